@@ -1,0 +1,281 @@
+"""Pins P6-P14 for the CPU oracle: moments, p-c formula, walk + forces, potential, leapfrog (no GPU).
+
+The checks are closed forms, textbook limits, brute force and invariants -- none re-uses the
+oracle's own formulas.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import bh_inputs
+import oracle
+
+
+def _state(cfg="c1", n=4096, seed=None):
+    pm, v, prm = bh_inputs.make(cfg, n=n, seed=seed)
+    return oracle.tree_build(pm, v), prm
+
+
+def _relerr(a, ref):
+    return np.linalg.norm(a[:, :3] - ref[:, :3], axis=1) / np.linalg.norm(ref[:, :3], axis=1)
+
+
+# ---------------------------------------------------------------- P6: moments
+def test_root_moments_match_direct_sums_and_boxes_tight():
+    st, _ = _state("c1", 16384)
+    t, p = st.tree, st.pos.astype(np.float64)
+    m, x = p[:, 3], p[:, :3]
+    M = m.sum()
+    com = (m[:, None] * x).sum(0) / M
+    r = x - com
+    Q = np.einsum("i,ij,ik->jk", m, r, r)
+    got = t.mom64[0]
+    assert abs(got[0] - M) < 1e-13 * M
+    assert np.allclose(got[1:4], com, rtol=0, atol=1e-12)
+    want = np.array([Q[0, 0], Q[1, 1], Q[2, 2], Q[0, 1], Q[0, 2], Q[1, 2]])
+    assert np.allclose(got[4:], want, rtol=1e-11, atol=1e-13)
+    # every cell: box is the exact min / max of its particles; moments of leaves by direct sums
+    for c in range(0, t.ncells, 37):
+        s = slice(int(t.pbegin[c]), int(t.pbegin[c] + t.pcount[c]))
+        assert np.array_equal(t.box[c, :3], st.pos[s, :3].min(0)) and np.array_equal(t.box[c, 3:], st.pos[s, :3].max(0))
+        mm, xx = m[s], x[s]
+        cc = (mm[:, None] * xx).sum(0) / mm.sum()
+        rr = xx - cc
+        qq = np.einsum("i,ij,ik->jk", mm, rr, rr)
+        assert np.allclose(t.mom64[c, 0], mm.sum(), rtol=1e-13)
+        assert np.allclose(t.mom64[c, 1:4], cc, atol=1e-12)
+        assert np.allclose(t.mom64[c, 4:], [qq[0, 0], qq[1, 1], qq[2, 2], qq[0, 1], qq[0, 2], qq[1, 2]],
+                           rtol=1e-9, atol=1e-16)
+
+
+def test_parallel_axis_identity_at_every_node():
+    st, _ = _state("c3", 20000)
+    t = st.tree
+    idx = [(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]
+    for c in np.nonzero(t.nchild > 0)[0]:
+        ch = np.arange(t.child_begin[c], t.child_begin[c] + t.nchild[c])
+        Mc, cc, Qc = t.mom64[ch, 0], t.mom64[ch, 1:4], t.mom64[ch, 4:]
+        M = Mc.sum()
+        com = (Mc[:, None] * cc).sum(0) / M
+        d = cc - com
+        Q = np.array([Qc[:, k].sum() + (Mc * d[:, a] * d[:, b]).sum() for k, (a, b) in enumerate(idx)])
+        assert abs(t.mom64[c, 0] - M) <= 1e-14 * M
+        assert np.allclose(t.mom64[c, 1:4], com, atol=1e-13)
+        assert np.allclose(t.mom64[c, 4:], Q, rtol=1e-10, atol=1e-18)
+
+
+# ---------------------------------------------------------------- P7: the p-c formula on a hand-made tree
+def _hand_tree(src, tgt):
+    """Root node with two leaf children: A = the source particles, B = the single target.
+
+    Bypasses keys/sort/tree so that the moments (O8), the MAC (O9) and the p-c formula (O10) are
+    exercised on a topology fixed by hand.
+    """
+    na = src.shape[0]
+    pos = np.concatenate([src, tgt]).astype(np.float32)
+    n = pos.shape[0]
+    lo = np.zeros(22, np.int64); lo[1] = 1; lo[2:] = 3
+    t = oracle.Tree(n, lo, np.array([0, 1, 1], np.int32), np.array([0, 0, 7], np.uint64),
+                    np.array([0, 0, na], np.int64), np.array([n, na, n - na], np.int64),
+                    np.array([1, -1, -1], np.int64), np.array([2, 0, 0], np.int32), np.array([-1, 0, 0], np.int64))
+    t.gcell = np.array([2], np.int64); t.gbegin = np.array([na], np.int64); t.gcount = np.array([n - na], np.int64)
+    oracle.moments(t, pos)
+    return t, pos
+
+
+def test_pc_closed_form_two_masses_on_axis():
+    # two equal masses m at (+-s, 0, 0), target on the axis at R: a_x = -(m/(R-s)^2 + m/(R+s)^2)
+    # = -(2m/R^2)(1 + 3 s^2/R^2 + 5 s^4/R^4 + ...); monopole + quadrupole keeps the first two terms.
+    m, s, R = 0.5, 0.125, 8.0
+    src = np.array([[-s, 0, 0, m], [s, 0, 0, m]])
+    t, pos = _hand_tree(src, np.array([[R, 0, 0, 1.0]]))
+    assert np.allclose(t.mom64[1], [2 * m, 0, 0, 0, 2 * m * s * s, 0, 0, 0, 0, 0], atol=1e-15)
+    r = oracle.walk_forces(t, pos, theta=0.5, eps=0.0)
+    assert r["npc"][0] == 1 and r["npp"][0] == 1          # cell A accepted, own leaf opened
+    ax, ay, az, phi = r["accpot"][2]
+    quad = -(2 * m / R ** 2) * (1 + 3 * s ** 2 / R ** 2)
+    exact = -(m / (R - s) ** 2 + m / (R + s) ** 2)
+    assert abs(ax - quad) < 1e-15 and ay == 0 and az == 0
+    assert abs(ax - exact) / abs(exact) < 6 * (s / R) ** 4   # next term is 5 s^4 / R^4
+    phi_quad = -(2 * m / R) * (1 + s ** 2 / R ** 2)
+    assert abs(phi - phi_quad) < 1e-15
+    # off axis (target on y): a_y = -2 m R / (R^2+s^2)^(3/2) = -(2m/R^2)(1 - 3 s^2 / (2 R^2) + ...)
+    t, pos = _hand_tree(src, np.array([[0, R, 0, 1.0]]))
+    r = oracle.walk_forces(t, pos, theta=0.5, eps=0.0)
+    ax, ay, az, phi = r["accpot"][2]
+    assert abs(ay + (2 * m / R ** 2) * (1 - 1.5 * s ** 2 / R ** 2)) < 1e-15 and ax == 0 and az == 0
+    assert abs(phi + (2 * m / R) * (1 - 0.5 * s ** 2 / R ** 2)) < 1e-15
+
+
+@pytest.mark.parametrize("eps", [0.0, 0.05, 0.2])
+def test_pc_error_falls_as_cube_of_size_over_distance(eps):
+    rng = np.random.default_rng(5)
+    s = 0.1
+    src = np.concatenate([rng.uniform(-s, s, (16, 3)), rng.uniform(0.5, 1.5, (16, 1))], axis=1).astype(np.float32)
+    dirn = np.array([0.3, -0.5, 0.81]); dirn /= np.linalg.norm(dirn)
+    errs, Rs = [], [1.0, 2.0, 4.0, 8.0]
+    for R in Rs:
+        t, pos = _hand_tree(src, np.array([np.append(R * dirn, 1.0)]))
+        r = oracle.walk_forces(t, pos, theta=0.9, eps=eps)
+        assert r["npc"][0] == 1
+        d = oracle.direct(pos, eps)[16]
+        got = r["accpot"][16]
+        errs.append((np.linalg.norm(got[:3] - d[:3]) / np.linalg.norm(d[:3]), abs(got[3] - d[3]) / abs(d[3])))
+    errs = np.array(errs)
+    for k in range(len(Rs) - 1):   # doubling R must cut the relative error by ~8 (octupole term); demand > 5
+        assert errs[k, 0] / errs[k + 1, 0] > 5.0, errs
+        assert errs[k, 1] / errs[k + 1, 1] > 5.0, errs
+    assert errs[-1, 0] < 5e-6
+
+
+def test_single_particle_cell_is_particle_particle():
+    src = np.array([[0.25, -0.5, 0.125, 0.75]])
+    t, pos = _hand_tree(src, np.array([[3.0, 1.0, -2.0, 1.0]]))
+    for eps in (0.0, 0.3):
+        r = oracle.walk_forces(t, pos, theta=0.5, eps=eps)
+        assert r["npc"][0] == 1
+        d = oracle.direct(pos, eps)[1]
+        assert np.allclose(r["accpot"][1], d, rtol=1e-15, atol=0)
+
+
+# ---------------------------------------------------------------- P8: walk + forces vs brute force
+def test_theta_to_zero_reproduces_direct_sum():
+    st, _ = _state("c1", 2048)
+    d = oracle.direct(st.pos, 0.01)
+    oracle.compute_forces(st, theta=1e-6, eps=0.01)
+    assert np.allclose(st.accpot, d, rtol=1e-12, atol=1e-13)
+    # every particle appears either as a particle or as a single-particle cell
+    assert np.all(st.npc + st.npp == st.tree.n)
+
+
+def test_tree_error_small_and_monotone_in_theta():
+    st, _ = _state("c1", 4096)
+    d = oracle.direct(st.pos, 0.0)
+    med = []
+    for th in (0.8, 0.6, 0.4, 0.2):
+        oracle.compute_forces(st, theta=th, eps=0.0)
+        med.append(np.median(_relerr(st.accpot, d)))
+    assert all(med[i] > med[i + 1] for i in range(3)), med
+    assert med[0] < 3e-3 and med[-1] < 3e-5, med
+
+
+def test_uniform_cube_vs_direct():
+    st, prm = _state("c3", 3000)
+    d = oracle.direct(st.pos, prm["eps"])
+    oracle.compute_forces(st, theta=prm["theta"], eps=prm["eps"])
+    e = _relerr(st.accpot, d)
+    assert np.median(e) < 2e-3 and e.max() < 0.2
+    assert np.max(np.abs(st.accpot[:, 3] - d[:, 3]) / np.abs(d[:, 3])) < 1e-3
+
+
+# ---------------------------------------------------------------- P9: MAC geometry
+def test_no_accepted_cell_contains_a_group_particle():
+    st, _ = _state("c1", 8192)
+    t = st.tree
+    for g in range(0, t.ngroups, 23):
+        r = oracle.walk_forces(t, st.pos, theta=1.0, eps=0.01, sel=[g], forces=False, want_lists=True)
+        b, e = t.gbegin[g], t.gbegin[g] + t.gcount[g]
+        cb, ce = t.pbegin[r["cells"]], t.pbegin[r["cells"]] + t.pcount[r["cells"]]
+        assert not np.any((cb < e) & (ce > b))
+        # lists cover every particle exactly once
+        assert t.pcount[r["cells"]].sum() + t.pcount[r["leaves"]].sum() == t.n
+        assert r["npp"][g] == t.pcount[r["leaves"]].sum() and r["npc"][g] == r["cells"].size
+
+
+# ---------------------------------------------------------------- P10 / P11: potential, momentum
+def test_plummer_potential_and_energies():
+    st, _ = _state("c1", 16384)
+    oracle.compute_forces(st, theta=0.5, eps=0.01)
+    a = bh_inputs.PLUMMER_A
+    p = st.pos.astype(np.float64)
+    r = np.linalg.norm(p[:, :3], axis=1)
+    phi_an = -1.0 / np.sqrt(r * r + a * a)
+    rel = np.abs(st.accpot[:, 3] - phi_an) / np.abs(phi_an)
+    assert np.median(rel) < 0.02 and np.percentile(rel, 99) < 0.12
+    W = 0.5 * np.sum(p[:, 3] * st.accpot[:, 3])
+    K = 0.5 * np.sum(p[:, 3] * np.sum(st.vel[:, :3].astype(np.float64) ** 2, axis=1))
+    assert abs(W + 0.5) < 0.02 and abs(K - 0.25) < 0.01      # -3 pi M^2 / (32 a) = -1/2; virial K = 1/4
+    # acceleration magnitude against the analytic field M r / (r^2 + a^2)^(3/2), outside the noisy core
+    sel = r > 0.5
+    ar = -np.sum(st.accpot[:, :3] * p[:, :3], axis=1) / r
+    an = r / np.power(r * r + a * a, 1.5)
+    assert np.median(np.abs(ar[sel] - an[sel]) / an[sel]) < 0.03
+
+
+def test_momentum_conservation():
+    st, _ = _state("c1", 4096)
+    m = st.pos[:, 3].astype(np.float64)
+    d = oracle.direct(st.pos, 0.01)
+    scale = np.sum(m * np.linalg.norm(d[:, :3], axis=1))
+    assert np.linalg.norm((m[:, None] * d[:, :3]).sum(0)) / scale < 1e-14
+    oracle.compute_forces(st, theta=0.75, eps=0.01)
+    assert np.linalg.norm((m[:, None] * st.accpot[:, :3]).sum(0)) / scale < 2e-4
+
+
+# ---------------------------------------------------------------- P12 / P13: leapfrog
+def _energy(st):
+    m = st.pos[:, 3].astype(np.float64)
+    K = 0.5 * np.sum(m * np.sum(st.vel[:, :3].astype(np.float64) ** 2, axis=1))
+    W = 0.5 * np.sum(m * st.accpot[:, 3])
+    return K + W
+
+
+def test_two_body_circular_orbit():
+    # two unit masses, separation 2 -> each at radius 1 feels a = 1/4: v = 1/2, period 4 pi
+    pm = np.array([[1, 0, 0, 1], [-1, 0, 0, 1]], np.float32)
+    v = np.array([[0, 0.5, 0, 0], [0, -0.5, 0, 0]], np.float32)
+    steps = 256
+    dt = 4 * math.pi / steps
+    st = oracle.compute_forces(oracle.tree_build(pm, v), 0.5, 0.0)
+    assert np.allclose(st.accpot[np.argsort(st.ids)], [[-0.25, 0, 0, -0.5], [0.25, 0, 0, -0.5]], atol=1e-15)
+    e0 = _energy(st)
+    rmin, rmax = 1.0, 1.0
+    for _ in range(steps):
+        st = oracle.leapfrog_step(st, 0.5, 0.0, dt)
+        rr = np.linalg.norm(st.pos[:, :3], axis=1)
+        rmin, rmax = min(rmin, rr.min()), max(rmax, rr.max())
+    o = np.argsort(st.ids)
+    assert np.allclose(st.pos[o, :3], pm[:, :3], atol=3e-3)        # back at the start after one period
+    assert rmax - rmin < 2e-3 and abs(_energy(st) - e0) < 1e-5
+
+
+def test_leapfrog_reversible_and_second_order():
+    pm, v, _ = bh_inputs.make("c1", n=512)
+    st0 = oracle.compute_forces(oracle.tree_build(pm, v), 1e-6, 0.05)     # direct-sum forces
+    # reversibility: n steps, flip v, n steps -> start (up to float32 rounding of x, v)
+    st = st0
+    for _ in range(4):
+        st = oracle.leapfrog_step(st, 1e-6, 0.05, 1 / 64)
+    st.vel = -st.vel
+    for _ in range(4):
+        st = oracle.leapfrog_step(st, 1e-6, 0.05, 1 / 64)
+    o, o0 = np.argsort(st.ids), np.argsort(st0.ids)
+    assert np.max(np.abs(st.pos[o, :3] - st0.pos[o0, :3])) < 2e-5
+    assert np.max(np.abs(-st.vel[o, :3] - st0.vel[o0, :3])) < 2e-5
+    # energy error over a fixed time span scales as dt^2 (softening 0.2 so that dt resolves every encounter)
+    sa = oracle.compute_forces(oracle.tree_build(pm, v), 1e-6, 0.2)
+    errs = []
+    for nst in (4, 8, 16):
+        st = sa
+        for _ in range(nst):
+            st = oracle.leapfrog_step(st, 1e-6, 0.2, 0.25 / nst)
+        errs.append(abs(_energy(st) - _energy(sa)))
+    assert 3.0 < errs[0] / errs[1] < 5.5 and 3.0 < errs[1] / errs[2] < 5.5, errs
+
+
+def test_energy_drift_c1_is_small():
+    pm, v, prm = bh_inputs.make("c1", n=4096)
+    st = oracle.compute_forces(oracle.tree_build(pm, v), prm["theta"], prm["eps"])
+    e0 = _energy(st)
+    for _ in range(4):
+        st = oracle.leapfrog_step(st, prm["theta"], prm["eps"], prm["dt"])
+    assert abs((_energy(st) - e0) / e0) < 2e-4      # context: the paper's merger, ~1e-4 (Table 2)
+
+
+# ---------------------------------------------------------------- P14: determinism
+def test_deterministic_across_runs():
+    st, prm = _state("c1", 8192)
+    a = oracle.walk_forces(st.tree, st.pos, 0.75, 0.01)
+    b = oracle.walk_forces(st.tree, st.pos, 0.75, 0.01)
+    assert np.array_equal(a["accpot"], b["accpot"]) and np.array_equal(a["npc"], b["npc"])
