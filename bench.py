@@ -1,0 +1,345 @@
+#!/usr/bin/env python
+"""bench.py -- particles/s per full Barnes-Hut step (build + walk + integrate) on B200.
+
+A "step" is one bh_leapfrog_step: kick, drift, S0-S6 tree build, S7+S8 walk + forces, kick.
+Default workload: BASELINE.json configs[1], the 1 M Plummer sphere (theta = 0.75, the value the paper's 2.8 M
+particles/s is quoted on; --theta 0.5 gives the other configured value).  Inputs are seeded and synthetic.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c2] [--theta T] [--impl ours|reference]
+
+N > 1 (torchrun, one rank per GPU): every rank steps its own replica of the workload ("replicas only", DESIGN.md
+multi-GPU section): no data-path collective, weak scaling; time = max over ranks.
+--impl reference times the CPU oracle (oracle/) on the host cores on a bounded sample of the same workload.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import bh_inputs  # noqa: E402
+
+PAPER_PARTICLES_PER_S = 2.8e6      # GTX480, Plummer N = 2^20, theta = 0.75
+FLOP_PP, FLOP_PC = 20, 64          # DESIGN.md flop convention (FMA = 2, rsqrt = 1)
+L2_FLUSH_BYTES = 256 << 20
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", str(self.idx)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        os.unlink(self.f.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _workload(args):
+    cfg = args.config
+    n = args.n or {"c1": 16_384, "c2": 1_048_576, "c3": 4_194_304, "c4": 16_777_216, "c5": 33_554_432}[cfg]
+    return cfg, n
+
+
+def _make_inputs(cfg, n, rank):
+    seed = bh_inputs.SEEDS[cfg] + 1000 * rank
+    pm, vel, prm = bh_inputs.make(cfg, n=n, seed=seed)
+    return pm, vel, prm
+
+
+# ------------------------------------------------------------------------------------------------ CPU oracle legs
+def oracle_sample(pm, vel, theta, eps, dt, budget_groups=None, seed=1):
+    """Time the oracle, as it stands, on a bounded sample of one step of this workload.
+
+    Full O1-O8 tree build on all n particles (single thread), then O9+O10 (OpenMP over groups) for a seeded random
+    subset of groups, then the O11 kicks/drift.  particles/s = particles of the sampled groups / (walk time of the
+    sample + the sample's share of the build and integration time).
+    """
+    import oracle
+    n = pm.shape[0]
+    t0 = time.perf_counter()
+    st = oracle.tree_build(pm, vel)
+    t_build = time.perf_counter() - t0
+    G = st.tree.ngroups
+    rng = np.random.default_rng(seed)
+    if budget_groups is None:
+        budget_groups = min(G, 65536)      # c2: every group, i.e. the whole step (~6 s on 8 cores)
+    sel = np.sort(rng.choice(G, size=min(G, budget_groups), replace=False)).astype(np.int64)
+    t0 = time.perf_counter()
+    oracle.compute_forces(st, theta, eps, sel=sel)
+    t_walk = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    a32 = np.nan_to_num(st.accpot).astype(np.float32)
+    v = oracle.kick(st.vel, a32, np.float32(0.5 * dt))
+    p = oracle.drift(st.pos, v, np.float32(dt))
+    v = oracle.kick(v, a32, np.float32(0.5 * dt))
+    t_int = time.perf_counter() - t0
+    n_s = int(st.tree.gcount[sel].sum())
+    frac = n_s / n
+    t_eff = t_walk + frac * (t_build + t_int)
+    inter = float((st.tree.gcount[sel] * (st.npc[sel] + st.npp[sel])).sum())
+    return dict(value=n_s / t_eff, particles=n_s, groups=int(sel.size), t_build=t_build, t_walk=t_walk, t_int=t_int,
+                interactions_per_s=inter / t_walk, cores=os.cpu_count())
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg, n = _workload(args)
+    pm, vel, prm = _make_inputs(cfg, n, 0)
+    theta = args.theta or prm["theta"]
+    vals, times = [], []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        r = oracle_sample(pm, vel, theta, prm["eps"], prm["dt"], budget_groups=args.ref_groups, seed=1 + i)
+        if i >= args.warmup:
+            vals.append(r["value"]); times.append(time.perf_counter() - t0)
+    v = float(np.mean(vals))
+    sample = (f"per step: full oracle tree build of n={n} (1 thread) + walk/forces of {r['groups']} seeded random groups "
+              f"({r['particles']} particles, OpenMP over groups); particles/s = sampled particles / (sample walk time + the "
+              f"sample's share of build + integration time)")
+    line = {"impl": "reference", "metric": "particles/sec per full step (build+walk+integrate)", "value": v, "unit": "particles/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * n / v,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": v / PAPER_PARTICLES_PER_S if cfg == "c2" and abs(theta - 0.75) < 1e-6 else None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg}: {n} particles, theta={theta}, eps={prm['eps']}, dt={prm['dt']}", "nleaf": 16, "ncrit": 64},
+            "cpu_baseline": {"value": v, "unit": "particles/s", "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ the CUDA path
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_1106_1900_b200 import BarnesHut
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg, n = _workload(args)
+    pm, vel, prm = _make_inputs(cfg, n, rank)
+    theta, eps, dt = args.theta or prm["theta"], prm["eps"], prm["dt"]
+    bh = BarnesHut(n, max_cells=args.max_cells)
+    bh.set_particles(pm, vel)
+    bh.tree_build()
+    bh.compute_forces(theta, eps)
+    bh.sync_status()
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    bh.set_stage_timing(True)
+
+    def one_step(ev0=None, ev1=None):
+        flush.fill_(1)                       # evict the previous step's working set from L2 (not timed)
+        if ev0 is not None:
+            ev0.record(stream)
+        bh.leapfrog_step(theta, eps, dt)
+        if ev1 is not None:
+            ev1.record(stream)
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    s0 = bh.sync_status()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    stage_acc = {}
+    wall0 = time.perf_counter()
+    for a, b in evs:
+        one_step(a, b)
+        for k, v in bh.stage_ms().items():   # per-stage CUDA events recorded by the library on the launching stream
+            stage_acc[k] = stage_acc.get(k, 0.0) + v
+    barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop() if rank == 0 else None
+    s1 = bh.sync_status()
+    ms = sum(a.elapsed_time(b) for a, b in evs)
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    value = world * n * args.steps / (ms_total * 1e-3)
+
+    # ---- e2e: the same step driven from HOST buffers through the C ABI (H2D and D2H inside the timed region)
+    hp = torch.from_numpy(pm).pin_memory(); hv = torch.from_numpy(vel).pin_memory()
+    hid = torch.arange(n, dtype=torch.int32).pin_memory()
+    ha = torch.empty((n, 4), dtype=torch.float32).pin_memory()
+    e2e_steps = max(1, min(args.steps, 8))
+
+    def host_step():
+        bh.set_particles(hp, hv, hid)        # H2D: pos+mass, vel, id
+        bh.tree_build()
+        bh.compute_forces(theta, eps)
+        bh.kick_drift(dt, dt)                # S9, kick-drift form
+        bh.get_particles(hp, hv, ha, hid)    # D2H: pos, vel, acc+pot, id
+        torch.cuda.synchronize()
+
+    bh.set_stage_timing(False)
+    for _ in range(2):
+        host_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        host_step()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = world * n * e2e_steps / float(t.item())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (k_walk): plain FP32 ALU bound, DESIGN.md
+    peaks, peak_kind = _peaks()
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    props = torch.cuda.get_device_properties(dev)
+    peak_tflops = props.multi_processor_count * 128 * 2 * sm_max * 1e6 / 1e12
+    walk_ms = stage_acc["walk"] / args.steps
+    flops = FLOP_PP * s1.sum_pp + FLOP_PC * s1.sum_pc            # of the last step's walk
+    achieved = flops / (walk_ms * 1e-3) / 1e12
+    prof = os.path.join(ROOT, "profiles", "walk_traffic.json")
+    traffic = json.load(open(prof)).get("dram_bytes_per_launch") if os.path.exists(prof) else None
+    build_ms = sum(stage_acc[k] for k in ("bbox", "keys", "sort", "reorder", "cells", "groups", "moments", "record")) / args.steps
+    roofline = {"bound": "alu", "kernel": "k_walk", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": achieved / peak_tflops, "traffic": traffic,
+                "peak_kind": f"148 SMs x 128 FP32 lanes x 2 flop x sm_max_mhz ({peak_kind} clock {sm_max:.0f} MHz), DESIGN.md",
+                "flop_convention": "20 per p-p, 64 per p-c (FMA=2, rsqrt=1); useful interactions only",
+                "walk_ms": walk_ms, "interactions_per_s": (s1.sum_pp + s1.sum_pc) / (walk_ms * 1e-3),
+                "frac_at_observed_clock": (achieved / (peak_tflops * clocks["sm_mhz"] / sm_max)) if clocks and clocks.get("sm_mhz") else None}
+
+    # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        r = oracle_sample(pm, vel, theta, eps, dt, budget_groups=args.ref_groups)
+        cpu = {"value": r["value"], "unit": "particles/s", "cores": r["cores"], "kind": "oracle",
+               "sample": (f"full oracle tree build of n={n} (1 thread, {r['t_build']:.2f} s) + walk/forces of {r['groups']} seeded "
+                          f"random groups = {r['particles']} particles (OpenMP, {r['t_walk']:.2f} s); particles/s = sampled "
+                          f"particles / (walk time + the sample's share of build+integration)"),
+               "interactions_per_s": r["interactions_per_s"]}
+
+    line = {
+        "metric": "particles/sec per full step (build+walk+integrate)", "value": value, "unit": "particles/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
+        "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": value / PAPER_PARTICLES_PER_S if (cfg == "c2" and abs(theta - 0.75) < 1e-6 and world == 1) else None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{cfg}: Plummer sphere n={n}" if cfg in ("c1", "c2") else f"{cfg}: n={n}",
+                   "theta": theta, "eps": eps, "dt": dt, "nleaf": 16, "ncrit": 64, "rebuild_every_step": True,
+                   "l2": f"{L2_FLUSH_BYTES >> 20} MiB buffer written between timed steps (outside the event pairs)",
+                   "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
+                   "cells": int(s1.n_cells), "groups": int(s1.n_groups), "levels": int(s1.n_levels),
+                   "pp_per_particle": s1.sum_pp / n, "pc_per_particle": s1.sum_pc / n, "mac_tests_per_group": s1.sum_mac / max(1, s1.n_groups)},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": "particles/s", "h2d_bytes_per_step": int(n * 36), "d2h_bytes_per_step": int(n * 52),
+                "steps": e2e_steps, "what": "bh_set_particles(host) + bh_tree_build + bh_compute_forces + bh_kick_drift + bh_get_particles(host), pinned host buffers"},
+        "gpu_launches": int(s1.launches - s0.launches),
+        "roofline": roofline,
+        "stages_ms": {k: v / args.steps for k, v in stage_acc.items()},
+        "build_ms": build_ms,
+        "wall_s_timed_region": wall,
+        "cpu_baseline": cpu,
+        "paper_context": "2.8 M particles/s on a GTX480, Plummer N=2^20, theta=0.75 (PAPER.md:182, 256)",
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=8)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c2", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--n", type=int, default=0)
+    ap.add_argument("--theta", type=float, default=0.0)
+    ap.add_argument("--max-cells", dest="max_cells", type=int, default=0)
+    ap.add_argument("--ref-groups", dest="ref_groups", type=int, default=None)
+    ap.add_argument("--no-cpu", dest="no_cpu", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                      # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,149 @@
+/* bh.h -- C ABI of the B200-native Barnes-Hut force pipeline (arxiv/paper_1106_1900, "Bonsai").
+ *
+ * One step of the paper's method (PAPER.md = /root/reference/PAPER.md, "L<n>" = line n):
+ *   S0 domain box (L374)            S1 60-bit Morton keys (L374-392)      S2 stable key radix sort (L59, L352, L362)
+ *   S3 reorder by the sort (L174)   S4 sparse octree, <= nleaf per leaf (L63-65, Fig.1-2)
+ *   S5 groups, <= ncrit (L75)       S6 monopole + quadrupole moments in fp64, boxes (L109-115, L127, L266)
+ *   S7 group walk, MAC d > l/theta + delta (L83-87, Eq.1)          S8 softened p-p / p-c forces + potentials (L85, L97)
+ *   S9 shared-step leapfrog (L105)
+ * Every step runs in hand-written sm_100a CUDA kernels inside this library; there is no CPU fallback.
+ *
+ * Conventions
+ *   - Units: N-body units, G = 1 (L238).  Arithmetic: fp32 except the moments (fp64), as in the paper (L154, L170).
+ *   - Particle layout: pos_mass = float[n][4] (x, y, z, m); vel = float[n][4] (vx, vy, vz, unused);
+ *     acc_pot = float[n][4] (ax, ay, az, phi); id = uint32[n] (caller identity).
+ *   - The library keeps the particle state inside the caller-provided WORKSPACE, in key-sorted order
+ *     (bh_tree_build re-sorts it; `id` follows the particles).  bh_set_particles / bh_get_particles copy in / out.
+ *   - Memory: the library never allocates device memory.  `d_workspace` is device memory owned by the caller
+ *     (e.g. a torch tensor) and must stay alive until bh_destroy.  Host objects are owned by the ctx.
+ *   - Streams: `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  bh_tree_build,
+ *     bh_compute_forces and bh_leapfrog_step only enqueue work: no host synchronisation, no host<->device copies,
+ *     so they can be captured into a CUDA graph.  One ctx = one stream at a time; not thread-safe.
+ *   - Errors: every call returns BH_OK (0) or a negative bh_status; nothing throws or exits.  Errors that only the
+ *     device can see (non-finite input, capacity overflow) are recorded in a device status word and reported by
+ *     bh_sync_status.
+ */
+#ifndef BH_B200_H
+#define BH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum bh_status {
+    BH_OK = 0,
+    BH_ERR_INVALID_ARG = -1, /* null pointer, n <= 0, n > n_max, theta <= 0 or non-finite, eps < 0, non-finite dt, bad config */
+    BH_ERR_WORKSPACE = -2,   /* workspace too small or not device memory */
+    BH_ERR_STATE = -3,       /* forces before build, step before forces, build before particles */
+    BH_ERR_CUDA = -4,        /* a CUDA runtime call failed (bh_last_cuda_error gives the code) */
+    BH_ERR_NONFINITE = -5,   /* deferred: NaN/Inf position or mass <= 0 seen by S0 (A27) */
+    BH_ERR_CAPACITY = -6     /* deferred: more cells than max_cells */
+} bh_status;
+
+/* Tunables.  Zero-initialise and override; 0 means "default". */
+typedef struct bh_config {
+    int32_t nleaf;     /* max particles per leaf, 1..64; default 16 (L63) */
+    int32_t ncrit;     /* max particles per group, 1..64; default 64 (L75) */
+    int64_t max_cells; /* cell capacity; default = the hard bound n_max + 20*(n_max/(nleaf+1)) + 1 */
+} bh_config;
+
+typedef struct bh_ctx bh_ctx;
+
+/* What a step produced.  Filled by bh_sync_status (which synchronises the stream). */
+typedef struct bh_stats {
+    int32_t status;        /* deferred device status: BH_OK, BH_ERR_NONFINITE or BH_ERR_CAPACITY */
+    int32_t n_levels;      /* deepest occupied level + 1 */
+    int64_t n;             /* particles */
+    int64_t n_cells;       /* tree cells (S4) */
+    int64_t n_groups;      /* groups (S5) */
+    int64_t sum_pc;        /* particle-cell interactions evaluated by the last bh_compute_forces: sum_g n_g * n_pc[g] */
+    int64_t sum_pp;        /* particle-particle interactions: sum_g n_g * n_pp[g] (includes the self term) */
+    int64_t sum_mac;       /* MAC evaluations (Eq.1) in the last walk */
+    int64_t launches;      /* kernels launched by this ctx since bh_create */
+    float   lo[3];         /* S0: domain corner */
+    float   hi[3];         /* S0: per-axis maximum */
+    int32_t domain_exp;    /* S0: cube side = 2^domain_exp */
+    int32_t reserved;
+} bh_stats;
+
+/* Device pointers into the workspace, valid until the next bh_tree_build / bh_set_particles (particle arrays) or
+ * bh_destroy.  All arrays are in the canonical numbering of DESIGN.md: cells level-major, ascending first particle
+ * within a level (A10); groups in particle order.  Filled by bh_export_tree, which enqueues one conversion kernel on
+ * `stream` (the caller synchronises before reading).  n_cells / n_groups come from bh_sync_status. */
+typedef struct bh_tree_view {
+    const float*    pos_mass;      /* float[n][4], sorted */
+    const float*    vel;           /* float[n][4], sorted */
+    const float*    acc_pot;       /* float[n][4], sorted; valid after bh_compute_forces */
+    const uint32_t* id;            /* uint32[n] */
+    const uint64_t* key;           /* uint64[n], sorted Morton keys (S1, S2) */
+    const uint32_t* perm;          /* uint32[n]: position BEFORE this build of the j-th sorted particle (S2) */
+    const uint32_t* level_offset;  /* uint32[22]: cells of level L are [level_offset[L], level_offset[L+1]) */
+    const int32_t*  cell_level;    /* int32[C] */
+    const uint64_t* cell_prefix;   /* uint64[C]: key >> (60 - 3 level) */
+    const uint32_t* cell_pbegin;   /* uint32[C]: first particle */
+    const uint32_t* cell_pcount;   /* uint32[C] */
+    const int32_t*  cell_child_begin; /* int32[C]: first child, -1 for a leaf */
+    const int32_t*  cell_nchild;   /* int32[C]: 0 for a leaf */
+    const int32_t*  cell_parent;   /* int32[C]: -1 for the root */
+    const double*   cell_mom64;    /* double[C][10]: M, com xyz, Qxx, Qyy, Qzz, Qxy, Qxz, Qyz (S6, fp64) */
+    const float*    cell_box;      /* float[C][6]: min xyz, max xyz (S6) */
+    const float*    cell_mom32;    /* float[C][10]: the fp32 roundings used by the walk; valid after bh_compute_forces */
+    const float*    cell_r2open;   /* float[C]: (l/theta + delta)^2 (Eq.1); valid after bh_compute_forces */
+    const uint32_t* group_begin;   /* uint32[G+1]: first particle of each group; group_begin[G] = n (S5) */
+    const uint32_t* group_cell;    /* uint32[G]: the cell a group comes from */
+    const uint32_t* group_npc;     /* uint32[G]: accepted cells per group (S7); valid after bh_compute_forces */
+    const uint32_t* group_npp;     /* uint32[G]: particles of opened leaves per group (S7) */
+} bh_tree_view;
+
+/* Bytes of device workspace needed for up to n_max particles (host-only, pure).  0 on a bad argument. */
+size_t bh_workspace_bytes(int64_t n_max, const bh_config* cfg);
+
+/* Create a context on the device that owns `d_workspace` (256-byte aligned device memory, `bytes` long).
+ * cfg may be NULL (defaults).  The device is taken from the pointer. */
+int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspace, size_t bytes);
+int bh_destroy(bh_ctx* ctx);
+
+/* Copy n particles into the workspace (cudaMemcpyAsync on `stream`; pointers may be host or device memory, host
+ * memory should be pinned for the copy to be asynchronous).  vel may be NULL (zeros); id may be NULL (0..n-1).
+ * Invalidates tree and forces. */
+int bh_set_particles(bh_ctx* ctx, int64_t n, const float* pos_mass, const float* vel, const uint32_t* id, void* stream);
+
+/* Copy the current (key-sorted) state out; any pointer may be NULL; host or device destinations. */
+int bh_get_particles(bh_ctx* ctx, float* pos_mass, float* vel, float* acc_pot, uint32_t* id, void* stream);
+
+/* S0-S6: domain, keys, sort, reorder, octree, groups, fp64 moments and boxes (L55-65, L107-115).  theta-independent. */
+int bh_tree_build(bh_ctx* ctx, void* stream);
+
+/* S7-S8 on the current tree: opening radii for `theta` (Eq.1), group walk, p-p and p-c forces + potentials
+ * with Plummer softening `eps` (L85, L97).  Needs bh_tree_build.  eps = 0 with coincident particles is undefined. */
+int bh_compute_forces(bh_ctx* ctx, float theta, float eps, void* stream);
+
+/* S9 around S0-S8 (L105): v += a dt/2; x += v dt; tree_build; compute_forces; v += a dt/2.  Needs valid forces. */
+int bh_leapfrog_step(bh_ctx* ctx, float theta, float eps, float dt, void* stream);
+
+/* S9 on its own (L105), the kick-drift form of the same leapfrog: v += a * dt_kick; x += v * dt_drift, with the
+ * accelerations of the last bh_compute_forces.  Invalidates tree and forces (the particles moved). */
+int bh_kick_drift(bh_ctx* ctx, float dt_kick, float dt_drift, void* stream);
+
+/* Synchronise `stream`, then report the deferred device status and the counters.  Returns the deferred status. */
+int bh_sync_status(bh_ctx* ctx, void* stream, bh_stats* out);
+
+/* Fill `out` with device pointers to the canonical tree arrays (see bh_tree_view). */
+int bh_export_tree(bh_ctx* ctx, bh_tree_view* out, void* stream);
+
+/* Per-stage device times of the last bh_tree_build + bh_compute_forces, in ms, when enabled (adds event records,
+ * do not enable under graph capture).  Order: bbox, keys, sort, reorder, cells, groups, moments, record (fp32 walk
+ * records + opening radii), walk (the S7+S8 kernel alone).  Synchronises. */
+int bh_set_stage_timing(bh_ctx* ctx, int enable);
+int bh_get_stage_ms(bh_ctx* ctx, float ms[9]);
+
+int bh_last_cuda_error(const bh_ctx* ctx);
+const char* bh_status_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BH_B200_H */

@@ -1,0 +1,7 @@
+"""B200-native Barnes-Hut force pipeline of arxiv/paper_1106_1900 (Bonsai): CUDA library + thin binding.
+
+``csrc/`` holds the sm_100a kernels and the C ABI of ``include/bh.h``; ``binding.py`` marshals arguments.
+Nothing here imports ``oracle/`` (test infrastructure); there is no CPU fallback.
+"""
+from .binding import (BarnesHut, BhError, BhStats, LIB_PATH, STAGES, SYMBOLS, load_library,  # noqa: F401
+                      workspace_bytes)

@@ -1,0 +1,231 @@
+"""ctypes binding of include/bh.h -- argument marshalling only; every step of the path runs in the CUDA library.
+
+PyTorch is used for device memory (the workspace tensor) and streams.  There is no CPU fallback: constructing a
+``BarnesHut`` without the compiled library or without a CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libbh_b200.so")
+
+BH_OK = 0
+STATUS = {0: "BH_OK", -1: "BH_ERR_INVALID_ARG", -2: "BH_ERR_WORKSPACE", -3: "BH_ERR_STATE", -4: "BH_ERR_CUDA",
+          -5: "BH_ERR_NONFINITE", -6: "BH_ERR_CAPACITY"}
+
+# every symbol include/bh.h declares (checked by tests/test_abi.py)
+SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", "bh_get_particles", "bh_tree_build",
+           "bh_compute_forces", "bh_leapfrog_step", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
+           "bh_get_stage_ms", "bh_last_cuda_error", "bh_status_string"]
+
+
+class BhConfig(C.Structure):
+    _fields_ = [("nleaf", C.c_int32), ("ncrit", C.c_int32), ("max_cells", C.c_int64)]
+
+
+class BhStats(C.Structure):
+    _fields_ = [("status", C.c_int32), ("n_levels", C.c_int32), ("n", C.c_int64), ("n_cells", C.c_int64),
+                ("n_groups", C.c_int64), ("sum_pc", C.c_int64), ("sum_pp", C.c_int64), ("sum_mac", C.c_int64),
+                ("launches", C.c_int64), ("lo", C.c_float * 3), ("hi", C.c_float * 3), ("domain_exp", C.c_int32),
+                ("reserved", C.c_int32)]
+
+
+_VIEW_FIELDS = ["pos_mass", "vel", "acc_pot", "id", "key", "perm", "level_offset", "cell_level", "cell_prefix",
+                "cell_pbegin", "cell_pcount", "cell_child_begin", "cell_nchild", "cell_parent", "cell_mom64", "cell_box",
+                "cell_mom32", "cell_r2open", "group_begin", "group_cell", "group_npc", "group_npp"]
+
+
+class BhTreeView(C.Structure):
+    _fields_ = [(name, C.c_void_p) for name in _VIEW_FIELDS]
+
+
+class BhError(RuntimeError):
+    def __init__(self, code: int, what: str = ""):
+        self.code = code
+        super().__init__(f"{STATUS.get(code, code)} {what}".strip())
+
+
+_lib = None
+
+
+def load_library():
+    """Load libbh_b200.so (built by paper_1106_1900_b200/build.py).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(f"{LIB_PATH} not built: run `python -c 'import __graft_entry__ as g; g.build()'`")
+    lib = C.CDLL(LIB_PATH)
+    lib.bh_workspace_bytes.restype = C.c_size_t
+    lib.bh_workspace_bytes.argtypes = [C.c_int64, C.POINTER(BhConfig)]
+    lib.bh_create.argtypes = [C.POINTER(C.c_void_p), C.c_int64, C.POINTER(BhConfig), C.c_void_p, C.c_size_t]
+    lib.bh_destroy.argtypes = [C.c_void_p]
+    lib.bh_set_particles.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.bh_get_particles.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.bh_tree_build.argtypes = [C.c_void_p, C.c_void_p]
+    lib.bh_compute_forces.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p]
+    lib.bh_leapfrog_step.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_void_p]
+    lib.bh_kick_drift.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p]
+    lib.bh_sync_status.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(BhStats)]
+    lib.bh_export_tree.argtypes = [C.c_void_p, C.POINTER(BhTreeView), C.c_void_p]
+    lib.bh_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
+    lib.bh_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    lib.bh_last_cuda_error.argtypes = [C.c_void_p]
+    lib.bh_status_string.restype = C.c_char_p
+    lib.bh_status_string.argtypes = [C.c_int]
+    for f in ("bh_create", "bh_destroy", "bh_set_particles", "bh_get_particles", "bh_tree_build", "bh_compute_forces",
+              "bh_leapfrog_step", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing", "bh_get_stage_ms",
+              "bh_last_cuda_error"):
+        getattr(lib, f).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def workspace_bytes(n_max: int, nleaf: int = 0, ncrit: int = 0, max_cells: int = 0) -> int:
+    cfg = BhConfig(nleaf, ncrit, max_cells)
+    return int(load_library().bh_workspace_bytes(n_max, C.byref(cfg)))
+
+
+STAGES = ["bbox", "keys", "sort", "reorder", "cells", "groups", "moments", "record", "walk"]
+
+
+def _ptr(x):
+    """Host (numpy / pinned torch) or device (torch cuda) buffer -> raw pointer; None -> NULL."""
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        assert x.flags["C_CONTIGUOUS"]
+        return x.ctypes.data
+    assert x.is_contiguous()
+    return x.data_ptr()
+
+
+class BarnesHut:
+    """One Barnes-Hut context on one GPU: same calls as include/bh.h (bh_tree_build, bh_compute_forces, bh_leapfrog_step)."""
+
+    def __init__(self, n_max: int, nleaf: int = 0, ncrit: int = 0, max_cells: int = 0, device=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1106_1900_b200 needs a CUDA device: there is no CPU fallback")
+        self.lib = load_library()
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        cfg = BhConfig(nleaf, ncrit, max_cells)
+        nbytes = int(self.lib.bh_workspace_bytes(n_max, C.byref(cfg)))
+        if nbytes == 0:
+            raise BhError(-1, "bad n_max / config")
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) & ~255
+        self._ws_off = base - self.workspace.data_ptr()
+        self._ws_base = base
+        self._ws_bytes = nbytes
+        h = C.c_void_p()
+        self._check(self.lib.bh_create(C.byref(h), n_max, C.byref(cfg), C.c_void_p(base), nbytes), "bh_create")
+        self.h = h
+        self.n_max = n_max
+        self.n = 0
+
+    # ------------------------------------------------------------------ helpers
+    def _check(self, rc: int, what: str = ""):
+        if rc != BH_OK:
+            extra = ""
+            if rc == -4 and getattr(self, "h", None):
+                extra = f" (cudaError {self.lib.bh_last_cuda_error(self.h)})"
+            raise BhError(rc, what + extra)
+
+    def _stream(self):
+        return C.c_void_p(torch.cuda.current_stream(self.device).cuda_stream)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.bh_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ------------------------------------------------------------------ the C ABI, one to one
+    def set_particles(self, pos_mass, vel=None, ids=None):
+        """pos_mass float32[n,4], vel float32[n,4] or None, ids uint32[n] or None; numpy, pinned or CUDA torch tensors."""
+        n = int(pos_mass.shape[0])
+        self._keep = (pos_mass, vel, ids)   # keep host buffers alive until the async copies are done
+        self._check(self.lib.bh_set_particles(self.h, n, _ptr(pos_mass), _ptr(vel), _ptr(ids), self._stream()), "bh_set_particles")
+        self.n = n
+
+    def get_particles(self, pos_mass=None, vel=None, acc_pot=None, ids=None):
+        self._check(self.lib.bh_get_particles(self.h, _ptr(pos_mass), _ptr(vel), _ptr(acc_pot), _ptr(ids), self._stream()),
+                    "bh_get_particles")
+
+    def tree_build(self):
+        self._check(self.lib.bh_tree_build(self.h, self._stream()), "bh_tree_build")
+
+    def compute_forces(self, theta: float, eps: float):
+        self._check(self.lib.bh_compute_forces(self.h, theta, eps, self._stream()), "bh_compute_forces")
+
+    def leapfrog_step(self, theta: float, eps: float, dt: float):
+        self._check(self.lib.bh_leapfrog_step(self.h, theta, eps, dt, self._stream()), "bh_leapfrog_step")
+
+    def kick_drift(self, dt_kick: float, dt_drift: float):
+        self._check(self.lib.bh_kick_drift(self.h, dt_kick, dt_drift, self._stream()), "bh_kick_drift")
+
+    def sync_status(self, check: bool = True) -> BhStats:
+        st = BhStats()
+        rc = self.lib.bh_sync_status(self.h, self._stream(), C.byref(st))
+        if check:
+            self._check(rc, "bh_sync_status")
+        return st
+
+    def set_stage_timing(self, enable: bool):
+        self._check(self.lib.bh_set_stage_timing(self.h, int(enable)))
+
+    def stage_ms(self) -> dict:
+        ms = (C.c_float * 9)()
+        self._check(self.lib.bh_get_stage_ms(self.h, ms), "bh_get_stage_ms")
+        return dict(zip(STAGES, [float(x) for x in ms]))
+
+    # ------------------------------------------------------------------ views of the workspace (no copies)
+    def _view(self, ptr: int, count: int, dtype: torch.dtype, shape=None):
+        if ptr is None or count == 0:
+            return torch.empty(0, dtype=dtype, device=self.device)
+        off = ptr - self.workspace.data_ptr()
+        nb = count * torch.empty(0, dtype=dtype).element_size()
+        t = self.workspace[off: off + nb].view(dtype)
+        return t.view(shape) if shape is not None else t
+
+    def export_tree(self) -> dict:
+        """Canonical arrays of bh_tree_view as torch tensors that alias the workspace (synchronises)."""
+        v = BhTreeView()
+        self._check(self.lib.bh_export_tree(self.h, C.byref(v), self._stream()), "bh_export_tree")
+        st = self.sync_status()
+        n, nc, ng = int(st.n), int(st.n_cells), int(st.n_groups)
+        f32, i32, u8 = torch.float32, torch.int32, torch.uint8
+        out = dict(stats=st, n=n, n_cells=nc, n_groups=ng)
+        out["pos_mass"] = self._view(v.pos_mass, n * 4, f32, (n, 4))
+        out["vel"] = self._view(v.vel, n * 4, f32, (n, 4))
+        out["acc_pot"] = self._view(v.acc_pot, n * 4, f32, (n, 4))
+        out["id"] = self._view(v.id, n, i32)                 # uint32 payload viewed as int32 (n < 2^31)
+        out["key"] = self._view(v.key, n, torch.int64)       # 60-bit keys fit a signed 64-bit view
+        out["perm"] = self._view(v.perm, n, i32)
+        out["level_offset"] = self._view(v.level_offset, 22, i32)
+        out["cell_level"] = self._view(v.cell_level, nc, i32)
+        out["cell_prefix"] = self._view(v.cell_prefix, nc, torch.int64)
+        out["cell_pbegin"] = self._view(v.cell_pbegin, nc, i32)
+        out["cell_pcount"] = self._view(v.cell_pcount, nc, i32)
+        out["cell_child_begin"] = self._view(v.cell_child_begin, nc, i32)
+        out["cell_nchild"] = self._view(v.cell_nchild, nc, i32)
+        out["cell_parent"] = self._view(v.cell_parent, nc, i32)
+        out["cell_mom64"] = self._view(v.cell_mom64, nc * 10, torch.float64, (nc, 10))
+        out["cell_box"] = self._view(v.cell_box, nc * 6, f32, (nc, 6))
+        out["cell_mom32"] = self._view(v.cell_mom32, nc * 10, f32, (nc, 10))
+        out["cell_r2open"] = self._view(v.cell_r2open, nc, f32)
+        out["group_begin"] = self._view(v.group_begin, ng + 1, i32)
+        out["group_cell"] = self._view(v.group_cell, ng, i32)
+        out["group_npc"] = self._view(v.group_npc, ng, i32)
+        out["group_npp"] = self._view(v.group_npp, ng, i32)
+        return out

@@ -1,0 +1,332 @@
+// api.cu -- the C ABI of include/bh.h: argument checking, workspace carving, stage sequencing.
+// No kernel arithmetic lives here; every step of the path is a kernel in the sibling translation units.
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "bh_internal.cuh"
+
+namespace bh {
+
+struct Carver {
+    unsigned char* base;
+    size_t off;
+    template <typename T>
+    T* take(size_t count) {
+        off = (off + 255) & ~(size_t)255;
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += count * sizeof(T);
+        return p;
+    }
+};
+
+struct Geometry {
+    int64_t n_max, max_cells, sort_tiles, tree_tiles, scan_sum_cap;
+    int32_t nleaf, ncrit;
+};
+
+static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
+    if (n_max < 1 || n_max > (int64_t)1 << 30) return false;
+    g->n_max = n_max;
+    g->nleaf = (cfg && cfg->nleaf) ? cfg->nleaf : 16;
+    g->ncrit = (cfg && cfg->ncrit) ? cfg->ncrit : 64;
+    if (g->nleaf < 1 || g->nleaf > kHaloMax || g->ncrit < 1 || g->ncrit > 64) return false;
+    const int64_t bound = n_max + kMaxLevel * (n_max / (g->nleaf + 1)) + 1;
+    g->max_cells = (cfg && cfg->max_cells > 0) ? cfg->max_cells : bound;
+    if (g->max_cells > bound) g->max_cells = bound;
+    if (g->max_cells < 1 || g->max_cells > ((int64_t)1 << 31) - 2) return false;
+    g->sort_tiles = div_up(n_max, kSortTile);
+    g->tree_tiles = div_up(n_max + 1, kTreeTile);
+    const int64_t biggest_scan = std::max<int64_t>(std::max<int64_t>((int64_t)kRadix * g->sort_tiles, (int64_t)kLevels * g->tree_tiles), n_max);
+    g->scan_sum_cap = div_up(biggest_scan, kScanTile) + 1;
+    return true;
+}
+
+static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
+    Carver c{base, 0};
+    Ws tmp;
+    Ws& o = w ? *w : tmp;
+    const size_t n = (size_t)g.n_max, C = (size_t)g.max_cells;
+    o.sc = c.take<DevScalars>(1);
+    for (int k = 0; k < 2; ++k) { o.pos[k] = c.take<float4>(n); o.vel[k] = c.take<float4>(n); o.idb[k] = c.take<uint32_t>(n); }
+    o.acc = c.take<float4>(n);
+    for (int k = 0; k < 2; ++k) { o.key[k] = c.take<uint64_t>(n); o.val[k] = c.take<uint32_t>(n); }
+    o.fl = c.take<uint8_t>(n + 1);
+    o.dep = c.take<uint8_t>(n);
+    o.gflag = c.take<uint8_t>(n);
+    o.gcell_at = c.take<uint32_t>(n);
+    o.gscan = c.take<uint32_t>(n);
+    o.g_begin = c.take<uint32_t>(n + 1);
+    o.g_cell = c.take<uint32_t>(n);
+    o.g_npc = c.take<uint32_t>(n);
+    o.g_npp = c.take<uint32_t>(n);
+    o.hist = c.take<uint32_t>((size_t)kRadix * g.sort_tiles);
+    o.hist_scan = c.take<uint32_t>((size_t)kRadix * g.sort_tiles);
+    o.scan_sums = c.take<uint32_t>((size_t)g.scan_sum_cap);
+    o.tile_cnt = c.take<uint32_t>((size_t)kLevels * g.tree_tiles);
+    o.tile_base = c.take<uint32_t>((size_t)kLevels * g.tree_tiles);
+    o.c_pbegin = c.take<uint32_t>(C);
+    o.c_pend = c.take<uint32_t>(C);
+    o.c_cbegin = c.take<uint32_t>(C);
+    o.c_cend = c.take<uint32_t>(C);
+    o.c_parent = c.take<uint32_t>(C);
+    o.mom64 = c.take<double>(10 * C);
+    o.box = c.take<float>(6 * C);
+    o.rec = c.take<float4>(4 * C);
+    o.e_level = c.take<int32_t>(C);
+    o.e_prefix = c.take<uint64_t>(C);
+    o.e_pcount = c.take<uint32_t>(C);
+    o.e_cbegin = c.take<int32_t>(C);
+    o.e_nchild = c.take<int32_t>(C);
+    o.e_parent = c.take<int32_t>(C);
+    o.e_mom32 = c.take<float>(10 * C);
+    o.e_r2open = c.take<float>(C);
+    return (c.off + 255) & ~(size_t)255;
+}
+
+}  // namespace bh
+
+using namespace bh;
+
+extern "C" {
+
+size_t bh_workspace_bytes(int64_t n_max, const bh_config* cfg) {
+    Geometry g;
+    if (!make_geometry(n_max, cfg, &g)) return 0;
+    return carve(g, nullptr, nullptr);
+}
+
+int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspace, size_t bytes) {
+    if (!out || !d_workspace) return BH_ERR_INVALID_ARG;
+    *out = nullptr;
+    Geometry g;
+    if (!make_geometry(n_max, cfg, &g)) return BH_ERR_INVALID_ARG;
+    if (((uintptr_t)d_workspace & 255) != 0) return BH_ERR_WORKSPACE;
+    if (carve(g, nullptr, nullptr) > bytes) return BH_ERR_WORKSPACE;
+    cudaPointerAttributes attr;
+    if (cudaPointerGetAttributes(&attr, d_workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+        (void)cudaGetLastError();
+        return BH_ERR_WORKSPACE;
+    }
+    bh_ctx* c = new (std::nothrow) bh_ctx();
+    if (!c) return BH_ERR_INVALID_ARG;
+    std::memset(c, 0, sizeof(*c));
+    c->device = attr.device;
+    c->n_max = n_max;
+    c->max_cells = g.max_cells;
+    c->nleaf = g.nleaf;
+    c->ncrit = g.ncrit;
+    c->sort_tiles = g.sort_tiles;
+    c->tree_tiles = g.tree_tiles;
+    c->scan_sum_cap = g.scan_sum_cap;
+    carve(g, static_cast<unsigned char*>(d_workspace), &c->ws);
+    int rc = BH_OK;
+    do {
+        if (cudaSetDevice(c->device) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
+        int sms = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
+        c->sm_count = sms;
+        if (walk_init(c) != BH_OK) { rc = BH_ERR_CUDA; break; }
+        for (int k = 0; k < 11; ++k)
+            if (cudaEventCreate(&c->ev[k]) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
+    } while (0);
+    if (rc != BH_OK) { delete c; return rc; }
+    *out = c;
+    return BH_OK;
+}
+
+int bh_destroy(bh_ctx* c) {
+    if (!c) return BH_ERR_INVALID_ARG;
+    cudaSetDevice(c->device);
+    for (int k = 0; k < 11; ++k)
+        if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+    delete c;
+    return BH_OK;
+}
+
+int bh_set_particles(bh_ctx* c, int64_t n, const float* pos_mass, const float* vel, const uint32_t* id, void* stream) {
+    if (!c || !pos_mass || n < 1 || n > c->n_max) return BH_ERR_INVALID_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    c->n = n;
+    c->cur = 0;
+    c->have_particles = c->have_tree = c->have_forces = false;
+    BH_CUDA(c, cudaMemcpyAsync(c->ws.pos[0], pos_mass, sizeof(float4) * (size_t)n, cudaMemcpyDefault, s));
+    if (vel) BH_CUDA(c, cudaMemcpyAsync(c->ws.vel[0], vel, sizeof(float4) * (size_t)n, cudaMemcpyDefault, s));
+    else BH_CUDA(c, cudaMemsetAsync(c->ws.vel[0], 0, sizeof(float4) * (size_t)n, s));
+    if (id) BH_CUDA(c, cudaMemcpyAsync(c->ws.idb[0], id, sizeof(uint32_t) * (size_t)n, cudaMemcpyDefault, s));
+    else { int rc = stage_iota(c, c->ws.idb[0], n, s); if (rc != BH_OK) return rc; }
+    BH_CUDA(c, cudaMemsetAsync(c->ws.acc, 0, sizeof(float4) * (size_t)n, s));
+    c->have_particles = true;
+    return BH_OK;
+}
+
+int bh_get_particles(bh_ctx* c, float* pos_mass, float* vel, float* acc_pot, uint32_t* id, void* stream) {
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->have_particles) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    const size_t n = (size_t)c->n;
+    if (pos_mass) BH_CUDA(c, cudaMemcpyAsync(pos_mass, c->ws.pos[c->cur], sizeof(float4) * n, cudaMemcpyDefault, s));
+    if (vel) BH_CUDA(c, cudaMemcpyAsync(vel, c->ws.vel[c->cur], sizeof(float4) * n, cudaMemcpyDefault, s));
+    if (acc_pot) BH_CUDA(c, cudaMemcpyAsync(acc_pot, c->ws.acc, sizeof(float4) * n, cudaMemcpyDefault, s));
+    if (id) BH_CUDA(c, cudaMemcpyAsync(id, c->ws.idb[c->cur], sizeof(uint32_t) * n, cudaMemcpyDefault, s));
+    return BH_OK;
+}
+
+int bh_tree_build(bh_ctx* c, void* stream) {
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->have_particles) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    c->have_tree = c->have_forces = false;
+    int rc;
+    if (c->timing) cudaEventRecord(c->ev[0], s);
+    if ((rc = stage_bbox_keys(c, s)) != BH_OK) return rc;      // records ev[1] between bbox and keys
+    if (c->timing) cudaEventRecord(c->ev[2], s);
+    if ((rc = stage_sort(c, s)) != BH_OK) return rc;
+    if (c->timing) cudaEventRecord(c->ev[3], s);
+    if ((rc = stage_reorder(c, s)) != BH_OK) return rc;
+    if (c->timing) cudaEventRecord(c->ev[4], s);
+    if ((rc = stage_cells(c, s)) != BH_OK) return rc;
+    if (c->timing) cudaEventRecord(c->ev[5], s);
+    if ((rc = stage_groups(c, s)) != BH_OK) return rc;
+    if (c->timing) cudaEventRecord(c->ev[6], s);
+    if ((rc = stage_moments(c, s)) != BH_OK) return rc;
+    if (c->timing) cudaEventRecord(c->ev[7], s);
+    c->have_tree = true;
+    return BH_OK;
+}
+
+int bh_compute_forces(bh_ctx* c, float theta, float eps, void* stream) {
+    if (!c || !(theta > 0.0f) || !std::isfinite(theta) || !(eps >= 0.0f) || !std::isfinite(eps)) return BH_ERR_INVALID_ARG;
+    if (!c->have_tree) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    int rc = stage_walk(c, theta, eps, s);      // records ev[8] (before the records), ev[9], ev[10] (around k_walk)
+    if (rc != BH_OK) return rc;
+    c->theta_last = theta;
+    c->have_forces = true;
+    return BH_OK;
+}
+
+int bh_leapfrog_step(bh_ctx* c, float theta, float eps, float dt, void* stream) {
+    if (!c || !std::isfinite(dt) || !(theta > 0.0f) || !std::isfinite(theta) || !(eps >= 0.0f) || !std::isfinite(eps))
+        return BH_ERR_INVALID_ARG;
+    if (!c->have_forces) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    const float h = 0.5f * dt;
+    int rc;
+    if ((rc = stage_kick_drift(c, h, dt, s)) != BH_OK) return rc;
+    if ((rc = bh_tree_build(c, stream)) != BH_OK) return rc;
+    if ((rc = bh_compute_forces(c, theta, eps, stream)) != BH_OK) return rc;
+    if ((rc = stage_kick(c, h, s)) != BH_OK) return rc;
+    return BH_OK;
+}
+
+int bh_kick_drift(bh_ctx* c, float dt_kick, float dt_drift, void* stream) {
+    if (!c || !std::isfinite(dt_kick) || !std::isfinite(dt_drift)) return BH_ERR_INVALID_ARG;
+    if (!c->have_forces) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    int rc = stage_kick_drift(c, dt_kick, dt_drift, s);
+    if (rc != BH_OK) return rc;
+    c->have_tree = c->have_forces = false;
+    return BH_OK;
+}
+
+int bh_sync_status(bh_ctx* c, void* stream, bh_stats* out) {
+    if (!c) return BH_ERR_INVALID_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    DevScalars h;
+    BH_CUDA(c, cudaMemcpyAsync(&h, c->ws.sc, sizeof(h), cudaMemcpyDeviceToHost, s));
+    BH_CUDA(c, cudaStreamSynchronize(s));
+    if (out) {
+        std::memset(out, 0, sizeof(*out));
+        out->status = c->have_tree ? h.status : BH_OK;
+        out->n = c->n;
+        out->launches = c->launches;
+        if (c->have_tree) {
+            out->n_levels = (int32_t)h.n_levels;
+            out->n_cells = h.n_cells;
+            out->n_groups = h.n_groups;
+            for (int k = 0; k < 3; ++k) { out->lo[k] = h.lo[k]; out->hi[k] = h.hi[k]; }
+            out->domain_exp = h.dom_e;
+        }
+        if (c->have_forces || c->theta_last > 0.0f) {
+            out->sum_pc = (int64_t)h.sum_pc;
+            out->sum_pp = (int64_t)h.sum_pp;
+            out->sum_mac = (int64_t)h.sum_mac;
+        }
+    }
+    return c->have_tree ? h.status : BH_OK;
+}
+
+int bh_export_tree(bh_ctx* c, bh_tree_view* v, void* stream) {
+    if (!c || !v) return BH_ERR_INVALID_ARG;
+    if (!c->have_tree) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    int rc = stage_export(c, s);
+    if (rc != BH_OK) return rc;
+    const Ws& w = c->ws;
+    v->pos_mass = reinterpret_cast<const float*>(w.pos[c->cur]);
+    v->vel = reinterpret_cast<const float*>(w.vel[c->cur]);
+    v->acc_pot = reinterpret_cast<const float*>(w.acc);
+    v->id = w.idb[c->cur];
+    v->key = w.key[c->sorted];
+    v->perm = w.val[c->sorted];
+    v->level_offset = c->ws.sc->level_offset;
+    v->cell_level = w.e_level;
+    v->cell_prefix = w.e_prefix;
+    v->cell_pbegin = w.c_pbegin;
+    v->cell_pcount = w.e_pcount;
+    v->cell_child_begin = w.e_cbegin;
+    v->cell_nchild = w.e_nchild;
+    v->cell_parent = w.e_parent;
+    v->cell_mom64 = w.mom64;
+    v->cell_box = w.box;
+    v->cell_mom32 = w.e_mom32;
+    v->cell_r2open = w.e_r2open;
+    v->group_begin = w.g_begin;
+    v->group_cell = w.g_cell;
+    v->group_npc = w.g_npc;
+    v->group_npp = w.g_npp;
+    return BH_OK;
+}
+
+int bh_set_stage_timing(bh_ctx* c, int enable) {
+    if (!c) return BH_ERR_INVALID_ARG;
+    c->timing = enable != 0;
+    return BH_OK;
+}
+
+int bh_get_stage_ms(bh_ctx* c, float ms[9]) {
+    if (!c || !ms) return BH_ERR_INVALID_ARG;
+    if (!c->timing || !c->have_forces) return BH_ERR_STATE;
+    BH_CUDA(c, cudaSetDevice(c->device));
+    BH_CUDA(c, cudaEventSynchronize(c->ev[10]));
+    for (int k = 0; k < 7; ++k) BH_CUDA(c, cudaEventElapsedTime(&ms[k], c->ev[k], c->ev[k + 1]));
+    BH_CUDA(c, cudaEventElapsedTime(&ms[7], c->ev[8], c->ev[9]));
+    BH_CUDA(c, cudaEventElapsedTime(&ms[8], c->ev[9], c->ev[10]));
+    return BH_OK;
+}
+
+int bh_last_cuda_error(const bh_ctx* c) { return c ? c->last_cuda : 0; }
+
+const char* bh_status_string(int status) {
+    switch (status) {
+        case BH_OK: return "ok";
+        case BH_ERR_INVALID_ARG: return "invalid argument";
+        case BH_ERR_WORKSPACE: return "workspace too small, misaligned or not device memory";
+        case BH_ERR_STATE: return "call out of order (particles -> tree_build -> compute_forces -> leapfrog_step)";
+        case BH_ERR_CUDA: return "CUDA runtime error";
+        case BH_ERR_NONFINITE: return "non-finite position or mass <= 0 in the input";
+        case BH_ERR_CAPACITY: return "tree needs more cells than max_cells";
+        default: return "unknown status";
+    }
+}
+
+}  // extern "C"

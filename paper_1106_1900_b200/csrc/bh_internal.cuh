@@ -1,0 +1,158 @@
+// bh_internal.cuh -- shared declarations of the CUDA library (not part of the C ABI).
+// Product code: never includes or links anything under oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/bh.h"
+
+namespace bh {
+
+constexpr int kMaxLevel = 20;
+constexpr int kKeyBits = 20;           // per axis
+constexpr int kLevels = kMaxLevel + 1; // levels 0..20
+constexpr uint32_t kNone = 0xFFFFFFFFu;
+
+// ---- sort geometry (S2)
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kSortPasses = 8;                 // 8 x 8 bits covers the 60-bit key
+constexpr int kSortThreads = 256;
+constexpr int kSortItemsPerThread = 16;
+constexpr int kSortTile = kSortThreads * kSortItemsPerThread;   // 4096 keys per block
+
+// ---- scan geometry
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 8;
+constexpr int kScanTile = kScanThreads * kScanItems;            // 2048 entries per block
+
+// ---- tree geometry (S4): one boundary per thread
+constexpr int kTreeTile = 256;
+constexpr int kHaloMax = 64;           // nleaf <= 64
+
+// Device-resident scalars (one struct, copied to the host by bh_sync_status).
+struct DevScalars {
+    uint32_t bb_min[3];      // order-preserving encodings of the per-axis minima / maxima (S0)
+    uint32_t bb_max[3];
+    int32_t status;          // deferred bh_status
+    int32_t dom_e;           // cube side = 2^dom_e
+    float lo[3];
+    float hi[3];
+    uint32_t level_offset[kLevels + 1];
+    uint32_t n_cells;
+    uint32_t n_groups;
+    uint32_t n_levels;
+    uint32_t walk_next;      // dynamic group counter of the walk
+    unsigned long long sum_pc;
+    unsigned long long sum_pp;
+    unsigned long long sum_mac;
+};
+
+// Pointers into the caller's workspace.
+struct Ws {
+    DevScalars* sc;
+    float4* pos[2];
+    float4* vel[2];
+    uint32_t* idb[2];
+    float4* acc;
+    uint64_t* key[2];
+    uint32_t* val[2];
+    uint8_t* fl;          // [n+1] first level at which boundary i starts a new run (0..21)
+    uint8_t* dep;         // [n]   level of the leaf holding particle i
+    uint8_t* gflag;       // [n]   1 where a group starts
+    uint32_t* gcell_at;   // [n]   cell of the group starting here
+    uint32_t* gscan;      // [n]   exclusive scan of gflag
+    uint32_t* g_begin;    // [n+1]
+    uint32_t* g_cell;     // [n]
+    uint32_t* g_npc;      // [n]
+    uint32_t* g_npp;      // [n]
+    uint32_t* hist;       // [kRadix * sortTiles]
+    uint32_t* hist_scan;  // same
+    uint32_t* scan_sums;  // partial sums of the generic scan
+    uint32_t* tile_cnt;   // [kLevels * treeTiles]
+    uint32_t* tile_base;  // same
+    uint32_t* c_pbegin;   // [max_cells]
+    uint32_t* c_pend;
+    uint32_t* c_cbegin;   // first child (0 for a leaf)
+    uint32_t* c_cend;     // one past the last child (0 for a leaf)
+    uint32_t* c_parent;
+    double* mom64;        // [max_cells][10]
+    float* box;           // [max_cells][6]
+    float4* rec;          // [max_cells][4] walk record: (com, r2open) (M, Qxx, Qyy, Qzz) (Qxy, Qxz, Qyz, 0) (first, count, leaf, 0)
+    // export (canonical arrays of bh_tree_view)
+    int32_t* e_level;
+    uint64_t* e_prefix;
+    uint32_t* e_pcount;
+    int32_t* e_cbegin;
+    int32_t* e_nchild;
+    int32_t* e_parent;
+    float* e_mom32;
+    float* e_r2open;
+};
+
+}  // namespace bh
+
+struct bh_ctx {
+    int device;
+    int sm_count;
+    int64_t n_max;
+    int64_t n;
+    int64_t max_cells;
+    int32_t nleaf, ncrit;
+    int cur;               // which of pos[2]/vel[2]/idb[2] holds the live state
+    int sorted;            // which of key[2]/val[2] holds the sorted keys / perm
+    bool have_particles, have_tree, have_forces;
+    int64_t launches;
+    int last_cuda;
+    float theta_last;
+    bh::Ws ws;
+    int64_t sort_tiles, tree_tiles, scan_sum_cap;
+    bool timing;
+    cudaEvent_t ev[11];
+};
+
+namespace bh {
+
+#define BH_CUDA(ctx, call)                                   \
+    do {                                                     \
+        cudaError_t _e = (call);                             \
+        if (_e != cudaSuccess) {                             \
+            (ctx)->last_cuda = (int)_e;                      \
+            return BH_ERR_CUDA;                              \
+        }                                                    \
+    } while (0)
+
+#define BH_LAUNCH(ctx, kernel, grid, block, smem, stream, ...)              \
+    do {                                                                    \
+        kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);         \
+        (ctx)->launches += 1;                                               \
+        cudaError_t _e = cudaPeekAtLastError();                             \
+        if (_e != cudaSuccess) {                                            \
+            (ctx)->last_cuda = (int)_e;                                     \
+            return BH_ERR_CUDA;                                             \
+        }                                                                   \
+    } while (0)
+
+static inline int64_t div_up(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// stage entry points (each only enqueues kernels on `s`)
+int stage_bbox_keys(bh_ctx* c, cudaStream_t s);       // S0, S1
+int stage_sort(bh_ctx* c, cudaStream_t s);            // S2
+int stage_reorder(bh_ctx* c, cudaStream_t s);         // S3
+int stage_cells(bh_ctx* c, cudaStream_t s);           // S4
+int stage_groups(bh_ctx* c, cudaStream_t s);          // S5
+int stage_moments(bh_ctx* c, cudaStream_t s);         // S6
+int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s);          // S6: fp32 walk record + r2open(theta)
+int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s);   // S7, S8
+int walk_init(bh_ctx* c);
+int stage_kick_drift(bh_ctx* c, float h, float dt, cudaStream_t s);  // S9
+int stage_kick(bh_ctx* c, float h, cudaStream_t s);                  // S9
+int stage_export(bh_ctx* c, cudaStream_t s);
+int stage_iota(bh_ctx* c, uint32_t* dst, int64_t n, cudaStream_t s);
+
+// generic exclusive scan (three kernels, no spinning): out[i] = sum_{j<i} in[j]; *total (device) = sum of all
+int scan_u32(bh_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, uint32_t* d_total, cudaStream_t s);
+int scan_u8(bh_ctx* c, const uint8_t* in, uint32_t* out, int64_t n, uint32_t* d_total, cudaStream_t s);
+
+}  // namespace bh

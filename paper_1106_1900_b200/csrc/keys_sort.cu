@@ -1,0 +1,339 @@
+// keys_sort.cu -- S0 domain box, S1 Morton keys, S2 stable LSD radix sort, S3 reorder, generic scan.
+// PAPER.md:374-392 (Appendix B: keys), PAPER.md:350-370 (Appendix A: scan, split, radix sort), PAPER.md:174 ("moving").
+#include <algorithm>
+#include "bh_internal.cuh"
+
+namespace bh {
+
+// ------------------------------------------------------------------------------------------ S0
+__device__ __forceinline__ uint32_t f2ord(float f) {
+    uint32_t u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float ord2f(uint32_t u) {
+    return __uint_as_float((u & 0x80000000u) ? (u & 0x7FFFFFFFu) : ~u);
+}
+
+__global__ void k_reset_build(DevScalars* sc) {
+    const int t = threadIdx.x;
+    if (t < 3) { sc->bb_min[t] = 0xFFFFFFFFu; sc->bb_max[t] = 0u; }
+    if (t == 0) { sc->status = BH_OK; sc->n_cells = 0; sc->n_groups = 0; sc->n_levels = 0; }
+}
+
+// Per-axis min / max (exact) and input validation (A27: finite positions, finite mass > 0).
+__global__ void __launch_bounds__(256) k_bbox(const float4* __restrict__ pos, int n, DevScalars* sc) {
+    float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
+    int bad = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const float4 p = pos[i];
+        bad |= !(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(p.w) && p.w > 0.0f);
+        mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
+        mn[1] = fminf(mn[1], p.y); mx[1] = fmaxf(mx[1], p.y);
+        mn[2] = fminf(mn[2], p.z); mx[2] = fmaxf(mx[2], p.z);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            mn[k] = fminf(mn[k], __shfl_xor_sync(0xFFFFFFFFu, mn[k], o));
+            mx[k] = fmaxf(mx[k], __shfl_xor_sync(0xFFFFFFFFu, mx[k], o));
+        }
+        bad |= __shfl_xor_sync(0xFFFFFFFFu, bad, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            atomicMin(&sc->bb_min[k], f2ord(mn[k]));
+            atomicMax(&sc->bb_max[k], f2ord(mx[k]));
+        }
+        if (bad) atomicMin(&sc->status, (int)BH_ERR_NONFINITE);
+    }
+}
+
+// Cube side 2^e with frexpf(ext) = (mu, e): the smallest power of two strictly above the extent (O1).
+__global__ void k_domain(DevScalars* sc) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    float ext = 0.0f;
+    for (int k = 0; k < 3; ++k) {
+        const float lo = ord2f(sc->bb_min[k]), hi = ord2f(sc->bb_max[k]);
+        sc->lo[k] = lo;
+        sc->hi[k] = hi;
+        ext = fmaxf(ext, __fsub_rn(hi, lo));
+    }
+    if (!isfinite(ext)) { atomicMin(&sc->status, (int)BH_ERR_NONFINITE); ext = 1.0f; }
+    if (ext == 0.0f) ext = 1.0f;
+    int e = 0;
+    (void)frexpf(ext, &e);
+    sc->dom_e = e;
+}
+
+// ------------------------------------------------------------------------------------------ S1
+// 20-bit dilate: bit b -> bit 3b (64-bit shift-and-mask form; the paper's List 1 is the 10-bit version).
+__device__ __forceinline__ uint64_t dilate20(uint32_t v) {
+    uint64_t x = v & 0xFFFFFu;
+    x = (x | (x << 32)) & 0x001F00000000FFFFull;
+    x = (x | (x << 16)) & 0x001F0000FF0000FFull;
+    x = (x | (x << 8)) & 0x100F00F00F00F00Full;
+    x = (x | (x << 4)) & 0x10C30C30C30C30C3ull;
+    x = (x | (x << 2)) & 0x1249249249249249ull;
+    return x;
+}
+
+__device__ __forceinline__ uint32_t grid_coord(float x, float lo, int sh) {
+    const float d = __fsub_rn(x, lo);              // the only rounding
+    const float s = ldexpf(d, sh);                 // exact power-of-two scaling
+    const float t = truncf(s);
+    uint32_t v = (t > 0.0f) ? (uint32_t)t : 0u;
+    return min(v, (1u << kKeyBits) - 1u);
+}
+
+__global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pos, int n, const DevScalars* __restrict__ sc,
+                                              uint64_t* __restrict__ key, uint32_t* __restrict__ val) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float lox = sc->lo[0], loy = sc->lo[1], loz = sc->lo[2];
+    const int sh = kKeyBits - sc->dom_e;
+    const float4 p = pos[i];
+    const uint32_t ix = grid_coord(p.x, lox, sh), iy = grid_coord(p.y, loy, sh), iz = grid_coord(p.z, loz, sh);
+    key[i] = (dilate20(ix) << 2) | (dilate20(iy) << 1) | dilate20(iz);   // x most significant in a triple (A4)
+    val[i] = (uint32_t)i;
+}
+
+__global__ void k_iota(uint32_t* dst, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = (uint32_t)i;
+}
+
+// ------------------------------------------------------------------------------------------ generic scan
+// Three kernels, no inter-block waiting: (A) per-tile sums, (B) one block scans the sums, (C) per-tile scan + offset.
+template <typename T>
+__device__ __forceinline__ uint32_t load_as_u32(const T* p, int64_t i) { return (uint32_t)p[i]; }
+
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total) {
+    // 256 threads; returns the exclusive prefix of v over the block
+    __shared__ uint32_t wsum[8];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    uint32_t base = 0, tot = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const uint32_t s = wsum[k];
+        if (k < w) base += s;
+        tot += s;
+    }
+    __syncthreads();
+    *total = tot;
+    return base + inc - v;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const T* __restrict__ in, int64_t n, uint32_t* __restrict__ sums) {
+    const int64_t base = (int64_t)blockIdx.x * kScanTile;
+    uint32_t s = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        const int64_t i = base + k * kScanThreads + threadIdx.x;
+        if (i < n) s += load_as_u32(in, i);
+    }
+    uint32_t tot;
+    (void)block_exclusive_scan(s, &tot);
+    if (threadIdx.x == 0) sums[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_sums(uint32_t* sums, int64_t m, uint32_t* d_total) {
+    // exclusive scan of sums[0..m) in place by one block; chunks of 256 with a running carry
+    uint32_t carry = 0;
+    for (int64_t b = 0; b < m; b += kScanThreads) {
+        const int64_t i = b + threadIdx.x;
+        const uint32_t v = (i < m) ? sums[i] : 0u;
+        uint32_t tot;
+        const uint32_t ex = block_exclusive_scan(v, &tot);
+        if (i < m) sums[i] = carry + ex;
+        carry += tot;
+    }
+    if (threadIdx.x == 0 && d_total) *d_total = carry;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kScanThreads) k_scan_apply(const T* __restrict__ in, int64_t n, const uint32_t* __restrict__ sums,
+                                                             uint32_t* __restrict__ out) {
+    // thread t owns kScanItems CONSECUTIVE entries, so the block scan of per-thread sums gives the order
+    const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
+    uint32_t v[kScanItems];
+    uint32_t s = 0;
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        const int64_t i = base + k;
+        v[k] = (i < n) ? load_as_u32(in, i) : 0u;
+        s += v[k];
+    }
+    uint32_t tot;
+    uint32_t ex = block_exclusive_scan(s, &tot) + sums[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < kScanItems; ++k) {
+        const int64_t i = base + k;
+        if (i < n) out[i] = ex;
+        ex += v[k];
+    }
+}
+
+template <typename T>
+static int scan_impl(bh_ctx* c, const T* in, uint32_t* out, int64_t n, uint32_t* d_total, cudaStream_t s) {
+    const int64_t tiles = div_up(n, kScanTile);
+    if (tiles > c->scan_sum_cap) return BH_ERR_WORKSPACE;
+    BH_LAUNCH(c, k_scan_reduce<T>, (unsigned)tiles, kScanThreads, 0, s, in, n, c->ws.scan_sums);
+    BH_LAUNCH(c, k_scan_sums, 1, kScanThreads, 0, s, c->ws.scan_sums, tiles, d_total);
+    BH_LAUNCH(c, k_scan_apply<T>, (unsigned)tiles, kScanThreads, 0, s, in, n, c->ws.scan_sums, out);
+    return BH_OK;
+}
+int scan_u32(bh_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, uint32_t* d_total, cudaStream_t s) {
+    return scan_impl<uint32_t>(c, in, out, n, d_total, s);
+}
+int scan_u8(bh_ctx* c, const uint8_t* in, uint32_t* out, int64_t n, uint32_t* d_total, cudaStream_t s) {
+    return scan_impl<uint8_t>(c, in, out, n, d_total, s);
+}
+
+// ------------------------------------------------------------------------------------------ S2
+// LSD radix sort, 8 bits per pass (the paper's 1-bit split generalised: PAPER.md:352, 362).
+// Per pass: per-tile digit histogram -> exclusive scan of the digit-major table -> stable scatter.
+__global__ void __launch_bounds__(kSortThreads) k_radix_hist(const uint64_t* __restrict__ key, int n, int shift, int tiles,
+                                                             uint32_t* __restrict__ hist) {
+    __shared__ uint32_t h[kRadix];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    const int base = blockIdx.x * kSortTile;
+#pragma unroll 4
+    for (int k = 0; k < kSortItemsPerThread; ++k) {
+        const int i = base + k * kSortThreads + threadIdx.x;
+        if (i < n) atomicAdd(&h[(uint32_t)(key[i] >> shift) & (kRadix - 1)], 1u);
+    }
+    __syncthreads();
+    hist[(size_t)threadIdx.x * tiles + blockIdx.x] = h[threadIdx.x];
+}
+
+// Stable scatter.  Warp w of the block owns the contiguous sub-tile [w*512, (w+1)*512): order = (warp, iteration, lane).
+__global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint64_t* __restrict__ key_in, const uint32_t* __restrict__ val_in,
+                                                                int n, int shift, int tiles, const uint32_t* __restrict__ hist_scan,
+                                                                uint64_t* __restrict__ key_out, uint32_t* __restrict__ val_out) {
+    constexpr int kWarps = kSortThreads / 32;
+    constexpr int kIters = kSortTile / kWarps / 32;   // 16
+    __shared__ uint32_t wcnt[kWarps][kRadix];
+    __shared__ uint32_t gbase[kRadix];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int j = threadIdx.x; j < kWarps * kRadix; j += kSortThreads) (&wcnt[0][0])[j] = 0;
+    gbase[threadIdx.x] = hist_scan[(size_t)threadIdx.x * tiles + blockIdx.x];
+    __syncthreads();
+
+    const int wbase = blockIdx.x * kSortTile + w * (kIters * 32);
+    const uint32_t lt = (1u << lane) - 1u;
+    uint64_t k[kIters];
+    uint32_t v[kIters];
+    uint32_t rank[kIters];
+#pragma unroll
+    for (int it = 0; it < kIters; ++it) {
+        const int i = wbase + it * 32 + lane;
+        const bool ok = i < n;
+        k[it] = ok ? key_in[i] : 0ull;
+        v[it] = ok ? val_in[i] : 0u;
+    }
+#pragma unroll
+    for (int it = 0; it < kIters; ++it) {
+        const int i = wbase + it * 32 + lane;
+        const bool ok = i < n;
+        const uint32_t d = (uint32_t)(k[it] >> shift) & (kRadix - 1);
+        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, ok ? d : 0xFFFFFFFFu);
+        const uint32_t before = __popc(peers & lt);
+        uint32_t old = 0;
+        if (ok) old = wcnt[w][d];
+        __syncwarp();
+        if (ok && before == 0) wcnt[w][d] = old + __popc(peers);
+        __syncwarp();
+        rank[it] = old + before;
+    }
+    __syncthreads();
+    {   // exclusive prefix over the warps for digit = threadIdx.x
+        uint32_t run = 0;
+#pragma unroll
+        for (int ww = 0; ww < kWarps; ++ww) {
+            const uint32_t t = wcnt[ww][threadIdx.x];
+            wcnt[ww][threadIdx.x] = run;
+            run += t;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < kIters; ++it) {
+        const int i = wbase + it * 32 + lane;
+        if (i < n) {
+            const uint32_t d = (uint32_t)(k[it] >> shift) & (kRadix - 1);
+            const uint32_t dst = gbase[d] + wcnt[w][d] + rank[it];
+            key_out[dst] = k[it];
+            val_out[dst] = v[it];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ S3
+__global__ void __launch_bounds__(256) k_reorder(const uint32_t* __restrict__ perm, int n,
+                                                 const float4* __restrict__ pos_in, const float4* __restrict__ vel_in,
+                                                 const uint32_t* __restrict__ id_in,
+                                                 float4* __restrict__ pos_out, float4* __restrict__ vel_out, uint32_t* __restrict__ id_out) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    const uint32_t src = perm[j];
+    pos_out[j] = pos_in[src];
+    vel_out[j] = vel_in[src];
+    id_out[j] = id_in[src];
+}
+
+// ------------------------------------------------------------------------------------------ host side
+int stage_iota(bh_ctx* c, uint32_t* dst, int64_t n, cudaStream_t s) {
+    BH_LAUNCH(c, k_iota, (unsigned)div_up(n, 256), 256, 0, s, dst, (int)n);
+    return BH_OK;
+}
+
+int stage_bbox_keys(bh_ctx* c, cudaStream_t s) {
+    const int n = (int)c->n;
+    BH_LAUNCH(c, k_reset_build, 1, 32, 0, s, c->ws.sc);
+    const int grid = (int)std::min<int64_t>(div_up(n, 256), (int64_t)c->sm_count * 8);
+    BH_LAUNCH(c, k_bbox, grid, 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc);
+    BH_LAUNCH(c, k_domain, 1, 32, 0, s, c->ws.sc);
+    if (c->timing) cudaEventRecord(c->ev[1], s);
+    BH_LAUNCH(c, k_keys, (unsigned)div_up(n, 256), 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc, c->ws.key[0], c->ws.val[0]);
+    return BH_OK;
+}
+
+int stage_sort(bh_ctx* c, cudaStream_t s) {
+    const int n = (int)c->n;
+    const int tiles = (int)div_up(n, kSortTile);
+    int src = 0;
+    for (int p = 0; p < kSortPasses; ++p) {
+        const int shift = p * kRadixBits;
+        BH_LAUNCH(c, k_radix_hist, tiles, kSortThreads, 0, s, c->ws.key[src], n, shift, tiles, c->ws.hist);
+        int rc = scan_u32(c, c->ws.hist, c->ws.hist_scan, (int64_t)kRadix * tiles, nullptr, s);
+        if (rc != BH_OK) return rc;
+        BH_LAUNCH(c, k_radix_scatter, tiles, kSortThreads, 0, s, c->ws.key[src], c->ws.val[src], n, shift, tiles,
+                  c->ws.hist_scan, c->ws.key[src ^ 1], c->ws.val[src ^ 1]);
+        src ^= 1;
+    }
+    c->sorted = src;
+    return BH_OK;
+}
+
+int stage_reorder(bh_ctx* c, cudaStream_t s) {
+    const int n = (int)c->n;
+    const int a = c->cur, b = c->cur ^ 1;
+    BH_LAUNCH(c, k_reorder, (unsigned)div_up(n, 256), 256, 0, s, c->ws.val[c->sorted], n, c->ws.pos[a], c->ws.vel[a],
+              c->ws.idb[a], c->ws.pos[b], c->ws.vel[b], c->ws.idb[b]);
+    c->cur = b;
+    return BH_OK;
+}
+
+}  // namespace bh

@@ -1,0 +1,171 @@
+// moments.cu -- S6: monopole + quadrupole moments and tight boxes, bottom-up, in binary64 with a fixed operation
+// order ("performed in double precision ... converted back to single precision"; Fig.4), then the
+// fp32 walk record with the opening radius of Eq.1.
+// Every fp64 operation is an explicit round-to-nearest intrinsic so that no multiply-add is ever fused: the fp32
+// roundings of these values feed the MAC, and a one-ulp difference would flip an opening decision somewhere.
+#include <algorithm>
+#include "bh_internal.cuh"
+
+namespace bh {
+
+struct Mom {
+    double M, S[3], com[3], Q[6];
+    float bmin[3], bmax[3];
+};
+
+__device__ __forceinline__ void mom_store(const Mom& m, double* __restrict__ mom64, float* __restrict__ box, uint32_t c) {
+    double* o = mom64 + 10 * (size_t)c;
+    o[0] = m.M; o[1] = m.com[0]; o[2] = m.com[1]; o[3] = m.com[2];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) o[4 + k] = m.Q[k];
+    float* b = box + 6 * (size_t)c;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { b[k] = m.bmin[k]; b[3 + k] = m.bmax[k]; }
+}
+
+// Leaves: M = sum m; S = sum m x; com = S / M; Q_jk = sum (m r_j) r_k, r = x - com; particles in ascending order.
+__global__ void __launch_bounds__(128) k_leaf_moments(const DevScalars* __restrict__ sc, const float4* __restrict__ pos,
+                                                      const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
+                                                      const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
+                                                      double* __restrict__ mom64, float* __restrict__ box) {
+    const uint32_t nc = sc->n_cells;
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
+        if (c_cend[c] != c_cbegin[c]) continue;   // node
+        const uint32_t b = c_pbegin[c], e = c_pend[c];
+        Mom m;
+        m.M = 0.0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { m.S[k] = 0.0; m.bmin[k] = INFINITY; m.bmax[k] = -INFINITY; }
+#pragma unroll
+        for (int k = 0; k < 6; ++k) m.Q[k] = 0.0;
+        for (uint32_t i = b; i < e; ++i) {
+            const float4 p = pos[i];
+            const double w = (double)p.w;
+            m.M = __dadd_rn(m.M, w);
+            m.S[0] = __dadd_rn(m.S[0], __dmul_rn(w, (double)p.x));
+            m.S[1] = __dadd_rn(m.S[1], __dmul_rn(w, (double)p.y));
+            m.S[2] = __dadd_rn(m.S[2], __dmul_rn(w, (double)p.z));
+            m.bmin[0] = fminf(m.bmin[0], p.x); m.bmax[0] = fmaxf(m.bmax[0], p.x);
+            m.bmin[1] = fminf(m.bmin[1], p.y); m.bmax[1] = fmaxf(m.bmax[1], p.y);
+            m.bmin[2] = fminf(m.bmin[2], p.z); m.bmax[2] = fmaxf(m.bmax[2], p.z);
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) m.com[k] = __ddiv_rn(m.S[k], m.M);
+        for (uint32_t i = b; i < e; ++i) {
+            const float4 p = pos[i];
+            const double w = (double)p.w;
+            const double rx = __dsub_rn((double)p.x, m.com[0]);
+            const double ry = __dsub_rn((double)p.y, m.com[1]);
+            const double rz = __dsub_rn((double)p.z, m.com[2]);
+            const double tx = __dmul_rn(w, rx), ty = __dmul_rn(w, ry), tz = __dmul_rn(w, rz);
+            m.Q[0] = __dadd_rn(m.Q[0], __dmul_rn(tx, rx));
+            m.Q[1] = __dadd_rn(m.Q[1], __dmul_rn(ty, ry));
+            m.Q[2] = __dadd_rn(m.Q[2], __dmul_rn(tz, rz));
+            m.Q[3] = __dadd_rn(m.Q[3], __dmul_rn(tx, ry));
+            m.Q[4] = __dadd_rn(m.Q[4], __dmul_rn(tx, rz));
+            m.Q[5] = __dadd_rn(m.Q[5], __dmul_rn(ty, rz));
+        }
+        mom_store(m, mom64, box, c);
+    }
+}
+
+// Nodes of one level: M = sum M_c; S = sum M_c com_c; com = S / M; Q_jk = sum_c ((Q + Q_c,jk) + (M_c d_j) d_k), d = com_c - com.
+__global__ void __launch_bounds__(128) k_node_moments(const DevScalars* __restrict__ sc, int level,
+                                                      const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
+                                                      double* __restrict__ mom64, float* __restrict__ box) {
+    const uint32_t lo = sc->level_offset[level], hi = sc->level_offset[level + 1];
+    for (uint32_t c = lo + blockIdx.x * blockDim.x + threadIdx.x; c < hi; c += gridDim.x * blockDim.x) {
+        const uint32_t cb = c_cbegin[c], ce = c_cend[c];
+        if (ce == cb) continue;   // leaf
+        Mom m;
+        m.M = 0.0;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { m.S[k] = 0.0; m.bmin[k] = INFINITY; m.bmax[k] = -INFINITY; }
+#pragma unroll
+        for (int k = 0; k < 6; ++k) m.Q[k] = 0.0;
+        for (uint32_t k2 = cb; k2 < ce; ++k2) {
+            const double* mc = mom64 + 10 * (size_t)k2;
+            const float* bc = box + 6 * (size_t)k2;
+            const double Mc = mc[0];
+            m.M = __dadd_rn(m.M, Mc);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                m.S[k] = __dadd_rn(m.S[k], __dmul_rn(Mc, mc[1 + k]));
+                m.bmin[k] = fminf(m.bmin[k], bc[k]);
+                m.bmax[k] = fmaxf(m.bmax[k], bc[3 + k]);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) m.com[k] = __ddiv_rn(m.S[k], m.M);
+        for (uint32_t k2 = cb; k2 < ce; ++k2) {
+            const double* mc = mom64 + 10 * (size_t)k2;
+            const double Mc = mc[0];
+            const double dx = __dsub_rn(mc[1], m.com[0]);
+            const double dy = __dsub_rn(mc[2], m.com[1]);
+            const double dz = __dsub_rn(mc[3], m.com[2]);
+            const double tx = __dmul_rn(Mc, dx), ty = __dmul_rn(Mc, dy), tz = __dmul_rn(Mc, dz);
+            m.Q[0] = __dadd_rn(__dadd_rn(m.Q[0], mc[4]), __dmul_rn(tx, dx));
+            m.Q[1] = __dadd_rn(__dadd_rn(m.Q[1], mc[5]), __dmul_rn(ty, dy));
+            m.Q[2] = __dadd_rn(__dadd_rn(m.Q[2], mc[6]), __dmul_rn(tz, dz));
+            m.Q[3] = __dadd_rn(__dadd_rn(m.Q[3], mc[7]), __dmul_rn(tx, dy));
+            m.Q[4] = __dadd_rn(__dadd_rn(m.Q[4], mc[8]), __dmul_rn(tx, dz));
+            m.Q[5] = __dadd_rn(__dadd_rn(m.Q[5], mc[9]), __dmul_rn(ty, dz));
+        }
+        mom_store(m, mom64, box, c);
+    }
+}
+
+// fp32 walk record (64 B per cell) with the opening radius of Eq.1:  l = longest side of the tight box (A14),
+// delta = |com - box centre|, r2open = (l / theta + delta)^2, all in single fp32 operations (O8).
+__global__ void __launch_bounds__(256) k_cell_record(const DevScalars* __restrict__ sc, float theta,
+                                                     const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
+                                                     const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
+                                                     const double* __restrict__ mom64, const float* __restrict__ box,
+                                                     float4* __restrict__ rec) {
+    const uint32_t nc = sc->n_cells;
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
+        const double* m = mom64 + 10 * (size_t)c;
+        const float* b = box + 6 * (size_t)c;
+        const float M = (float)m[0];
+        const float cx = (float)m[1], cy = (float)m[2], cz = (float)m[3];
+        float l = fmaxf(fmaxf(__fsub_rn(b[3], b[0]), __fsub_rn(b[4], b[1])), __fsub_rn(b[5], b[2]));
+        l = fmaxf(l, 0.0f);
+        const float ux = __fsub_rn(cx, __fmul_rn(0.5f, __fadd_rn(b[0], b[3])));
+        const float uy = __fsub_rn(cy, __fmul_rn(0.5f, __fadd_rn(b[1], b[4])));
+        const float uz = __fsub_rn(cz, __fmul_rn(0.5f, __fadd_rn(b[2], b[5])));
+        const float s2 = __fadd_rn(__fadd_rn(__fmul_rn(ux, ux), __fmul_rn(uy, uy)), __fmul_rn(uz, uz));
+        const float delta = __fsqrt_rn(s2);
+        const float ropen = __fadd_rn(__fdiv_rn(l, theta), delta);
+        const float r2open = __fmul_rn(ropen, ropen);
+        const uint32_t cb = c_cbegin[c], ce = c_cend[c];
+        const bool leaf = (ce == cb);
+        uint4 link;
+        link.x = leaf ? c_pbegin[c] : cb;
+        link.y = leaf ? (c_pend[c] - c_pbegin[c]) : (ce - cb);
+        link.z = leaf ? 1u : 0u;
+        link.w = 0u;
+        float4* r = rec + 4 * (size_t)c;
+        r[0] = make_float4(cx, cy, cz, r2open);
+        r[1] = make_float4(M, (float)m[4], (float)m[5], (float)m[6]);
+        r[2] = make_float4((float)m[7], (float)m[8], (float)m[9], 0.0f);
+        r[3] = make_float4(__uint_as_float(link.x), __uint_as_float(link.y), __uint_as_float(link.z), 0.0f);
+    }
+}
+
+int stage_moments(bh_ctx* c, cudaStream_t s) {
+    const int grid = (int)std::min<int64_t>(div_up(c->max_cells, 128), (int64_t)c->sm_count * 16);
+    BH_LAUNCH(c, k_leaf_moments, grid, 128, 0, s, c->ws.sc, c->ws.pos[c->cur], c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin,
+              c->ws.c_cend, c->ws.mom64, c->ws.box);
+    for (int L = kMaxLevel - 1; L >= 0; --L)
+        BH_LAUNCH(c, k_node_moments, grid, 128, 0, s, c->ws.sc, L, c->ws.c_cbegin, c->ws.c_cend, c->ws.mom64, c->ws.box);
+    return BH_OK;
+}
+
+int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s) {
+    const int grid = (int)std::min<int64_t>(div_up(c->max_cells, 256), (int64_t)c->sm_count * 16);
+    BH_LAUNCH(c, k_cell_record, grid, 256, 0, s, c->ws.sc, theta, c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin, c->ws.c_cend,
+              c->ws.mom64, c->ws.box, c->ws.rec);
+    return BH_OK;
+}
+
+}  // namespace bh
