@@ -40,13 +40,28 @@ __global__ void __launch_bounds__(256) k_bbox(const float4* __restrict__ pos, in
         }
         bad |= __shfl_xor_sync(0xFFFFFFFFu, bad, o);
     }
+    __shared__ float smn[8][3], smx[8][3];
+    __shared__ int sbad[8];
+    const int w = threadIdx.x >> 5;
     if ((threadIdx.x & 31) == 0) {
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            atomicMin(&sc->bb_min[k], f2ord(mn[k]));
-            atomicMax(&sc->bb_max[k], f2ord(mx[k]));
-        }
-        if (bad) atomicMin(&sc->status, (int)BH_ERR_NONFINITE);
+        for (int k = 0; k < 3; ++k) { smn[w][k] = mn[k]; smx[w][k] = mx[k]; }
+        sbad[w] = bad;
+    }
+    __syncthreads();
+    if (threadIdx.x < 3) {          // one atomic pair per axis per block
+        const int k = threadIdx.x;
+        float a = smn[0][k], b = smx[0][k];
+#pragma unroll
+        for (int ww = 1; ww < 8; ++ww) { a = fminf(a, smn[ww][k]); b = fmaxf(b, smx[ww][k]); }
+        atomicMin(&sc->bb_min[k], f2ord(a));
+        atomicMax(&sc->bb_max[k], f2ord(b));
+    }
+    if (threadIdx.x == 32) {
+        int any = 0;
+#pragma unroll
+        for (int ww = 0; ww < 8; ++ww) any |= sbad[ww];
+        if (any) atomicMin(&sc->status, (int)BH_ERR_NONFINITE);
     }
 }
 
@@ -302,7 +317,7 @@ int stage_iota(bh_ctx* c, uint32_t* dst, int64_t n, cudaStream_t s) {
 int stage_bbox_keys(bh_ctx* c, cudaStream_t s) {
     const int n = (int)c->n;
     BH_LAUNCH(c, k_reset_build, 1, 32, 0, s, c->ws.sc);
-    const int grid = (int)std::min<int64_t>(div_up(n, 256), (int64_t)c->sm_count * 8);
+    const int grid = (int)std::min<int64_t>(div_up(n, 256 * 4), (int64_t)c->sm_count * 8);
     BH_LAUNCH(c, k_bbox, grid, 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc);
     BH_LAUNCH(c, k_domain, 1, 32, 0, s, c->ws.sc);
     if (c->timing) cudaEventRecord(c->ev[1], s);

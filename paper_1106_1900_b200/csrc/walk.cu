@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(kWalkThreads, 2) k_walk(DevScalars* sc, const 
     }
 }
 
-__global__ void k_walk_reset(DevScalars* sc) {
+__global__ void k_reset_counters(DevScalars* sc) {
     if (threadIdx.x == 0) { sc->walk_next = 0; sc->sum_pc = 0; sc->sum_pp = 0; sc->sum_mac = 0; }
 }
 
@@ -317,7 +317,7 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
     if (c->timing) cudaEventRecord(c->ev[8], s);
     int rc = stage_cell_record(c, theta, s);
     if (rc != BH_OK) return rc;
-    BH_LAUNCH(c, k_walk_reset, 1, 32, 0, s, c->ws.sc);
+    BH_LAUNCH(c, k_reset_counters, 1, 32, 0, s, c->ws.sc);
     if (c->timing) cudaEventRecord(c->ev[9], s);
     const size_t smem = sizeof(WarpShared) * kWalkWarps;
     const int grid = c->sm_count * 2;

@@ -1,0 +1,66 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (1 M Plummer, theta 0.75 / 0.5).
+
+Tree arrays, moments and per-group counts are compared in full (bit-exact); forces on a seeded random sample of
+4096 groups, which the oracle computes one by one (groups are independent).  The larger configs (c3 always; c4, c5
+when BH_FULL_PARITY=1, they need minutes of single-threaded oracle time) use the same protocol.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import bh_inputs
+from parity_common import check_forces, compare_counts, compare_tree, gpu_tree, oracle_state
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def BH():
+    import __graft_entry__ as g
+    g.build()
+    from paper_1106_1900_b200 import BarnesHut
+    return BarnesHut
+
+
+def _sampled_parity(BH, cfg, thetas, n=None, nsample=4096):
+    pm, vel, prm = bh_inputs.make(cfg, n=n)
+    bh = BH(pm.shape[0])
+    out = {}
+    for theta in thetas:
+        g = gpu_tree(bh, pm, vel, theta, prm["eps"])
+        rng = np.random.default_rng(1234)
+        sel = np.sort(rng.choice(g["n_groups"], size=min(nsample, g["n_groups"]), replace=False)).astype(np.int64)
+        st = oracle_state(pm, vel, theta, prm["eps"], sel=sel)
+        bad = compare_tree(g, st)
+        compare_counts(g, st, sel=sel, problems=bad)
+        assert not bad, f"{cfg} theta={theta}:\n" + "\n".join(bad)
+        out[theta] = check_forces(g, st, sel=sel)
+        # counts of ALL groups, without forces (cheap for the oracle: MAC tests only)
+        st_all = oracle_state(pm, vel, theta, prm["eps"], forces=False)
+        assert not compare_counts(g, st_all)
+        s = g["stats"]
+        assert s.sum_pc == int((st_all.tree.gcount * st_all.npc).sum())
+        assert s.sum_pp == int((st_all.tree.gcount * st_all.npp).sum())
+    bh.close()
+    return out
+
+
+def test_c2_plummer_1m_full_size():
+    import __graft_entry__ as g
+    g.build()
+    from paper_1106_1900_b200 import BarnesHut
+    e = _sampled_parity(BarnesHut, "c2", (0.75, 0.5))
+    print("c2 force errors", e)
+
+
+def test_c3_uniform_cube_4m_full_size(BH):
+    e = _sampled_parity(BH, "c3", (0.5,))
+    print("c3 force errors", e)
+
+
+@pytest.mark.skipif(os.environ.get("BH_FULL_PARITY") != "1", reason="set BH_FULL_PARITY=1 (minutes of oracle time, ~40 GB host RAM)")
+@pytest.mark.parametrize("cfg", ["c4", "c5"])
+def test_large_configs_full_size(BH, cfg):
+    e = _sampled_parity(BH, cfg, (0.4,))
+    print(cfg, "force errors", e)
