@@ -8,12 +8,22 @@
 //     of 7 x 20 + slack entries always admits a pure depth-first descent, so the stack cannot overflow.
 //   * each lane tests one cell:  d = distance from the group's tight box to the cell's centre of mass,
 //     accept iff d^2 > r2open = (l/theta + delta)^2  (Eq.1), in exactly the fp32 operations of DESIGN.md O9.
-//   * accepted cells are staged (48 B each) in a shared-memory ring; opened leaves contribute their particles (16 B each)
-//     to a second ring; whenever a ring holds 32 entries every lane sweeps them for its own target particle(s)
-//     ("each thread ... progresses over the data in the on-chip memory and accumulates partial interactions").
+//   * accepted cells are staged in a shared-memory ring; opened leaves contribute their particles to a second ring;
+//     whenever a ring holds 32 entries the warp sweeps them.
 //   * the group's own particles are skipped while staging and handled by a final self block with j != i (A19).
+//
+// Evaluation layout (what differs from the paper's one-thread-per-particle sweep, and why):
+//   (1) Lane use.  A group holds n <= 64 targets (mean ~19), so "one target per lane" idles ~half of the warp.  The
+//       paper's remedy is up to 4 threads per particle (L81, L97); here it is taken to its end: n is rounded up to a
+//       multiple of 4 and split in binary, 32 + 32 + 16 + 8 + 4 -> "slots" with T = 2^K targets each.  In a slot,
+//       lane l serves target (l mod T) and sub-list (l div T): the 32 / T sub-lists interleave the ring entries, and a
+//       butterfly of shuffles adds the sub-list sums at the end of the group.  Every lane does useful work (>= 93 %).
+//   (2) FP32 rate.  On sm_100a scalar FFMA issues at half rate; the full 128 lanes/clk/SM needs the packed f32x2 forms
+//       (FFMA2/FMUL2/FADD2, measured 71.8 vs 37-45 TFLOP/s).  The rings therefore store PAIRS of entries interleaved
+//       (x0, x1, y0, y1, ...), one LDS.128 yields two packed operands, and each lane evaluates two list entries per
+//       instruction for its target.  Partial sums per 32-entry batch are added to the running totals (accuracy).
 // Forces: Plummer-softened p-p, and p-c with monopole + quadrupole (second-order expansion of the softened kernel,
-// DESIGN.md O10).  fp32 FMA arithmetic + MUFU.RSQ; partial sums per 32-entry batch are added to the running totals.
+// DESIGN.md O10): 35 packed fp32 operations + 2 MUFU.RSQ per PAIR of p-c interactions, 13 + 2 per pair of p-p.
 #include <algorithm>
 #include "bh_internal.cuh"
 
@@ -23,21 +33,30 @@ constexpr int kWalkWarps = 8;
 constexpr int kWalkThreads = kWalkWarps * 32;
 constexpr int kStackCap = 1024;
 constexpr int kStackReserve = 160;   // >= 7 * 20 + 7: room for a pure depth-first descent
-constexpr int kRing = 64;            // ring capacity (entries), power of two, >= 63
+constexpr int kRing = 64;            // ring capacity in entries (power of two, >= 63)
+constexpr int kRingPairs = kRing / 2;
+constexpr int kPcPair = 28;          // floats per p-c pair: 12 fields x 2 + 4 pad (112 B stride: no bank conflict for 8 pairs)
+constexpr int kPpPair = 8;           // floats per p-p pair: x0 x1 y0 y1 z0 z1 m0 m1
 
+// p-c pair fields f = 0..11: x y z M | Qm_xx Qm_yy Qm_zz Qm_xy | Qm_xz Qm_yz nTh n3Th, with Qm = -3 Q, nTh = -T/2,
+// n3Th = -3T/2; entry e lives in pair e >> 1, half e & 1, at float index pair * kPcPair + 2 f + half.
 struct __align__(16) WarpShared {
-    float4 pc[kRing][3];             // (com.xyz, M) (1.5 Qxx, 1.5 Qyy, 1.5 Qzz, 1.5 Qxy) (1.5 Qxz, 1.5 Qyz, -T/2, -3T/2)
-    float4 pp[kRing];                // (x, y, z, m)
+    float pc[kRingPairs * kPcPair];
+    float pp[kRingPairs * kPpPair];
     uint32_t stack[kStackCap];
     uint32_t run_begin[32];
     uint32_t run_off[36];
 };
 
-__device__ __forceinline__ float rsqrt_approx(float x) {
-    float y;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
+typedef unsigned long long f2;   // two fp32 values in one 64-bit register: low word = even entry, high word = odd entry
+
+__device__ __forceinline__ f2 pk(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void upk(f2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { f2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { f2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { f2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ f2 rsqrt2(f2 v) { float lo, hi; upk(v, lo, hi); return pk(rsqrt_approx(lo), rsqrt_approx(hi)); }
 
 __device__ __forceinline__ int warp_excl_scan(int v, int lane, int& total) {
     int inc = v;
@@ -50,132 +69,225 @@ __device__ __forceinline__ int warp_excl_scan(int v, int lane, int& total) {
     return inc - v;
 }
 
-struct Acc4 { float x, y, z, p; };   // acceleration and MINUS the potential
+// One slot: T = 2^K targets; this lane's target position and running sums (acceleration, MINUS the potential).
+struct Slot { float tx, ty, tz, ax, ay, az, p; };
 
-// p-c: 36 fp32 operations + 1 rsqrt per interaction.  Staged values: M, Q'' = 1.5 Q, nTh = -T/2, n3Th = -3T/2.
-//   -phi += M/rho + nTh/rho^3 + w''/rho^5,          w'' = dr.Q''.dr = 1.5 w
-//   a    += dr (M/rho^3 + n3Th/rho^5 + 5 w''/rho^7) - 2 q''/rho^5,   q'' = Q'' dr = 1.5 q
-template <int NT>
-__device__ __forceinline__ void eval_pc(const WarpShared* ws, int head, int count, const float (&tx)[NT], const float (&ty)[NT],
-                                        const float (&tz)[NT], Acc4 (&acc)[NT], float eps2) {
-    Acc4 loc[NT];
-#pragma unroll
-    for (int t = 0; t < NT; ++t) loc[t] = Acc4{0.f, 0.f, 0.f, 0.f};
-#pragma unroll 4
-    for (int j = 0; j < count; ++j) {
-        const int e = (head + j) & (kRing - 1);
-        const float4 a = ws->pc[e][0], b = ws->pc[e][1], c = ws->pc[e][2];
-#pragma unroll
-        for (int t = 0; t < NT; ++t) {
-            const float dx = a.x - tx[t], dy = a.y - ty[t], dz = a.z - tz[t];
-            const float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2)));
-            const float ri = rsqrt_approx(r2);
-            const float ri2 = ri * ri, ri3 = ri * ri2, ri5 = ri3 * ri2, ri7 = ri5 * ri2;
-            const float qx = fmaf(b.x, dx, fmaf(b.w, dy, c.x * dz));
-            const float qy = fmaf(b.w, dx, fmaf(b.y, dy, c.y * dz));
-            const float qz = fmaf(c.x, dx, fmaf(c.y, dy, b.z * dz));
-            const float w = fmaf(dx, qx, fmaf(dy, qy, dz * qz));
-            loc[t].p = fmaf(a.w, ri, fmaf(c.z, ri3, fmaf(w, ri5, loc[t].p)));
-            const float br = fmaf(5.0f * w, ri7, fmaf(c.w, ri5, a.w * ri3));
-            const float c5 = -2.0f * ri5;
-            loc[t].x = fmaf(qx, c5, fmaf(dx, br, loc[t].x));
-            loc[t].y = fmaf(qy, c5, fmaf(dy, br, loc[t].y));
-            loc[t].z = fmaf(qz, c5, fmaf(dz, br, loc[t].z));
-        }
+struct Consts { f2 e2, mhalf, m2p5; };
+
+// p-c over `npairs` ring pairs starting at pair `hp`; lane takes pairs sub, sub + S, ...  (S = 32 >> K sub-lists).
+//   -phi += M/rho + nTh/rho^3 - w/(2 rho^5),                 q = Qm dr = -3 Q dr,  w = dr.q
+//   a    += dr (M/rho^3 + n3Th/rho^5 - 5 w/(2 rho^7)) + q/rho^5
+template <int K>
+__device__ __forceinline__ void eval_pc(const WarpShared* ws, int hp, int npairs, Slot& s, const Consts& k, int lane) {
+    constexpr int S = 32 >> K;
+    const f2 ntx = pk(-s.tx, -s.tx), nty = pk(-s.ty, -s.ty), ntz = pk(-s.tz, -s.tz);
+    f2 ax = 0ull, ay = 0ull, az = 0ull, P = 0ull;
+#pragma unroll 2
+    for (int p = lane >> K; p < npairs; p += S) {
+        const ulonglong2* src = reinterpret_cast<const ulonglong2*>(ws->pc + ((hp + p) & (kRingPairs - 1)) * kPcPair);
+        const ulonglong2 v0 = src[0], v1 = src[1], v2 = src[2], v3 = src[3], v4 = src[4], v5 = src[5];
+        const f2 dx = add2(v0.x, ntx), dy = add2(v0.y, nty), dz = add2(v1.x, ntz);
+        const f2 r2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, k.e2)));
+        const f2 ri = rsqrt2(r2);
+        const f2 ri2 = mul2(ri, ri), ri3 = mul2(ri, ri2), ri5 = mul2(ri3, ri2);
+        const f2 qx = fma2(v2.x, dx, fma2(v3.y, dy, mul2(v4.x, dz)));
+        const f2 qy = fma2(v3.y, dx, fma2(v2.y, dy, mul2(v4.y, dz)));
+        const f2 qz = fma2(v4.x, dx, fma2(v4.y, dy, mul2(v3.x, dz)));
+        const f2 w = fma2(dx, qx, fma2(dy, qy, mul2(dz, qz)));
+        const f2 t = mul2(w, ri5);
+        P = fma2(v1.y, ri, fma2(v5.x, ri3, fma2(t, k.mhalf, P)));
+        const f2 br = fma2(mul2(t, ri2), k.m2p5, fma2(v5.y, ri5, mul2(v1.y, ri3)));
+        ax = fma2(qx, ri5, fma2(dx, br, ax));
+        ay = fma2(qy, ri5, fma2(dy, br, ay));
+        az = fma2(qz, ri5, fma2(dz, br, az));
     }
-#pragma unroll
-    for (int t = 0; t < NT; ++t) { acc[t].x += loc[t].x; acc[t].y += loc[t].y; acc[t].z += loc[t].z; acc[t].p += loc[t].p; }
+    float lo, hi;
+    upk(ax, lo, hi); s.ax += lo + hi;
+    upk(ay, lo, hi); s.ay += lo + hi;
+    upk(az, lo, hi); s.az += lo + hi;
+    upk(P, lo, hi); s.p += lo + hi;
 }
 
-// p-p: 13 fp32 operations + 1 rsqrt.  kSelf: sources are the group's own particles; entry j is target index j (skip j == i).
-template <int NT, bool kSelf>
-__device__ __forceinline__ void eval_pp(const WarpShared* ws, int head, int count, const float (&tx)[NT], const float (&ty)[NT],
-                                        const float (&tz)[NT], Acc4 (&acc)[NT], float eps2, int lane) {
-    Acc4 loc[NT];
-#pragma unroll
-    for (int t = 0; t < NT; ++t) loc[t] = Acc4{0.f, 0.f, 0.f, 0.f};
-#pragma unroll 4
-    for (int j = 0; j < count; ++j) {
-        const float4 s = ws->pp[(head + j) & (kRing - 1)];
-#pragma unroll
-        for (int t = 0; t < NT; ++t) {
-            const float dx = s.x - tx[t], dy = s.y - ty[t], dz = s.z - tz[t];
-            const float r2 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, eps2)));
-            float ri = rsqrt_approx(r2);
-            if (kSelf) ri = (j == lane + 32 * t) ? 0.0f : ri;
-            const float ri2 = ri * ri;
-            const float mr = s.w * ri;
-            const float mr3 = mr * ri2;
-            loc[t].p += mr;
-            loc[t].x = fmaf(dx, mr3, loc[t].x);
-            loc[t].y = fmaf(dy, mr3, loc[t].y);
-            loc[t].z = fmaf(dz, mr3, loc[t].z);
+// p-p.  kSelf: the ring holds the group's own `nself` particles from entry 0; entry j is target index j: skip j == tidx
+// and the massless pad entry j >= nself (it sits ON the last own particle: r = 0 would give 0 * inf when eps = 0).
+template <int K, bool kSelf>
+__device__ __forceinline__ void eval_pp(const WarpShared* ws, int hp, int npairs, Slot& s, const Consts& k, int lane, int tidx, int nself) {
+    constexpr int S = 32 >> K;
+    const f2 ntx = pk(-s.tx, -s.tx), nty = pk(-s.ty, -s.ty), ntz = pk(-s.tz, -s.tz);
+    f2 ax = 0ull, ay = 0ull, az = 0ull, P = 0ull;
+#pragma unroll 2
+    for (int p = lane >> K; p < npairs; p += S) {
+        const ulonglong2* src = reinterpret_cast<const ulonglong2*>(ws->pp + ((hp + p) & (kRingPairs - 1)) * kPpPair);
+        const ulonglong2 v0 = src[0], v1 = src[1];
+        const f2 dx = add2(v0.x, ntx), dy = add2(v0.y, nty), dz = add2(v1.x, ntz);
+        const f2 r2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, k.e2)));
+        f2 ri;
+        if (kSelf) {
+            float lo, hi;
+            upk(r2, lo, hi);
+            lo = (2 * p == tidx) ? 0.0f : rsqrt_approx(lo);
+            hi = (2 * p + 1 == tidx || 2 * p + 1 >= nself) ? 0.0f : rsqrt_approx(hi);
+            ri = pk(lo, hi);
+        } else {
+            ri = rsqrt2(r2);
         }
+        const f2 ri2 = mul2(ri, ri);
+        const f2 mr = mul2(v1.y, ri);
+        const f2 mr3 = mul2(mr, ri2);
+        P = add2(P, mr);
+        ax = fma2(dx, mr3, ax);
+        ay = fma2(dy, mr3, ay);
+        az = fma2(dz, mr3, az);
     }
-#pragma unroll
-    for (int t = 0; t < NT; ++t) { acc[t].x += loc[t].x; acc[t].y += loc[t].y; acc[t].z += loc[t].z; acc[t].p += loc[t].p; }
+    float lo, hi;
+    upk(ax, lo, hi); s.ax += lo + hi;
+    upk(ay, lo, hi); s.ay += lo + hi;
+    upk(az, lo, hi); s.az += lo + hi;
+    upk(P, lo, hi); s.p += lo + hi;
 }
 
-template <int NT>
-__device__ __forceinline__ void walk_group(WarpShared* ws, const int lane, const uint32_t g, const uint32_t gb, const uint32_t ge,
-                                           const float4* __restrict__ pos, const float4* __restrict__ rec, float eps2,
-                                           float4* __restrict__ acc_out, uint32_t* __restrict__ g_npc, uint32_t* __restrict__ g_npp,
-                                           DevScalars* sc) {
+// The five slots of a group: A, B (32 targets each), C (16), D (8), E (4).
+struct Slots {
+    Slot a, b, c, d, e;
+    bool hasA, hasB, hasC, hasD, hasE;
+    int baseC, baseD, baseE;
+};
+
+__device__ __forceinline__ void eval_pc_all(const WarpShared* ws, int hp, int npairs, Slots& S, const Consts& k, int lane) {
+    if (S.hasA) eval_pc<5>(ws, hp, npairs, S.a, k, lane);
+    if (S.hasB) eval_pc<5>(ws, hp, npairs, S.b, k, lane);
+    if (S.hasC) eval_pc<4>(ws, hp, npairs, S.c, k, lane);
+    if (S.hasD) eval_pc<3>(ws, hp, npairs, S.d, k, lane);
+    if (S.hasE) eval_pc<2>(ws, hp, npairs, S.e, k, lane);
+}
+
+template <bool kSelf>
+__device__ __forceinline__ void eval_pp_all(const WarpShared* ws, int hp, int npairs, Slots& S, const Consts& k, int lane, int nself) {
+    if (S.hasA) eval_pp<5, kSelf>(ws, hp, npairs, S.a, k, lane, lane, nself);
+    if (S.hasB) eval_pp<5, kSelf>(ws, hp, npairs, S.b, k, lane, 32 + lane, nself);
+    if (S.hasC) eval_pp<4, kSelf>(ws, hp, npairs, S.c, k, lane, S.baseC + (lane & 15), nself);
+    if (S.hasD) eval_pp<3, kSelf>(ws, hp, npairs, S.d, k, lane, S.baseD + (lane & 7), nself);
+    if (S.hasE) eval_pp<2, kSelf>(ws, hp, npairs, S.e, k, lane, S.baseE + (lane & 3), nself);
+}
+
+__device__ __forceinline__ void slot_init(Slot& s, const float4* __restrict__ pos, uint32_t gb, int ng, int tidx) {
+    const float4 p = __ldg(pos + gb + min(tidx, ng - 1));   // idle target slots shadow the last particle (results discarded)
+    s.tx = p.x; s.ty = p.y; s.tz = p.z;
+    s.ax = s.ay = s.az = s.p = 0.0f;
+}
+
+// Add the sub-list sums of a slot (lanes that share l mod T) and store the T targets.
+template <int K>
+__device__ __forceinline__ void slot_finish(Slot& s, int lane, int tbase, int ng, uint32_t gb, float4* __restrict__ acc_out) {
+#pragma unroll
+    for (int o = 1 << K; o < 32; o <<= 1) {
+        s.ax += __shfl_xor_sync(0xFFFFFFFFu, s.ax, o);
+        s.ay += __shfl_xor_sync(0xFFFFFFFFu, s.ay, o);
+        s.az += __shfl_xor_sync(0xFFFFFFFFu, s.az, o);
+        s.p += __shfl_xor_sync(0xFFFFFFFFu, s.p, o);
+    }
+    const int idx = tbase + lane;
+    if (lane < (1 << K) && idx < ng) acc_out[gb + idx] = make_float4(s.ax, s.ay, s.az, -s.p);
+}
+
+__device__ __forceinline__ void pc_store(float* ring, int e, float x, float y, float z, float M, float qxx, float qyy, float qzz,
+                                         float qxy, float qxz, float qyz, float nth, float n3th) {
+    float* d = ring + (e >> 1) * kPcPair + (e & 1);
+    d[0] = x; d[2] = y; d[4] = z; d[6] = M; d[8] = qxx; d[10] = qyy; d[12] = qzz; d[14] = qxy; d[16] = qxz; d[18] = qyz;
+    d[20] = nth; d[22] = n3th;
+}
+__device__ __forceinline__ void pp_store(float* ring, int e, float x, float y, float z, float m) {
+    float* d = ring + (e >> 1) * kPpPair + (e & 1);
+    d[0] = x; d[2] = y; d[4] = z; d[6] = m;
+}
+// An odd tail gets a massless partner at the position of the last real entry (a position no target can coincide with).
+__device__ __forceinline__ void pc_pad(float* ring, int e_last) {
+    const float* s = ring + (e_last >> 1) * kPcPair + (e_last & 1);
+    pc_store(ring, (e_last + 1) & (kRing - 1), s[0], s[2], s[4], 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f);
+}
+__device__ __forceinline__ void pp_pad(float* ring, int e_last) {
+    const float* s = ring + (e_last >> 1) * kPpPair + (e_last & 1);
+    pp_store(ring, (e_last + 1) & (kRing - 1), s[0], s[2], s[4], 0.f);
+}
+
+__device__ __noinline__ void walk_group(WarpShared* ws, const int lane, const uint32_t g, const uint32_t gb, const uint32_t ge,
+                                        const float4* __restrict__ pos, const float4* __restrict__ rec, float eps2,
+                                        float4* __restrict__ acc_out, uint32_t* __restrict__ g_npc, uint32_t* __restrict__ g_npp,
+                                        DevScalars* sc) {
     const uint32_t lt = (1u << lane) - 1u;
     const int ng = (int)(ge - gb);
-    float tx[NT], ty[NT], tz[NT];
-    Acc4 acc[NT];
-    float4 tp[NT];
+    Consts k;
+    k.e2 = pk(eps2, eps2);
+    k.mhalf = pk(-0.5f, -0.5f);
+    k.m2p5 = pk(-2.5f, -2.5f);
+
+    // ---- the group's tight box (A13) and its own particles
+    float4 own[2];
     float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
-    for (int t = 0; t < NT; ++t) {
-        const int idx = lane + 32 * t;
-        tp[t] = pos[gb + min(idx, ng - 1)];          // idle lanes shadow the last particle (results discarded)
-        tx[t] = tp[t].x; ty[t] = tp[t].y; tz[t] = tp[t].z;
-        acc[t] = Acc4{0.f, 0.f, 0.f, 0.f};
-        mn[0] = fminf(mn[0], tx[t]); mx[0] = fmaxf(mx[0], tx[t]);
-        mn[1] = fminf(mn[1], ty[t]); mx[1] = fmaxf(mx[1], ty[t]);
-        mn[2] = fminf(mn[2], tz[t]); mx[2] = fmaxf(mx[2], tz[t]);
+    for (int t = 0; t < 2; ++t) {
+        own[t] = __ldg(pos + gb + min(lane + 32 * t, ng - 1));
+        mn[0] = fminf(mn[0], own[t].x); mx[0] = fmaxf(mx[0], own[t].x);
+        mn[1] = fminf(mn[1], own[t].y); mx[1] = fmaxf(mx[1], own[t].y);
+        mn[2] = fminf(mn[2], own[t].z); mx[2] = fmaxf(mx[2], own[t].z);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1)
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            mn[k] = fminf(mn[k], __shfl_xor_sync(0xFFFFFFFFu, mn[k], o));
-            mx[k] = fmaxf(mx[k], __shfl_xor_sync(0xFFFFFFFFu, mx[k], o));
+        for (int a = 0; a < 3; ++a) {
+            mn[a] = fminf(mn[a], __shfl_xor_sync(0xFFFFFFFFu, mn[a], o));
+            mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xFFFFFFFFu, mx[a], o));
         }
+
+    // ---- slots: n rounded up to a multiple of 4, split as 32 + 32 + 16 + 8 + 4
+    Slots S;
+    {
+        const int m = (ng + 3) & ~3;
+        const int full = m >> 5, rem = m & 31;
+        S.hasA = full >= 1; S.hasB = full == 2;
+        S.hasC = (rem & 16) != 0; S.hasD = (rem & 8) != 0; S.hasE = (rem & 4) != 0;
+        int base = 32 * full;
+        S.baseC = base; base += S.hasC ? 16 : 0;
+        S.baseD = base; base += S.hasD ? 8 : 0;
+        S.baseE = base;
+        slot_init(S.a, pos, gb, ng, lane);
+        slot_init(S.b, pos, gb, ng, 32 + lane);
+        slot_init(S.c, pos, gb, ng, S.baseC + (lane & 15));
+        slot_init(S.d, pos, gb, ng, S.baseD + (lane & 7));
+        slot_init(S.e, pos, gb, ng, S.baseE + (lane & 3));
+    }
 
     int sp = 1;
     if (lane == 0) ws->stack[0] = 0u;   // the root (A17)
     __syncwarp();
-    int pc_head = 0, pc_cnt = 0, pp_head = 0, pp_cnt = 0;
+    int pc_head = 0, pc_cnt = 0, pp_head = 0, pp_cnt = 0;   // heads are even (entries are consumed 32 at a time)
     uint32_t npc = 0, npp = 0, nmac = 0;
 
     while (sp > 0) {
-        int k = (kStackCap - kStackReserve - sp) / 7;
-        k = max(1, min(k, 32));
-        k = min(k, sp);
-        const bool valid = lane < k;
+        int kpop = (kStackCap - kStackReserve - sp) / 7;
+        kpop = max(1, min(kpop, 32));
+        kpop = min(kpop, sp);
+        const bool valid = lane < kpop;
         uint32_t cell = 0;
         if (valid) cell = ws->stack[sp - 1 - lane];
-        sp -= k;
-        nmac += (uint32_t)k;
+        sp -= kpop;
+        nmac += (uint32_t)kpop;
         __syncwarp();
         bool accept = false, isleaf = false, isnode = false;
-        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0, r2 = r0, r3 = r0;
         uint32_t first = 0, cnt = 0;
         if (valid) {
-            r0 = __ldg(rec + 4 * (size_t)cell);
+            const float4* rp = rec + 4 * (size_t)cell;     // the whole 64 B record in one round trip
+            r0 = __ldg(rp); r1 = __ldg(rp + 1); r2 = __ldg(rp + 2); r3 = __ldg(rp + 3);
             const float dx = fmaxf(fmaxf(__fsub_rn(mn[0], r0.x), __fsub_rn(r0.x, mx[0])), 0.0f);
             const float dy = fmaxf(fmaxf(__fsub_rn(mn[1], r0.y), __fsub_rn(r0.y, mx[1])), 0.0f);
             const float dz = fmaxf(fmaxf(__fsub_rn(mn[2], r0.z), __fsub_rn(r0.z, mx[2])), 0.0f);
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
             accept = d2 > r0.w;
             if (!accept) {
-                const float4 l = __ldg(rec + 4 * (size_t)cell + 3);
-                first = __float_as_uint(l.x);
-                cnt = __float_as_uint(l.y);
-                isleaf = __float_as_uint(l.z) != 0u;
+                first = __float_as_uint(r3.x);
+                cnt = __float_as_uint(r3.y);
+                isleaf = __float_as_uint(r3.z) != 0u;
                 isnode = !isleaf;
             }
         }
@@ -183,19 +295,17 @@ __device__ __forceinline__ void walk_group(WarpShared* ws, const int lane, const
         const uint32_t amask = __ballot_sync(0xFFFFFFFFu, accept);
         if (amask) {
             if (accept) {
-                const float4 r1 = __ldg(rec + 4 * (size_t)cell + 1), r2 = __ldg(rec + 4 * (size_t)cell + 2);
                 const float T = (r1.y + r1.z) + r1.w;
-                const int slot = (pc_head + pc_cnt + __popc(amask & lt)) & (kRing - 1);
-                ws->pc[slot][0] = make_float4(r0.x, r0.y, r0.z, r1.x);
-                ws->pc[slot][1] = make_float4(1.5f * r1.y, 1.5f * r1.z, 1.5f * r1.w, 1.5f * r2.x);
-                ws->pc[slot][2] = make_float4(1.5f * r2.y, 1.5f * r2.z, -0.5f * T, -1.5f * T);
+                const int e = (pc_head + pc_cnt + __popc(amask & lt)) & (kRing - 1);
+                pc_store(ws->pc, e, r0.x, r0.y, r0.z, r1.x, -3.0f * r1.y, -3.0f * r1.z, -3.0f * r1.w, -3.0f * r2.x, -3.0f * r2.y,
+                         -3.0f * r2.z, -0.5f * T, -1.5f * T);
             }
             const int na = __popc(amask);
             pc_cnt += na;
             npc += (uint32_t)na;
             __syncwarp();
             if (pc_cnt >= 32) {
-                eval_pc<NT>(ws, pc_head, 32, tx, ty, tz, acc, eps2);
+                eval_pc_all(ws, pc_head >> 1, 16, S, k, lane);
                 pc_head = (pc_head + 32) & (kRing - 1);
                 pc_cnt -= 32;
                 __syncwarp();
@@ -228,11 +338,14 @@ __device__ __forceinline__ void walk_group(WarpShared* ws, const int lane, const
                     keep = !(src >= gb && src < ge);
                 }
                 const uint32_t kmask = __ballot_sync(0xFFFFFFFFu, keep);
-                if (keep) ws->pp[(pp_head + pp_cnt + __popc(kmask & lt)) & (kRing - 1)] = __ldg(pos + src);
+                if (keep) {
+                    const float4 p = __ldg(pos + src);
+                    pp_store(ws->pp, (pp_head + pp_cnt + __popc(kmask & lt)) & (kRing - 1), p.x, p.y, p.z, p.w);
+                }
                 pp_cnt += __popc(kmask);
                 __syncwarp();
                 if (pp_cnt >= 32) {
-                    eval_pp<NT, false>(ws, pp_head, 32, tx, ty, tz, acc, eps2, lane);
+                    eval_pp_all<false>(ws, pp_head >> 1, 16, S, k, lane, 0);
                     pp_head = (pp_head + 32) & (kRing - 1);
                     pp_cnt -= 32;
                     __syncwarp();
@@ -256,24 +369,35 @@ __device__ __forceinline__ void walk_group(WarpShared* ws, const int lane, const
             __syncwarp();
         }
     }
-    // ---- flush the rings
-    if (pc_cnt > 0) eval_pc<NT>(ws, pc_head, pc_cnt, tx, ty, tz, acc, eps2);
-    if (pp_cnt > 0) eval_pp<NT, false>(ws, pp_head, pp_cnt, tx, ty, tz, acc, eps2, lane);
-    __syncwarp();
-    // ---- self block: the group's own particles, j != i
-#pragma unroll
-    for (int t = 0; t < NT; ++t) {
-        const int idx = lane + 32 * t;
-        if (idx < ng) ws->pp[idx] = tp[t];
+    // ---- flush the rings (an odd tail gets a massless partner)
+    if (pc_cnt > 0) {
+        if ((pc_cnt & 1) && lane == 0) pc_pad(ws->pc, (pc_head + pc_cnt - 1) & (kRing - 1));
+        __syncwarp();
+        eval_pc_all(ws, pc_head >> 1, (pc_cnt + 1) >> 1, S, k, lane);
+    }
+    if (pp_cnt > 0) {
+        if ((pp_cnt & 1) && lane == 0) pp_pad(ws->pp, (pp_head + pp_cnt - 1) & (kRing - 1));
+        __syncwarp();
+        eval_pp_all<false>(ws, pp_head >> 1, (pp_cnt + 1) >> 1, S, k, lane, 0);
     }
     __syncwarp();
-    eval_pp<NT, true>(ws, 0, ng, tx, ty, tz, acc, eps2, lane);
-    __syncwarp();
+    // ---- self block: the group's own particles, entry j = target index j, j != i
 #pragma unroll
-    for (int t = 0; t < NT; ++t) {
+    for (int t = 0; t < 2; ++t) {
         const int idx = lane + 32 * t;
-        if (idx < ng) acc_out[gb + idx] = make_float4(acc[t].x, acc[t].y, acc[t].z, -acc[t].p);
+        if (idx < ng) pp_store(ws->pp, idx, own[t].x, own[t].y, own[t].z, own[t].w);
     }
+    __syncwarp();
+    if ((ng & 1) && lane == 0) pp_pad(ws->pp, ng - 1);
+    __syncwarp();
+    eval_pp_all<true>(ws, 0, (ng + 1) >> 1, S, k, lane, ng);
+    __syncwarp();
+    // ---- add the sub-list sums and store
+    if (S.hasA) slot_finish<5>(S.a, lane, 0, ng, gb, acc_out);
+    if (S.hasB) slot_finish<5>(S.b, lane, 32, ng, gb, acc_out);
+    if (S.hasC) slot_finish<4>(S.c, lane, S.baseC, ng, gb, acc_out);
+    if (S.hasD) slot_finish<3>(S.d, lane, S.baseD, ng, gb, acc_out);
+    if (S.hasE) slot_finish<2>(S.e, lane, S.baseE, ng, gb, acc_out);
     if (lane == 0) {
         g_npc[g] = npc;
         g_npp[g] = npp;
@@ -296,10 +420,7 @@ __global__ void __launch_bounds__(kWalkThreads, 2) k_walk(DevScalars* sc, const 
         g = __shfl_sync(0xFFFFFFFFu, g, 0);
         if (g >= ngroups) break;
         const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
-        if (ge - gb <= 32u)
-            walk_group<1>(ws, lane, g, gb, ge, pos, rec, eps2, acc_out, g_npc, g_npp, sc);
-        else
-            walk_group<2>(ws, lane, g, gb, ge, pos, rec, eps2, acc_out, g_npc, g_npp, sc);
+        walk_group(ws, lane, g, gb, ge, pos, rec, eps2, acc_out, g_npc, g_npp, sc);
         __syncwarp();
     }
 }
