@@ -32,7 +32,7 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
-    cmd = [NVCC] + FLAGS + ["-o", LIB] + sources()
+    cmd = [NVCC] + FLAGS + os.environ.get("BH_NVCC_EXTRA", "").split() + ["-o", LIB] + sources()
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         print(r.stdout)

@@ -79,7 +79,7 @@ struct Ws {
     uint32_t* c_parent;
     double* mom64;        // [max_cells][10]
     float* box;           // [max_cells][6]
-    float4* rec;          // [max_cells][4] walk record: (com, r2open) (M, Qxx, Qyy, Qzz) (Qxy, Qxz, Qyz, 0) (first, count, leaf, 0)
+    float4* rec;          // [4][max_cells] walk record planes: (com, r2open) (M, -3Qxx, -3Qyy, -3Qzz) (-3Qxy, -3Qxz, -3Qyz, -T/2) (first, count, leaf, -3T/2)
     // export (canonical arrays of bh_tree_view)
     int32_t* e_level;
     uint64_t* e_prefix;
