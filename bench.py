@@ -97,10 +97,30 @@ def _workload(args):
     return cfg, n
 
 
+def rank_seed(cfg: str, rank: int) -> int:
+    """Every rank steps its own replica of the workload: same recipe, different seed."""
+    return bh_inputs.SEEDS[cfg] + 1000 * rank
+
+
 def _make_inputs(cfg, n, rank):
-    seed = bh_inputs.SEEDS[cfg] + 1000 * rank
-    pm, vel, prm = bh_inputs.make(cfg, n=n, seed=seed)
+    pm, vel, prm = bh_inputs.make(cfg, n=n, seed=rank_seed(cfg, rank))
     return pm, vel, prm
+
+
+def max_over_ranks(x: float, world: int, device=None) -> float:
+    """The job's time is the slowest rank's: one all-reduce(MAX) of a scalar (NCCL on GPUs, gloo in the CPU test)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(world: int, n_per_rank: int, steps: int, seconds: float) -> float:
+    """Whole-job particles/s: every rank advanced n_per_rank particles `steps` times in `seconds` (max over ranks)."""
+    return world * n_per_rank * steps / seconds
 
 
 # ------------------------------------------------------------------------------------------------ CPU oracle legs
@@ -225,11 +245,8 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     s1 = bh.sync_status()
     ms = sum(a.elapsed_time(b) for a, b in evs)
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
-    value = world * n * args.steps / (ms_total * 1e-3)
+    ms_total = max_over_ranks(ms, world, dev)
+    value = job_throughput(world, n, args.steps, ms_total * 1e-3)
 
     # ---- e2e: the same step driven from HOST buffers through the C ABI (H2D and D2H inside the timed region)
     hp = torch.from_numpy(pm).pin_memory(); hv = torch.from_numpy(vel).pin_memory()
@@ -255,11 +272,8 @@ def run_ours(args):
     for _ in range(e2e_steps):
         host_step()
     barrier()
-    e2e_s = max(time.perf_counter() - t0, 1e-9)
-    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * n * e2e_steps / float(t.item())
+    e2e_s = max_over_ranks(max(time.perf_counter() - t0, 1e-9), world, dev)
+    e2e_value = job_throughput(world, n, e2e_steps, e2e_s)
 
     if rank != 0:
         if world > 1:

@@ -1,0 +1,61 @@
+"""Host-side logic of the N > 1 path of bench.py, on CPU with the gloo backend and world size 2 (no GPU).
+
+DESIGN.md section 9: replicas only -- each rank steps its own replica (its own seed), no data-path collective; the
+job's time is the slowest rank's (all-reduce MAX of one scalar); rank 0 alone reports; the reference arm runs on
+rank 0 only.  The ranks here also run the oracle on their replica to show the replicas really differ.
+"""
+import os
+import subprocess
+import sys
+import textwrap
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+WORKER = textwrap.dedent("""
+    import json, os, sys
+    sys.path.insert(0, %r)
+    import numpy as np
+    import torch.distributed as dist
+    import bench, bh_inputs, oracle
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    dist.init_process_group("gloo")
+    pm, vel, prm = bench._make_inputs("c1", 2048, rank)
+    st = oracle.tree_build(pm, vel)
+    local_ms = 10.0 * (rank + 1)                        # rank 1 is the slow one
+    total_ms = bench.max_over_ranks(local_ms, world)
+    value = bench.job_throughput(world, 2048, 4, total_ms * 1e-3)
+    out = dict(rank=rank, seed=bench.rank_seed("c1", rank), checksum=float(np.float64(pm[:, :3]).sum()),
+               cells=st.tree.ncells, total_ms=total_ms, value=value)
+    print("RANKOUT " + json.dumps(out), flush=True)
+    dist.barrier()
+    dist.destroy_process_group()
+""") % ROOT
+
+
+def test_two_ranks_gloo(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", "29731", str(script)]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    import json
+    outs = sorted((json.loads(l.split("RANKOUT ", 1)[1]) for l in r.stdout.splitlines() if "RANKOUT " in l), key=lambda o: o["rank"])
+    assert [o["rank"] for o in outs] == [0, 1]
+    assert outs[0]["seed"] != outs[1]["seed"] and outs[0]["checksum"] != outs[1]["checksum"]      # different replicas
+    assert outs[0]["total_ms"] == outs[1]["total_ms"] == 20.0                                      # max over ranks
+    assert outs[0]["value"] == 2 * 2048 * 4 / 20e-3                                                 # whole-job aggregate
+
+
+def test_reference_arm_runs_on_rank0_only():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                        "--warmup", "0", "--config", "c1"], capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    assert r.returncode == 0 and r.stdout.strip() == ""          # other ranks exit 0 without work
+    env["RANK"] = "0"
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                        "--warmup", "0", "--config", "c1"], capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    import json
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "particles/s"
