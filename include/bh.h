@@ -48,6 +48,11 @@ typedef struct bh_config {
     int32_t nleaf;     /* max particles per leaf, 1..64; default 16 (L63) */
     int32_t ncrit;     /* max particles per group, 1..64; default 64 (L75) */
     int64_t max_cells; /* cell capacity; default = the hard bound n_max + 20*(n_max/(nleaf+1)) + 1 */
+    int64_t list_entries; /* capacity of the interaction-list buffer (S7 -> S8), 4-byte entries; default
+                           * clamp(320 * n_max, 2^22, 2^30).  Bounds memory only: groups whose lists do not fit are walked and
+                           * evaluated by the fused kernel, with identical counts and forces within rounding. */
+    int32_t walk_mode; /* 0 (default): list walk + list evaluation, fused kernel for what does not fit; 1: fused kernel only */
+    int32_t reserved;
 } bh_config;
 
 typedef struct bh_ctx bh_ctx;

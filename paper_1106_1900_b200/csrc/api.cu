@@ -21,8 +21,8 @@ struct Carver {
 };
 
 struct Geometry {
-    int64_t n_max, max_cells, sort_tiles, tree_tiles, scan_sum_cap;
-    int32_t nleaf, ncrit;
+    int64_t n_max, max_cells, sort_tiles, tree_tiles, scan_sum_cap, list_entries;
+    int32_t nleaf, ncrit, walk_mode;
 };
 
 static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
@@ -35,6 +35,11 @@ static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
     g->max_cells = (cfg && cfg->max_cells > 0) ? cfg->max_cells : bound;
     if (g->max_cells > bound) g->max_cells = bound;
     if (g->max_cells < 1 || g->max_cells > ((int64_t)1 << 31) - 2) return false;
+    g->list_entries = (cfg && cfg->list_entries > 0) ? cfg->list_entries
+                                                     : std::min<int64_t>(std::max<int64_t>(320 * n_max, (int64_t)1 << 22), (int64_t)1 << 30);
+    if (g->list_entries > ((int64_t)1 << 31)) return false;
+    g->walk_mode = cfg ? cfg->walk_mode : 0;
+    if (g->walk_mode < 0 || g->walk_mode > 1) return false;
     g->sort_tiles = div_up(n_max, kSortTile);
     g->tree_tiles = div_up(n_max + 1, kTreeTile);
     const int64_t biggest_scan = std::max<int64_t>(std::max<int64_t>((int64_t)kRadix * g->sort_tiles, (int64_t)kLevels * g->tree_tiles), n_max);
@@ -72,7 +77,15 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     o.c_parent = c.take<uint32_t>(C);
     o.mom64 = c.take<double>(10 * C);
     o.box = c.take<float>(6 * C);
-    o.rec = c.take<float4>(4 * C);
+    o.trec = c.take<float4>(C);
+    o.tlink = c.take<uint2>(C);
+    o.erec = c.take<float4>(3 * C);
+    o.ctl = c.take<WalkCtl>(1);
+    o.lists = c.take<uint32_t>((size_t)g.list_entries);
+    o.g_pcoff = c.take<uint32_t>(n);
+    o.g_ppoff = c.take<uint32_t>(n);
+    o.g_lpp = c.take<uint32_t>(n);
+    o.deferred = c.take<uint32_t>(n);
     o.e_level = c.take<int32_t>(C);
     o.e_prefix = c.take<uint64_t>(C);
     o.e_pcount = c.take<uint32_t>(C);
@@ -116,6 +129,8 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
     c->max_cells = g.max_cells;
     c->nleaf = g.nleaf;
     c->ncrit = g.ncrit;
+    c->list_entries = g.list_entries;
+    c->walk_mode = g.walk_mode;
     c->sort_tiles = g.sort_tiles;
     c->tree_tiles = g.tree_tiles;
     c->scan_sum_cap = g.scan_sum_cap;

@@ -31,6 +31,9 @@ constexpr int kScanTile = kScanThreads * kScanItems;            // 2048 entries 
 constexpr int kTreeTile = 256;
 constexpr int kHaloMax = 64;           // nleaf <= 64
 
+// ---- walk (S7, S8): waves of groups whose interaction lists share the list buffer
+constexpr int kMaxWaves = 255;
+
 // Device-resident scalars (one struct, copied to the host by bh_sync_status).
 struct DevScalars {
     uint32_t bb_min[3];      // order-preserving encodings of the per-axis minima / maxima (S0)
@@ -47,6 +50,15 @@ struct DevScalars {
     unsigned long long sum_pc;
     unsigned long long sum_pp;
     unsigned long long sum_mac;
+};
+
+// Walk control block (device): wave boundaries in groups, work counters, the groups deferred to the fused kernel.
+struct WalkCtl {
+    uint32_t wave_g[kMaxWaves + 1];
+    uint32_t list_next[kMaxWaves + 1];
+    uint32_t eval_next[kMaxWaves + 1];
+    uint32_t n_deferred;
+    uint32_t fused_next;
 };
 
 // Pointers into the caller's workspace.
@@ -79,7 +91,15 @@ struct Ws {
     uint32_t* c_parent;
     double* mom64;        // [max_cells][10]
     float* box;           // [max_cells][6]
-    float4* rec;          // [4][max_cells] walk record planes: (com, r2open) (M, -3Qxx, -3Qyy, -3Qzz) (-3Qxy, -3Qxz, -3Qyz, -T/2) (first, count, leaf, -3T/2)
+    float4* trec;         // [max_cells] walk record: (com, r2open)
+    uint2* tlink;         // [max_cells] walk record: (first child | first particle, count | leaf << 31)
+    float4* erec;         // [max_cells][3] evaluation record: (com, M) (Qm_xx, Qm_yy, Qm_zz, Qm_xy) (Qm_xz, Qm_yz, -T/2, -3T/2), Qm = -3 Q
+    WalkCtl* ctl;
+    uint32_t* lists;      // [list_entries] interaction lists: cell indices / particle indices
+    uint32_t* g_pcoff;    // [n] first entry of the group's cell list (kNone: deferred to the fused kernel)
+    uint32_t* g_ppoff;    // [n] first entry of the group's particle list
+    uint32_t* g_lpp;      // [n] length of the particle list (g_npp minus the group's own particles)
+    uint32_t* deferred;   // [n] groups whose lists did not fit
     // export (canonical arrays of bh_tree_view)
     int32_t* e_level;
     uint64_t* e_prefix;
@@ -106,6 +126,8 @@ struct bh_ctx {
     int64_t launches;
     int last_cuda;
     float theta_last;
+    int64_t list_entries;
+    int walk_mode;
     bh::Ws ws;
     int64_t sort_tiles, tree_tiles, scan_sum_cap;
     bool timing;
@@ -146,6 +168,16 @@ int stage_moments(bh_ctx* c, cudaStream_t s);         // S6
 int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s);          // S6: fp32 walk record + r2open(theta)
 int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s);   // S7, S8
 int walk_init(bh_ctx* c);
+int walk_eval_init(bh_ctx* c);
+struct WalkListOut {       // what k_walk_lists writes
+    DevScalars* sc;
+    WalkCtl* ctl;
+    uint32_t *g_pcoff, *g_ppoff, *g_lpp, *g_npc, *g_npp, *deferred;
+};
+WalkListOut walk_list_out(bh_ctx* c);
+int stage_walk_prepare(bh_ctx* c, int nwaves, uint32_t wave_particles, cudaStream_t s);
+int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t arena_entries, cudaStream_t s);   // S7
+int stage_walk_eval(bh_ctx* c, int wave, float eps, cudaStream_t s);                           // S8
 int stage_kick_drift(bh_ctx* c, float h, float dt, cudaStream_t s);  // S9
 int stage_kick(bh_ctx* c, float h, cudaStream_t s);                  // S9
 int stage_export(bh_ctx* c, cudaStream_t s);

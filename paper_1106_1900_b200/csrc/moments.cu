@@ -115,14 +115,15 @@ __global__ void __launch_bounds__(128) k_node_moments(const DevScalars* __restri
     }
 }
 
-// fp32 walk record (4 planes of float4 per cell: (com, r2open) (M, Qm_xx, Qm_yy, Qm_zz) (Qm_xy, Qm_xz, Qm_yz, nTh) (first, count, leaf, n3Th))
+// fp32 records per cell: what the walk tests (trec: com, r2open; tlink: first child / particle, count | leaf << 31) and what
+// the force loop consumes (erec, 48 B: (com, M) (Qm_xx, Qm_yy, Qm_zz, Qm_xy) (Qm_xz, Qm_yz, nTh, n3Th)),
 // with the opening radius of Eq.1:  l = longest side of the tight box (A14),
 // delta = |com - box centre|, r2open = (l / theta + delta)^2, all in single fp32 operations (O8).
 __global__ void __launch_bounds__(256) k_cell_record(const DevScalars* __restrict__ sc, float theta,
                                                      const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
                                                      const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
                                                      const double* __restrict__ mom64, const float* __restrict__ box,
-                                                     float4* __restrict__ rec, size_t rstride) {
+                                                     float4* __restrict__ trec, uint2* __restrict__ tlink, float4* __restrict__ erec) {
     const uint32_t nc = sc->n_cells;
     for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
         const double* m = mom64 + 10 * (size_t)c;
@@ -140,19 +141,17 @@ __global__ void __launch_bounds__(256) k_cell_record(const DevScalars* __restric
         const float r2open = __fmul_rn(ropen, ropen);
         const uint32_t cb = c_cbegin[c], ce = c_cend[c];
         const bool leaf = (ce == cb);
-        uint4 link;
+        uint2 link;
         link.x = leaf ? c_pbegin[c] : cb;
-        link.y = leaf ? (c_pend[c] - c_pbegin[c]) : (ce - cb);
-        link.z = leaf ? 1u : 0u;
-        link.w = 0u;
-        // walk record: what the force loop consumes, pre-scaled once: Qm = -3 Q, nTh = -T/2, n3Th = -3T/2 (T = trace of Q)
+        link.y = leaf ? ((c_pend[c] - c_pbegin[c]) | 0x80000000u) : (ce - cb);
+        // evaluation record, pre-scaled once: Qm = -3 Q, nTh = -T/2, n3Th = -3T/2 (T = trace of Q)
         const float qxx = (float)m[4], qyy = (float)m[5], qzz = (float)m[6], qxy = (float)m[7], qxz = (float)m[8], qyz = (float)m[9];
         const float T = (qxx + qyy) + qzz;
-        // four planes (structure of arrays): siblings are consecutive cells, so a popped run of them shares cache lines
-        rec[c] = make_float4(cx, cy, cz, r2open);
-        rec[rstride + c] = make_float4(M, -3.0f * qxx, -3.0f * qyy, -3.0f * qzz);
-        rec[2 * rstride + c] = make_float4(-3.0f * qxy, -3.0f * qxz, -3.0f * qyz, -0.5f * T);
-        rec[3 * rstride + c] = make_float4(__uint_as_float(link.x), __uint_as_float(link.y), __uint_as_float(link.z), -1.5f * T);
+        trec[c] = make_float4(cx, cy, cz, r2open);
+        tlink[c] = link;
+        erec[3 * (size_t)c] = make_float4(cx, cy, cz, M);
+        erec[3 * (size_t)c + 1] = make_float4(-3.0f * qxx, -3.0f * qyy, -3.0f * qzz, -3.0f * qxy);
+        erec[3 * (size_t)c + 2] = make_float4(-3.0f * qxz, -3.0f * qyz, -0.5f * T, -1.5f * T);
     }
 }
 
@@ -168,7 +167,7 @@ int stage_moments(bh_ctx* c, cudaStream_t s) {
 int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s) {
     const int grid = (int)std::min<int64_t>(div_up(c->max_cells, 256), (int64_t)c->sm_count * 16);
     BH_LAUNCH(c, k_cell_record, grid, 256, 0, s, c->ws.sc, theta, c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin, c->ws.c_cend,
-              c->ws.mom64, c->ws.box, c->ws.rec, (size_t)c->max_cells);
+              c->ws.mom64, c->ws.box, c->ws.trec, c->ws.tlink, c->ws.erec);
     return BH_OK;
 }
 

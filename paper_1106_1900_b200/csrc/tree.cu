@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(256) k_group_write(const uint8_t* __restrict__
 __global__ void __launch_bounds__(256) k_export(const DevScalars* __restrict__ sc, const uint64_t* __restrict__ key,
                                                 const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
                                                 const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
-                                                const uint32_t* __restrict__ c_parent, const float4* __restrict__ rec, const double* __restrict__ mom64,
+                                                const uint32_t* __restrict__ c_parent, const float4* __restrict__ trec, const double* __restrict__ mom64,
                                                 int32_t* __restrict__ e_level, uint64_t* __restrict__ e_prefix, uint32_t* __restrict__ e_pcount,
                                                 int32_t* __restrict__ e_cbegin, int32_t* __restrict__ e_nchild, int32_t* __restrict__ e_parent,
                                                 float* __restrict__ e_mom32, float* __restrict__ e_r2open) {
@@ -204,7 +204,7 @@ __global__ void __launch_bounds__(256) k_export(const DevScalars* __restrict__ s
         float* m = e_mom32 + 10 * (size_t)c;
 #pragma unroll
         for (int k = 0; k < 10; ++k) m[k] = (float)mom64[10 * (size_t)c + k];   // the fp32 roundings the walk record is built from
-        e_r2open[c] = rec[c].w;
+        e_r2open[c] = trec[c].w;
     }
 }
 
@@ -238,7 +238,7 @@ int stage_groups(bh_ctx* c, cudaStream_t s) {
 int stage_export(bh_ctx* c, cudaStream_t s) {
     const int grid = (int)std::min<int64_t>(div_up(c->max_cells, 256), (int64_t)c->sm_count * 16);
     BH_LAUNCH(c, k_export, grid, 256, 0, s, c->ws.sc, c->ws.key[c->sorted], c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin,
-              c->ws.c_cend, c->ws.c_parent, c->ws.rec, c->ws.mom64, c->ws.e_level, c->ws.e_prefix, c->ws.e_pcount, c->ws.e_cbegin,
+              c->ws.c_cend, c->ws.c_parent, c->ws.trec, c->ws.mom64, c->ws.e_level, c->ws.e_prefix, c->ws.e_pcount, c->ws.e_cbegin,
               c->ws.e_nchild, c->ws.e_parent, c->ws.e_mom32, c->ws.e_r2open);
     return BH_OK;
 }

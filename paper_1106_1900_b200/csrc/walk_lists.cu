@@ -1,0 +1,237 @@
+// walk_lists.cu -- S7: the group tree-walk with the MAC of Eq.1, writing the interaction lists.
+//
+// The paper keeps the two lists of a group in the shared memory of the block that also evaluates them (L83-87).  Here
+// the walk and the evaluation are two kernels with different shapes: the walk is a chain of dependent cache round trips
+// (pop -> load cell -> test -> push children) that wants many light warps per SM; the evaluation (walk_eval.cu) is a dense
+// FP32 loop that wants 128 registers per thread.  The lists travel through device memory as 4-byte indices -- 4 B against
+// ~20 x 64 flops per entry, i.e. nothing next to the arithmetic they feed.
+//
+// One warp walks one group; the eight warps of a block draw from a chunk of 32 CONSECUTIVE groups (Morton neighbours test
+// nearly the same cells, so the block's loads hit L1).  Per group:
+//   * frontier: a LIFO of OPENED NODES (first child, child count) in shared memory.  The paper walks breadth-first with two
+//     stacks of cells (L83-87); the interaction lists are SETS, so any traversal order produces the same lists and counts.
+//     A step pops up to four nodes and gives each of their (up to 8, consecutive) children to one lane: a node of the
+//     sparse octree has ~7.8 children, so the lanes are full and the eight records of a node arrive as one 128 B line.
+//     Depth-first popping bounds the frontier: the pop width shrinks when the stack nears its capacity and a reserve of
+//     7 x 20 + slack entries always admits a pure depth-first descent, so the stack cannot overflow.
+//   * each lane tests its cell with exactly the fp32 operations of DESIGN.md O9 (mac_accept).
+//   * accepted cells -> the group's cell list; opened nodes -> back onto the stack (one 8-byte entry, ballot-compacted);
+//     opened leaves -> a small queue that is expanded 32 leaves at a time into the group's particle list, minus the
+//     group's own particles (A19).
+// List memory: every warp owns an arena of the list buffer; cell lists grow upward from its bottom, particle lists
+// downward from its top, so both lists of a group are contiguous.  A group that does not fit is rolled back and handed
+// to the fused fallback kernel (walk.cu), so the capacity of the list buffer bounds memory, never correctness.
+#include "walk_common.cuh"
+
+namespace bh {
+
+constexpr int kListWarps = 8;
+constexpr int kListThreads = kListWarps * 32;
+constexpr int kLStackCap = 512;       // opened nodes
+constexpr int kLStackReserve = 160;   // >= 7 * 20 + 7: room for a pure depth-first descent
+constexpr int kLeafQueue = 64;
+constexpr int kGroupChunk = 32;       // consecutive groups a block claims at a time
+
+struct ListArena { uint32_t pc_top, pp_bot; };
+struct WalkSums { unsigned long long pc, pp, mac; };
+struct ListWarpShared {
+    uint2 stack[kLStackCap];
+    uint2 leafq[kLeafQueue];
+};
+
+// Expand `k` <= 32 queued leaves (entries q[0..k)) into the particle list, which grows downward from pp_bot.
+// Returns false if the list does not fit above pc_top.
+__device__ __forceinline__ bool flush_leaves(const uint2* q, int k, int lane, uint32_t gb, uint32_t ge, uint32_t* __restrict__ lists,
+                                             uint32_t pc_top, uint32_t& pp_bot, uint32_t& npp) {
+    uint32_t first = 0, cnt = 0;
+    if (lane < k) { const uint2 e = q[lane]; first = e.x; cnt = e.y; }
+    // [first, first + cnt) minus the group's own [gb, ge) = [first, a) and [b, first + cnt)
+    const uint32_t end = first + cnt;
+    const uint32_t a = min(end, max(first, gb));
+    const uint32_t b = max(first, min(end, ge));
+    const uint32_t n1 = a - first, kept = n1 + (end - b);
+    int total;
+    const int off = warp_excl_scan((int)kept, lane, total);
+    npp += __reduce_add_sync(0xFFFFFFFFu, cnt);
+    if ((uint32_t)total > pp_bot - pc_top) return false;
+    pp_bot -= (uint32_t)total;
+    uint32_t* dst = lists + pp_bot + off;
+#pragma unroll 4
+    for (uint32_t t = 0; t < kept; ++t) dst[t] = (t < n1) ? first + t : b + (t - n1);
+    return true;
+}
+
+__device__ __forceinline__ void list_group(ListWarpShared* ws, const int lane, const uint32_t g, const uint32_t gb, const uint32_t ge,
+                                           const float4* __restrict__ pos, const float4* __restrict__ trec, const uint2* __restrict__ tlink,
+                                           const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
+                                           const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
+                                           uint32_t* __restrict__ lists, ListArena& ar, WalkListOut o, WalkSums& sums) {
+    const uint32_t lt = (1u << lane) - 1u;
+    const int ng = (int)(ge - gb);
+    // ---- group box (A13).  A group that is a whole cell has that cell's box (exact min / max of the same particles);
+    //      a chunk of a level-20 overflow leaf takes it from its particles.
+    float mn[3], mx[3];
+    {
+        const uint32_t gc = __ldg(g_cell + g);
+        if (__ldg(c_pend + gc) - __ldg(c_pbegin + gc) == (uint32_t)ng) {
+            const float* b = box + 6 * (size_t)gc;
+            mn[0] = __ldg(b); mn[1] = __ldg(b + 1); mn[2] = __ldg(b + 2);
+            mx[0] = __ldg(b + 3); mx[1] = __ldg(b + 4); mx[2] = __ldg(b + 5);
+        } else {
+            group_box(pos, gb, ng, lane, nullptr, mn, mx);
+        }
+    }
+
+    const uint32_t pc0 = ar.pc_top, pp0 = ar.pp_bot;
+    uint32_t pc_top = pc0, pp_bot = pp0;
+    uint32_t npp = 0, nmac = 0;
+    bool fits = true;
+    int sp = 1, lq = 0;
+    if (lane == 0) ws->stack[0] = make_uint2(0u, 1u);   // the root (A17) as the only child of a virtual node
+    __syncwarp();
+
+    while (sp > 0) {
+        int kpop = (kLStackCap - kLStackReserve - sp) / 7;
+        kpop = max(1, min(kpop, 4));
+        kpop = min(kpop, sp);
+        const int r = lane >> 3;
+        bool valid = false, accept = false, isleaf = false, isnode = false;
+        uint32_t cell = 0;
+        uint2 lk = make_uint2(0u, 0u);
+        if (r < kpop) {
+            const uint2 e = ws->stack[sp - 1 - r];
+            valid = (uint32_t)(lane & 7) < e.y;
+            cell = e.x + (uint32_t)(lane & 7);
+        }
+        if (valid) {
+            const float4 r0 = __ldg(trec + cell);
+            lk = __ldg(tlink + cell);
+            accept = mac_accept(mn, mx, r0);
+            isleaf = !accept && (lk.y >> 31) != 0u;
+            isnode = !accept && !isleaf;
+        }
+        sp -= kpop;
+        __syncwarp();
+        nmac += (uint32_t)__popc(__ballot_sync(0xFFFFFFFFu, valid));
+        // ---- accepted cells -> cell list
+        const uint32_t amask = __ballot_sync(0xFFFFFFFFu, accept);
+        if (amask) {
+            const uint32_t na = (uint32_t)__popc(amask);
+            if (pc_top + na > pp_bot) { fits = false; break; }
+            if (accept) lists[pc_top + (uint32_t)__popc(amask & lt)] = cell;
+            pc_top += na;
+        }
+        // ---- opened nodes -> back onto the stack (kpop <= (cap - reserve - sp) / 7 guarantees room for 8 per popped node)
+        const uint32_t nmask = __ballot_sync(0xFFFFFFFFu, isnode);
+        if (isnode) ws->stack[sp + __popc(nmask & lt)] = lk;
+        sp += __popc(nmask);
+        // ---- opened leaves -> queue; expanded 32 at a time
+        const uint32_t lmask = __ballot_sync(0xFFFFFFFFu, isleaf);
+        if (lmask) {
+            if (isleaf) ws->leafq[lq + __popc(lmask & lt)] = make_uint2(lk.x, lk.y & 0x7FFFFFFFu);
+            lq += __popc(lmask);
+            __syncwarp();
+            if (lq >= 32) {
+                lq -= 32;
+                if (!flush_leaves(ws->leafq + lq, 32, lane, gb, ge, lists, pc_top, pp_bot, npp)) { fits = false; break; }
+            }
+        }
+        __syncwarp();
+    }
+    if (fits && lq > 0) fits = flush_leaves(ws->leafq, lq, lane, gb, ge, lists, pc_top, pp_bot, npp);
+
+    if (fits) {
+        ar.pc_top = pc_top;
+        ar.pp_bot = pp_bot;
+        if (lane == 0) {
+            o.g_pcoff[g] = pc0;
+            o.g_ppoff[g] = pp_bot;
+            o.g_lpp[g] = pp0 - pp_bot;
+            o.g_npc[g] = pc_top - pc0;
+            o.g_npp[g] = npp;
+        }
+        sums.pc += (unsigned long long)(pc_top - pc0) * (unsigned long long)ng;
+        sums.pp += (unsigned long long)npp * (unsigned long long)ng;
+        sums.mac += nmac;
+    } else if (lane == 0) {            // roll back; the fused kernel walks and evaluates this group
+        o.g_pcoff[g] = kNone;
+        o.deferred[atomicAdd(&o.ctl->n_deferred, 1u)] = g;
+    }
+    __syncwarp();
+}
+
+__global__ void __launch_bounds__(kListThreads, 5) k_walk_lists(WalkListOut o, int wave, const float4* __restrict__ pos,
+                                                                const float4* __restrict__ trec, const uint2* __restrict__ tlink,
+                                                                const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
+                                                                const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
+                                                                const uint32_t* __restrict__ g_begin, uint32_t* __restrict__ lists,
+                                                                uint32_t arena_entries) {
+    __shared__ ListWarpShared s_ws[kListWarps];
+    __shared__ uint32_t s_chunk, s_taken;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t g0 = o.ctl->wave_g[wave], g1 = o.ctl->wave_g[wave + 1];
+    ListArena ar;
+    ar.pc_top = (blockIdx.x * kListWarps + warp) * arena_entries;
+    ar.pp_bot = ar.pc_top + arena_entries;
+    WalkSums sums = {0ull, 0ull, 0ull};
+    for (;;) {
+        __syncthreads();               // everyone is done with the previous chunk's counters
+        if (threadIdx.x == 0) { s_chunk = atomicAdd(&o.ctl->list_next[wave], (uint32_t)kGroupChunk); s_taken = 0; }
+        __syncthreads();
+        const uint32_t base = g0 + s_chunk;
+        if (base >= g1) break;
+        const uint32_t nchunk = min((uint32_t)kGroupChunk, g1 - base);
+        for (;;) {
+            uint32_t i = 0;
+            if (lane == 0) i = atomicAdd(&s_taken, 1u);
+            i = __shfl_sync(0xFFFFFFFFu, i, 0);
+            if (i >= nchunk) break;
+            const uint32_t g = base + i;
+            const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
+            list_group(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
+        }
+    }
+    if (lane == 0 && sums.mac) {
+        atomicAdd(&o.sc->sum_pc, sums.pc);
+        atomicAdd(&o.sc->sum_pp, sums.pp);
+        atomicAdd(&o.sc->sum_mac, sums.mac);
+    }
+}
+
+// Wave boundaries (first group whose first particle is >= w * wave_particles) and counter reset: one tiny launch per walk.
+__global__ void k_walk_prepare(DevScalars* sc, WalkCtl* ctl, const uint32_t* __restrict__ g_begin, int nwaves, uint32_t wave_particles) {
+    const int t = threadIdx.x;
+    const uint32_t G = sc->n_groups;
+    if (t <= nwaves) {
+        uint32_t lo = 0, hi = G;           // lower_bound of t * wave_particles in g_begin[0..G)
+        const unsigned long long target = (unsigned long long)t * wave_particles;
+        if (t == nwaves) lo = G;
+        else
+            while (lo < hi) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if ((unsigned long long)g_begin[mid] < target) lo = mid + 1; else hi = mid;
+            }
+        ctl->wave_g[t] = lo;
+        ctl->list_next[t] = 0;
+        ctl->eval_next[t] = 0;
+    }
+    if (t == 0) {
+        ctl->n_deferred = 0;
+        ctl->fused_next = 0;
+        sc->sum_pc = 0; sc->sum_pp = 0; sc->sum_mac = 0;
+    }
+}
+
+int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t arena_entries, cudaStream_t s) {
+    WalkListOut o = walk_list_out(c);
+    BH_LAUNCH(c, k_walk_lists, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
+              c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, arena_entries);
+    return BH_OK;
+}
+
+int stage_walk_prepare(bh_ctx* c, int nwaves, uint32_t wave_particles, cudaStream_t s) {
+    BH_LAUNCH(c, k_walk_prepare, 1, kMaxWaves + 1, 0, s, c->ws.sc, c->ws.ctl, c->ws.g_begin, nwaves, wave_particles);
+    return BH_OK;
+}
+
+}  // namespace bh

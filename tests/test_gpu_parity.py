@@ -47,6 +47,19 @@ def test_parity_other_opening_angles_and_softening(BH, theta, eps):
     _full_parity(BH, pm, vel, theta, eps)
 
 
+@pytest.mark.parametrize("cfg", [dict(walk_mode=1), dict(list_entries=3000), dict(list_entries=40000), dict(list_entries=1)])
+def test_walk_paths_agree(BH, cfg):
+    """Fused kernel only; list buffer too small for most / some / all groups (deferred to the fused kernel): same counts, same forces."""
+    pm, vel, prm = bh_inputs.make("c1", n=6000, seed=13)
+    _full_parity(BH, pm, vel, prm["theta"], prm["eps"], **cfg)
+
+
+def test_walk_in_several_waves(BH):
+    """A list buffer that forces several waves (contiguous particle ranges walked and evaluated one after the other)."""
+    pm, vel, prm = bh_inputs.make("c1", n=40000, seed=17)
+    _full_parity(BH, pm, vel, prm["theta"], prm["eps"], list_entries=1 << 20)
+
+
 @pytest.mark.parametrize("n", [1, 2, 16, 17, 64, 65])
 def test_tiny_inputs(BH, n):
     pm, vel, prm = bh_inputs.make("c1", n=n, seed=11)
