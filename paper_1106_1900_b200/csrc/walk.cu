@@ -153,7 +153,7 @@ __device__ __noinline__ void walk_group(WarpShared* ws, const int lane, const ui
                 pp_cnt += __popc(kmask);
                 __syncwarp();
                 if (pp_cnt >= 32) {
-                    eval_pp_all<false, kRingPairs>(ws->pp, ws->own, ws->tot, pp_head >> 1, 16, m, ng, k, lane);
+                    eval_pp_all<false, kRingPairs, true>(ws->pp, ws->own, ws->tot, pp_head >> 1, 16, m, ng, k, lane);
                     pp_head = (pp_head + 32) & (kRing - 1);
                     pp_cnt -= 32;
                     __syncwarp();
@@ -162,7 +162,7 @@ __device__ __noinline__ void walk_group(WarpShared* ws, const int lane, const ui
             __syncwarp();
         }
         if (pc_cnt >= 32) {
-            eval_pc_all<kRingPairs>(ws->pc, ws->own, ws->tot, pc_head >> 1, 16, m, ng, k, lane);
+            eval_pc_all<kRingPairs, true, false>(ws->pc, ws->own, ws->tot, pc_head >> 1, 16, m, ng, k, lane);
             pc_head = (pc_head + 32) & (kRing - 1);
             pc_cnt -= 32;
             __syncwarp();
@@ -172,12 +172,12 @@ __device__ __noinline__ void walk_group(WarpShared* ws, const int lane, const ui
     if (pc_cnt > 0) {
         if ((pc_cnt & 1) && lane == 0) pc_pad(ws->pc, (pc_head + pc_cnt - 1) & (kRing - 1));
         __syncwarp();
-        eval_pc_all<kRingPairs>(ws->pc, ws->own, ws->tot, pc_head >> 1, (pc_cnt + 1) >> 1, m, ng, k, lane);
+        eval_pc_all<kRingPairs, true, false>(ws->pc, ws->own, ws->tot, pc_head >> 1, (pc_cnt + 1) >> 1, m, ng, k, lane);
     }
     if (pp_cnt > 0) {
         if ((pp_cnt & 1) && lane == 0) pp_pad(ws->pp, (pp_head + pp_cnt - 1) & (kRing - 1));
         __syncwarp();
-        eval_pp_all<false, kRingPairs>(ws->pp, ws->own, ws->tot, pp_head >> 1, (pp_cnt + 1) >> 1, m, ng, k, lane);
+        eval_pp_all<false, kRingPairs, true>(ws->pp, ws->own, ws->tot, pp_head >> 1, (pp_cnt + 1) >> 1, m, ng, k, lane);
     }
     __syncwarp();
     // ---- self block: the group's own particles, entry j = target index j, j != i
@@ -189,7 +189,7 @@ __device__ __noinline__ void walk_group(WarpShared* ws, const int lane, const ui
     __syncwarp();
     if ((ng & 1) && lane == 0) pp_pad(ws->pp, ng - 1);
     __syncwarp();
-    eval_pp_all<true, kRingPairs>(ws->pp, ws->own, ws->tot, 0, (ng + 1) >> 1, m, ng, k, lane);
+    eval_pp_all<true, kRingPairs, true>(ws->pp, ws->own, ws->tot, 0, (ng + 1) >> 1, m, ng, k, lane);
     __syncwarp();
     totals_finish(ws->tot, m, lane, ng, gb, acc_out);
     __syncwarp();

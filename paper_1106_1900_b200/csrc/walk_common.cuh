@@ -62,16 +62,6 @@ __device__ __forceinline__ Consts make_consts(float eps2) {
 
 struct Acc2 { f2 ax, ay, az, p; };
 
-__device__ __forceinline__ void acc_flush(float4* tot, const Acc2& a) {
-    float4 t = *tot;
-    float lo, hi;
-    upk(a.ax, lo, hi); t.x += lo + hi;
-    upk(a.ay, lo, hi); t.y += lo + hi;
-    upk(a.az, lo, hi); t.z += lo + hi;
-    upk(a.p, lo, hi); t.w += lo + hi;
-    *tot = t;
-}
-
 // One pair of p-c entries on one target.  With rho^2 = |dr|^2 + eps^2, u = 1/rho^2, q = Qm dr = -3 Q dr, w = dr.q:
 //   -phi += (1/rho)   (M + u (nTh - w u / 2))
 //   a    += (1/rho^5) (q + dr (M rho^2 + n3Th - 5 w u / 2))
@@ -94,9 +84,28 @@ __device__ __forceinline__ void pc_one(const ulonglong2& v0, const ulonglong2& v
     a.az = fma2(fma2(dz, c, qz), ri5, a.az);
 }
 
-// p-c sweep of one slot over `npairs` ring pairs starting at pair `hp` of a ring of `kPairs` pairs (power of two).
-// Lane: targets t0, t1; pairs sub, sub + S, ...
-template <int kPairs>
+// Running sums <-> packed accumulators: a sweep starts from (total, 0) and stores low + high, so the only extra
+// arithmetic per slot and sweep is one add per component.
+__device__ __forceinline__ Acc2 acc_load(const float4* tot) {
+    const float4 t = *tot;
+    Acc2 a;
+    a.ax = pk(t.x, 0.f); a.ay = pk(t.y, 0.f); a.az = pk(t.z, 0.f); a.p = pk(t.w, 0.f);
+    return a;
+}
+__device__ __forceinline__ void acc_store(float4* tot, const Acc2& a) {
+    float4 t;
+    float lo, hi;
+    upk(a.ax, lo, hi); t.x = lo + hi;
+    upk(a.ay, lo, hi); t.y = lo + hi;
+    upk(a.az, lo, hi); t.z = lo + hi;
+    upk(a.p, lo, hi); t.w = lo + hi;
+    *tot = t;
+}
+
+// p-c sweep of one slot over `npairs` ring pairs starting at pair `hp` of a ring of `kPairs` pairs (power of two; the
+// ring never wraps when kWrap is false).  Lane: targets t0, t1; pairs sub, sub + S, ...  kUnroll2: two pairs per
+// iteration (four independent interaction chains per lane hide the rsqrt and FMA latencies with few resident warps).
+template <int kPairs, bool kWrap, bool kUnroll2>
 __device__ __forceinline__ void eval_pc_slot(const float* ring, const float4* own, SlotTotals* tot, int hp, int npairs, int K, int tbase,
                                              int slot, int ng, const Consts& k, int lane) {
     const int L = 1 << (K - 1), sub = lane >> (K - 1), S = 32 >> (K - 1);
@@ -104,15 +113,28 @@ __device__ __forceinline__ void eval_pc_slot(const float* ring, const float4* ow
     const float4 T0 = own[min(t0, ng - 1)], T1 = own[min(t1, ng - 1)];   // idle targets shadow the last particle
     const f2 ntx0 = pk(-T0.x, -T0.x), nty0 = pk(-T0.y, -T0.y), ntz0 = pk(-T0.z, -T0.z);
     const f2 ntx1 = pk(-T1.x, -T1.x), nty1 = pk(-T1.y, -T1.y), ntz1 = pk(-T1.z, -T1.z);
-    Acc2 a0 = {0ull, 0ull, 0ull, 0ull}, a1 = {0ull, 0ull, 0ull, 0ull};
-    for (int p = sub; p < npairs; p += S) {
-        const ulonglong2* src = reinterpret_cast<const ulonglong2*>(ring + ((hp + p) & (kPairs - 1)) * kPcPair);
+    Acc2 a0 = acc_load(&tot[slot][0][lane]), a1 = acc_load(&tot[slot][1][lane]);
+    int p = sub;
+    if (kUnroll2) {
+        for (; p + S < npairs; p += 2 * S) {
+            const ulonglong2* sa = reinterpret_cast<const ulonglong2*>(ring + (kWrap ? ((hp + p) & (kPairs - 1)) : (hp + p)) * kPcPair);
+            const ulonglong2* sb = reinterpret_cast<const ulonglong2*>(ring + (kWrap ? ((hp + p + S) & (kPairs - 1)) : (hp + p + S)) * kPcPair);
+            const ulonglong2 v0 = sa[0], v1 = sa[1], v2 = sa[2], v3 = sa[3], v4 = sa[4], v5 = sa[5];
+            const ulonglong2 w0 = sb[0], w1 = sb[1], w2 = sb[2], w3 = sb[3], w4 = sb[4], w5 = sb[5];
+            pc_one(v0, v1, v2, v3, v4, v5, ntx0, nty0, ntz0, k, a0);
+            pc_one(v0, v1, v2, v3, v4, v5, ntx1, nty1, ntz1, k, a1);
+            pc_one(w0, w1, w2, w3, w4, w5, ntx0, nty0, ntz0, k, a0);
+            pc_one(w0, w1, w2, w3, w4, w5, ntx1, nty1, ntz1, k, a1);
+        }
+    }
+    for (; p < npairs; p += S) {
+        const ulonglong2* src = reinterpret_cast<const ulonglong2*>(ring + (kWrap ? ((hp + p) & (kPairs - 1)) : (hp + p)) * kPcPair);
         const ulonglong2 v0 = src[0], v1 = src[1], v2 = src[2], v3 = src[3], v4 = src[4], v5 = src[5];
         pc_one(v0, v1, v2, v3, v4, v5, ntx0, nty0, ntz0, k, a0);
         pc_one(v0, v1, v2, v3, v4, v5, ntx1, nty1, ntz1, k, a1);
     }
-    acc_flush(&tot[slot][0][lane], a0);
-    acc_flush(&tot[slot][1][lane], a1);
+    acc_store(&tot[slot][0][lane], a0);
+    acc_store(&tot[slot][1][lane], a1);
 }
 
 // p-p, one pair of entries on one target.  kSelf: the ring holds the group's own `ng` particles from entry 0 and entry j is
@@ -142,7 +164,7 @@ __device__ __forceinline__ void pp_one(const ulonglong2& v0, const ulonglong2& v
     a.az = fma2(dz, mr3, a.az);
 }
 
-template <bool kSelf, int kPairs>
+template <bool kSelf, int kPairs, bool kWrap>
 __device__ __forceinline__ void eval_pp_slot(const float* ring, const float4* own, SlotTotals* tot, int hp, int npairs, int K, int tbase,
                                              int slot, int ng, const Consts& k, int lane) {
     const int L = 1 << (K - 1), sub = lane >> (K - 1), S = 32 >> (K - 1);
@@ -150,34 +172,34 @@ __device__ __forceinline__ void eval_pp_slot(const float* ring, const float4* ow
     const float4 T0 = own[min(t0, ng - 1)], T1 = own[min(t1, ng - 1)];
     const f2 ntx0 = pk(-T0.x, -T0.x), nty0 = pk(-T0.y, -T0.y), ntz0 = pk(-T0.z, -T0.z);
     const f2 ntx1 = pk(-T1.x, -T1.x), nty1 = pk(-T1.y, -T1.y), ntz1 = pk(-T1.z, -T1.z);
-    Acc2 a0 = {0ull, 0ull, 0ull, 0ull}, a1 = {0ull, 0ull, 0ull, 0ull};
+    Acc2 a0 = acc_load(&tot[slot][0][lane]), a1 = acc_load(&tot[slot][1][lane]);
     for (int p = sub; p < npairs; p += S) {
-        const ulonglong2* src = reinterpret_cast<const ulonglong2*>(ring + ((hp + p) & (kPairs - 1)) * kPpPair);
+        const ulonglong2* src = reinterpret_cast<const ulonglong2*>(ring + (kWrap ? ((hp + p) & (kPairs - 1)) : (hp + p)) * kPpPair);
         const ulonglong2 v0 = src[0], v1 = src[1];
         pp_one<kSelf>(v0, v1, ntx0, nty0, ntz0, k, a0, 2 * p, t0, ng);
         pp_one<kSelf>(v0, v1, ntx1, nty1, ntz1, k, a1, 2 * p, t1, ng);
     }
-    acc_flush(&tot[slot][0][lane], a0);
-    acc_flush(&tot[slot][1][lane], a1);
+    acc_store(&tot[slot][0][lane], a0);
+    acc_store(&tot[slot][1][lane], a1);
 }
 
 // The slots of a group are the set bits K = 6 (alone) or 5..2 of m = roundup4(n): a slot of 2^K targets each.  They are
 // enumerated on the fly (slot index = rank of the bit from the top, first target = sum of the higher bits).
-template <int kPairs>
+template <int kPairs, bool kWrap, bool kUnroll2>
 __device__ __forceinline__ void eval_pc_all(const float* ring, const float4* own, SlotTotals* tot, int hp, int npairs, int m, int ng,
                                             const Consts& k, int lane) {
     int slot = 0, base = 0;
 #pragma unroll
     for (int K = 6; K >= 2; --K)
-        if (m & (1 << K)) { eval_pc_slot<kPairs>(ring, own, tot, hp, npairs, K, base, slot, ng, k, lane); ++slot; base += 1 << K; }
+        if (m & (1 << K)) { eval_pc_slot<kPairs, kWrap, kUnroll2>(ring, own, tot, hp, npairs, K, base, slot, ng, k, lane); ++slot; base += 1 << K; }
 }
-template <bool kSelf, int kPairs>
+template <bool kSelf, int kPairs, bool kWrap>
 __device__ __forceinline__ void eval_pp_all(const float* ring, const float4* own, SlotTotals* tot, int hp, int npairs, int m, int ng,
                                             const Consts& k, int lane) {
     int slot = 0, base = 0;
 #pragma unroll
     for (int K = 6; K >= 2; --K)
-        if (m & (1 << K)) { eval_pp_slot<kSelf, kPairs>(ring, own, tot, hp, npairs, K, base, slot, ng, k, lane); ++slot; base += 1 << K; }
+        if (m & (1 << K)) { eval_pp_slot<kSelf, kPairs, kWrap>(ring, own, tot, hp, npairs, K, base, slot, ng, k, lane); ++slot; base += 1 << K; }
 }
 
 __device__ __forceinline__ void totals_clear(SlotTotals* tot, int lane) {
