@@ -1,13 +1,24 @@
 // walk_eval.cu -- S8: evaluation of the interaction lists written by walk_lists.cu.
 //
 // One warp owns one group at a time (groups are independent units of work) and pulls the next group from a
-// device counter.  The lists are streamed in batches of 128 entries ("Nblock"):
-//   * the indices of batch b + 2 are loaded while the records of batch b + 1 are in flight and batch b is evaluated;
-//   * records (48 B per accepted cell, 16 B per particle) are gathered with cp.async (LDGSTS) straight into a raw
-//     shared-memory buffer -- no registers are held across the sweep, and the gather's L2 latency hides behind arithmetic;
-//   * the raw records are then transposed into the pair-interleaved ring the packed FFMA2 sweep reads
-//     (walk_common.cuh): entry p is paired with entry p + ceil(k/2) of a batch of k, an odd tail gets a massless partner.
-// The group's own particles form the last, "self" block with j != i (A19).
+// device counter.  What differs from the paper's one-thread-per-particle sweep, and why:
+//   (1) FP32 rate.  On sm_100a the full 128 FP32 lanes/clk/SM need the packed forms FFMA2 / FMUL2 / FADD2; a scalar
+//       FFMA issues at half rate.  A 64-bit register here holds TWO TARGETS (particles of the group); the list entry is
+//       a scalar operand that the packed instructions broadcast to both halves (the `.F32` operand form of the SASS), so
+//       the records are used exactly as they sit in memory: no pairing of entries, no transposition, no padding entry.
+//   (2) Lane use.  A group holds ng <= 64 targets (mean ~19; work-weighted mean ~27).  A lane serves R = 2, 4 or 6
+//       targets (R/2 packed registers per coordinate); L = ceil(ng / R) lanes cover the group, and the warp is split into
+//       S = floor(32 / L) such teams, each sweeping every S-th entry of the list ("up to 4 threads per particle",
+//       PAPER.md:81, 97, taken to its end).  R is chosen per group to maximise the useful lanes ng S / (32 R) (c2: 91 %).
+//       The sums stay in registers for the whole group; the S partial sums per target are added once, through shared
+//       memory, in a fixed order (deterministic).
+//   (3) Shared-memory delivery.  An entry costs three LDS.128 per lane whatever R is, so R = 4 or 6 halves or thirds the
+//       shared-memory traffic per interaction; R = 2 sweeps two entries per iteration for independent work instead.
+//   (4) The lists are streamed in batches of 128 entries ("Nblock"): the indices of batch b + 2 are loaded
+//       and the records of batch b + 1 are gathered by cp.async (LDGSTS) into the other half of a double buffer while
+//       batch b is swept; no registers are held across the sweep and the gather's L2 latency hides behind arithmetic.
+// The group's own particles form the last batch, with j != i (A19).
+// Forces: DESIGN.md O10 -- 33 packed operations + 2 MUFU.RSQ per entry and target pair (p-c), 13 + 2 (p-p).
 #include <algorithm>
 #include "walk_common.cuh"
 
@@ -15,16 +26,13 @@ namespace bh {
 
 constexpr int kEvalWarps = 4;
 constexpr int kEvalThreads = kEvalWarps * 32;
-constexpr int kEvalBlocksPerSM = 3;          // 12 warps / SM at up to 168 registers: few, fat warps (two pairs in flight per lane)
-constexpr int kBatch = 128;                  // list entries per sweep
-constexpr int kBatchPairs = kBatch / 2;
+constexpr int kEvalBlocksPerSM = 4;          // 16 warps / SM at <= 128 registers
+constexpr int kBatch = 128;                  // list entries per batch
 constexpr int kPerLane = kBatch / 32;        // entries a lane gathers per batch
 
 struct __align__(16) EvalShared {
-    float ring[kBatchPairs * kPcPair];       // pair-interleaved operands of the current batch (p-c: 112 B / pair; p-p: 32 B / pair)
-    float4 raw[kBatch * 3];                  // cp.async landing zone: 3 x float4 per cell, 1 x float4 per particle
-    float4 own[64];                          // the group's particles (targets; sources of the self block)
-    SlotTotals tot[kMaxSlots];
+    float4 buf[2][kBatch * 3];               // cp.async landing zones: 3 x float4 per cell, 1 x float4 per particle
+    float tx[64], ty[64], tz[64];            // negated target coordinates: a lane reads its pairs with one 64-bit load each
 };
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
@@ -34,124 +42,209 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-struct Idx { uint32_t v[kPerLane]; };
+__device__ __forceinline__ f2 bc(float s) { return pk(s, s); }   // ptxas folds this into the broadcast operand form
 
-// A list (kPc: accepted cells, 48 B records; else: particles, 16 B) is streamed through raw -> ring -> sweep.
-template <bool kPc>
-__device__ __forceinline__ void load_idx(const uint32_t* __restrict__ list, int n, int b, int lane, Idx& ix) {
-#pragma unroll
-    for (int j = 0; j < kPerLane; ++j) {
-        const int e = b * kBatch + j * 32 + lane;
-        if (e < n) ix.v[j] = __ldg(list + e);
-    }
-}
-template <bool kPc>
-__device__ __forceinline__ void issue(EvalShared* ws, const float4* __restrict__ src, int n, int b, int lane, const Idx& ix) {
-#pragma unroll
-    for (int j = 0; j < kPerLane; ++j) {
-        const int le = j * 32 + lane;
-        if (b * kBatch + le < n) {
-            if (kPc) {
-                const float4* s = src + 3 * (size_t)ix.v[j];
-                float4* d = ws->raw + 3 * le;
-                cp_async16(d, s); cp_async16(d + 1, s + 1); cp_async16(d + 2, s + 2);
-            } else {
-                cp_async16(ws->raw + le, src + ix.v[j]);
-            }
-        }
-    }
-    cp_async_commit();
-}
-// raw -> ring: pair p = (entry p, entry p + h) of a batch of len entries, h = ceil(len / 2); an odd tail gets a massless
-// partner at its own position (a position no target can coincide with).
-template <bool kPc>
-__device__ __forceinline__ void transpose(EvalShared* ws, int len, int h, int lane) {
-#pragma unroll
-    for (int j = 0; j < kBatchPairs / 32; ++j) {
-        const int p = j * 32 + lane;
-        if (p < h) {
-            const bool two = p + h < len;
-            if (kPc) {
-                const float4* a = ws->raw + 3 * p;
-                const float4* b = ws->raw + 3 * (p + h);
-                const float4 a0 = a[0], a1 = a[1], a2 = a[2];
-                float4 b0 = make_float4(a0.x, a0.y, a0.z, 0.f), b1 = make_float4(0.f, 0.f, 0.f, 0.f), b2 = b1;
-                if (two) { b0 = b[0]; b1 = b[1]; b2 = b[2]; }
-                float4* d = reinterpret_cast<float4*>(ws->ring + p * kPcPair);
-                d[0] = make_float4(a0.x, b0.x, a0.y, b0.y);
-                d[1] = make_float4(a0.z, b0.z, a0.w, b0.w);
-                d[2] = make_float4(a1.x, b1.x, a1.y, b1.y);
-                d[3] = make_float4(a1.z, b1.z, a1.w, b1.w);
-                d[4] = make_float4(a2.x, b2.x, a2.y, b2.y);
-                d[5] = make_float4(a2.z, b2.z, a2.w, b2.w);
-            } else {
-                const float4 a0 = ws->raw[p];
-                float4 b0 = make_float4(a0.x, a0.y, a0.z, 0.f);
-                if (two) b0 = ws->raw[p + h];
-                float4* d = reinterpret_cast<float4*>(ws->ring + p * kPpPair);
-                d[0] = make_float4(a0.x, b0.x, a0.y, b0.y);
-                d[1] = make_float4(a0.z, b0.z, a0.w, b0.w);
-            }
-        }
-    }
+// One p-c entry on one packed pair of targets.  Record: v0 = (com, M), v1 = (Qm_xx, Qm_yy, Qm_zz, Qm_xy),
+// v2 = (Qm_xz, Qm_yz, nTh, n3Th) with Qm = -3 Q, nTh = -T/2, n3Th = -3T/2.  rho^2 = |dr|^2 + eps^2, u = 1/rho^2,
+// q = Qm dr, w = dr.q:   -phi += (1/rho) (M + u (nTh - w u / 2)),   a += (1/rho^5) (q + dr (M rho^2 + n3Th - 5 w u / 2)).
+__device__ __forceinline__ void pc_bc(const float4& v0, const float4& v1, const float4& v2, f2 ntx, f2 nty, f2 ntz, const Consts& k, Acc2& a) {
+    const f2 dx = add2(bc(v0.x), ntx), dy = add2(bc(v0.y), nty), dz = add2(bc(v0.z), ntz);
+    const f2 r2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, k.e2)));
+    const f2 ri = rsqrt2(r2);
+    const f2 u = mul2(ri, ri), uu = mul2(u, u), ri5 = mul2(ri, uu);
+    const f2 qx = fma2(bc(v1.x), dx, fma2(bc(v1.w), dy, mul2(bc(v2.x), dz)));
+    const f2 qy = fma2(bc(v1.w), dx, fma2(bc(v1.y), dy, mul2(bc(v2.y), dz)));
+    const f2 qz = fma2(bc(v2.x), dx, fma2(bc(v2.y), dy, mul2(bc(v1.z), dz)));
+    const f2 w = fma2(dx, qx, fma2(dy, qy, mul2(dz, qz)));
+    const f2 wu = mul2(w, u);
+    a.p = fma2(ri, fma2(u, fma2(wu, k.mhalf, bc(v2.z)), bc(v0.w)), a.p);
+    const f2 c = fma2(bc(v0.w), r2, fma2(wu, k.m2p5, bc(v2.w)));
+    a.ax = fma2(fma2(dx, c, qx), ri5, a.ax);
+    a.ay = fma2(fma2(dy, c, qy), ri5, a.ay);
+    a.az = fma2(fma2(dz, c, qz), ri5, a.az);
 }
 
+// One p-p entry on one packed pair of targets tA, tA + 1.  kSelf: the entry is particle `e` of the group itself: skip
+// e == target (A19) and the shadow targets >= ng (they sit ON a real particle: r = 0 would give 0 * inf when eps = 0).
+template <bool kSelf>
+__device__ __forceinline__ void pp_bc(const float4& v, f2 ntx, f2 nty, f2 ntz, const Consts& k, Acc2& a, int e, int tA, int ng) {
+    const f2 dx = add2(bc(v.x), ntx), dy = add2(bc(v.y), nty), dz = add2(bc(v.z), ntz);
+    const f2 r2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, k.e2)));
+    f2 ri;
+    if (kSelf) {
+        float lo, hi;
+        upk(r2, lo, hi);
+        lo = (e == tA || tA >= ng) ? 0.0f : rsqrt_approx(lo);
+        hi = (e == tA + 1 || tA + 1 >= ng) ? 0.0f : rsqrt_approx(hi);
+        ri = pk(lo, hi);
+    } else {
+        ri = rsqrt2(r2);
+    }
+    const f2 ri2 = mul2(ri, ri);
+    const f2 mr = mul2(bc(v.w), ri);
+    const f2 mr3 = mul2(mr, ri2);
+    a.p = add2(a.p, mr);
+    a.ax = fma2(dx, mr3, a.ax);
+    a.ay = fma2(dy, mr3, a.ay);
+    a.az = fma2(dz, mr3, a.az);
+}
+
+// The evaluation of one group with R = 2 * R2 targets per lane.  Batches: nbpc of accepted cells, nbpp of particles of
+// opened leaves, then the group's own particles.
+template <int R2>
 __device__ __forceinline__ void eval_group(EvalShared* ws, const int lane, const uint32_t gb, const int ng, const float4* __restrict__ pos,
                                            const float4* __restrict__ erec, const uint32_t* __restrict__ lpc, const int npc,
                                            const uint32_t* __restrict__ lpp, const int npp, const Consts& k, float4* __restrict__ acc_out) {
+    constexpr int R = 2 * R2;
+    constexpr int U = R2 == 1 ? 2 : 1;           // entries per iteration: two independent chains per lane in every case but R2 = 3 (three)
+    const int L = (ng + R - 1) / R, S = 32 / L;
+    const int team = lane / L, tl = lane - team * L;
+    const bool active = team < S;
+    const int t0 = tl * R;                       // first target of this lane
+    f2 ntx[R2], nty[R2], ntz[R2];
+    Acc2 a[R2];
+    // targets: staged through shared memory so that every packed pair arrives in an aligned register pair (one LDS.64)
 #pragma unroll
-    for (int t = 0; t < 2; ++t) {
-        const int idx = lane + 32 * t;
-        if (idx < ng) ws->own[idx] = __ldg(pos + gb + idx);
+    for (int h = 0; h < 2; ++h) {
+        const int t = lane + 32 * h;
+        const float4 P = __ldg(pos + gb + min(t, ng - 1));   // idle targets shadow the last particle
+        ws->tx[t] = -P.x; ws->ty[t] = -P.y; ws->tz[t] = -P.z;
     }
-    const int m = (ng + 3) & ~3;
-    totals_clear(ws->tot, lane);
+    __syncwarp();
+#pragma unroll
+    for (int j = 0; j < R2; ++j) {
+        const int t = min(t0 + 2 * j, 62);
+        ntx[j] = *reinterpret_cast<const f2*>(ws->tx + t);
+        nty[j] = *reinterpret_cast<const f2*>(ws->ty + t);
+        ntz[j] = *reinterpret_cast<const f2*>(ws->tz + t);
+        a[j].ax = a[j].ay = a[j].az = a[j].p = 0ull;
+    }
     const int nbpc = (npc + kBatch - 1) / kBatch, nbpp = (npp + kBatch - 1) / kBatch;
+    const int nb = nbpc + nbpp + 1;
+    const int e0 = active ? team : (1 << 28);    // idle lanes (32 - S L of them) skip the sweeps
 
-    Idx ix, ixp;
-    load_idx<true>(lpc, npc, 0, lane, ix);
-    load_idx<false>(lpp, npp, 0, lane, ixp);
-    __syncwarp();                      // `own`, `tot` visible; the previous group's sweeps are done with ring / raw
-    if (nbpc > 0) issue<true>(ws, erec, npc, 0, lane, ix); else issue<false>(ws, pos, npp, 0, lane, ixp);
-    load_idx<true>(lpc, npc, 1, lane, ix);
-    // ---- accepted cells
-    for (int b = 0; b < nbpc; ++b) {
-        const int len = min(kBatch, npc - kBatch * b), h = (len + 1) >> 1;
-        cp_async_wait_all();
-        __syncwarp();
-        transpose<true>(ws, len, h, lane);
-        __syncwarp();
-        // request the next batch, then sweep this one while those copies are in flight
-        if (b + 1 < nbpc) { issue<true>(ws, erec, npc, b + 1, lane, ix); load_idx<true>(lpc, npc, b + 2, lane, ix); }
-        else issue<false>(ws, pos, npp, 0, lane, ixp);
-        eval_pc_all<kBatchPairs, false, true>(ws->ring, ws->own, ws->tot, 0, h, m, ng, k, lane);
-        __syncwarp();
-    }
-    // ---- particles of opened leaves
-    if (nbpp > 1) load_idx<false>(lpp, npp, 1, lane, ixp);
-    for (int b = 0; b < nbpp; ++b) {
-        const int len = min(kBatch, npp - kBatch * b), h = (len + 1) >> 1;
-        cp_async_wait_all();
-        __syncwarp();
-        transpose<false>(ws, len, h, lane);
-        __syncwarp();
-        if (b + 1 < nbpp) { issue<false>(ws, pos, npp, b + 1, lane, ixp); load_idx<false>(lpp, npp, b + 2, lane, ixp); }
-        eval_pp_all<false, kBatchPairs, false>(ws->ring, ws->own, ws->tot, 0, h, m, ng, k, lane);
-        __syncwarp();
-    }
-    cp_async_wait_all();
-    // ---- self block: the group's own particles, entry j = target index j, j != i
+    uint32_t ix[kPerLane];
+    // indices of batch b (cells, particles, or the group's own particles)
+    auto load_idx = [&](int b) {
+        if (b < nbpc) {
 #pragma unroll
-    for (int t = 0; t < 2; ++t) {
-        const int idx = lane + 32 * t;
-        if (idx < ng) { const float4 p = ws->own[idx]; pp_store(ws->ring, idx, p.x, p.y, p.z, p.w); }
+            for (int j = 0; j < kPerLane; ++j) { const int e = b * kBatch + j * 32 + lane; if (e < npc) ix[j] = __ldg(lpc + e); }
+        } else if (b < nbpc + nbpp) {
+#pragma unroll
+            for (int j = 0; j < kPerLane; ++j) { const int e = (b - nbpc) * kBatch + j * 32 + lane; if (e < npp) ix[j] = __ldg(lpp + e); }
+        } else {
+#pragma unroll
+            for (int j = 0; j < kPerLane; ++j) ix[j] = gb + (uint32_t)(j * 32 + lane);
+        }
+    };
+    auto batch_len = [&](int b) { return b < nbpc ? min(kBatch, npc - kBatch * b) : b < nbpc + nbpp ? min(kBatch, npp - kBatch * (b - nbpc)) : ng; };
+    // gather the records of batch b into half b & 1 of the buffer
+    auto issue = [&](int b) {
+        float4* dst = ws->buf[b & 1];
+        const int len = batch_len(b);
+        if (b < nbpc) {
+#pragma unroll
+            for (int j = 0; j < kPerLane; ++j) {
+                const int le = j * 32 + lane;
+                if (le < len) {
+                    const float4* s = erec + 3 * (size_t)ix[j];
+                    float4* d = dst + 3 * le;
+                    cp_async16(d, s); cp_async16(d + 1, s + 1); cp_async16(d + 2, s + 2);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < kPerLane; ++j) {
+                const int le = j * 32 + lane;
+                if (le < len) cp_async16(dst + le, pos + ix[j]);
+            }
+        }
+        cp_async_commit();
+    };
+
+    load_idx(0);
+    __syncwarp();                      // the previous group's reduction is done with the buffer
+    issue(0);
+    if (nb > 1) load_idx(1);
+    for (int b = 0; b < nb; ++b) {
+        cp_async_wait_all();
+        __syncwarp();                  // batch b has landed for every lane; everyone is done sweeping batch b - 1
+        if (b + 1 < nb) { issue(b + 1); if (b + 2 < nb) load_idx(b + 2); }
+        const float4* buf = ws->buf[b & 1];
+        const int len = batch_len(b);
+        if (b < nbpc) {
+            const float4* p = buf + 3 * min(e0, len);
+            const float4* const end = buf + 3 * len;
+            const int step = 3 * S;
+            if (U == 2) {
+                for (; p + step < end; p += 2 * step) {
+                    const float4 v0 = p[0], v1 = p[1], v2 = p[2];
+                    const float4 w0 = p[step], w1 = p[step + 1], w2 = p[step + 2];
+#pragma unroll
+                    for (int j = 0; j < R2; ++j) pc_bc(v0, v1, v2, ntx[j], nty[j], ntz[j], k, a[j]);
+#pragma unroll
+                    for (int j = 0; j < R2; ++j) pc_bc(w0, w1, w2, ntx[j], nty[j], ntz[j], k, a[j]);
+                }
+            }
+            for (; p < end; p += step) {
+                const float4 v0 = p[0], v1 = p[1], v2 = p[2];
+#pragma unroll
+                for (int j = 0; j < R2; ++j) pc_bc(v0, v1, v2, ntx[j], nty[j], ntz[j], k, a[j]);
+            }
+        } else if (b + 1 < nb) {
+            const float4* p = buf + min(e0, len);
+            const float4* const end = buf + len;
+            for (; p + S < end; p += 2 * S) {
+                const float4 v = p[0], w = p[S];
+#pragma unroll
+                for (int j = 0; j < R2; ++j) pp_bc<false>(v, ntx[j], nty[j], ntz[j], k, a[j], 0, 0, 0);
+#pragma unroll
+                for (int j = 0; j < R2; ++j) pp_bc<false>(w, ntx[j], nty[j], ntz[j], k, a[j], 0, 0, 0);
+            }
+            for (; p < end; p += S) {
+                const float4 v = p[0];
+#pragma unroll
+                for (int j = 0; j < R2; ++j) pp_bc<false>(v, ntx[j], nty[j], ntz[j], k, a[j], 0, 0, 0);
+            }
+        } else {
+            for (int e = e0; e < len; e += S) {
+                const float4 v = buf[e];
+#pragma unroll
+                for (int j = 0; j < R2; ++j) pp_bc<true>(v, ntx[j], nty[j], ntz[j], k, a[j], e, t0 + 2 * j, ng);
+            }
+        }
     }
-    if ((ng & 1) && lane == 0) { const float4 p = ws->own[ng - 1]; pp_store(ws->ring, ng, p.x, p.y, p.z, 0.f); }
+    __syncwarp();                      // every lane is done with the last batch
+    // ---- add the S partial sums of every target in team order and store (ax, ay, az, phi)
+    float4* red = ws->buf[0];
+    const int mpad = L * R;
+    if (active) {
+#pragma unroll
+        for (int j = 0; j < R2; ++j) {
+            float xl, xh, yl, yh, zl, zh, pl, ph;
+            upk(a[j].ax, xl, xh); upk(a[j].ay, yl, yh); upk(a[j].az, zl, zh); upk(a[j].p, pl, ph);
+            red[team * mpad + t0 + 2 * j] = make_float4(xl, yl, zl, pl);
+            red[team * mpad + t0 + 2 * j + 1] = make_float4(xh, yh, zh, ph);
+        }
+    }
     __syncwarp();
-    eval_pp_all<true, kBatchPairs, false>(ws->ring, ws->own, ws->tot, 0, (ng + 1) >> 1, m, ng, k, lane);
-    __syncwarp();
-    totals_finish(ws->tot, m, lane, ng, gb, acc_out);
-    __syncwarp();
+    for (int t = lane; t < ng; t += 32) {
+        float4 r = red[t];
+        for (int s = 1; s < S; ++s) {
+            const float4 q = red[s * mpad + t];
+            r.x += q.x; r.y += q.y; r.z += q.z; r.w += q.w;
+        }
+        acc_out[gb + t] = make_float4(r.x, r.y, r.z, -r.w);
+    }
+}
+
+// Targets per lane (R = 2 R2) that maximise the useful lanes ng S / (32 R); ties go to the larger R (less shared-memory traffic).
+__device__ __forceinline__ int choose_r2(int ng) {
+    const int s1 = 32 / ((ng + 1) / 2), s2 = 32 / ((ng + 3) / 4), s3 = 32 / ((ng + 5) / 6);
+    const int q1 = 6 * s1, q2 = 3 * s2, q3 = 2 * s3;
+    if (q3 >= q2 && q3 >= q1) return 3;
+    if (q2 >= q1) return 2;
+    return 1;
 }
 
 __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(WalkCtl* __restrict__ ctl, int wave, const float4* __restrict__ pos,
@@ -172,8 +265,15 @@ __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(Wa
         const uint32_t pcoff = __ldg(g_pcoff + g);
         if (pcoff == kNone) continue;          // deferred to the fused kernel
         const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
-        eval_group(ws, lane, gb, (int)(ge - gb), pos, erec, lists + pcoff, (int)__ldg(g_npc + g), lists + __ldg(g_ppoff + g),
-                   (int)__ldg(g_lpp + g), k, acc_out);
+        const int ng = (int)(ge - gb), npc = (int)__ldg(g_npc + g), npp = (int)__ldg(g_lpp + g);
+        const uint32_t* lpc = lists + pcoff;
+        const uint32_t* lpp = lists + __ldg(g_ppoff + g);
+        switch (choose_r2(ng)) {
+            case 1: eval_group<1>(ws, lane, gb, ng, pos, erec, lpc, npc, lpp, npp, k, acc_out); break;
+            case 2: eval_group<2>(ws, lane, gb, ng, pos, erec, lpc, npc, lpp, npp, k, acc_out); break;
+            default: eval_group<3>(ws, lane, gb, ng, pos, erec, lpc, npc, lpp, npp, k, acc_out); break;
+        }
+        __syncwarp();
     }
 }
 
