@@ -75,6 +75,7 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     o.c_cbegin = c.take<uint32_t>(C);
     o.c_cend = c.take<uint32_t>(C);
     o.c_parent = c.take<uint32_t>(C);
+    o.c_arrive = c.take<uint32_t>(C);
     o.mom64 = c.take<double>(10 * C);
     o.box = c.take<float>(6 * C);
     o.trec = c.take<float4>(C);

@@ -89,6 +89,7 @@ struct Ws {
     uint32_t* c_cbegin;   // first child (0 for a leaf)
     uint32_t* c_cend;     // one past the last child (0 for a leaf)
     uint32_t* c_parent;
+    uint32_t* c_arrive;   // [max_cells] children that have published their moments (S6)
     double* mom64;        // [max_cells][10]
     float* box;           // [max_cells][6]
     float4* trec;         // [max_cells] walk record: (com, r2open)

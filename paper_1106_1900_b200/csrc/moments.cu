@@ -23,95 +23,108 @@ __device__ __forceinline__ void mom_store(const Mom& m, double* __restrict__ mom
     for (int k = 0; k < 3; ++k) { b[k] = m.bmin[k]; b[3 + k] = m.bmax[k]; }
 }
 
-// Leaves: M = sum m; S = sum m x; com = S / M; Q_jk = sum (m r_j) r_k, r = x - com; particles in ascending order.
-__global__ void __launch_bounds__(128) k_leaf_moments(const DevScalars* __restrict__ sc, const float4* __restrict__ pos,
-                                                      const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
-                                                      const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
-                                                      double* __restrict__ mom64, float* __restrict__ box) {
-    const uint32_t nc = sc->n_cells;
-    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
-        if (c_cend[c] != c_cbegin[c]) continue;   // node
-        const uint32_t b = c_pbegin[c], e = c_pend[c];
-        Mom m;
-        m.M = 0.0;
+// Leaf: M = sum m; S = sum m x; com = S / M; Q_jk = sum (m r_j) r_k, r = x - com; particles in ascending order.
+__device__ __forceinline__ void leaf_moments(Mom& m, const float4* __restrict__ pos, uint32_t b, uint32_t e) {
+    m.M = 0.0;
 #pragma unroll
-        for (int k = 0; k < 3; ++k) { m.S[k] = 0.0; m.bmin[k] = INFINITY; m.bmax[k] = -INFINITY; }
+    for (int k = 0; k < 3; ++k) { m.S[k] = 0.0; m.bmin[k] = INFINITY; m.bmax[k] = -INFINITY; }
 #pragma unroll
-        for (int k = 0; k < 6; ++k) m.Q[k] = 0.0;
-        for (uint32_t i = b; i < e; ++i) {
-            const float4 p = pos[i];
-            const double w = (double)p.w;
-            m.M = __dadd_rn(m.M, w);
-            m.S[0] = __dadd_rn(m.S[0], __dmul_rn(w, (double)p.x));
-            m.S[1] = __dadd_rn(m.S[1], __dmul_rn(w, (double)p.y));
-            m.S[2] = __dadd_rn(m.S[2], __dmul_rn(w, (double)p.z));
-            m.bmin[0] = fminf(m.bmin[0], p.x); m.bmax[0] = fmaxf(m.bmax[0], p.x);
-            m.bmin[1] = fminf(m.bmin[1], p.y); m.bmax[1] = fmaxf(m.bmax[1], p.y);
-            m.bmin[2] = fminf(m.bmin[2], p.z); m.bmax[2] = fmaxf(m.bmax[2], p.z);
-        }
+    for (int k = 0; k < 6; ++k) m.Q[k] = 0.0;
+    for (uint32_t i = b; i < e; ++i) {
+        const float4 p = __ldg(pos + i);
+        const double w = (double)p.w;
+        m.M = __dadd_rn(m.M, w);
+        m.S[0] = __dadd_rn(m.S[0], __dmul_rn(w, (double)p.x));
+        m.S[1] = __dadd_rn(m.S[1], __dmul_rn(w, (double)p.y));
+        m.S[2] = __dadd_rn(m.S[2], __dmul_rn(w, (double)p.z));
+        m.bmin[0] = fminf(m.bmin[0], p.x); m.bmax[0] = fmaxf(m.bmax[0], p.x);
+        m.bmin[1] = fminf(m.bmin[1], p.y); m.bmax[1] = fmaxf(m.bmax[1], p.y);
+        m.bmin[2] = fminf(m.bmin[2], p.z); m.bmax[2] = fmaxf(m.bmax[2], p.z);
+    }
 #pragma unroll
-        for (int k = 0; k < 3; ++k) m.com[k] = __ddiv_rn(m.S[k], m.M);
-        for (uint32_t i = b; i < e; ++i) {
-            const float4 p = pos[i];
-            const double w = (double)p.w;
-            const double rx = __dsub_rn((double)p.x, m.com[0]);
-            const double ry = __dsub_rn((double)p.y, m.com[1]);
-            const double rz = __dsub_rn((double)p.z, m.com[2]);
-            const double tx = __dmul_rn(w, rx), ty = __dmul_rn(w, ry), tz = __dmul_rn(w, rz);
-            m.Q[0] = __dadd_rn(m.Q[0], __dmul_rn(tx, rx));
-            m.Q[1] = __dadd_rn(m.Q[1], __dmul_rn(ty, ry));
-            m.Q[2] = __dadd_rn(m.Q[2], __dmul_rn(tz, rz));
-            m.Q[3] = __dadd_rn(m.Q[3], __dmul_rn(tx, ry));
-            m.Q[4] = __dadd_rn(m.Q[4], __dmul_rn(tx, rz));
-            m.Q[5] = __dadd_rn(m.Q[5], __dmul_rn(ty, rz));
-        }
-        mom_store(m, mom64, box, c);
+    for (int k = 0; k < 3; ++k) m.com[k] = __ddiv_rn(m.S[k], m.M);
+    for (uint32_t i = b; i < e; ++i) {
+        const float4 p = __ldg(pos + i);
+        const double w = (double)p.w;
+        const double rx = __dsub_rn((double)p.x, m.com[0]);
+        const double ry = __dsub_rn((double)p.y, m.com[1]);
+        const double rz = __dsub_rn((double)p.z, m.com[2]);
+        const double tx = __dmul_rn(w, rx), ty = __dmul_rn(w, ry), tz = __dmul_rn(w, rz);
+        m.Q[0] = __dadd_rn(m.Q[0], __dmul_rn(tx, rx));
+        m.Q[1] = __dadd_rn(m.Q[1], __dmul_rn(ty, ry));
+        m.Q[2] = __dadd_rn(m.Q[2], __dmul_rn(tz, rz));
+        m.Q[3] = __dadd_rn(m.Q[3], __dmul_rn(tx, ry));
+        m.Q[4] = __dadd_rn(m.Q[4], __dmul_rn(tx, rz));
+        m.Q[5] = __dadd_rn(m.Q[5], __dmul_rn(ty, rz));
     }
 }
 
-// Nodes of one level: M = sum M_c; S = sum M_c com_c; com = S / M; Q_jk = sum_c ((Q + Q_c,jk) + (M_c d_j) d_k), d = com_c - com.
-__global__ void __launch_bounds__(128) k_node_moments(const DevScalars* __restrict__ sc, int level,
-                                                      const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
-                                                      double* __restrict__ mom64, float* __restrict__ box) {
-    const uint32_t lo = sc->level_offset[level], hi = sc->level_offset[level + 1];
-    for (uint32_t c = lo + blockIdx.x * blockDim.x + threadIdx.x; c < hi; c += gridDim.x * blockDim.x) {
-        const uint32_t cb = c_cbegin[c], ce = c_cend[c];
-        if (ce == cb) continue;   // leaf
+// Node: M = sum M_c; S = sum M_c com_c; com = S / M; Q_jk = sum_c ((Q + Q_c,jk) + (M_c d_j) d_k), d = com_c - com; children
+// in ascending order.  The children were written by other threads of this launch: read them from L2 (ld.global.cg).
+__device__ __forceinline__ void node_moments(Mom& m, const double* mom64, const float* box, uint32_t cb, uint32_t ce) {
+    m.M = 0.0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { m.S[k] = 0.0; m.bmin[k] = INFINITY; m.bmax[k] = -INFINITY; }
+#pragma unroll
+    for (int k = 0; k < 6; ++k) m.Q[k] = 0.0;
+    for (uint32_t k2 = cb; k2 < ce; ++k2) {
+        const double* mc = mom64 + 10 * (size_t)k2;
+        const float* bc = box + 6 * (size_t)k2;
+        const double Mc = __ldcg(mc);
+        m.M = __dadd_rn(m.M, Mc);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            m.S[k] = __dadd_rn(m.S[k], __dmul_rn(Mc, __ldcg(mc + 1 + k)));
+            m.bmin[k] = fminf(m.bmin[k], __ldcg(bc + k));
+            m.bmax[k] = fmaxf(m.bmax[k], __ldcg(bc + 3 + k));
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) m.com[k] = __ddiv_rn(m.S[k], m.M);
+    for (uint32_t k2 = cb; k2 < ce; ++k2) {
+        const double* mc = mom64 + 10 * (size_t)k2;
+        const double Mc = __ldcg(mc);
+        const double dx = __dsub_rn(__ldcg(mc + 1), m.com[0]);
+        const double dy = __dsub_rn(__ldcg(mc + 2), m.com[1]);
+        const double dz = __dsub_rn(__ldcg(mc + 3), m.com[2]);
+        const double tx = __dmul_rn(Mc, dx), ty = __dmul_rn(Mc, dy), tz = __dmul_rn(Mc, dz);
+        m.Q[0] = __dadd_rn(__dadd_rn(m.Q[0], __ldcg(mc + 4)), __dmul_rn(tx, dx));
+        m.Q[1] = __dadd_rn(__dadd_rn(m.Q[1], __ldcg(mc + 5)), __dmul_rn(ty, dy));
+        m.Q[2] = __dadd_rn(__dadd_rn(m.Q[2], __ldcg(mc + 6)), __dmul_rn(tz, dz));
+        m.Q[3] = __dadd_rn(__dadd_rn(m.Q[3], __ldcg(mc + 7)), __dmul_rn(tx, dy));
+        m.Q[4] = __dadd_rn(__dadd_rn(m.Q[4], __ldcg(mc + 8)), __dmul_rn(tx, dz));
+        m.Q[5] = __dadd_rn(__dadd_rn(m.Q[5], __ldcg(mc + 9)), __dmul_rn(ty, dz));
+    }
+}
+
+// The whole bottom-up pass in ONE launch (the paper goes level by level: one launch per level, ~20
+// dependent launches that are nearly all empty).  A thread computes a leaf, publishes it (store, fence) and counts itself
+// in at the parent (c_arrive, zeroed by k_emit_cells); whoever arrives last at a node finds all of its children
+// published, computes the node and climbs on.  Nobody waits, so the launch cannot deadlock; every node is still computed
+// from its children in ascending order, so the values are bit-identical to the level-by-level pass.
+__global__ void __launch_bounds__(128) k_moments(const DevScalars* __restrict__ sc, const float4* __restrict__ pos,
+                                                 const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
+                                                 const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
+                                                 const uint32_t* __restrict__ c_parent, uint32_t* __restrict__ c_arrive,
+                                                 double* mom64, float* box) {
+    const uint32_t nc = sc->n_cells;
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
+        if (c_cend[c] != c_cbegin[c]) continue;   // node: computed by its last child
         Mom m;
-        m.M = 0.0;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) { m.S[k] = 0.0; m.bmin[k] = INFINITY; m.bmax[k] = -INFINITY; }
-#pragma unroll
-        for (int k = 0; k < 6; ++k) m.Q[k] = 0.0;
-        for (uint32_t k2 = cb; k2 < ce; ++k2) {
-            const double* mc = mom64 + 10 * (size_t)k2;
-            const float* bc = box + 6 * (size_t)k2;
-            const double Mc = mc[0];
-            m.M = __dadd_rn(m.M, Mc);
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                m.S[k] = __dadd_rn(m.S[k], __dmul_rn(Mc, mc[1 + k]));
-                m.bmin[k] = fminf(m.bmin[k], bc[k]);
-                m.bmax[k] = fmaxf(m.bmax[k], bc[3 + k]);
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < 3; ++k) m.com[k] = __ddiv_rn(m.S[k], m.M);
-        for (uint32_t k2 = cb; k2 < ce; ++k2) {
-            const double* mc = mom64 + 10 * (size_t)k2;
-            const double Mc = mc[0];
-            const double dx = __dsub_rn(mc[1], m.com[0]);
-            const double dy = __dsub_rn(mc[2], m.com[1]);
-            const double dz = __dsub_rn(mc[3], m.com[2]);
-            const double tx = __dmul_rn(Mc, dx), ty = __dmul_rn(Mc, dy), tz = __dmul_rn(Mc, dz);
-            m.Q[0] = __dadd_rn(__dadd_rn(m.Q[0], mc[4]), __dmul_rn(tx, dx));
-            m.Q[1] = __dadd_rn(__dadd_rn(m.Q[1], mc[5]), __dmul_rn(ty, dy));
-            m.Q[2] = __dadd_rn(__dadd_rn(m.Q[2], mc[6]), __dmul_rn(tz, dz));
-            m.Q[3] = __dadd_rn(__dadd_rn(m.Q[3], mc[7]), __dmul_rn(tx, dy));
-            m.Q[4] = __dadd_rn(__dadd_rn(m.Q[4], mc[8]), __dmul_rn(tx, dz));
-            m.Q[5] = __dadd_rn(__dadd_rn(m.Q[5], mc[9]), __dmul_rn(ty, dz));
-        }
+        leaf_moments(m, pos, c_pbegin[c], c_pend[c]);
         mom_store(m, mom64, box, c);
+        uint32_t cur = c;
+        for (;;) {
+            const uint32_t par = c_parent[cur];
+            if (par == kNone) break;
+            const uint32_t cb = c_cbegin[par], ce = c_cend[par];
+            __threadfence();                                   // publish `cur` before counting in
+            if (atomicAdd(c_arrive + par, 1u) != ce - cb - 1u) break;
+            __threadfence();                                   // all children are published; do not read them early
+            node_moments(m, mom64, box, cb, ce);
+            mom_store(m, mom64, box, par);
+            cur = par;
+        }
     }
 }
 
@@ -156,11 +169,9 @@ __global__ void __launch_bounds__(256) k_cell_record(const DevScalars* __restric
 }
 
 int stage_moments(bh_ctx* c, cudaStream_t s) {
-    const int grid = (int)std::min<int64_t>(div_up(c->max_cells, 128), (int64_t)c->sm_count * 16);
-    BH_LAUNCH(c, k_leaf_moments, grid, 128, 0, s, c->ws.sc, c->ws.pos[c->cur], c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin,
-              c->ws.c_cend, c->ws.mom64, c->ws.box);
-    for (int L = kMaxLevel - 1; L >= 0; --L)
-        BH_LAUNCH(c, k_node_moments, grid, 128, 0, s, c->ws.sc, L, c->ws.c_cbegin, c->ws.c_cend, c->ws.mom64, c->ws.box);
+    const int grid = (int)std::min<int64_t>(div_up(std::min<int64_t>(c->max_cells, c->n + c->n / 2 + 1), 128), (int64_t)c->sm_count * 16);
+    BH_LAUNCH(c, k_moments, grid, 128, 0, s, c->ws.sc, c->ws.pos[c->cur], c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin,
+              c->ws.c_cend, c->ws.c_parent, c->ws.c_arrive, c->ws.mom64, c->ws.box);
     return BH_OK;
 }
 

@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(kTreeTile) k_emit_cells(const uint8_t* __restr
                                                           const uint32_t* __restrict__ tile_base, uint32_t max_cells,
                                                           uint32_t* __restrict__ c_pbegin, uint32_t* __restrict__ c_pend,
                                                           uint32_t* __restrict__ c_cbegin, uint32_t* __restrict__ c_cend,
-                                                          uint32_t* __restrict__ c_parent) {
+                                                          uint32_t* __restrict__ c_parent, uint32_t* __restrict__ c_arrive) {
     constexpr int kWarps = kTreeTile / 32;
     __shared__ uint32_t wc[kLevels][kWarps];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -132,6 +132,7 @@ __global__ void __launch_bounds__(kTreeTile) k_emit_cells(const uint8_t* __restr
                 uint32_t par = kNone;
                 if (L > 0) par = (myfl <= L - 1) ? S[L - 1] : S[L - 1] - 1u;
                 c_parent[c] = par;
+                c_arrive[c] = 0u;                // children counted in by k_moments
             }
         }
         if (i > 0 && myfl <= L && L <= prevdep) {   // a level-L cell ends here
@@ -218,7 +219,7 @@ int stage_cells(bh_ctx* c, cudaStream_t s) {
     if (rc != BH_OK) return rc;
     BH_LAUNCH(c, k_tree_finalize, 1, 32, 0, s, c->ws.tile_base, tiles, &c->ws.sc->n_cells, (uint32_t)c->max_cells, c->ws.sc);
     BH_LAUNCH(c, k_emit_cells, tiles, kTreeTile, 0, s, c->ws.fl, c->ws.dep, n, tiles, c->ws.tile_base, (uint32_t)c->max_cells,
-              c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin, c->ws.c_cend, c->ws.c_parent);
+              c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin, c->ws.c_cend, c->ws.c_parent, c->ws.c_arrive);
     return BH_OK;
 }
 
