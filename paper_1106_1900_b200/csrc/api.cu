@@ -26,7 +26,7 @@ struct Geometry {
 };
 
 static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
-    if (n_max < 1 || n_max > (int64_t)1 << 30) return false;
+    if (n_max < 1 || n_max >= (int64_t)1 << 30) return false;   // counts must fit 30 bits (sort look-back words)
     g->n_max = n_max;
     g->nleaf = (cfg && cfg->nleaf) ? cfg->nleaf : 16;
     g->ncrit = (cfg && cfg->ncrit) ? cfg->ncrit : 64;
@@ -65,8 +65,9 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     o.g_cell = c.take<uint32_t>(n);
     o.g_npc = c.take<uint32_t>(n);
     o.g_npp = c.take<uint32_t>(n);
-    o.hist = c.take<uint32_t>((size_t)kRadix * g.sort_tiles);
-    o.hist_scan = c.take<uint32_t>((size_t)kRadix * g.sort_tiles);
+    o.sort_ghist = c.take<uint32_t>((size_t)kSortPasses * kRadix + kSortPasses + (size_t)kSortPasses * kRadix * g.sort_tiles);
+    o.sort_ticket = o.sort_ghist ? o.sort_ghist + kSortPasses * kRadix : nullptr;
+    o.sort_status = o.sort_ghist ? o.sort_ticket + kSortPasses : nullptr;
     o.scan_sums = c.take<uint32_t>((size_t)g.scan_sum_cap);
     o.tile_cnt = c.take<uint32_t>((size_t)kLevels * g.tree_tiles);
     o.tile_base = c.take<uint32_t>((size_t)kLevels * g.tree_tiles);
@@ -142,7 +143,7 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
         int sms = 0;
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
         c->sm_count = sms;
-        if (walk_init(c) != BH_OK) { rc = BH_ERR_CUDA; break; }
+        if (walk_init(c) != BH_OK || sort_init(c) != BH_OK) { rc = BH_ERR_CUDA; break; }
         for (int k = 0; k < 11; ++k)
             if (cudaEventCreate(&c->ev[k]) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
     } while (0);

@@ -79,8 +79,9 @@ struct Ws {
     uint32_t* g_cell;     // [n]
     uint32_t* g_npc;      // [n]
     uint32_t* g_npp;      // [n]
-    uint32_t* hist;       // [kRadix * sortTiles]
-    uint32_t* hist_scan;  // same
+    uint32_t* sort_ghist;  // [kSortPasses][kRadix] keys per digit value, all passes (counted by k_keys)
+    uint32_t* sort_ticket; // [kSortPasses] tile tickets                       (contiguous with sort_ghist and
+    uint32_t* sort_status; // [kSortPasses][sortTiles][kRadix] look-back words  sort_status: one memset)
     uint32_t* scan_sums;  // partial sums of the generic scan
     uint32_t* tile_cnt;   // [kLevels * treeTiles]
     uint32_t* tile_base;  // same
@@ -169,6 +170,7 @@ int stage_moments(bh_ctx* c, cudaStream_t s);         // S6
 int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s);          // S6: fp32 walk record + r2open(theta)
 int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s);   // S7, S8
 int walk_init(bh_ctx* c);
+int sort_init(bh_ctx* c);
 int walk_eval_init(bh_ctx* c);
 struct WalkListOut {       // what k_walk_lists writes
     DevScalars* sc;

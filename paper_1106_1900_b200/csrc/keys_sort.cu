@@ -102,16 +102,27 @@ __device__ __forceinline__ uint32_t grid_coord(float x, float lo, int sh) {
     return min(v, (1u << kKeyBits) - 1u);
 }
 
+// Also counts, for every sort pass, how many keys carry each digit value (ghist[pass][digit]): the sort then needs no
+// histogram pass of its own.
 __global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pos, int n, const DevScalars* __restrict__ sc,
-                                              uint64_t* __restrict__ key, uint32_t* __restrict__ val) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+                                              uint64_t* __restrict__ key, uint32_t* __restrict__ val, uint32_t* __restrict__ ghist) {
+    __shared__ uint32_t h[kSortPasses * kRadix];
+    for (int j = threadIdx.x; j < kSortPasses * kRadix; j += blockDim.x) h[j] = 0;
+    __syncthreads();
     const float lox = sc->lo[0], loy = sc->lo[1], loz = sc->lo[2];
     const int sh = kKeyBits - sc->dom_e;
-    const float4 p = pos[i];
-    const uint32_t ix = grid_coord(p.x, lox, sh), iy = grid_coord(p.y, loy, sh), iz = grid_coord(p.z, loz, sh);
-    key[i] = (dilate20(ix) << 2) | (dilate20(iy) << 1) | dilate20(iz);   // x most significant in a triple (A4)
-    val[i] = (uint32_t)i;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const float4 p = pos[i];
+        const uint32_t ix = grid_coord(p.x, lox, sh), iy = grid_coord(p.y, loy, sh), iz = grid_coord(p.z, loz, sh);
+        const uint64_t k = (dilate20(ix) << 2) | (dilate20(iy) << 1) | dilate20(iz);   // x most significant in a triple (A4)
+        key[i] = k;
+        val[i] = (uint32_t)i;
+#pragma unroll
+        for (int q = 0; q < kSortPasses; ++q) atomicAdd(&h[q * kRadix + ((uint32_t)(k >> (q * kRadixBits)) & (kRadix - 1))], 1u);
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < kSortPasses * kRadix; j += blockDim.x)
+        if (h[j]) atomicAdd(&ghist[j], h[j]);
 }
 
 __global__ void k_iota(uint32_t* dst, int n) {
@@ -216,37 +227,44 @@ int scan_u8(bh_ctx* c, const uint8_t* in, uint32_t* out, int64_t n, uint32_t* d_
 }
 
 // ------------------------------------------------------------------------------------------ S2
-// LSD radix sort, 8 bits per pass (the paper's 1-bit split generalised: PAPER.md:352, 362).
-// Per pass: per-tile digit histogram -> exclusive scan of the digit-major table -> stable scatter.
-__global__ void __launch_bounds__(kSortThreads) k_radix_hist(const uint64_t* __restrict__ key, int n, int shift, int tiles,
-                                                             uint32_t* __restrict__ hist) {
-    __shared__ uint32_t h[kRadix];
-    h[threadIdx.x] = 0;
-    __syncthreads();
-    const int base = blockIdx.x * kSortTile;
-#pragma unroll 4
-    for (int k = 0; k < kSortItemsPerThread; ++k) {
-        const int i = base + k * kSortThreads + threadIdx.x;
-        if (i < n) atomicAdd(&h[(uint32_t)(key[i] >> shift) & (kRadix - 1)], 1u);
-    }
-    __syncthreads();
-    hist[(size_t)threadIdx.x * tiles + blockIdx.x] = h[threadIdx.x];
+// Stable LSD radix sort, 8 bits per pass (the paper's 1-bit split generalised: PAPER.md:352, 362), ONE kernel
+// per pass.  The digit histograms of all passes were counted while the keys were made (k_keys).  A pass ranks a tile of
+// 4096 keys, publishes the tile's digit counts and obtains the counts of all earlier tiles by a decoupled look-back
+// (status word = flag | count: AGGREGATE = this tile only, PREFIX = this tile and all before it), so no key is read
+// twice and there is no separate histogram or scan launch.  Tiles are numbered by an atomic ticket, so a tile only ever
+// waits for tiles whose blocks are already running: the look-back cannot deadlock.
+constexpr uint32_t kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kCountMask = (1u << 30) - 1u;
+constexpr uint32_t kSpinLimit = 1u << 22;   // ~1 s of polling
+
+__device__ __forceinline__ uint32_t ld_relaxed(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed(uint32_t* p, uint32_t v) {
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// Stable scatter.  Warp w of the block owns the contiguous sub-tile [w*512, (w+1)*512): order = (warp, iteration, lane).
-__global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint64_t* __restrict__ key_in, const uint32_t* __restrict__ val_in,
-                                                                int n, int shift, int tiles, const uint32_t* __restrict__ hist_scan,
-                                                                uint64_t* __restrict__ key_out, uint32_t* __restrict__ val_out) {
+// Warp w of the block owns the contiguous sub-tile [w*512, (w+1)*512): order = (warp, iteration, lane).
+__global__ void __launch_bounds__(kSortThreads) k_radix_pass(const uint64_t* __restrict__ key_in, const uint32_t* __restrict__ val_in,
+                                                             int n, int shift, const uint32_t* __restrict__ ghist, uint32_t* ticket,
+                                                             uint32_t* status, uint64_t* __restrict__ key_out,
+                                                             uint32_t* __restrict__ val_out, DevScalars* sc) {
     constexpr int kWarps = kSortThreads / 32;
     constexpr int kIters = kSortTile / kWarps / 32;   // 16
     __shared__ uint32_t wcnt[kWarps][kRadix];
-    __shared__ uint32_t gbase[kRadix];
+    __shared__ uint32_t gbase[kRadix], lbase[kRadix];
+    __shared__ uint32_t s_tile;
+    extern __shared__ __align__(16) unsigned char xch[];
+    uint64_t* skey = reinterpret_cast<uint64_t*>(xch);
+    uint32_t* sval = reinterpret_cast<uint32_t*>(xch + kSortTile * 8);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
     for (int j = threadIdx.x; j < kWarps * kRadix; j += kSortThreads) (&wcnt[0][0])[j] = 0;
-    gbase[threadIdx.x] = hist_scan[(size_t)threadIdx.x * tiles + blockIdx.x];
     __syncthreads();
+    const uint32_t tile = s_tile;
 
-    const int wbase = blockIdx.x * kSortTile + w * (kIters * 32);
+    const int wbase = (int)tile * kSortTile + w * (kIters * 32);
     const uint32_t lt = (1u << lane) - 1u;
     uint64_t k[kIters];
     uint32_t v[kIters];
@@ -263,7 +281,15 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint64_t* 
         const int i = wbase + it * 32 + lane;
         const bool ok = i < n;
         const uint32_t d = (uint32_t)(k[it] >> shift) & (kRadix - 1);
-        const uint32_t peers = __match_any_sync(0xFFFFFFFFu, ok ? d : 0xFFFFFFFFu);
+        // lanes with the same digit: one ballot per digit bit (the MATCH instruction is far slower than nine votes)
+        uint32_t peers = __ballot_sync(0xFFFFFFFFu, ok);
+        if (!ok) peers = ~peers;
+#pragma unroll
+        for (int b = 0; b < kRadixBits; ++b) {
+            const bool bit = (d >> b) & 1u;
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
+            peers &= bit ? m : ~m;
+        }
         const uint32_t before = __popc(peers & lt);
         uint32_t old = 0;
         if (ok) old = wcnt[w][d];
@@ -273,26 +299,71 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint64_t* 
         rank[it] = old + before;
     }
     __syncthreads();
-    {   // exclusive prefix over the warps for digit = threadIdx.x
-        uint32_t run = 0;
+    // ---- digit = threadIdx.x: exclusive prefix over the warps, the tile's count, and the look-back over earlier tiles
+    const uint32_t d = threadIdx.x;
+    uint32_t tcount = 0;
 #pragma unroll
-        for (int ww = 0; ww < kWarps; ++ww) {
-            const uint32_t t = wcnt[ww][threadIdx.x];
-            wcnt[ww][threadIdx.x] = run;
-            run += t;
-        }
+    for (int ww = 0; ww < kWarps; ++ww) {
+        const uint32_t t = wcnt[ww][d];
+        wcnt[ww][d] = tcount;
+        tcount += t;
     }
+    uint32_t excl = 0;
+    if (tile == 0) {
+        st_relaxed(status + d, kFlagPrefix | tcount);
+    } else {
+        st_relaxed(status + (size_t)tile * kRadix + d, kFlagAgg | tcount);
+        // look back eight tiles per round trip; the words are consumed in order, nearest tile first
+        int t = (int)tile - 1;
+        uint32_t spins = 0;
+        bool done = false;
+        while (!done) {
+            uint32_t wd[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) wd[j] = (t - j >= 0) ? ld_relaxed(status + (size_t)(t - j) * kRadix + d) : kFlagPrefix;
+            int used = 0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                if (done || used != j) continue;
+                if (wd[j] & kFlagPrefix) { excl += wd[j] & kCountMask; done = true; }
+                else if (wd[j] & kFlagAgg) { excl += wd[j] & kCountMask; used = j + 1; }
+            }
+            t -= used;                                   // resume at the first tile that had nothing to report yet
+            if (!done && used == 0 && ++spins > kSpinLimit) { atomicMin(&sc->status, (int)BH_ERR_CUDA); break; }   // never hang the device
+        }
+        st_relaxed(status + (size_t)tile * kRadix + d, kFlagPrefix | (excl + tcount));
+    }
+    uint32_t dummy;
+    const uint32_t dbase = block_exclusive_scan(ghist[d], &dummy);   // first output slot of digit d
+    const uint32_t dstart = block_exclusive_scan(tcount, &dummy);    // first slot of digit d inside the tile, sorted by digit
+    gbase[d] = dbase + excl - dstart;                                // output slot = gbase[digit] + slot inside the sorted tile
+    lbase[d] = dstart;
     __syncthreads();
+    // ---- exchange through shared memory: the tile leaves sorted by digit, so every digit's run is written contiguously
 #pragma unroll
     for (int it = 0; it < kIters; ++it) {
         const int i = wbase + it * 32 + lane;
         if (i < n) {
-            const uint32_t d = (uint32_t)(k[it] >> shift) & (kRadix - 1);
-            const uint32_t dst = gbase[d] + wcnt[w][d] + rank[it];
-            key_out[dst] = k[it];
-            val_out[dst] = v[it];
+            const uint32_t dg = (uint32_t)(k[it] >> shift) & (kRadix - 1);
+            const uint32_t lp = lbase[dg] + wcnt[w][dg] + rank[it];
+            skey[lp] = k[it];
+            sval[lp] = v[it];
         }
     }
+    __syncthreads();
+    const int cnt = min(kSortTile, n - (int)tile * kSortTile);
+#pragma unroll 4
+    for (int lp = threadIdx.x; lp < cnt; lp += kSortThreads) {
+        const uint64_t kk = skey[lp];
+        const uint32_t dst = gbase[(uint32_t)(kk >> shift) & (kRadix - 1)] + (uint32_t)lp;
+        key_out[dst] = kk;
+        val_out[dst] = sval[lp];
+    }
+}
+
+int sort_init(bh_ctx* c) {
+    BH_CUDA(c, cudaFuncSetAttribute(k_radix_pass, cudaFuncAttributeMaxDynamicSharedMemorySize, kSortTile * 12));
+    return BH_OK;
 }
 
 // ------------------------------------------------------------------------------------------ S3
@@ -317,11 +388,15 @@ int stage_iota(bh_ctx* c, uint32_t* dst, int64_t n, cudaStream_t s) {
 int stage_bbox_keys(bh_ctx* c, cudaStream_t s) {
     const int n = (int)c->n;
     BH_LAUNCH(c, k_reset_build, 1, 32, 0, s, c->ws.sc);
+    // sort bookkeeping (digit histograms, tile tickets, look-back status words of every pass): one memset per build
+    const int tiles = (int)div_up(n, kSortTile);
+    BH_CUDA(c, cudaMemsetAsync(c->ws.sort_ghist, 0, sizeof(uint32_t) * ((size_t)kSortPasses * kRadix + kSortPasses + (size_t)kSortPasses * kRadix * tiles), s));
     const int grid = (int)std::min<int64_t>(div_up(n, 256 * 4), (int64_t)c->sm_count * 8);
     BH_LAUNCH(c, k_bbox, grid, 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc);
     BH_LAUNCH(c, k_domain, 1, 32, 0, s, c->ws.sc);
     if (c->timing) cudaEventRecord(c->ev[1], s);
-    BH_LAUNCH(c, k_keys, (unsigned)div_up(n, 256), 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc, c->ws.key[0], c->ws.val[0]);
+    const int kgrid = (int)std::min<int64_t>(div_up(n, 256), (int64_t)c->sm_count * 8);
+    BH_LAUNCH(c, k_keys, kgrid, 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc, c->ws.key[0], c->ws.val[0], c->ws.sort_ghist);
     return BH_OK;
 }
 
@@ -331,11 +406,8 @@ int stage_sort(bh_ctx* c, cudaStream_t s) {
     int src = 0;
     for (int p = 0; p < kSortPasses; ++p) {
         const int shift = p * kRadixBits;
-        BH_LAUNCH(c, k_radix_hist, tiles, kSortThreads, 0, s, c->ws.key[src], n, shift, tiles, c->ws.hist);
-        int rc = scan_u32(c, c->ws.hist, c->ws.hist_scan, (int64_t)kRadix * tiles, nullptr, s);
-        if (rc != BH_OK) return rc;
-        BH_LAUNCH(c, k_radix_scatter, tiles, kSortThreads, 0, s, c->ws.key[src], c->ws.val[src], n, shift, tiles,
-                  c->ws.hist_scan, c->ws.key[src ^ 1], c->ws.val[src ^ 1]);
+        BH_LAUNCH(c, k_radix_pass, tiles, kSortThreads, kSortTile * 12, s, c->ws.key[src], c->ws.val[src], n, shift, c->ws.sort_ghist + p * kRadix,
+                  c->ws.sort_ticket + p, c->ws.sort_status + (size_t)p * kRadix * tiles, c->ws.key[src ^ 1], c->ws.val[src ^ 1], c->ws.sc);
         src ^= 1;
     }
     c->sorted = src;
