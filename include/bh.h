@@ -52,7 +52,8 @@ typedef struct bh_config {
                            * clamp(320 * n_max, 2^22, 2^30).  Bounds memory only: groups whose lists do not fit are walked and
                            * evaluated by the fused kernel, with identical counts and forces within rounding. */
     int32_t walk_mode; /* 0 (default): list walk + list evaluation, fused kernel for what does not fit; 1: fused kernel only */
-    int32_t reserved;
+    int32_t walk_waves; /* 0 (default): as few waves as the list buffer allows (normally 1); k > 1: at least k waves of groups,
+                         * run as a pipeline (list walk of wave w + 1 beside the evaluation of wave w); 0..255 */
 } bh_config;
 
 typedef struct bh_ctx bh_ctx;
@@ -144,6 +145,12 @@ int bh_export_tree(bh_ctx* ctx, bh_tree_view* out, void* stream);
  * records + opening radii), walk (the S7+S8 kernel alone).  Synchronises. */
 int bh_set_stage_timing(bh_ctx* ctx, int enable);
 int bh_get_stage_ms(bh_ctx* ctx, float ms[9]);
+
+/* Device timeline of the last bh_compute_forces (profiling aid; synchronises `stream`).  The walk runs as a pipeline
+ * over waves of groups (S7 list walk of wave w + 1 beside the S8 evaluation of wave w); for wave w,
+ * ns[4w .. 4w+3] = %globaltimer nanoseconds of {first list block start, last list block end, first evaluation block
+ * start, last evaluation block end}.  Returns the number of waves written (<= capacity_waves), or a negative status. */
+int bh_get_walk_timeline(bh_ctx* ctx, void* stream, int64_t* ns, int capacity_waves);
 
 int bh_last_cuda_error(const bh_ctx* ctx);
 const char* bh_status_string(int status);

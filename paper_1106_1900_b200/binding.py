@@ -21,12 +21,12 @@ STATUS = {0: "BH_OK", -1: "BH_ERR_INVALID_ARG", -2: "BH_ERR_WORKSPACE", -3: "BH_
 # every symbol include/bh.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", "bh_get_particles", "bh_tree_build",
            "bh_compute_forces", "bh_leapfrog_step", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
-           "bh_get_stage_ms", "bh_last_cuda_error", "bh_status_string"]
+           "bh_get_stage_ms", "bh_get_walk_timeline", "bh_last_cuda_error", "bh_status_string"]
 
 
 class BhConfig(C.Structure):
     _fields_ = [("nleaf", C.c_int32), ("ncrit", C.c_int32), ("max_cells", C.c_int64), ("list_entries", C.c_int64),
-                ("walk_mode", C.c_int32), ("reserved", C.c_int32)]
+                ("walk_mode", C.c_int32), ("walk_waves", C.c_int32)]
 
 
 class BhStats(C.Structure):
@@ -76,6 +76,8 @@ def load_library():
     lib.bh_export_tree.argtypes = [C.c_void_p, C.POINTER(BhTreeView), C.c_void_p]
     lib.bh_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
     lib.bh_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    lib.bh_get_walk_timeline.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_int64), C.c_int]
+    lib.bh_get_walk_timeline.restype = C.c_int
     lib.bh_last_cuda_error.argtypes = [C.c_void_p]
     lib.bh_status_string.restype = C.c_char_p
     lib.bh_status_string.argtypes = [C.c_int]
@@ -87,8 +89,9 @@ def load_library():
     return lib
 
 
-def workspace_bytes(n_max: int, nleaf: int = 0, ncrit: int = 0, max_cells: int = 0, list_entries: int = 0, walk_mode: int = 0) -> int:
-    cfg = BhConfig(nleaf, ncrit, max_cells, list_entries, walk_mode, 0)
+def workspace_bytes(n_max: int, nleaf: int = 0, ncrit: int = 0, max_cells: int = 0, list_entries: int = 0, walk_mode: int = 0,
+                    walk_waves: int = 0) -> int:
+    cfg = BhConfig(nleaf, ncrit, max_cells, list_entries, walk_mode, walk_waves)
     return int(load_library().bh_workspace_bytes(n_max, C.byref(cfg)))
 
 
@@ -110,12 +113,12 @@ class BarnesHut:
     """One Barnes-Hut context on one GPU: same calls as include/bh.h (bh_tree_build, bh_compute_forces, bh_leapfrog_step)."""
 
     def __init__(self, n_max: int, nleaf: int = 0, ncrit: int = 0, max_cells: int = 0, list_entries: int = 0, walk_mode: int = 0,
-                 device=None):
+                 walk_waves: int = 0, device=None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1106_1900_b200 needs a CUDA device: there is no CPU fallback")
         self.lib = load_library()
         self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
-        cfg = BhConfig(nleaf, ncrit, max_cells, list_entries, walk_mode, 0)
+        cfg = BhConfig(nleaf, ncrit, max_cells, list_entries, walk_mode, walk_waves)
         nbytes = int(self.lib.bh_workspace_bytes(n_max, C.byref(cfg)))
         if nbytes == 0:
             raise BhError(-1, "bad n_max / config")
@@ -190,6 +193,15 @@ class BarnesHut:
         ms = (C.c_float * 9)()
         self._check(self.lib.bh_get_stage_ms(self.h, ms), "bh_get_stage_ms")
         return dict(zip(STAGES, [float(x) for x in ms]))
+
+    def walk_timeline(self, max_waves: int = 256):
+        """[(lists_start, lists_end, eval_start, eval_end)] per wave of the last walk, ns relative to the first start."""
+        buf = (C.c_int64 * (4 * max_waves))()
+        w = self.lib.bh_get_walk_timeline(self.h, self._stream(), buf, max_waves)
+        if w < 0:
+            self._check(w, "bh_get_walk_timeline")
+        t0 = min(buf[4 * i] for i in range(w)) if w else 0
+        return [tuple(int(buf[4 * i + j] - t0) for j in range(4)) for i in range(w)]
 
     # ------------------------------------------------------------------ views of the workspace (no copies)
     def _view(self, ptr: int, count: int, dtype: torch.dtype, shape=None):

@@ -22,7 +22,7 @@ struct Carver {
 
 struct Geometry {
     int64_t n_max, max_cells, sort_tiles, tree_tiles, scan_sum_cap, list_entries;
-    int32_t nleaf, ncrit, walk_mode;
+    int32_t nleaf, ncrit, walk_mode, walk_waves;
 };
 
 static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
@@ -40,6 +40,8 @@ static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
     if (g->list_entries > ((int64_t)1 << 31)) return false;
     g->walk_mode = cfg ? cfg->walk_mode : 0;
     if (g->walk_mode < 0 || g->walk_mode > 1) return false;
+    g->walk_waves = cfg ? cfg->walk_waves : 0;
+    if (g->walk_waves < 0 || g->walk_waves > kMaxWaves) return false;
     g->sort_tiles = div_up(n_max, kSortTile);
     g->tree_tiles = div_up(n_max + 1, kTreeTile);
     const int64_t biggest_scan = std::max<int64_t>(std::max<int64_t>((int64_t)kRadix * g->sort_tiles, (int64_t)kLevels * g->tree_tiles), n_max);
@@ -133,6 +135,7 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
     c->ncrit = g.ncrit;
     c->list_entries = g.list_entries;
     c->walk_mode = g.walk_mode;
+    c->walk_waves = g.walk_waves;
     c->sort_tiles = g.sort_tiles;
     c->tree_tiles = g.tree_tiles;
     c->scan_sum_cap = g.scan_sum_cap;
@@ -147,7 +150,7 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
         for (int k = 0; k < 11; ++k)
             if (cudaEventCreate(&c->ev[k]) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
     } while (0);
-    if (rc != BH_OK) { delete c; return rc; }
+    if (rc != BH_OK) { walk_destroy(c); delete c; return rc; }
     *out = c;
     return BH_OK;
 }
@@ -157,6 +160,7 @@ int bh_destroy(bh_ctx* c) {
     cudaSetDevice(c->device);
     for (int k = 0; k < 11; ++k)
         if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+    walk_destroy(c);
     delete c;
     return BH_OK;
 }
@@ -329,6 +333,26 @@ int bh_get_stage_ms(bh_ctx* c, float ms[9]) {
     BH_CUDA(c, cudaEventElapsedTime(&ms[7], c->ev[8], c->ev[9]));
     BH_CUDA(c, cudaEventElapsedTime(&ms[8], c->ev[9], c->ev[10]));
     return BH_OK;
+}
+
+int bh_get_walk_timeline(bh_ctx* c, void* stream, int64_t* ns, int capacity_waves) {
+    if (!c || !ns || capacity_waves < 1) return BH_ERR_INVALID_ARG;
+    if (!c->have_forces) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    static_assert(sizeof(unsigned long long) == sizeof(int64_t), "timeline words");
+    WalkCtl* h = new (std::nothrow) WalkCtl;
+    if (!h) return BH_ERR_INVALID_ARG;
+    cudaError_t e = cudaMemcpyAsync(h, c->ws.ctl, sizeof(WalkCtl), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { delete h; c->last_cuda = (int)e; return BH_ERR_CUDA; }
+    int w = 0;
+    for (; w < capacity_waves && w < kMaxWaves && h->t_end[1][w] != 0ull; ++w) {
+        ns[4 * w + 0] = (int64_t)h->t_start[0][w]; ns[4 * w + 1] = (int64_t)h->t_end[0][w];
+        ns[4 * w + 2] = (int64_t)h->t_start[1][w]; ns[4 * w + 3] = (int64_t)h->t_end[1][w];
+    }
+    delete h;
+    return w;
 }
 
 int bh_last_cuda_error(const bh_ctx* c) { return c ? c->last_cuda : 0; }

@@ -59,7 +59,16 @@ struct WalkCtl {
     uint32_t eval_next[kMaxWaves + 1];
     uint32_t n_deferred;
     uint32_t fused_next;
+    // %globaltimer (ns) of the first block start / last block end of every list walk [0] and evaluation [1] (bh_get_walk_timeline)
+    unsigned long long t_start[2][kMaxWaves + 1];
+    unsigned long long t_end[2][kMaxWaves + 1];
 };
+
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 
 // Pointers into the caller's workspace.
 struct Ws {
@@ -130,10 +139,14 @@ struct bh_ctx {
     float theta_last;
     int64_t list_entries;
     int walk_mode;
+    int walk_waves;
     bh::Ws ws;
     int64_t sort_tiles, tree_tiles, scan_sum_cap;
     bool timing;
     cudaEvent_t ev[11];
+    // walk pipeline (walk.cu): the list walk of wave w + 1 runs beside the evaluation of wave w on internal streams
+    cudaStream_t s_lists, s_eval2;
+    cudaEvent_t ev_fork, ev_join, ev_lists[bh::kMaxWaves + 1], ev_eval[bh::kMaxWaves + 1];
 };
 
 namespace bh {
@@ -172,6 +185,8 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s);   // S7, S8
 int walk_init(bh_ctx* c);
 int sort_init(bh_ctx* c);
 int walk_eval_init(bh_ctx* c);
+int walk_lists_init(bh_ctx* c);
+int walk_destroy(bh_ctx* c);
 struct WalkListOut {       // what k_walk_lists writes
     DevScalars* sc;
     WalkCtl* ctl;
@@ -179,8 +194,8 @@ struct WalkListOut {       // what k_walk_lists writes
 };
 WalkListOut walk_list_out(bh_ctx* c);
 int stage_walk_prepare(bh_ctx* c, int nwaves, uint32_t wave_particles, cudaStream_t s);
-int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t arena_entries, cudaStream_t s);   // S7
-int stage_walk_eval(bh_ctx* c, int wave, float eps, cudaStream_t s);                           // S8
+int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t arena_base, uint32_t arena_entries, cudaStream_t s);   // S7
+int stage_walk_eval(bh_ctx* c, int wave, float eps, int blocks_per_sm, cudaStream_t s);                           // S8
 int stage_kick_drift(bh_ctx* c, float h, float dt, cudaStream_t s);  // S9
 int stage_kick(bh_ctx* c, float h, cudaStream_t s);                  // S9
 int stage_export(bh_ctx* c, cudaStream_t s);

@@ -240,33 +240,91 @@ WalkListOut walk_list_out(bh_ctx* c) {
 
 int walk_init(bh_ctx* c) {
     BH_CUDA(c, cudaFuncSetAttribute(k_walk_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(WarpShared) * kWalkWarps)));
+    BH_CUDA(c, cudaStreamCreateWithFlags(&c->s_lists, cudaStreamNonBlocking));
+    BH_CUDA(c, cudaStreamCreateWithFlags(&c->s_eval2, cudaStreamNonBlocking));
+    BH_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+    BH_CUDA(c, cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+    for (int k = 0; k <= kMaxWaves; ++k) {
+        BH_CUDA(c, cudaEventCreateWithFlags(&c->ev_lists[k], cudaEventDisableTiming));
+        BH_CUDA(c, cudaEventCreateWithFlags(&c->ev_eval[k], cudaEventDisableTiming));
+    }
     return walk_eval_init(c);
+}
+
+int walk_destroy(bh_ctx* c) {
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
+    for (int k = 0; k <= kMaxWaves; ++k) {
+        if (c->ev_lists[k]) cudaEventDestroy(c->ev_lists[k]);
+        if (c->ev_eval[k]) cudaEventDestroy(c->ev_eval[k]);
+    }
+    if (c->s_lists) cudaStreamDestroy(c->s_lists);
+    if (c->s_eval2) cudaStreamDestroy(c->s_eval2);
+    return BH_OK;
 }
 
 // Expected list entries per particle (cells + particles per group / group size), from the measured c2 figures
 // (80 at theta = 0.75, 189 at theta = 0.5) and the theta^-3 growth of the opened volume; only sizes the waves.
 static double list_entries_per_particle(float theta) { return 32.0 / ((double)theta * theta * theta) + 16.0; }
 
+constexpr int kPipeEvalBlocks = 3;    // evaluation blocks per SM while a list walk runs beside them (12 warps x 128 registers)
+constexpr int kPipeListBlocks = 1;    // ... which leaves registers and shared memory for this many list blocks per SM
+
+// One wave (the default whenever the lists of all groups fit the list buffer): list walk, then evaluation, on the caller's
+// stream.  Several waves (the buffer is too small, or bh_config.walk_waves asks for them): a two-stage pipeline over
+// contiguous particle ranges.  The list walk of wave w + 1 runs BESIDE the evaluation of wave w (internal stream
+// s_lists); the evaluations alternate between the caller's stream and s_eval2 so that the tail of one wave overlaps the
+// head of the next; the list buffer is used in halves (wave parity), and the list walk of wave w + 2 waits for the
+// evaluation of wave w.  Everything is joined back into the caller's stream with events: no host synchronisation, and
+// the fork/join pattern can be captured into a CUDA graph.
+// Measured on B200 (c2, bh_get_walk_timeline): the pipeline does overlap, but it does not pay at this size -- 12
+// evaluation warps + 8 list warps per SM take 2.96 ms (8 waves) against 2.36 ms for one wave: the list walk is bound
+// by instruction issue (~5800 warp instructions per group), so beside the evaluation it starves; hence the default.
 int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
     if (c->timing) cudaEventRecord(c->ev[8], s);
     int rc = stage_cell_record(c, theta, s);
     if (rc != BH_OK) return rc;
     if (c->timing) cudaEventRecord(c->ev[9], s);
-    // ---- waves: contiguous particle ranges whose lists are expected to fit the list buffer 1.5 times over
+    const bool fused_only = c->walk_mode == 1;
+    // ---- waves: each must fit half of the list buffer 1.5 times over
     const double need = 1.5 * list_entries_per_particle(theta) * (double)c->n;
     int64_t nwaves = (int64_t)std::ceil(need / (double)c->list_entries);
-    nwaves = std::min<int64_t>(nwaves, std::max<int64_t>(1, c->n / 8192));
+    if (nwaves > 1) nwaves = (int64_t)std::ceil(2.0 * need / (double)c->list_entries);   // pipelined: halves of the buffer
+    nwaves = std::max<int64_t>(nwaves, c->walk_waves);   // bh_config.walk_waves: 0 = as few as the list buffer allows
+    nwaves = std::min<int64_t>(nwaves, std::max<int64_t>(1, c->n / 4096));
     nwaves = std::max<int64_t>(1, std::min<int64_t>(nwaves, kMaxWaves));
     const int64_t wave_particles = div_up(c->n, nwaves);
-    const bool fused_only = c->walk_mode == 1;
     if ((rc = stage_walk_prepare(c, (int)nwaves, (uint32_t)wave_particles, s)) != BH_OK) return rc;
     if (!fused_only) {
-        // one block of eight warps per ~128 particles (~7 groups), at most 5 resident blocks per SM
-        const int grid = (int)std::max<int64_t>(1, std::min<int64_t>(div_up(wave_particles, 128), (int64_t)c->sm_count * 5));
-        const uint32_t arena = (uint32_t)std::min<int64_t>(c->list_entries / ((int64_t)grid * 8), (int64_t)1 << 30);
-        for (int w = 0; w < (int)nwaves; ++w) {
-            if ((rc = stage_walk_lists(c, w, grid, arena, s)) != BH_OK) return rc;
-            if ((rc = stage_walk_eval(c, w, eps, s)) != BH_OK) return rc;
+        const int W = (int)nwaves;
+        const uint32_t half = (uint32_t)std::min<int64_t>(c->list_entries / 2, (int64_t)1 << 30);
+        // one block of eight warps per ~128 particles (~7 groups); alone on the device: up to 5 resident blocks per SM
+        const int grid_alone = (int)std::max<int64_t>(1, std::min<int64_t>(div_up(wave_particles, 128), (int64_t)c->sm_count * 5));
+        const int grid_beside = (int)std::max<int64_t>(1, std::min<int64_t>(div_up(wave_particles, 128), (int64_t)c->sm_count * kPipeListBlocks));
+        if (W == 1) {
+            const uint32_t whole = (uint32_t)std::min<int64_t>(c->list_entries, (int64_t)1 << 30);
+            if ((rc = stage_walk_lists(c, 0, grid_alone, 0u, whole / ((uint32_t)grid_alone * 8u), s)) != BH_OK) return rc;
+            if ((rc = stage_walk_eval(c, 0, eps, 99, s)) != BH_OK) return rc;
+        } else {
+            cudaStream_t sl = c->s_lists, s2 = c->s_eval2;
+            BH_CUDA(c, cudaEventRecord(c->ev_fork, s));
+            BH_CUDA(c, cudaStreamWaitEvent(sl, c->ev_fork, 0));
+            BH_CUDA(c, cudaStreamWaitEvent(s2, c->ev_fork, 0));
+            for (int w = 0; w < W; ++w) {
+                // lists of wave w (nothing runs beside wave 0: it gets the whole device)
+                if (w >= 2) BH_CUDA(c, cudaStreamWaitEvent(sl, c->ev_eval[w - 2], 0));
+                const int grid = (w == 0) ? grid_alone : grid_beside;
+                if ((rc = stage_walk_lists(c, w, grid, (w & 1) ? half : 0u, half / ((uint32_t)grid * 8u), sl)) != BH_OK) return rc;
+                BH_CUDA(c, cudaEventRecord(c->ev_lists[w], sl));
+                // evaluation of wave w
+                cudaStream_t se = (w & 1) ? s2 : s;
+                BH_CUDA(c, cudaStreamWaitEvent(se, c->ev_lists[w], 0));
+                if ((rc = stage_walk_eval(c, w, eps, (w + 1 < W) ? kPipeEvalBlocks : 99, se)) != BH_OK) return rc;
+                BH_CUDA(c, cudaEventRecord(c->ev_eval[w], se));
+            }
+            // join: the caller's stream continues after every evaluation (and with them every list walk)
+            for (int w = std::max(0, W - 2); w < W; ++w)
+                if (w & 1) BH_CUDA(c, cudaStreamWaitEvent(s, c->ev_eval[w], 0));
         }
     }
     const size_t smem = sizeof(WarpShared) * kWalkWarps;

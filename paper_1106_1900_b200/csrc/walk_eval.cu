@@ -257,6 +257,7 @@ __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(Wa
     const int lane = threadIdx.x & 31;
     const uint32_t g0 = ctl->wave_g[wave], g1 = ctl->wave_g[wave + 1];
     const Consts k = make_consts(eps2);
+    if (threadIdx.x == 0) atomicMin(&ctl->t_start[1][wave], global_ns());
     for (;;) {
         uint32_t g = 0;
         if (lane == 0) g = g0 + atomicAdd(&ctl->eval_next[wave], 1u);
@@ -275,16 +276,19 @@ __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(Wa
         }
         __syncwarp();
     }
+    if (lane == 0) atomicMax(&ctl->t_end[1][wave], global_ns());
 }
 
 int walk_eval_init(bh_ctx* c) {
     BH_CUDA(c, cudaFuncSetAttribute(k_walk_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(EvalShared) * kEvalWarps)));
-    return BH_OK;
+    // the same (largest) shared-memory carve-out as k_walk_lists, so that blocks of both kernels can share an SM
+    BH_CUDA(c, cudaFuncSetAttribute(k_walk_eval, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
+    return walk_lists_init(c);
 }
 
-int stage_walk_eval(bh_ctx* c, int wave, float eps, cudaStream_t s) {
+int stage_walk_eval(bh_ctx* c, int wave, float eps, int blocks_per_sm, cudaStream_t s) {
     const size_t smem = sizeof(EvalShared) * kEvalWarps;
-    const int grid = c->sm_count * kEvalBlocksPerSM;
+    const int grid = c->sm_count * std::min(blocks_per_sm, kEvalBlocksPerSM);
     BH_LAUNCH(c, k_walk_eval, grid, kEvalThreads, smem, s, c->ws.ctl, wave, c->ws.pos[c->cur], c->ws.erec, c->ws.g_begin, c->ws.lists,
               c->ws.g_pcoff, c->ws.g_npc, c->ws.g_ppoff, c->ws.g_lpp, eps * eps, c->ws.acc);
     return BH_OK;

@@ -30,7 +30,14 @@ constexpr int kListThreads = kListWarps * 32;
 constexpr int kLStackCap = 512;       // opened nodes
 constexpr int kLStackReserve = 160;   // >= 7 * 20 + 7: room for a pure depth-first descent
 constexpr int kLeafQueue = 64;
-constexpr int kGroupChunk = 32;       // consecutive groups a block claims at a time
+#ifndef BH_GROUP_CHUNK
+#define BH_GROUP_CHUNK 32
+#endif
+#ifndef BH_KSUB
+#define BH_KSUB 2
+#endif
+constexpr int kGroupChunk = BH_GROUP_CHUNK;   // consecutive groups a block claims at a time
+constexpr int kSub = BH_KSUB;               // sub-batches of 4 nodes (32 children) popped per step: 4 records in flight per lane
 
 struct ListArena { uint32_t pc_top, pp_bot; };
 struct WalkSums { unsigned long long pc, pp, mac; };
@@ -90,50 +97,64 @@ __device__ __forceinline__ void list_group(ListWarpShared* ws, const int lane, c
     if (lane == 0) ws->stack[0] = make_uint2(0u, 1u);   // the root (A17) as the only child of a virtual node
     __syncwarp();
 
-    while (sp > 0) {
+    while (sp > 0 && fits) {
+        // pop up to 4 kSub nodes; lane = (node r of a sub-batch, child c8); all records are requested before any is used
         int kpop = (kLStackCap - kLStackReserve - sp) / 7;
-        kpop = max(1, min(kpop, 4));
+        kpop = max(1, min(kpop, 4 * kSub));
         kpop = min(kpop, sp);
-        const int r = lane >> 3;
-        bool valid = false, accept = false, isleaf = false, isnode = false;
-        uint32_t cell = 0;
-        uint2 lk = make_uint2(0u, 0u);
-        if (r < kpop) {
-            const uint2 e = ws->stack[sp - 1 - r];
-            valid = (uint32_t)(lane & 7) < e.y;
-            cell = e.x + (uint32_t)(lane & 7);
+        const int r = lane >> 3, c8 = lane & 7;
+        bool valid[kSub];
+        uint32_t cell[kSub];
+        float4 r0[kSub];
+        uint2 lk[kSub];
+#pragma unroll
+        for (int j = 0; j < kSub; ++j) {
+            valid[j] = false;
+            cell[j] = 0u;
+            const int idx = 4 * j + r;
+            if (idx < kpop) {
+                const uint2 e = ws->stack[sp - 1 - idx];
+                valid[j] = (uint32_t)c8 < e.y;
+                cell[j] = e.x + (uint32_t)c8;
+            }
         }
-        if (valid) {
-            const float4 r0 = __ldg(trec + cell);
-            lk = __ldg(tlink + cell);
-            accept = mac_accept(mn, mx, r0);
-            isleaf = !accept && (lk.y >> 31) != 0u;
-            isnode = !accept && !isleaf;
+#pragma unroll
+        for (int j = 0; j < kSub; ++j) {
+            r0[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+            lk[j] = make_uint2(0u, 0u);
+            if (valid[j]) { r0[j] = __ldg(trec + cell[j]); lk[j] = __ldg(tlink + cell[j]); }
         }
         sp -= kpop;
-        __syncwarp();
-        nmac += (uint32_t)__popc(__ballot_sync(0xFFFFFFFFu, valid));
-        // ---- accepted cells -> cell list
-        const uint32_t amask = __ballot_sync(0xFFFFFFFFu, accept);
-        if (amask) {
-            const uint32_t na = (uint32_t)__popc(amask);
-            if (pc_top + na > pp_bot) { fits = false; break; }
-            if (accept) lists[pc_top + (uint32_t)__popc(amask & lt)] = cell;
-            pc_top += na;
-        }
-        // ---- opened nodes -> back onto the stack (kpop <= (cap - reserve - sp) / 7 guarantees room for 8 per popped node)
-        const uint32_t nmask = __ballot_sync(0xFFFFFFFFu, isnode);
-        if (isnode) ws->stack[sp + __popc(nmask & lt)] = lk;
-        sp += __popc(nmask);
-        // ---- opened leaves -> queue; expanded 32 at a time
-        const uint32_t lmask = __ballot_sync(0xFFFFFFFFu, isleaf);
-        if (lmask) {
-            if (isleaf) ws->leafq[lq + __popc(lmask & lt)] = make_uint2(lk.x, lk.y & 0x7FFFFFFFu);
-            lq += __popc(lmask);
-            __syncwarp();
-            if (lq >= 32) {
-                lq -= 32;
-                if (!flush_leaves(ws->leafq + lq, 32, lane, gb, ge, lists, pc_top, pp_bot, npp)) { fits = false; break; }
+        __syncwarp();                 // every lane has read its stack entries: the slots may be overwritten
+#pragma unroll
+        for (int j = 0; j < kSub; ++j) {
+            if (4 * j >= kpop) break;
+            const bool accept = valid[j] && mac_accept(mn, mx, r0[j]);
+            const bool isleaf = valid[j] && !accept && (lk[j].y >> 31) != 0u;
+            const bool isnode = valid[j] && !accept && !isleaf;
+            nmac += (uint32_t)__popc(__ballot_sync(0xFFFFFFFFu, valid[j]));
+            // ---- accepted cells -> cell list
+            const uint32_t amask = __ballot_sync(0xFFFFFFFFu, accept);
+            if (amask) {
+                const uint32_t na = (uint32_t)__popc(amask);
+                if (pc_top + na > pp_bot) { fits = false; break; }
+                if (accept) lists[pc_top + (uint32_t)__popc(amask & lt)] = cell[j];
+                pc_top += na;
+            }
+            // ---- opened nodes -> back onto the stack (kpop <= (cap - reserve - sp) / 7 guarantees room for 8 per popped node)
+            const uint32_t nmask = __ballot_sync(0xFFFFFFFFu, isnode);
+            if (isnode) ws->stack[sp + __popc(nmask & lt)] = lk[j];
+            sp += __popc(nmask);
+            // ---- opened leaves -> queue; expanded 32 at a time
+            const uint32_t lmask = __ballot_sync(0xFFFFFFFFu, isleaf);
+            if (lmask) {
+                if (isleaf) ws->leafq[lq + __popc(lmask & lt)] = make_uint2(lk[j].x, lk[j].y & 0x7FFFFFFFu);
+                lq += __popc(lmask);
+                __syncwarp();
+                if (lq >= 32) {
+                    lq -= 32;
+                    if (!flush_leaves(ws->leafq + lq, 32, lane, gb, ge, lists, pc_top, pp_bot, npp)) { fits = false; break; }
+                }
             }
         }
         __syncwarp();
@@ -160,18 +181,19 @@ __device__ __forceinline__ void list_group(ListWarpShared* ws, const int lane, c
     __syncwarp();
 }
 
-__global__ void __launch_bounds__(kListThreads, 5) k_walk_lists(WalkListOut o, int wave, const float4* __restrict__ pos,
+__global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, int wave, const float4* __restrict__ pos,
                                                                 const float4* __restrict__ trec, const uint2* __restrict__ tlink,
                                                                 const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
                                                                 const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
                                                                 const uint32_t* __restrict__ g_begin, uint32_t* __restrict__ lists,
-                                                                uint32_t arena_entries) {
+                                                                uint32_t arena_base, uint32_t arena_entries) {
     __shared__ ListWarpShared s_ws[kListWarps];
     __shared__ uint32_t s_chunk, s_taken;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t g0 = o.ctl->wave_g[wave], g1 = o.ctl->wave_g[wave + 1];
+    if (threadIdx.x == 0) atomicMin(&o.ctl->t_start[0][wave], global_ns());
     ListArena ar;
-    ar.pc_top = (blockIdx.x * kListWarps + warp) * arena_entries;
+    ar.pc_top = arena_base + (blockIdx.x * kListWarps + warp) * arena_entries;
     ar.pp_bot = ar.pc_top + arena_entries;
     WalkSums sums = {0ull, 0ull, 0ull};
     for (;;) {
@@ -191,6 +213,7 @@ __global__ void __launch_bounds__(kListThreads, 5) k_walk_lists(WalkListOut o, i
             list_group(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
         }
     }
+    if (threadIdx.x == 0) atomicMax(&o.ctl->t_end[0][wave], global_ns());
     if (lane == 0 && sums.mac) {
         atomicAdd(&o.sc->sum_pc, sums.pc);
         atomicAdd(&o.sc->sum_pp, sums.pp);
@@ -214,6 +237,8 @@ __global__ void k_walk_prepare(DevScalars* sc, WalkCtl* ctl, const uint32_t* __r
         ctl->wave_g[t] = lo;
         ctl->list_next[t] = 0;
         ctl->eval_next[t] = 0;
+        ctl->t_start[0][t] = ctl->t_start[1][t] = ~0ull;
+        ctl->t_end[0][t] = ctl->t_end[1][t] = 0ull;
     }
     if (t == 0) {
         ctl->n_deferred = 0;
@@ -222,10 +247,15 @@ __global__ void k_walk_prepare(DevScalars* sc, WalkCtl* ctl, const uint32_t* __r
     }
 }
 
-int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t arena_entries, cudaStream_t s) {
+int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t arena_base, uint32_t arena_entries, cudaStream_t s) {
     WalkListOut o = walk_list_out(c);
     BH_LAUNCH(c, k_walk_lists, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
-              c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, arena_entries);
+              c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, arena_base, arena_entries);
+    return BH_OK;
+}
+
+int walk_lists_init(bh_ctx* c) {
+    BH_CUDA(c, cudaFuncSetAttribute(k_walk_lists, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
     return BH_OK;
 }
 

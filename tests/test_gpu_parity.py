@@ -54,10 +54,12 @@ def test_walk_paths_agree(BH, cfg):
     _full_parity(BH, pm, vel, prm["theta"], prm["eps"], **cfg)
 
 
-def test_walk_in_several_waves(BH):
-    """A list buffer that forces several waves (contiguous particle ranges walked and evaluated one after the other)."""
+@pytest.mark.parametrize("cfg", [dict(list_entries=1 << 20), dict(walk_waves=5), dict(walk_waves=2, list_entries=1 << 22)])
+def test_walk_in_several_waves(BH, cfg):
+    """Several waves (forced by a small list buffer, or asked for): the list walk of wave w + 1 runs beside the evaluation of
+    wave w on internal streams; same counts, same forces."""
     pm, vel, prm = bh_inputs.make("c1", n=40000, seed=17)
-    _full_parity(BH, pm, vel, prm["theta"], prm["eps"], list_entries=1 << 20)
+    _full_parity(BH, pm, vel, prm["theta"], prm["eps"], **cfg)
 
 
 @pytest.mark.parametrize("n", [1, 2, 16, 17, 64, 65])
