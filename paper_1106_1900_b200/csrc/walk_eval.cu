@@ -14,9 +14,9 @@
 //       memory, in a fixed order (deterministic).
 //   (3) Shared-memory delivery.  An entry costs three LDS.128 per lane whatever R is, so R = 4 or 6 halves or thirds the
 //       shared-memory traffic per interaction; R = 2 sweeps two entries per iteration for independent work instead.
-//   (4) The lists are streamed in batches of 128 entries ("Nblock"): the indices of batch b + 2 are loaded
-//       and the records of batch b + 1 are gathered by cp.async (LDGSTS) into the other half of a double buffer while
-//       batch b is swept; no registers are held across the sweep and the gather's L2 latency hides behind arithmetic.
+//   (4) The lists are streamed in batches of 128 entries ("Nblock"): while batch b is swept, the records of
+//       batch b + 1 and the indices of batch b + 2 are copied by cp.async (LDGSTS) into the other halves of two double
+//       buffers; no register waits for a load across the sweep, and the L2 latency hides behind arithmetic.
 // The group's own particles form the last batch, with j != i (A19).
 // Forces: DESIGN.md O10 -- 33 packed operations + 2 MUFU.RSQ per entry and target pair (p-c), 13 + 2 (p-p).
 #include <algorithm>
@@ -32,12 +32,17 @@ constexpr int kPerLane = kBatch / 32;        // entries a lane gathers per batch
 
 struct __align__(16) EvalShared {
     float4 buf[2][kBatch * 3];               // cp.async landing zones: 3 x float4 per cell, 1 x float4 per particle
+    uint32_t idx[2][kBatch];                 // list indices of the next batches (cp.async as well)
     float tx[64], ty[64], tz[64];            // negated target coordinates: a lane reads its pairs with one 64-bit load each
 };
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
     const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* smem_dst, const void* gsrc) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
@@ -123,53 +128,62 @@ __device__ __forceinline__ void eval_group(EvalShared* ws, const int lane, const
     const int nb = nbpc + nbpp + 1;
     const int e0 = active ? team : (1 << 28);    // idle lanes (32 - S L of them) skip the sweeps
 
-    uint32_t ix[kPerLane];
-    // indices of batch b (cells, particles, or the group's own particles)
-    auto load_idx = [&](int b) {
-        if (b < nbpc) {
+    auto batch_len = [&](int b) { return b < nbpc ? min(kBatch, npc - kBatch * b) : b < nbpc + nbpp ? min(kBatch, npp - kBatch * (b - nbpc)) : ng; };
+    // copy the list indices of batch b (cells or particles; the self batch has none) into half b & 1 of the index buffer.
+    // They travel by cp.async like the records, so no register waits for them: lane l fetches and later reads entries
+    // l, l + 32, ... itself.
+    auto fetch_idx = [&](int b) {
+        if (b >= nbpc + nbpp) return;
+        const uint32_t* src = b < nbpc ? lpc + b * kBatch : lpp + (b - nbpc) * kBatch;
+        const int len = batch_len(b);
+        uint32_t* dst = ws->idx[b & 1];
 #pragma unroll
-            for (int j = 0; j < kPerLane; ++j) { const int e = b * kBatch + j * 32 + lane; if (e < npc) ix[j] = __ldg(lpc + e); }
-        } else if (b < nbpc + nbpp) {
-#pragma unroll
-            for (int j = 0; j < kPerLane; ++j) { const int e = (b - nbpc) * kBatch + j * 32 + lane; if (e < npp) ix[j] = __ldg(lpp + e); }
-        } else {
-#pragma unroll
-            for (int j = 0; j < kPerLane; ++j) ix[j] = gb + (uint32_t)(j * 32 + lane);
+        for (int j = 0; j < kPerLane; ++j) {
+            const int le = j * 32 + lane;
+            if (le < len) cp_async4(dst + le, src + le);
         }
     };
-    auto batch_len = [&](int b) { return b < nbpc ? min(kBatch, npc - kBatch * b) : b < nbpc + nbpp ? min(kBatch, npp - kBatch * (b - nbpc)) : ng; };
-    // gather the records of batch b into half b & 1 of the buffer
+    // gather the records of batch b into half b & 1 of the record buffer
     auto issue = [&](int b) {
         float4* dst = ws->buf[b & 1];
+        const uint32_t* sidx = ws->idx[b & 1];
         const int len = batch_len(b);
         if (b < nbpc) {
 #pragma unroll
             for (int j = 0; j < kPerLane; ++j) {
                 const int le = j * 32 + lane;
                 if (le < len) {
-                    const float4* s = erec + 3 * (size_t)ix[j];
+                    const float4* s = erec + 3 * (size_t)sidx[le];
                     float4* d = dst + 3 * le;
                     cp_async16(d, s); cp_async16(d + 1, s + 1); cp_async16(d + 2, s + 2);
                 }
+            }
+        } else if (b < nbpc + nbpp) {
+#pragma unroll
+            for (int j = 0; j < kPerLane; ++j) {
+                const int le = j * 32 + lane;
+                if (le < len) cp_async16(dst + le, pos + sidx[le]);
             }
         } else {
 #pragma unroll
             for (int j = 0; j < kPerLane; ++j) {
                 const int le = j * 32 + lane;
-                if (le < len) cp_async16(dst + le, pos + ix[j]);
+                if (le < len) cp_async16(dst + le, pos + gb + le);
             }
         }
-        cp_async_commit();
     };
 
-    load_idx(0);
-    __syncwarp();                      // the previous group's reduction is done with the buffer
+    __syncwarp();                      // the previous group's reduction is done with the buffers
+    fetch_idx(0);
+    cp_async_commit();
+    cp_async_wait_all();               // (the only index round trip that nothing hides: one per group)
     issue(0);
-    if (nb > 1) load_idx(1);
+    fetch_idx(1);
+    cp_async_commit();
     for (int b = 0; b < nb; ++b) {
         cp_async_wait_all();
-        __syncwarp();                  // batch b has landed for every lane; everyone is done sweeping batch b - 1
-        if (b + 1 < nb) { issue(b + 1); if (b + 2 < nb) load_idx(b + 2); }
+        __syncwarp();                  // batch b (and the indices of b + 1) have landed; everyone is done sweeping batch b - 1
+        if (b + 1 < nb) { issue(b + 1); fetch_idx(b + 2); cp_async_commit(); }
         const float4* buf = ws->buf[b & 1];
         const int len = batch_len(b);
         if (b < nbpc) {
