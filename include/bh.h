@@ -142,9 +142,11 @@ int bh_export_tree(bh_ctx* ctx, bh_tree_view* out, void* stream);
 
 /* Per-stage device times of the last bh_tree_build + bh_compute_forces, in ms, when enabled (adds event records,
  * do not enable under graph capture).  Order: bbox, keys, sort, reorder, cells, groups, moments, record (fp32 walk
- * records + opening radii), walk (the S7+S8 kernel alone).  Synchronises. */
+ * records + opening radii), walk (S7 + S8: list walk, evaluation, fallback kernel), lists (k_walk_lists alone), eval
+ * (k_walk_eval alone); the last two are 0 when the walk ran as a pipeline of several waves (the kernels overlap: see
+ * bh_get_walk_timeline).  Synchronises. */
 int bh_set_stage_timing(bh_ctx* ctx, int enable);
-int bh_get_stage_ms(bh_ctx* ctx, float ms[9]);
+int bh_get_stage_ms(bh_ctx* ctx, float ms[11]);
 
 /* Device timeline of the last bh_compute_forces (profiling aid; synchronises `stream`).  The walk runs as a pipeline
  * over waves of groups (S7 list walk of wave w + 1 beside the S8 evaluation of wave w); for wave w,

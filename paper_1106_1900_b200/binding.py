@@ -95,7 +95,7 @@ def workspace_bytes(n_max: int, nleaf: int = 0, ncrit: int = 0, max_cells: int =
     return int(load_library().bh_workspace_bytes(n_max, C.byref(cfg)))
 
 
-STAGES = ["bbox", "keys", "sort", "reorder", "cells", "groups", "moments", "record", "walk"]
+STAGES = ["bbox", "keys", "sort", "reorder", "cells", "groups", "moments", "record", "walk", "lists", "eval"]
 
 
 def _ptr(x):
@@ -190,7 +190,7 @@ class BarnesHut:
         self._check(self.lib.bh_set_stage_timing(self.h, int(enable)))
 
     def stage_ms(self) -> dict:
-        ms = (C.c_float * 9)()
+        ms = (C.c_float * 11)()
         self._check(self.lib.bh_get_stage_ms(self.h, ms), "bh_get_stage_ms")
         return dict(zip(STAGES, [float(x) for x in ms]))
 

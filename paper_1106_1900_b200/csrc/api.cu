@@ -147,7 +147,7 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
         c->sm_count = sms;
         if (walk_init(c) != BH_OK || sort_init(c) != BH_OK) { rc = BH_ERR_CUDA; break; }
-        for (int k = 0; k < 11; ++k)
+        for (int k = 0; k < 13; ++k)
             if (cudaEventCreate(&c->ev[k]) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
     } while (0);
     if (rc != BH_OK) { walk_destroy(c); delete c; return rc; }
@@ -158,7 +158,7 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
 int bh_destroy(bh_ctx* c) {
     if (!c) return BH_ERR_INVALID_ARG;
     cudaSetDevice(c->device);
-    for (int k = 0; k < 11; ++k)
+    for (int k = 0; k < 13; ++k)
         if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     walk_destroy(c);
     delete c;
@@ -324,7 +324,7 @@ int bh_set_stage_timing(bh_ctx* c, int enable) {
     return BH_OK;
 }
 
-int bh_get_stage_ms(bh_ctx* c, float ms[9]) {
+int bh_get_stage_ms(bh_ctx* c, float ms[11]) {
     if (!c || !ms) return BH_ERR_INVALID_ARG;
     if (!c->timing || !c->have_forces) return BH_ERR_STATE;
     BH_CUDA(c, cudaSetDevice(c->device));
@@ -332,6 +332,11 @@ int bh_get_stage_ms(bh_ctx* c, float ms[9]) {
     for (int k = 0; k < 7; ++k) BH_CUDA(c, cudaEventElapsedTime(&ms[k], c->ev[k], c->ev[k + 1]));
     BH_CUDA(c, cudaEventElapsedTime(&ms[7], c->ev[8], c->ev[9]));
     BH_CUDA(c, cudaEventElapsedTime(&ms[8], c->ev[9], c->ev[10]));
+    ms[9] = ms[10] = 0.0f;
+    if (c->walk_split_timed) {
+        BH_CUDA(c, cudaEventElapsedTime(&ms[9], c->ev[9], c->ev[11]));
+        BH_CUDA(c, cudaEventElapsedTime(&ms[10], c->ev[11], c->ev[12]));
+    }
     return BH_OK;
 }
 

@@ -286,6 +286,7 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
     if (rc != BH_OK) return rc;
     if (c->timing) cudaEventRecord(c->ev[9], s);
     const bool fused_only = c->walk_mode == 1;
+    c->walk_split_timed = false;
     // ---- waves: each must fit half of the list buffer 1.5 times over
     const double need = 1.5 * list_entries_per_particle(theta) * (double)c->n;
     int64_t nwaves = (int64_t)std::ceil(need / (double)c->list_entries);
@@ -304,7 +305,10 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
         if (W == 1) {
             const uint32_t whole = (uint32_t)std::min<int64_t>(c->list_entries, (int64_t)1 << 30);
             if ((rc = stage_walk_lists(c, 0, grid_alone, 0u, whole / ((uint32_t)grid_alone * 8u), s)) != BH_OK) return rc;
+            if (c->timing) cudaEventRecord(c->ev[11], s);
             if ((rc = stage_walk_eval(c, 0, eps, 99, s)) != BH_OK) return rc;
+            if (c->timing) cudaEventRecord(c->ev[12], s);
+            c->walk_split_timed = c->timing;
         } else {
             cudaStream_t sl = c->s_lists, s2 = c->s_eval2;
             BH_CUDA(c, cudaEventRecord(c->ev_fork, s));
