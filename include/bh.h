@@ -154,6 +154,14 @@ int bh_get_stage_ms(bh_ctx* ctx, float ms[11]);
  * start, last evaluation block end}.  Returns the number of waves written (<= capacity_waves), or a negative status. */
 int bh_get_walk_timeline(bh_ctx* ctx, void* stream, int64_t* ns, int capacity_waves);
 
+/* The accuracy reference of PAPER.md:196-200 (Eq.2: |a_tree - a_direct| / |a_direct|): softened O(N^2) direct summation
+ * in binary64 from the fp32 inputs, on the GPU (the paper uses a double-precision GPU direct code for the same purpose).
+ * d_pos_mass: float[n][4] DEVICE pointer (x, y, z, m); targets are particles [t0, t1); d_acc_pot: double[n][4] DEVICE
+ * pointer, rows t0..t1-1 receive (ax, ay, az, phi), other rows are not touched.  phi_i = -sum_{j != i} m_j / rho_ij,
+ * a_i = sum_{j != i} m_j (x_j - x_i) / rho_ij^3, rho^2 = |x_j - x_i|^2 + eps^2.  Needs no ctx; only enqueues work on
+ * `stream`; both pointers are borrowed.  Not on the per-step path.  Returns BH_OK, BH_ERR_INVALID_ARG or BH_ERR_CUDA. */
+int bh_direct_forces(const float* d_pos_mass, int64_t n, float eps, int64_t t0, int64_t t1, double* d_acc_pot, void* stream);
+
 int bh_last_cuda_error(const bh_ctx* ctx);
 const char* bh_status_string(int status);
 

@@ -3,5 +3,5 @@
 ``csrc/`` holds the sm_100a kernels and the C ABI of ``include/bh.h``; ``binding.py`` marshals arguments.
 Nothing here imports ``oracle/`` (test infrastructure); there is no CPU fallback.
 """
-from .binding import (BarnesHut, BhError, BhStats, LIB_PATH, STAGES, SYMBOLS, load_library,  # noqa: F401
+from .binding import (BarnesHut, BhError, BhStats, LIB_PATH, STAGES, SYMBOLS, direct_forces, load_library,  # noqa: F401
                       workspace_bytes)

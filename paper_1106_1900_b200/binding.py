@@ -21,7 +21,7 @@ STATUS = {0: "BH_OK", -1: "BH_ERR_INVALID_ARG", -2: "BH_ERR_WORKSPACE", -3: "BH_
 # every symbol include/bh.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", "bh_get_particles", "bh_tree_build",
            "bh_compute_forces", "bh_leapfrog_step", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
-           "bh_get_stage_ms", "bh_get_walk_timeline", "bh_last_cuda_error", "bh_status_string"]
+           "bh_get_stage_ms", "bh_get_walk_timeline", "bh_direct_forces", "bh_last_cuda_error", "bh_status_string"]
 
 
 class BhConfig(C.Structure):
@@ -78,6 +78,8 @@ def load_library():
     lib.bh_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
     lib.bh_get_walk_timeline.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_int64), C.c_int]
     lib.bh_get_walk_timeline.restype = C.c_int
+    lib.bh_direct_forces.argtypes = [C.c_void_p, C.c_int64, C.c_float, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
+    lib.bh_direct_forces.restype = C.c_int
     lib.bh_last_cuda_error.argtypes = [C.c_void_p]
     lib.bh_status_string.restype = C.c_char_p
     lib.bh_status_string.argtypes = [C.c_int]
@@ -93,6 +95,23 @@ def workspace_bytes(n_max: int, nleaf: int = 0, ncrit: int = 0, max_cells: int =
                     walk_waves: int = 0) -> int:
     cfg = BhConfig(nleaf, ncrit, max_cells, list_entries, walk_mode, walk_waves)
     return int(load_library().bh_workspace_bytes(n_max, C.byref(cfg)))
+
+
+def direct_forces(pos_mass: torch.Tensor, eps: float, t0: int = 0, t1: int | None = None, out: torch.Tensor | None = None) -> torch.Tensor:
+    """bh_direct_forces: binary64 O(N^2) direct sum on the GPU for targets [t0, t1).  pos_mass: CUDA float32[n,4];
+    returns (or fills) a CUDA float64[n,4] tensor (ax, ay, az, phi); rows outside the range are left as they are (NaN if new)."""
+    if not (pos_mass.is_cuda and pos_mass.dtype == torch.float32 and pos_mass.is_contiguous() and pos_mass.dim() == 2 and pos_mass.shape[1] == 4):
+        raise BhError(-1, "pos_mass must be a contiguous CUDA float32[n,4] tensor")
+    n = int(pos_mass.shape[0])
+    t1 = n if t1 is None else t1
+    if out is None:
+        out = torch.full((n, 4), float("nan"), dtype=torch.float64, device=pos_mass.device)
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and tuple(out.shape) == (n, 4)
+    rc = load_library().bh_direct_forces(pos_mass.data_ptr(), n, eps, t0, t1, out.data_ptr(),
+                                         C.c_void_p(torch.cuda.current_stream(pos_mass.device).cuda_stream))
+    if rc != BH_OK:
+        raise BhError(rc, "bh_direct_forces")
+    return out
 
 
 STAGES = ["bbox", "keys", "sort", "reorder", "cells", "groups", "moments", "record", "walk", "lists", "eval"]
