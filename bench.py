@@ -209,7 +209,7 @@ def run_ours(args):
     cfg, n = _workload(args)
     pm, vel, prm = _make_inputs(cfg, n, rank)
     theta, eps, dt = args.theta or prm["theta"], prm["eps"], prm["dt"]
-    bh = BarnesHut(n, max_cells=args.max_cells)
+    bh = BarnesHut(n, max_cells=args.max_cells, list_entries=args.list_entries, walk_waves=args.walk_waves)
     bh.set_particles(pm, vel)
     bh.tree_build()
     bh.compute_forces(theta, eps)
@@ -363,6 +363,8 @@ def main():
     ap.add_argument("--n", type=int, default=0)
     ap.add_argument("--theta", type=float, default=0.0)
     ap.add_argument("--max-cells", dest="max_cells", type=int, default=0)
+    ap.add_argument("--list-entries", dest="list_entries", type=int, default=0, help="capacity of the interaction-list buffer (0: default)")
+    ap.add_argument("--walk-waves", dest="walk_waves", type=int, default=0, help="k > 1: pipelined walk over at least k waves (0: default)")
     ap.add_argument("--ref-groups", dest="ref_groups", type=int, default=None)
     ap.add_argument("--no-cpu", dest="no_cpu", action="store_true")
     ap.add_argument("--no-e2e", dest="no_e2e", action="store_true", help="skip the host-buffer leg (for profiling runs)")

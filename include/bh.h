@@ -52,8 +52,9 @@ typedef struct bh_config {
                            * clamp(320 * n_max, 2^22, 2^30).  Bounds memory only: groups whose lists do not fit are walked and
                            * evaluated by the fused kernel, with identical counts and forces within rounding. */
     int32_t walk_mode; /* 0 (default): list walk + list evaluation, fused kernel for what does not fit; 1: fused kernel only */
-    int32_t walk_waves; /* 0 (default): as few waves as the list buffer allows (normally 1); k > 1: at least k waves of groups,
-                         * run as a pipeline (list walk of wave w + 1 beside the evaluation of wave w); 0..255 */
+    int32_t walk_waves; /* 0 (default): as few waves of groups as the list buffer allows (normally 1), one after the other;
+                         * k > 1: at least k waves, run as a pipeline (list walk of wave w + 1 beside the evaluation of
+                         * wave w on internal streams); 0..255 */
 } bh_config;
 
 typedef struct bh_ctx bh_ctx;

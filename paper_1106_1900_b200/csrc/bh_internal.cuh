@@ -57,6 +57,7 @@ struct WalkCtl {
     uint32_t wave_g[kMaxWaves + 1];
     uint32_t list_next[kMaxWaves + 1];
     uint32_t eval_next[kMaxWaves + 1];
+    uint32_t arena_next[kMaxWaves + 1];   // list-region cursor of each wave (chunks handed to walking warps)
     uint32_t n_deferred;
     uint32_t fused_next;
     // %globaltimer (ns) of the first block start / last block end of every list walk [0] and evaluation [1] (bh_get_walk_timeline)
@@ -195,7 +196,7 @@ struct WalkListOut {       // what k_walk_lists writes
 };
 WalkListOut walk_list_out(bh_ctx* c);
 int stage_walk_prepare(bh_ctx* c, int nwaves, uint32_t wave_particles, cudaStream_t s);
-int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t arena_base, uint32_t arena_entries, cudaStream_t s);   // S7
+int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t region_base, uint32_t region_entries, cudaStream_t s);   // S7
 int stage_walk_eval(bh_ctx* c, int wave, float eps, int blocks_per_sm, cudaStream_t s);                           // S8
 int stage_kick_drift(bh_ctx* c, float h, float dt, cudaStream_t s);  // S9
 int stage_kick(bh_ctx* c, float h, cudaStream_t s);                  // S9

@@ -270,16 +270,16 @@ static double list_entries_per_particle(float theta) { return 32.0 / ((double)th
 constexpr int kPipeEvalBlocks = 3;    // evaluation blocks per SM while a list walk runs beside them (12 warps x 128 registers)
 constexpr int kPipeListBlocks = 1;    // ... which leaves registers and shared memory for this many list blocks per SM
 
-// One wave (the default whenever the lists of all groups fit the list buffer): list walk, then evaluation, on the caller's
-// stream.  Several waves (the buffer is too small, or bh_config.walk_waves asks for them): a two-stage pipeline over
-// contiguous particle ranges.  The list walk of wave w + 1 runs BESIDE the evaluation of wave w (internal stream
-// s_lists); the evaluations alternate between the caller's stream and s_eval2 so that the tail of one wave overlaps the
-// head of the next; the list buffer is used in halves (wave parity), and the list walk of wave w + 2 waits for the
-// evaluation of wave w.  Everything is joined back into the caller's stream with events: no host synchronisation, and
-// the fork/join pattern can be captured into a CUDA graph.
-// Measured on B200 (c2, bh_get_walk_timeline): the pipeline does overlap, but it does not pay at this size -- 12
-// evaluation warps + 8 list warps per SM take 2.96 ms (8 waves) against 2.36 ms for one wave: the list walk is bound
-// by instruction issue (~5800 warp instructions per group), so beside the evaluation it starves; hence the default.
+// Waves are contiguous particle ranges whose lists are expected to fit the list buffer; normally there is one.  By
+// default the waves run one after the other on the caller's stream (list walk, evaluation, list walk, ...).
+// bh_config.walk_waves = k > 1 asks for a two-stage PIPELINE over at least k waves instead: the list walk of wave w + 1
+// runs BESIDE the evaluation of wave w (internal stream s_lists); the evaluations alternate between the caller's stream
+// and s_eval2 so that the tail of one wave overlaps the head of the next; the list buffer is used in halves (wave
+// parity), and the list walk of wave w + 2 waits for the evaluation of wave w.  Everything is joined back into the
+// caller's stream with events: no host synchronisation, and the fork/join pattern can be captured into a CUDA graph.
+// Measured on B200 (c2, bh_get_walk_timeline): the pipeline does overlap, but it does not pay -- 12 evaluation warps +
+// 8 list warps per SM take 2.96 ms (8 waves) against 2.38 ms for one wave: the list walk is bound by instruction issue
+// (~5800 warp instructions per group), so beside the evaluation it starves.  Hence opt-in.
 int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
     if (c->timing) cudaEventRecord(c->ev[8], s);
     int rc = stage_cell_record(c, theta, s);
@@ -287,11 +287,11 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
     if (c->timing) cudaEventRecord(c->ev[9], s);
     const bool fused_only = c->walk_mode == 1;
     c->walk_split_timed = false;
-    // ---- waves: each must fit half of the list buffer 1.5 times over
+    // ---- waves: each must fit the list buffer (pipelined: half of it) 1.5 times over
+    const bool pipelined = c->walk_waves > 1;            // bh_config.walk_waves: 0 = as few waves as the buffer allows, one after the other
     const double need = 1.5 * list_entries_per_particle(theta) * (double)c->n;
-    int64_t nwaves = (int64_t)std::ceil(need / (double)c->list_entries);
-    if (nwaves > 1) nwaves = (int64_t)std::ceil(2.0 * need / (double)c->list_entries);   // pipelined: halves of the buffer
-    nwaves = std::max<int64_t>(nwaves, c->walk_waves);   // bh_config.walk_waves: 0 = as few as the list buffer allows
+    int64_t nwaves = (int64_t)std::ceil((pipelined ? 2.0 : 1.0) * need / (double)c->list_entries);
+    nwaves = std::max<int64_t>(nwaves, c->walk_waves);
     nwaves = std::min<int64_t>(nwaves, std::max<int64_t>(1, c->n / 4096));
     nwaves = std::max<int64_t>(1, std::min<int64_t>(nwaves, kMaxWaves));
     const int64_t wave_particles = div_up(c->n, nwaves);
@@ -302,13 +302,16 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
         // one block of eight warps per ~128 particles (~7 groups); alone on the device: up to 5 resident blocks per SM
         const int grid_alone = (int)std::max<int64_t>(1, std::min<int64_t>(div_up(wave_particles, 128), (int64_t)c->sm_count * 5));
         const int grid_beside = (int)std::max<int64_t>(1, std::min<int64_t>(div_up(wave_particles, 128), (int64_t)c->sm_count * kPipeListBlocks));
-        if (W == 1) {
+        if (!pipelined || W == 1) {
+            // one wave after the other on the caller's stream; every wave has the whole list buffer and the whole device
             const uint32_t whole = (uint32_t)std::min<int64_t>(c->list_entries, (int64_t)1 << 30);
-            if ((rc = stage_walk_lists(c, 0, grid_alone, 0u, whole / ((uint32_t)grid_alone * 8u), s)) != BH_OK) return rc;
-            if (c->timing) cudaEventRecord(c->ev[11], s);
-            if ((rc = stage_walk_eval(c, 0, eps, 99, s)) != BH_OK) return rc;
-            if (c->timing) cudaEventRecord(c->ev[12], s);
-            c->walk_split_timed = c->timing;
+            for (int w = 0; w < W; ++w) {
+                if ((rc = stage_walk_lists(c, w, grid_alone, 0u, whole, s)) != BH_OK) return rc;
+                if (W == 1 && c->timing) cudaEventRecord(c->ev[11], s);
+                if ((rc = stage_walk_eval(c, w, eps, 99, s)) != BH_OK) return rc;
+                if (W == 1 && c->timing) cudaEventRecord(c->ev[12], s);
+            }
+            c->walk_split_timed = c->timing && W == 1;
         } else {
             cudaStream_t sl = c->s_lists, s2 = c->s_eval2;
             BH_CUDA(c, cudaEventRecord(c->ev_fork, s));
@@ -318,7 +321,7 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
                 // lists of wave w (nothing runs beside wave 0: it gets the whole device)
                 if (w >= 2) BH_CUDA(c, cudaStreamWaitEvent(sl, c->ev_eval[w - 2], 0));
                 const int grid = (w == 0) ? grid_alone : grid_beside;
-                if ((rc = stage_walk_lists(c, w, grid, (w & 1) ? half : 0u, half / ((uint32_t)grid * 8u), sl)) != BH_OK) return rc;
+                if ((rc = stage_walk_lists(c, w, grid, (w & 1) ? half : 0u, half, sl)) != BH_OK) return rc;
                 BH_CUDA(c, cudaEventRecord(c->ev_lists[w], sl));
                 // evaluation of wave w
                 cudaStream_t se = (w & 1) ? s2 : s;

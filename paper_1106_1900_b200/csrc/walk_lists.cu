@@ -18,9 +18,12 @@
 //   * accepted cells -> the group's cell list; opened nodes -> back onto the stack (one 8-byte entry, ballot-compacted);
 //     opened leaves -> a small queue that is expanded 32 leaves at a time into the group's particle list, minus the
 //     group's own particles (A19).
-// List memory: every warp owns an arena of the list buffer; cell lists grow upward from its bottom, particle lists
-// downward from its top, so both lists of a group are contiguous.  A group that does not fit is rolled back and handed
-// to the fused fallback kernel (walk.cu), so the capacity of the list buffer bounds memory, never correctness.
+// List memory: a warp takes chunks of the wave's list region from a device cursor; inside a chunk cell lists grow upward
+// from the bottom, particle lists downward from the top, so both lists of a group are contiguous.  A group that does not
+// fit the rest of its warp's chunk is walked again in a fresh chunk; a group that does not fit a whole chunk, or finds
+// the region used up, is handed to the fused fallback kernel (walk.cu): the capacity of the list buffer bounds memory,
+// never correctness.
+#include <algorithm>
 #include "walk_common.cuh"
 
 namespace bh {
@@ -68,7 +71,7 @@ __device__ __forceinline__ bool flush_leaves(const uint2* q, int k, int lane, ui
     return true;
 }
 
-__device__ __forceinline__ void list_group(ListWarpShared* ws, const int lane, const uint32_t g, const uint32_t gb, const uint32_t ge,
+__device__ __forceinline__ bool list_group(ListWarpShared* ws, const int lane, const uint32_t g, const uint32_t gb, const uint32_t ge,
                                            const float4* __restrict__ pos, const float4* __restrict__ trec, const uint2* __restrict__ tlink,
                                            const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
                                            const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
@@ -174,11 +177,21 @@ __device__ __forceinline__ void list_group(ListWarpShared* ws, const int lane, c
         sums.pc += (unsigned long long)(pc_top - pc0) * (unsigned long long)ng;
         sums.pp += (unsigned long long)npp * (unsigned long long)ng;
         sums.mac += nmac;
-    } else if (lane == 0) {            // roll back; the fused kernel walks and evaluates this group
-        o.g_pcoff[g] = kNone;
-        o.deferred[atomicAdd(&o.ctl->n_deferred, 1u)] = g;
     }
     __syncwarp();
+    return fits;                       // false: nothing was committed (the entries written so far are simply abandoned)
+}
+
+// A chunk of the wave's list region for this warp (bump allocation from a device cursor).  False when the region is used up.
+__device__ __forceinline__ bool alloc_chunk(WalkCtl* ctl, int wave, int lane, uint32_t region_base, uint32_t region_entries,
+                                            uint32_t chunk_entries, ListArena& ar) {
+    uint32_t off = 0;
+    if (lane == 0) off = atomicAdd(&ctl->arena_next[wave], chunk_entries);
+    off = __shfl_sync(0xFFFFFFFFu, off, 0);
+    if (off > region_entries || region_entries - off < chunk_entries) { ar.pc_top = ar.pp_bot = 0u; return false; }
+    ar.pc_top = region_base + off;
+    ar.pp_bot = ar.pc_top + chunk_entries;
+    return true;
 }
 
 __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, int wave, const float4* __restrict__ pos,
@@ -186,15 +199,14 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
                                                                 const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
                                                                 const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
                                                                 const uint32_t* __restrict__ g_begin, uint32_t* __restrict__ lists,
-                                                                uint32_t arena_base, uint32_t arena_entries) {
+                                                                uint32_t region_base, uint32_t region_entries, uint32_t chunk_entries) {
     __shared__ ListWarpShared s_ws[kListWarps];
     __shared__ uint32_t s_chunk, s_taken;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t g0 = o.ctl->wave_g[wave], g1 = o.ctl->wave_g[wave + 1];
     if (threadIdx.x == 0) atomicMin(&o.ctl->t_start[0][wave], global_ns());
-    ListArena ar;
-    ar.pc_top = arena_base + (blockIdx.x * kListWarps + warp) * arena_entries;
-    ar.pp_bot = ar.pc_top + arena_entries;
+    ListArena ar = {0u, 0u};           // this warp's current chunk of the list region: cell lists grow up, particle lists down
+    uint32_t last_total = 0u;          // entries of the last group this warp listed: Morton neighbours need about as many
     WalkSums sums = {0ull, 0ull, 0ull};
     for (;;) {
         __syncthreads();               // everyone is done with the previous chunk's counters
@@ -210,7 +222,27 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
             if (i >= nchunk) break;
             const uint32_t g = base + i;
             const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
-            list_group(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
+            // a fresh chunk if this one will probably not do; a second try in a fresh chunk if it did not; a group that does
+            // not fit a whole chunk (or finds the region used up) goes to the fused kernel instead
+            bool fresh = false;
+            if (ar.pp_bot - ar.pc_top < last_total + (last_total >> 2) + 64u) {
+                fresh = true;
+                alloc_chunk(o.ctl, wave, lane, region_base, region_entries, chunk_entries, ar);
+            }
+            const uint32_t before = ar.pp_bot - ar.pc_top;
+            bool ok = before != 0u && list_group(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
+            if (!ok && !fresh && alloc_chunk(o.ctl, wave, lane, region_base, region_entries, chunk_entries, ar)) {
+                const uint32_t b2 = ar.pp_bot - ar.pc_top;
+                ok = list_group(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
+                if (ok) last_total = b2 - (ar.pp_bot - ar.pc_top);
+            } else if (ok) {
+                last_total = before - (ar.pp_bot - ar.pc_top);
+            }
+            if (!ok && lane == 0) {
+                o.g_pcoff[g] = kNone;
+                o.deferred[atomicAdd(&o.ctl->n_deferred, 1u)] = g;
+            }
+            __syncwarp();
         }
     }
     if (threadIdx.x == 0) atomicMax(&o.ctl->t_end[0][wave], global_ns());
@@ -237,6 +269,7 @@ __global__ void k_walk_prepare(DevScalars* sc, WalkCtl* ctl, const uint32_t* __r
         ctl->wave_g[t] = lo;
         ctl->list_next[t] = 0;
         ctl->eval_next[t] = 0;
+        ctl->arena_next[t] = 0;
         ctl->t_start[0][t] = ctl->t_start[1][t] = ~0ull;
         ctl->t_end[0][t] = ctl->t_end[1][t] = 0ull;
     }
@@ -247,10 +280,13 @@ __global__ void k_walk_prepare(DevScalars* sc, WalkCtl* ctl, const uint32_t* __r
     }
 }
 
-int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t arena_base, uint32_t arena_entries, cudaStream_t s) {
+int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t region_base, uint32_t region_entries, cudaStream_t s) {
+    // chunk: a third of a warp's even share of the region, within [4096, 65536] entries (a group's lists must fit one chunk)
+    const uint32_t share = region_entries / ((uint32_t)grid * kListWarps * 3u);
+    const uint32_t chunk_entries = std::min(std::max(std::min(share, 65536u), 4096u), region_entries);
     WalkListOut o = walk_list_out(c);
     BH_LAUNCH(c, k_walk_lists, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
-              c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, arena_base, arena_entries);
+              c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries);
     return BH_OK;
 }
 
