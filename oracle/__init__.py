@@ -141,23 +141,27 @@ def moments(t: Tree, pos_sorted) -> Tree:
     return t
 
 
-def cell_floats(t: Tree, theta: float):
+MAC_EQ1 = 0       # PAPER.md:125, Eq.1: d(group box, centre of mass) > l / theta + delta
+MAC_MINDIST = 1   # PAPER.md:129 "minimal distance MAC [31]" (reading A28): d(group box, cell box) > l / theta
+
+
+def cell_floats(t: Tree, theta: float, mac_kind: int = MAC_EQ1):
     """O8 float outputs: (mom32 float32[C,10], mac float32[C,3] = l, delta, r2_open)."""
     mom32 = np.empty((t.ncells, 10), np.float32)
     mac = np.empty((t.ncells, 3), np.float32)
-    lib().orc_cell_floats(C.c_int64(t.ncells), _p(t.mom64), _p(t.box), C.c_float(theta), _p(mom32), _p(mac))
+    lib().orc_cell_floats(C.c_int64(t.ncells), _p(t.mom64), _p(t.box), C.c_float(theta), C.c_int32(mac_kind), _p(mom32), _p(mac))
     return mom32, mac
 
 
 def walk_forces(t: Tree, pos_sorted, theta: float, eps: float, sel=None, forces: bool = True,
-                want_lists: bool = False):
+                want_lists: bool = False, mac_kind: int = MAC_EQ1):
     """O9 + O10 for the selected groups (default: all).
 
     Returns dict(npc int64[G], npp int64[G], accpot float64[N,4] or None, mom32, mac[, cells, leaves]).
     Entries of npc / npp / accpot outside the selection are -1 / NaN.
     """
     pm = _f32c(pos_sorted)
-    mom32, mac = cell_floats(t, theta)
+    mom32, mac = cell_floats(t, theta, mac_kind)
     G = t.ngroups
     sel = np.arange(G, dtype=np.int64) if sel is None else np.ascontiguousarray(sel, np.int64)
     npc = np.full(G, -1, np.int64)
@@ -169,7 +173,7 @@ def walk_forces(t: Tree, pos_sorted, theta: float, eps: float, sel=None, forces:
         lc = np.full(t.ncells, -1, np.int64)
         ll = np.full(t.ncells, -1, np.int64)
     lib().orc_walk_forces(C.c_int64(t.n), _p(pm), _p(t.nchild), _p(t.child_begin), _p(t.pbegin), _p(t.pcount),
-                          _p(mom32), _p(mac), _p(t.gbegin), _p(t.gcount), _p(t.gbox),
+                          _p(mom32), _p(mac), C.c_int32(mac_kind), _p(t.box), _p(t.gbegin), _p(t.gcount), _p(t.gbox),
                           C.c_int64(sel.shape[0]), _p(sel), C.c_float(eps), _p(npc), _p(npp), _p(acc),
                           _p(lc), C.c_int64(t.ncells), _p(ll), C.c_int64(t.ncells))
     out = dict(npc=npc, npp=npp, accpot=acc, mom32=mom32, mac=mac)
@@ -242,9 +246,9 @@ def tree_build(pos_mass, vel=None, ids=None, nleaf: int = NLEAF, ncrit: int = NC
     return State(ps, vs, idss, perm, ks, lo, e, t)
 
 
-def compute_forces(st: State, theta: float, eps: float, sel=None, forces: bool = True) -> State:
+def compute_forces(st: State, theta: float, eps: float, sel=None, forces: bool = True, mac_kind: int = MAC_EQ1) -> State:
     """O9 + O10."""
-    r = walk_forces(st.tree, st.pos, theta, eps, sel=sel, forces=forces)
+    r = walk_forces(st.tree, st.pos, theta, eps, sel=sel, forces=forces, mac_kind=mac_kind)
     st.npc, st.npp, st.accpot, st.mom32, st.mac = r["npc"], r["npp"], r["accpot"], r["mom32"], r["mac"]
     return st
 

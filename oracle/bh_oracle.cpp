@@ -273,7 +273,10 @@ void orc_moments(int64_t C, const int64_t* level_offset, const int32_t* nchild,
 // l = max_k (bmax_k -f bmin_k); gc_k = 0.5f *f (bmin_k +f bmax_k); u = com~ -f gc;
 // delta = sqrtf(((ux*ux) +f (uy*uy)) +f (uz*uz)); r_open = (l /f theta) +f delta; r2_open = r_open *f r_open.
 // mom32: float[C][10] (same order as mom64);  mac: float[C][3] = l, delta, r2_open.
-void orc_cell_floats(int64_t C, const double* mom64, const float* box, float theta,
+// mac_kind 0: Eq.1 (L125), r_open = l / theta + delta.  mac_kind 1: the minimum-distance MAC the paper also implemented
+// (L129, [31]; reading A28): r_open = l / theta, to be compared with the distance between the group's box and the
+// cell's tight BOX instead of its centre of mass (orc_walk_forces).
+void orc_cell_floats(int64_t C, const double* mom64, const float* box, float theta, int32_t mac_kind,
                      float* mom32, float* mac) {
     for (int64_t c = 0; c < C; ++c) {
         for (int k = 0; k < 10; ++k) mom32[10 * c + k] = (float)mom64[10 * c + k];
@@ -286,7 +289,7 @@ void orc_cell_floats(int64_t C, const double* mom64, const float* box, float the
         }
         const float s2 = ((u[0] * u[0]) + (u[1] * u[1])) + (u[2] * u[2]);
         const float delta = sqrtf(s2);
-        const float ropen = (l / theta) + delta;
+        const float ropen = mac_kind == 1 ? (l / theta) : (l / theta) + delta;
         mac[3 * c + 0] = l;
         mac[3 * c + 1] = delta;
         mac[3 * c + 2] = ropen * ropen;
@@ -309,6 +312,7 @@ void orc_group_boxes(int64_t G, const int64_t* gbegin, const int64_t* gcount, co
 // O9 (L83, L87, Eq.1; A16, A17): breadth-first from the root;  d_k = max(max(gmin_k -f com_k, com_k -f gmax_k), 0);
 //   d2 = fmaf(dz, dz, fmaf(dy, dy, dx *f dx));  d2 > r2_open -> cell list; else leaf -> particle list; else
 //   children queued.  n_pc = accepted cells, n_pp = sum of pcount over opened leaves.
+//   mac_kind 1 (L129, A28): d_k = max(max(gmin_k -f cmax_k, cmin_k -f gmax_k), 0) with the cell's tight box, r2_open = (l / theta)^2.
 // O10 (L85, L109; A18, A19, A22), binary64 from the float inputs, eps2 = eps * eps:
 //   p-p (j != i): dr = x_j - x_i, rho2 = |dr|^2 + eps2: phi -= m_j / rho; a += m_j dr / rho^3.
 //   p-c: dr = com - x_i, T = Qxx+Qyy+Qzz, q = Q dr, w = dr . q:
@@ -319,7 +323,7 @@ void orc_group_boxes(int64_t G, const int64_t* gbegin, const int64_t* gcount, co
 void orc_walk_forces(int64_t n, const float* pos4,
                      const int32_t* nchild, const int64_t* child_begin,
                      const int64_t* pbegin, const int64_t* pcount,
-                     const float* mom32, const float* mac,
+                     const float* mom32, const float* mac, int32_t mac_kind, const float* box,
                      const int64_t* gbegin, const int64_t* gcount, const float* gbox,
                      int64_t nsel, const int64_t* sel, float eps,
                      int64_t* npc, int64_t* npp, double* accpot,
@@ -338,7 +342,12 @@ void orc_walk_forces(int64_t n, const float* pos4,
             const int64_t c = queue[head++];
             const float* cm = mom32 + 10 * c + 1;
             float d[3];
-            for (int k = 0; k < 3; ++k) d[k] = std::max(std::max(gb[k] - cm[k], cm[k] - gb[3 + k]), 0.0f);
+            if (mac_kind == 1) {      // A28: per-axis gap between the group's box and the cell's tight box (0 where they overlap)
+                const float* cb = box + 6 * c;
+                for (int k = 0; k < 3; ++k) d[k] = std::max(std::max(gb[k] - cb[3 + k], cb[k] - gb[3 + k]), 0.0f);
+            } else {
+                for (int k = 0; k < 3; ++k) d[k] = std::max(std::max(gb[k] - cm[k], cm[k] - gb[3 + k]), 0.0f);
+            }
             const float d2 = fmaf(d[2], d[2], fmaf(d[1], d[1], d[0] * d[0]));
             if (d2 > mac[3 * c + 2]) {
                 cells_acc.push_back(c);

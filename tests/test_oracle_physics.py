@@ -279,3 +279,57 @@ def test_deterministic_across_runs():
     a = oracle.walk_forces(st.tree, st.pos, 0.75, 0.01)
     b = oracle.walk_forces(st.tree, st.pos, 0.75, 0.01)
     assert np.array_equal(a["accpot"], b["accpot"]) and np.array_equal(a["npc"], b["npc"])
+
+
+# ---------------------------------------------------------------- minimum-distance MAC (reading A28)
+def _mindist_accept_np(gbox, cbox, theta):
+    """A28 restated in numpy float32: per-axis gap between two boxes, d2 by fused multiply-adds, accept iff d2 > (l / theta)^2."""
+    f = np.float32
+    d = np.maximum(np.maximum(gbox[:3] - cbox[3:], cbox[:3] - gbox[3:]), f(0)).astype(np.float32)
+    d2 = f(np.float64(d[0]) * np.float64(d[0]))                      # one rounding: the product of two floats is exact in double
+    d2 = f(np.float64(d[1]) * np.float64(d[1]) + np.float64(d2))     # fmaf: exact product + addend, one rounding
+    d2 = f(np.float64(d[2]) * np.float64(d[2]) + np.float64(d2))
+    l = np.max((cbox[3:] - cbox[:3]).astype(np.float32))
+    r = f(l / f(theta))
+    return d2 > f(r * r)
+
+
+def test_mindist_mac_lists_equal_a_walk_written_from_the_definition():
+    st, _ = _state("c1", 3000)
+    t = st.tree
+    theta = 0.6
+    for g in range(0, t.ngroups, 7):
+        r = oracle.walk_forces(t, st.pos, theta=theta, eps=0.01, sel=[g], forces=False, want_lists=True, mac_kind=oracle.MAC_MINDIST)
+        cells, leaves, todo = [], [], [0]
+        while todo:
+            c = todo.pop()
+            if _mindist_accept_np(t.gbox[g], t.box[c], theta):
+                cells.append(c)
+            elif t.nchild[c] == 0:
+                leaves.append(c)
+            else:
+                todo.extend(range(t.child_begin[c], t.child_begin[c] + t.nchild[c]))
+        assert sorted(cells) == sorted(r["cells"].tolist()) and sorted(leaves) == sorted(r["leaves"].tolist())
+        # an accepted cell's box is strictly separated from the group's box, and the lists cover every particle once
+        for c in cells:
+            gap = np.maximum(np.maximum(t.gbox[g][:3] - t.box[c][3:], t.box[c][:3] - t.gbox[g][3:]), 0)
+            assert np.any(gap > 0)
+        assert t.pcount[cells].sum() + t.pcount[leaves].sum() == t.n
+
+
+def test_mindist_mac_limits_and_accuracy():
+    st, _ = _state("c1", 4096)
+    d = oracle.direct(st.pos, 0.01)
+    # theta -> 0: the direct sum
+    oracle.compute_forces(st, theta=1e-6, eps=0.01, mac_kind=oracle.MAC_MINDIST)
+    assert _relerr(st.accpot, d).max() < 1e-12          # (accepted cells are single particles: l = 0, exact)
+    # same theta: opens more than Eq.1 and is more accurate (the paper: smaller error, more interactions, L129)
+    oracle.compute_forces(st, theta=0.75, eps=0.01)
+    n0, e0 = st.npc.sum() + st.npp.sum(), _relerr(st.accpot, d)
+    oracle.compute_forces(st, theta=0.75, eps=0.01, mac_kind=oracle.MAC_MINDIST)
+    n1, e1 = st.npc.sum() + st.npp.sum(), _relerr(st.accpot, d)
+    assert n1 > n0 and np.median(e1) < np.median(e0) and np.quantile(e1, 0.99) < np.quantile(e0, 0.99)
+    # r2_open is (l / theta)^2 with l the longest side of the tight box
+    l = (st.tree.box[:, 3:] - st.tree.box[:, :3]).max(axis=1).astype(np.float32)
+    r = (l / np.float32(0.75)).astype(np.float32)
+    assert np.array_equal(st.mac[:, 2], (r * r).astype(np.float32))
