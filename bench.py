@@ -211,6 +211,7 @@ def run_ours(args):
     theta, eps, dt = args.theta or prm["theta"], prm["eps"], prm["dt"]
     bh = BarnesHut(n, max_cells=args.max_cells, list_entries=args.list_entries, walk_waves=args.walk_waves)
     bh.set_particles(pm, vel)
+    bh.set_mac(args.mac)
     bh.tree_build()
     bh.compute_forces(theta, eps)
     bh.sync_status()
@@ -331,7 +332,7 @@ def run_ours(args):
         "vs_baseline": value / PAPER_PARTICLES_PER_S if (cfg == "c2" and abs(theta - 0.75) < 1e-6 and world == 1) else None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{cfg}: Plummer sphere n={n}" if cfg in ("c1", "c2") else f"{cfg}: n={n}",
-                   "theta": theta, "eps": eps, "dt": dt, "nleaf": 16, "ncrit": 64, "rebuild_every_step": True,
+                   "theta": theta, "eps": eps, "dt": dt, "nleaf": 16, "ncrit": 64, "mac": "min_distance" if args.mac else "eq1", "rebuild_every_step": True,
                    "l2": f"{L2_FLUSH_BYTES >> 20} MiB buffer written between timed steps (outside the event pairs)",
                    "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
                    "cells": int(s1.n_cells), "groups": int(s1.n_groups), "levels": int(s1.n_levels),
@@ -365,6 +366,7 @@ def main():
     ap.add_argument("--max-cells", dest="max_cells", type=int, default=0)
     ap.add_argument("--list-entries", dest="list_entries", type=int, default=0, help="capacity of the interaction-list buffer (0: default)")
     ap.add_argument("--walk-waves", dest="walk_waves", type=int, default=0, help="k > 1: pipelined walk over at least k waves (0: default)")
+    ap.add_argument("--mac", type=int, default=0, choices=[0, 1], help="0: Eq.1 (the metric's configuration); 1: minimum-distance MAC (PAPER.md:129)")
     ap.add_argument("--ref-groups", dest="ref_groups", type=int, default=None)
     ap.add_argument("--no-cpu", dest="no_cpu", action="store_true")
     ap.add_argument("--no-e2e", dest="no_e2e", action="store_true", help="skip the host-buffer leg (for profiling runs)")

@@ -128,6 +128,14 @@ int bh_tree_build(bh_ctx* ctx, void* stream);
  * with Plummer softening `eps` (L85, L97).  Needs bh_tree_build.  eps = 0 with coincident particles is undefined. */
 int bh_compute_forces(bh_ctx* ctx, float theta, float eps, void* stream);
 
+/* Which multipole acceptance criterion S7 uses from the next bh_compute_forces on (the tree need not be rebuilt).
+ *   BH_MAC_EQ1 (default): Eq.1 (L125): d > l / theta + delta, d = distance between the group's box and the cell's centre of
+ *     mass, l = longest side of the cell's tight box, delta = |centre of mass - box centre|.
+ *   BH_MAC_MIN_DISTANCE: the minimum-distance MAC the paper also implemented (L129, [31]; A28): d > l / theta with
+ *     d = distance between the group's box and the cell's tight BOX.  Opens more cells: smaller error, more interactions. */
+enum { BH_MAC_EQ1 = 0, BH_MAC_MIN_DISTANCE = 1 };
+int bh_set_mac(bh_ctx* ctx, int mac);
+
 /* S9 around S0-S8 (L105): v += a dt/2; x += v dt; tree_build; compute_forces; v += a dt/2.  Needs valid forces. */
 int bh_leapfrog_step(bh_ctx* ctx, float theta, float eps, float dt, void* stream);
 

@@ -1,6 +1,6 @@
 """The acceleration-error experiment of PAPER.md:196-204 (section 4.2.1, Eq.2, Fig.8-9), on synthetic Plummer spheres.
 
-    python -m paper_1106_1900_b200.accuracy [--n 32768 131072 1048576] [--theta 0.2 0.3 ... 0.8] [--eps 0.0]
+    python -m paper_1106_1900_b200.accuracy [--n 32768 131072 1048576] [--theta 0.2 0.3 ... 0.8] [--eps 0.0] [--mac 0|1]
 
 For every N: one tree build, one binary64 direct summation on the GPU (bh_direct_forces, the paper's "double precision
 version of Sapporo"), then for every opening angle the fp32 tree forces (bh_compute_forces) and the distribution of
@@ -41,10 +41,11 @@ def exceeded_by(err: np.ndarray, fraction: float) -> float:
     return float(np.quantile(err, 1.0 - fraction))
 
 
-def run(n: int, thetas, eps: float, seed: int | None = None):
+def run(n: int, thetas, eps: float, seed: int | None = None, mac: int = 0):
     pm, vel, _ = bh_inputs.make("c2", n=n, seed=seed)
     bh = BarnesHut(n)
     bh.set_particles(pm, vel)
+    bh.set_mac(mac)
     bh.tree_build()
     bh.compute_forces(float(thetas[0]), eps)
     t = bh.export_tree()                                   # sorted particles (device views of the workspace)
@@ -64,7 +65,7 @@ def run(n: int, thetas, eps: float, seed: int | None = None):
         walk_ms = ev0.elapsed_time(ev1)
         a_tree = t["acc_pot"].cpu().numpy()
         err = relative_error(a_tree, a_direct)
-        out.append({"n": n, "theta": float(th), "eps": eps, "exceeded_by_50pct": exceeded_by(err, 0.5),
+        out.append({"n": n, "theta": float(th), "eps": eps, "mac": "min_distance" if mac else "eq1", "exceeded_by_50pct": exceeded_by(err, 0.5),
                     "exceeded_by_10pct": exceeded_by(err, 0.1), "exceeded_by_1pct": exceeded_by(err, 0.01), "max": float(err.max()),
                     "pp_per_particle": st.sum_pp / n, "pc_per_particle": st.sum_pc / n, "walk_ms": walk_ms,
                     "direct_ms": direct_ms, "direct_pairs_per_s": n * (n - 1) / (direct_ms * 1e-3)})
@@ -77,9 +78,10 @@ def main():
     ap.add_argument("--n", type=int, nargs="+", default=[32768, 131072, 1048576])
     ap.add_argument("--theta", type=float, nargs="+", default=[0.2, 0.3, 0.4, 0.5, 0.6, 0.7, 0.8])
     ap.add_argument("--eps", type=float, default=0.0)
+    ap.add_argument("--mac", type=int, default=0, choices=[0, 1], help="0: Eq.1; 1: minimum-distance MAC (PAPER.md:129)")
     args = ap.parse_args()
     for n in args.n:
-        for row in run(n, args.theta, args.eps):
+        for row in run(n, args.theta, args.eps, mac=args.mac):
             print(json.dumps(row), flush=True)
 
 

@@ -318,6 +318,13 @@ int bh_export_tree(bh_ctx* c, bh_tree_view* v, void* stream) {
     return BH_OK;
 }
 
+int bh_set_mac(bh_ctx* c, int mac) {
+    if (!c || (mac != BH_MAC_EQ1 && mac != BH_MAC_MIN_DISTANCE)) return BH_ERR_INVALID_ARG;
+    c->mac_kind = mac;
+    c->have_forces = false;
+    return BH_OK;
+}
+
 int bh_set_stage_timing(bh_ctx* c, int enable) {
     if (!c) return BH_ERR_INVALID_ARG;
     c->timing = enable != 0;

@@ -141,6 +141,7 @@ struct bh_ctx {
     int64_t list_entries;
     int walk_mode;
     int walk_waves;
+    int mac_kind;          // 0: Eq.1, 1: minimum distance (bh_set_mac)
     bh::Ws ws;
     int64_t sort_tiles, tree_tiles, scan_sum_cap;
     bool timing;

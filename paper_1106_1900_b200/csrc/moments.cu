@@ -132,7 +132,7 @@ __global__ void __launch_bounds__(128) k_moments(const DevScalars* __restrict__ 
 // the force loop consumes (erec, 48 B: (com, M) (Qm_xx, Qm_yy, Qm_zz, Qm_xy) (Qm_xz, Qm_yz, nTh, n3Th)),
 // with the opening radius of Eq.1:  l = longest side of the tight box (A14),
 // delta = |com - box centre|, r2open = (l / theta + delta)^2, all in single fp32 operations (O8).
-__global__ void __launch_bounds__(256) k_cell_record(const DevScalars* __restrict__ sc, float theta,
+__global__ void __launch_bounds__(256) k_cell_record(const DevScalars* __restrict__ sc, float theta, int mac_kind,
                                                      const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
                                                      const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
                                                      const double* __restrict__ mom64, const float* __restrict__ box,
@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(256) k_cell_record(const DevScalars* __restric
         const float uz = __fsub_rn(cz, __fmul_rn(0.5f, __fadd_rn(b[2], b[5])));
         const float s2 = __fadd_rn(__fadd_rn(__fmul_rn(ux, ux), __fmul_rn(uy, uy)), __fmul_rn(uz, uz));
         const float delta = __fsqrt_rn(s2);
-        const float ropen = __fadd_rn(__fdiv_rn(l, theta), delta);
+        const float ropen = mac_kind == 1 ? __fdiv_rn(l, theta) : __fadd_rn(__fdiv_rn(l, theta), delta);   // A28 / Eq.1
         const float r2open = __fmul_rn(ropen, ropen);
         const uint32_t cb = c_cbegin[c], ce = c_cend[c];
         const bool leaf = (ce == cb);
@@ -177,7 +177,7 @@ int stage_moments(bh_ctx* c, cudaStream_t s) {
 
 int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s) {
     const int grid = (int)std::min<int64_t>(div_up(c->max_cells, 256), (int64_t)c->sm_count * 16);
-    BH_LAUNCH(c, k_cell_record, grid, 256, 0, s, c->ws.sc, theta, c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin, c->ws.c_cend,
+    BH_LAUNCH(c, k_cell_record, grid, 256, 0, s, c->ws.sc, theta, c->mac_kind, c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin, c->ws.c_cend,
               c->ws.mom64, c->ws.box, c->ws.trec, c->ws.tlink, c->ws.erec);
     return BH_OK;
 }

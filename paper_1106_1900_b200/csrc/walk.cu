@@ -43,9 +43,10 @@ __device__ __forceinline__ void pp_pad(float* ring, int e_last) {
     pp_store(ring, (e_last + 1) & (kRing - 1), s[0], s[2], s[4], 0.f);
 }
 
+template <int kMac>
 __device__ __noinline__ void walk_group(WarpShared* ws, const int lane, const uint32_t g, const uint32_t gb, const uint32_t ge,
                                         const float4* __restrict__ pos, const float4* __restrict__ trec, const uint2* __restrict__ tlink,
-                                        const float4* __restrict__ erec, float eps2, float4* __restrict__ acc_out,
+                                        const float* __restrict__ box, const float4* __restrict__ erec, float eps2, float4* __restrict__ acc_out,
                                         uint32_t* __restrict__ g_npc, uint32_t* __restrict__ g_npp, DevScalars* sc) {
     const uint32_t lt = (1u << lane) - 1u;
     const int ng = (int)(ge - gb);
@@ -72,7 +73,7 @@ __device__ __noinline__ void walk_group(WarpShared* ws, const int lane, const ui
             cell = ws->stack[sp - 1 - lane];
             const float4 r0 = __ldg(trec + cell);
             const uint2 lk = __ldg(tlink + cell);
-            accept = mac_accept(mn, mx, r0);
+            accept = kMac == kMacMinDist ? mac_accept_box(mn, mx, load_cell_box(box, cell), r0.w) : mac_accept(mn, mx, r0);
             if (!accept) {
                 first = lk.x;
                 cnt = lk.y & 0x7FFFFFFFu;
@@ -203,9 +204,10 @@ __device__ __noinline__ void walk_group(WarpShared* ws, const int lane, const ui
 }
 
 // The groups k_walk_lists deferred (ctl->n_deferred of them; with `all` != 0: every group, the list path is bypassed).
+template <int kMac>
 __global__ void __launch_bounds__(kWalkThreads, 2) k_walk_fused(DevScalars* sc, WalkCtl* ctl, int all, const uint32_t* __restrict__ deferred,
                                                                 const float4* __restrict__ pos, const float4* __restrict__ trec,
-                                                                const uint2* __restrict__ tlink, const float4* __restrict__ erec,
+                                                                const uint2* __restrict__ tlink, const float* __restrict__ box, const float4* __restrict__ erec,
                                                                 const uint32_t* __restrict__ g_begin, float eps2, float4* __restrict__ acc_out,
                                                                 uint32_t* __restrict__ g_npc, uint32_t* __restrict__ g_npp) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -220,7 +222,7 @@ __global__ void __launch_bounds__(kWalkThreads, 2) k_walk_fused(DevScalars* sc, 
         if (i >= count) break;
         const uint32_t g = all ? i : deferred[i];
         const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
-        walk_group(ws, lane, g, gb, ge, pos, trec, tlink, erec, eps2, acc_out, g_npc, g_npp, sc);
+        walk_group<kMac>(ws, lane, g, gb, ge, pos, trec, tlink, box, erec, eps2, acc_out, g_npc, g_npp, sc);
         __syncwarp();
     }
 }
@@ -239,7 +241,8 @@ WalkListOut walk_list_out(bh_ctx* c) {
 }
 
 int walk_init(bh_ctx* c) {
-    BH_CUDA(c, cudaFuncSetAttribute(k_walk_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(WarpShared) * kWalkWarps)));
+    BH_CUDA(c, cudaFuncSetAttribute(k_walk_fused<kMacEq1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(WarpShared) * kWalkWarps)));
+    BH_CUDA(c, cudaFuncSetAttribute(k_walk_fused<kMacMinDist>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(WarpShared) * kWalkWarps)));
     BH_CUDA(c, cudaStreamCreateWithFlags(&c->s_lists, cudaStreamNonBlocking));
     BH_CUDA(c, cudaStreamCreateWithFlags(&c->s_eval2, cudaStreamNonBlocking));
     BH_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
@@ -335,8 +338,12 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
         }
     }
     const size_t smem = sizeof(WarpShared) * kWalkWarps;
-    BH_LAUNCH(c, k_walk_fused, c->sm_count * 2, kWalkThreads, smem, s, c->ws.sc, c->ws.ctl, fused_only ? 1 : 0, c->ws.deferred,
-              c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.erec, c->ws.g_begin, eps * eps, c->ws.acc, c->ws.g_npc, c->ws.g_npp);
+    if (c->mac_kind == kMacMinDist)
+        BH_LAUNCH(c, k_walk_fused<kMacMinDist>, c->sm_count * 2, kWalkThreads, smem, s, c->ws.sc, c->ws.ctl, fused_only ? 1 : 0, c->ws.deferred,
+                  c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.erec, c->ws.g_begin, eps * eps, c->ws.acc, c->ws.g_npc, c->ws.g_npp);
+    else
+        BH_LAUNCH(c, k_walk_fused<kMacEq1>, c->sm_count * 2, kWalkThreads, smem, s, c->ws.sc, c->ws.ctl, fused_only ? 1 : 0, c->ws.deferred,
+                  c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.erec, c->ws.g_begin, eps * eps, c->ws.acc, c->ws.g_npc, c->ws.g_npp);
     if (c->timing) cudaEventRecord(c->ev[10], s);
     return BH_OK;
 }

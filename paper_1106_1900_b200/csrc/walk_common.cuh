@@ -277,4 +277,23 @@ __device__ __forceinline__ bool mac_accept(const float mn[3], const float mx[3],
     return d2 > com_r2.w;
 }
 
+// The minimum-distance MAC the paper also implemented ([31]; reading A28): the distance is taken
+// between the group's box and the cell's tight BOX, and compared with l / theta: accept iff d^2 > r2open, with
+// d_k = max(max(gmin_k - cmax_k, cmin_k - gmax_k), 0) in the same single fp32 operations as Eq.1's test.
+constexpr int kMacEq1 = 0, kMacMinDist = 1;
+struct CellBox { float2 a, b, c; };        // (min x, min y) (min z, max x) (max y, max z): the row of `box` as three 8-byte loads
+__device__ __forceinline__ CellBox load_cell_box(const float* __restrict__ box, uint32_t cell) {
+    const float2* p = reinterpret_cast<const float2*>(box + 6 * (size_t)cell);
+    CellBox r;
+    r.a = __ldg(p); r.b = __ldg(p + 1); r.c = __ldg(p + 2);
+    return r;
+}
+__device__ __forceinline__ bool mac_accept_box(const float mn[3], const float mx[3], const CellBox& cb, float r2open) {
+    const float dx = fmaxf(fmaxf(__fsub_rn(mn[0], cb.b.y), __fsub_rn(cb.a.x, mx[0])), 0.0f);
+    const float dy = fmaxf(fmaxf(__fsub_rn(mn[1], cb.c.x), __fsub_rn(cb.a.y, mx[1])), 0.0f);
+    const float dz = fmaxf(fmaxf(__fsub_rn(mn[2], cb.c.y), __fsub_rn(cb.b.x, mx[2])), 0.0f);
+    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+    return d2 > r2open;
+}
+
 }  // namespace bh

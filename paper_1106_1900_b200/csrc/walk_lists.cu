@@ -71,6 +71,7 @@ __device__ __forceinline__ bool flush_leaves(const uint2* q, int k, int lane, ui
     return true;
 }
 
+template <int kMac>
 __device__ __forceinline__ bool list_group(ListWarpShared* ws, const int lane, const uint32_t g, const uint32_t gb, const uint32_t ge,
                                            const float4* __restrict__ pos, const float4* __restrict__ trec, const uint2* __restrict__ tlink,
                                            const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
@@ -110,6 +111,7 @@ __device__ __forceinline__ bool list_group(ListWarpShared* ws, const int lane, c
         uint32_t cell[kSub];
         float4 r0[kSub];
         uint2 lk[kSub];
+        CellBox cbx[kMac == kMacMinDist ? kSub : 1];
 #pragma unroll
         for (int j = 0; j < kSub; ++j) {
             valid[j] = false;
@@ -125,14 +127,18 @@ __device__ __forceinline__ bool list_group(ListWarpShared* ws, const int lane, c
         for (int j = 0; j < kSub; ++j) {
             r0[j] = make_float4(0.f, 0.f, 0.f, 0.f);
             lk[j] = make_uint2(0u, 0u);
-            if (valid[j]) { r0[j] = __ldg(trec + cell[j]); lk[j] = __ldg(tlink + cell[j]); }
+            if (valid[j]) {
+                r0[j] = __ldg(trec + cell[j]);
+                lk[j] = __ldg(tlink + cell[j]);
+                if (kMac == kMacMinDist) cbx[j] = load_cell_box(box, cell[j]);
+            }
         }
         sp -= kpop;
         __syncwarp();                 // every lane has read its stack entries: the slots may be overwritten
 #pragma unroll
         for (int j = 0; j < kSub; ++j) {
             if (4 * j >= kpop) break;
-            const bool accept = valid[j] && mac_accept(mn, mx, r0[j]);
+            const bool accept = valid[j] && (kMac == kMacMinDist ? mac_accept_box(mn, mx, cbx[j], r0[j].w) : mac_accept(mn, mx, r0[j]));
             const bool isleaf = valid[j] && !accept && (lk[j].y >> 31) != 0u;
             const bool isnode = valid[j] && !accept && !isleaf;
             nmac += (uint32_t)__popc(__ballot_sync(0xFFFFFFFFu, valid[j]));
@@ -194,6 +200,7 @@ __device__ __forceinline__ bool alloc_chunk(WalkCtl* ctl, int wave, int lane, ui
     return true;
 }
 
+template <int kMac>
 __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, int wave, const float4* __restrict__ pos,
                                                                 const float4* __restrict__ trec, const uint2* __restrict__ tlink,
                                                                 const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
@@ -230,10 +237,10 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
                 alloc_chunk(o.ctl, wave, lane, region_base, region_entries, chunk_entries, ar);
             }
             const uint32_t before = ar.pp_bot - ar.pc_top;
-            bool ok = before != 0u && list_group(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
+            bool ok = before != 0u && list_group<kMac>(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
             if (!ok && !fresh && alloc_chunk(o.ctl, wave, lane, region_base, region_entries, chunk_entries, ar)) {
                 const uint32_t b2 = ar.pp_bot - ar.pc_top;
-                ok = list_group(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
+                ok = list_group<kMac>(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
                 if (ok) last_total = b2 - (ar.pp_bot - ar.pc_top);
             } else if (ok) {
                 last_total = before - (ar.pp_bot - ar.pc_top);
@@ -285,13 +292,19 @@ int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t region_base, uint32
     const uint32_t share = region_entries / ((uint32_t)grid * kListWarps * 3u);
     const uint32_t chunk_entries = std::min(std::max(std::min(share, 65536u), 4096u), region_entries);
     WalkListOut o = walk_list_out(c);
-    BH_LAUNCH(c, k_walk_lists, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
+    if (c->mac_kind == kMacMinDist) {
+        BH_LAUNCH(c, k_walk_lists<kMacMinDist>, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
+                  c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries);
+        return BH_OK;
+    }
+    BH_LAUNCH(c, k_walk_lists<kMacEq1>, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
               c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries);
     return BH_OK;
 }
 
 int walk_lists_init(bh_ctx* c) {
-    BH_CUDA(c, cudaFuncSetAttribute(k_walk_lists, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
+    BH_CUDA(c, cudaFuncSetAttribute(k_walk_lists<kMacEq1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
+    BH_CUDA(c, cudaFuncSetAttribute(k_walk_lists<kMacMinDist>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
     return BH_OK;
 }
 

@@ -14,9 +14,10 @@ RMS_TOL = 1e-5
 MAX_TOL = 1e-4
 
 
-def gpu_tree(bh, pos_mass, vel, theta, eps, ids=None):
+def gpu_tree(bh, pos_mass, vel, theta, eps, ids=None, mac=0):
     """set_particles + tree_build + compute_forces + export, as numpy arrays."""
     bh.set_particles(pos_mass, vel, ids)
+    bh.set_mac(mac)
     bh.tree_build()
     bh.compute_forces(theta, eps)
     return export_numpy(bh)
@@ -110,7 +111,7 @@ def check_forces(g, st, sel=None):
     return e
 
 
-def oracle_state(pos_mass, vel, theta, eps, ids=None, sel=None, forces=True, nleaf=16, ncrit=64):
+def oracle_state(pos_mass, vel, theta, eps, ids=None, sel=None, forces=True, nleaf=16, ncrit=64, mac=0):
     st = oracle.tree_build(pos_mass, vel, ids, nleaf, ncrit)
-    oracle.compute_forces(st, theta, eps, sel=sel, forces=forces)
+    oracle.compute_forces(st, theta, eps, sel=sel, forces=forces, mac_kind=mac)
     return st

@@ -23,10 +23,10 @@ def BH():
     return BarnesHut
 
 
-def _full_parity(BH, pm, vel, theta, eps, **cfg):
+def _full_parity(BH, pm, vel, theta, eps, mac=0, **cfg):
     bh = BH(pm.shape[0], **cfg)
-    g = gpu_tree(bh, pm, vel, theta, eps)
-    st = oracle_state(pm, vel, theta, eps, nleaf=cfg.get("nleaf", 0) or 16, ncrit=cfg.get("ncrit", 0) or 64)
+    g = gpu_tree(bh, pm, vel, theta, eps, mac=mac)
+    st = oracle_state(pm, vel, theta, eps, nleaf=cfg.get("nleaf", 0) or 16, ncrit=cfg.get("ncrit", 0) or 64, mac=mac)
     bad = compare_tree(g, st)
     compare_counts(g, st, problems=bad)
     assert not bad, "\n".join(bad)
@@ -60,6 +60,38 @@ def test_walk_in_several_waves(BH, cfg):
     wave w on internal streams; same counts, same forces."""
     pm, vel, prm = bh_inputs.make("c1", n=40000, seed=17)
     _full_parity(BH, pm, vel, prm["theta"], prm["eps"], **cfg)
+
+
+@pytest.mark.parametrize("cfg,n,theta,extra", [("c1", 16384, 0.75, {}), ("c1", 4097, 0.5, {}), ("c3", 12289, 0.6, {}), ("c1", 6000, 0.75, dict(walk_mode=1)),
+                                               ("c1", 6000, 0.75, dict(list_entries=40000)), ("c1", 40000, 0.75, dict(walk_waves=3))])
+def test_minimum_distance_mac_parity(BH, cfg, n, theta, extra):
+    """The minimum-distance MAC (A28) through every walk path: counts bit-exact, forces within tolerance."""
+    pm, vel, prm = bh_inputs.make(cfg, n=n, seed=41)
+    g, st, _ = _full_parity(BH, pm, vel, theta, prm["eps"], mac=1, **extra)
+    # and it is a different walk from Eq.1's: more interactions on the same tree
+    st0 = oracle_state(pm, vel, theta, prm["eps"], forces=False)
+    assert g["group_npc"].sum() + g["group_npp"].sum() > st0.npc.sum() + st0.npp.sum()
+
+
+def test_switching_the_mac_needs_no_rebuild(BH):
+    pm, vel, prm = bh_inputs.make("c1", n=5000, seed=43)
+    bh = BH(5000)
+    g0 = gpu_tree(bh, pm, vel, 0.75, prm["eps"])
+    bh.set_mac(1)
+    with pytest.raises(Exception):
+        bh.leapfrog_step(0.75, prm["eps"], prm["dt"])          # forces of the old criterion are no longer valid
+    bh.compute_forces(0.75, prm["eps"])
+    g1 = export_numpy(bh)
+    st1 = oracle_state(pm, vel, 0.75, prm["eps"], mac=1)
+    bad = compare_counts(g1, st1)
+    assert not bad, "\n".join(bad)
+    check_forces(g1, st1)
+    bh.set_mac(0)
+    bh.compute_forces(0.75, prm["eps"])
+    g2 = export_numpy(bh)
+    assert np.array_equal(g2["group_npc"], g0["group_npc"]) and np.array_equal(g2["acc_pot"], g0["acc_pot"])
+    with pytest.raises(Exception):
+        bh.set_mac(2)
 
 
 @pytest.mark.parametrize("n", [1, 2, 16, 17, 64, 65])
