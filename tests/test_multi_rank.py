@@ -40,7 +40,9 @@ def test_two_ranks_gloo(tmp_path):
     r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
     assert r.returncode == 0, r.stderr[-2000:]
     import json
-    outs = sorted((json.loads(l.split("RANKOUT ", 1)[1]) for l in r.stdout.splitlines() if "RANKOUT " in l), key=lambda o: o["rank"])
+    import re
+    # the two ranks share one pipe: their lines may arrive glued together, so cut at the marker, not at newlines
+    outs = sorted((json.loads(m) for m in re.findall(r"RANKOUT (\{[^{}]*\})", r.stdout)), key=lambda o: o["rank"])
     assert [o["rank"] for o in outs] == [0, 1]
     assert outs[0]["seed"] != outs[1]["seed"] and outs[0]["checksum"] != outs[1]["checksum"]      # different replicas
     assert outs[0]["total_ms"] == outs[1]["total_ms"] == 20.0                                      # max over ranks
