@@ -249,6 +249,40 @@ def run_ours(args):
     ms_total = max_over_ranks(ms, world, dev)
     value = job_throughput(world, n, args.steps, ms_total * 1e-3)
 
+    # ---- block time-step ingredients, rank 0 reports: moments refreshed on
+    #      the existing cells against a full rebuild, and the walk of the groups with an active particle (a dense core
+    #      holding `--active-fraction` of the particles) against the walk of all groups
+    block = None
+    if args.active_fraction > 0.0:
+        t = bh.export_tree()
+        r = torch.linalg.vector_norm(t["pos_mass"][:, :3], dim=1)
+        active = (r <= torch.quantile(r[:: max(1, n // 1_000_000)], args.active_fraction)).to(torch.uint8).contiguous()
+        cum = torch.cat([torch.zeros(1, dtype=torch.int64, device=dev), torch.cumsum(active.to(torch.int64), 0)])
+        gb = t["group_begin"].to(torch.int64)
+        n_active_groups = int(((cum[gb[1:]] - cum[gb[:-1]]) > 0).sum())
+        ea, eb, ec = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        t_ref, t_act = [], []
+        sub = dt / 16.0                      # a sub-step of the block hierarchy: the particles move by dt / 16 on the cells of a fresh build
+        for _ in range(5):
+            bh.tree_build()
+            bh.compute_forces(theta, eps)
+            bh.kick_drift(0.5 * sub, sub)
+            flush.fill_(1)
+            ea.record(stream)
+            bh.refresh_moments()
+            eb.record(stream)
+            bh.compute_forces_active(theta, eps, active)
+            ec.record(stream)
+            torch.cuda.synchronize()
+            t_ref.append(ea.elapsed_time(eb)); t_act.append(eb.elapsed_time(ec))
+        sa = bh.sync_status()
+        block = {"active_fraction": args.active_fraction, "active_particles": int(active.sum()), "active_groups": n_active_groups,
+                 "groups": int(sa.n_groups), "refresh_moments_ms": statistics.median(t_ref), "forces_active_ms": statistics.median(t_act),
+                 "sub_step": sub, "interactions_active": int(sa.sum_pc + sa.sum_pp),
+                 "what": "fresh build + forces (untimed), bh_kick_drift by dt/16 (untimed), then timed: bh_refresh_moments (S6 on the "
+                         "existing cells) and bh_compute_forces_active (S7 + S8 of the groups with an active particle); compare "
+                         "refresh_moments_ms with build_ms and forces_active_ms with stages_ms.walk + stages_ms.record"}
+
     # ---- e2e: the same step driven from HOST buffers through the C ABI (H2D and D2H inside the timed region)
     hp = torch.from_numpy(pm).pin_memory(); hv = torch.from_numpy(vel).pin_memory()
     hid = torch.arange(n, dtype=torch.int32).pin_memory()
@@ -346,6 +380,7 @@ def run_ours(args):
         "build_ms": build_ms,
         "build_hbm": build_hbm,
         "wall_s_timed_region": wall,
+        "block_step": block,
         "cpu_baseline": cpu,
         "paper_context": "2.8 M particles/s on a GTX480, Plummer N=2^20, theta=0.75 (PAPER.md:182, 256)",
     }
@@ -366,6 +401,8 @@ def main():
     ap.add_argument("--max-cells", dest="max_cells", type=int, default=0)
     ap.add_argument("--list-entries", dest="list_entries", type=int, default=0, help="capacity of the interaction-list buffer (0: default)")
     ap.add_argument("--walk-waves", dest="walk_waves", type=int, default=0, help="k > 1: pipelined walk over at least k waves (0: default)")
+    ap.add_argument("--active-fraction", dest="active_fraction", type=float, default=0.05,
+                    help="block time-step leg: fraction of the particles (the densest core) that is active; 0 skips the leg")
     ap.add_argument("--mac", type=int, default=0, choices=[0, 1], help="0: Eq.1 (the metric's configuration); 1: minimum-distance MAC (PAPER.md:129)")
     ap.add_argument("--ref-groups", dest="ref_groups", type=int, default=None)
     ap.add_argument("--no-cpu", dest="no_cpu", action="store_true")

@@ -128,6 +128,20 @@ int bh_tree_build(bh_ctx* ctx, void* stream);
  * with Plummer softening `eps` (L85, L97).  Needs bh_tree_build.  eps = 0 with coincident particles is undefined. */
 int bh_compute_forces(bh_ctx* ctx, float theta, float eps, void* stream);
 
+/* Block time-steps (L105 "... or on a subset of particles in case of the block-time step regime"; L264-266).  The paper
+ * gives two device-side ingredients and leaves the step criterion open (not part of this library, A23):
+ *
+ * bh_refresh_moments: S6 again on the EXISTING cells and groups after the particles moved (bh_kick_drift): "it is
+ *   sufficient to only recompute the multipole moments of tree-cells that have updated child particles" (L266) -- here of
+ *   all cells, in one launch; the tight boxes follow the particles, so the cell size l grows as L266 describes.  Needs a
+ *   topology from an earlier bh_tree_build on this particle set; afterwards bh_compute_forces(_active) may be called.
+ * bh_compute_forces_active: S7 + S8 for the groups that hold at least one ACTIVE particle only ("the tree-traverse time is
+ *   reduced by a factor N_groups / N_active", L264).  d_active: uint8[n] DEVICE pointer in the current (key-sorted)
+ *   particle order, non-zero = active; borrowed for the duration of the enqueued work.  Particles of other groups keep
+ *   their acc_pot; group_npc / group_npp of other groups read 0; sum_pc / sum_pp count the walked groups only. */
+int bh_refresh_moments(bh_ctx* ctx, void* stream);
+int bh_compute_forces_active(bh_ctx* ctx, float theta, float eps, const uint8_t* d_active, void* stream);
+
 /* Which multipole acceptance criterion S7 uses from the next bh_compute_forces on (the tree need not be rebuilt).
  *   BH_MAC_EQ1 (default): Eq.1 (L125): d > l / theta + delta, d = distance between the group's box and the cell's centre of
  *     mass, l = longest side of the cell's tight box, delta = |centre of mass - box centre|.

@@ -20,7 +20,7 @@ STATUS = {0: "BH_OK", -1: "BH_ERR_INVALID_ARG", -2: "BH_ERR_WORKSPACE", -3: "BH_
 
 # every symbol include/bh.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", "bh_get_particles", "bh_tree_build",
-           "bh_compute_forces", "bh_set_mac", "bh_leapfrog_step", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
+           "bh_compute_forces", "bh_refresh_moments", "bh_compute_forces_active", "bh_set_mac", "bh_leapfrog_step", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
            "bh_get_stage_ms", "bh_get_walk_timeline", "bh_direct_forces", "bh_last_cuda_error", "bh_status_string"]
 
 
@@ -70,6 +70,10 @@ def load_library():
     lib.bh_get_particles.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.bh_tree_build.argtypes = [C.c_void_p, C.c_void_p]
     lib.bh_compute_forces.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p]
+    lib.bh_refresh_moments.argtypes = [C.c_void_p, C.c_void_p]
+    lib.bh_refresh_moments.restype = C.c_int
+    lib.bh_compute_forces_active.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
+    lib.bh_compute_forces_active.restype = C.c_int
     lib.bh_set_mac.argtypes = [C.c_void_p, C.c_int]
     lib.bh_set_mac.restype = C.c_int
     lib.bh_leapfrog_step.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_void_p]
@@ -193,6 +197,17 @@ class BarnesHut:
 
     def compute_forces(self, theta: float, eps: float):
         self._check(self.lib.bh_compute_forces(self.h, theta, eps, self._stream()), "bh_compute_forces")
+
+    def refresh_moments(self):
+        """S6 on the existing cells after the particles moved (block time-steps)."""
+        self._check(self.lib.bh_refresh_moments(self.h, self._stream()), "bh_refresh_moments")
+
+    def compute_forces_active(self, theta: float, eps: float, active: torch.Tensor):
+        """S7 + S8 for the groups with an active particle; active: CUDA uint8[n] in the current sorted order."""
+        if not (active.is_cuda and active.dtype == torch.uint8 and active.is_contiguous() and active.numel() == self.n):
+            raise BhError(-1, "active must be a contiguous CUDA uint8[n] tensor")
+        self._keep_active = active
+        self._check(self.lib.bh_compute_forces_active(self.h, theta, eps, active.data_ptr(), self._stream()), "bh_compute_forces_active")
 
     def set_mac(self, mac: int):
         """0: Eq.1 (default); 1: minimum-distance MAC."""

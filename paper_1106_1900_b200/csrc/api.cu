@@ -171,7 +171,7 @@ int bh_set_particles(bh_ctx* c, int64_t n, const float* pos_mass, const float* v
     BH_CUDA(c, cudaSetDevice(c->device));
     c->n = n;
     c->cur = 0;
-    c->have_particles = c->have_tree = c->have_forces = false;
+    c->have_particles = c->have_topology = c->have_tree = c->have_forces = false;
     BH_CUDA(c, cudaMemcpyAsync(c->ws.pos[0], pos_mass, sizeof(float4) * (size_t)n, cudaMemcpyDefault, s));
     if (vel) BH_CUDA(c, cudaMemcpyAsync(c->ws.vel[0], vel, sizeof(float4) * (size_t)n, cudaMemcpyDefault, s));
     else BH_CUDA(c, cudaMemsetAsync(c->ws.vel[0], 0, sizeof(float4) * (size_t)n, s));
@@ -200,7 +200,7 @@ int bh_tree_build(bh_ctx* c, void* stream) {
     if (!c->have_particles) return BH_ERR_STATE;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     BH_CUDA(c, cudaSetDevice(c->device));
-    c->have_tree = c->have_forces = false;
+    c->have_topology = c->have_tree = c->have_forces = false;
     int rc;
     if (c->timing) cudaEventRecord(c->ev[0], s);
     if ((rc = stage_bbox_keys(c, s)) != BH_OK) return rc;      // records ev[1] between bbox and keys
@@ -215,20 +215,45 @@ int bh_tree_build(bh_ctx* c, void* stream) {
     if (c->timing) cudaEventRecord(c->ev[6], s);
     if ((rc = stage_moments(c, s)) != BH_OK) return rc;
     if (c->timing) cudaEventRecord(c->ev[7], s);
+    c->have_topology = c->have_tree = true;
+    return BH_OK;
+}
+
+int bh_refresh_moments(bh_ctx* c, void* stream) {
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->have_topology) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    c->have_forces = false;
+    int rc = stage_moments(c, s);
+    if (rc != BH_OK) return rc;
     c->have_tree = true;
     return BH_OK;
 }
 
-int bh_compute_forces(bh_ctx* c, float theta, float eps, void* stream) {
+static int compute_forces_impl(bh_ctx* c, float theta, float eps, const uint8_t* d_active, void* stream) {
     if (!c || !(theta > 0.0f) || !std::isfinite(theta) || !(eps >= 0.0f) || !std::isfinite(eps)) return BH_ERR_INVALID_ARG;
     if (!c->have_tree) return BH_ERR_STATE;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     BH_CUDA(c, cudaSetDevice(c->device));
-    int rc = stage_walk(c, theta, eps, s);      // records ev[8] (before the records), ev[9], ev[10] (around k_walk)
+    int rc;
+    if (d_active && (rc = stage_group_active(c, d_active, s)) != BH_OK) return rc;
+    c->active = d_active;
+    rc = stage_walk(c, theta, eps, s);      // records ev[8] (before the records), ev[9], ev[10] (around S7 + S8)
+    c->active = nullptr;
     if (rc != BH_OK) return rc;
     c->theta_last = theta;
     c->have_forces = true;
     return BH_OK;
+}
+
+int bh_compute_forces(bh_ctx* c, float theta, float eps, void* stream) { return compute_forces_impl(c, theta, eps, nullptr, stream); }
+
+int bh_compute_forces_active(bh_ctx* c, float theta, float eps, const uint8_t* d_active, void* stream) {
+    if (!d_active) return BH_ERR_INVALID_ARG;
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, d_active) != cudaSuccess || a.type != cudaMemoryTypeDevice) { (void)cudaGetLastError(); return BH_ERR_INVALID_ARG; }
+    return compute_forces_impl(c, theta, eps, d_active, stream);
 }
 
 int bh_leapfrog_step(bh_ctx* c, float theta, float eps, float dt, void* stream) {
@@ -253,7 +278,7 @@ int bh_kick_drift(bh_ctx* c, float dt_kick, float dt_drift, void* stream) {
     BH_CUDA(c, cudaSetDevice(c->device));
     int rc = stage_kick_drift(c, dt_kick, dt_drift, s);
     if (rc != BH_OK) return rc;
-    c->have_tree = c->have_forces = false;
+    c->have_tree = c->have_forces = false;      // the topology (cells, groups) stays: bh_refresh_moments can revive the tree
     return BH_OK;
 }
 

@@ -13,6 +13,7 @@ constexpr int kMaxLevel = 20;
 constexpr int kKeyBits = 20;           // per axis
 constexpr int kLevels = kMaxLevel + 1; // levels 0..20
 constexpr uint32_t kNone = 0xFFFFFFFFu;
+constexpr uint32_t kSkip = 0xFFFFFFFEu;   // g_pcoff of a group that is not active in this walk (>= kSkip: nothing to evaluate)
 
 // ---- sort geometry (S2)
 constexpr int kRadixBits = 8;
@@ -134,7 +135,8 @@ struct bh_ctx {
     int32_t nleaf, ncrit;
     int cur;               // which of pos[2]/vel[2]/idb[2] holds the live state
     int sorted;            // which of key[2]/val[2] holds the sorted keys / perm
-    bool have_particles, have_tree, have_forces;
+    bool have_particles, have_topology, have_tree, have_forces;   // topology: cells + groups; tree: topology + current moments
+    const uint8_t* active;   // per-particle flags of bh_compute_forces_active during that call (nullptr: every group)
     int64_t launches;
     int last_cuda;
     float theta_last;
@@ -185,6 +187,7 @@ int stage_groups(bh_ctx* c, cudaStream_t s);          // S5
 int stage_moments(bh_ctx* c, cudaStream_t s);         // S6
 int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s);          // S6: fp32 walk record + r2open(theta)
 int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s);   // S7, S8
+int stage_group_active(bh_ctx* c, const uint8_t* d_active, cudaStream_t s);   // groups with an active particle -> ws.gflag[g]
 int walk_init(bh_ctx* c);
 int sort_init(bh_ctx* c);
 int walk_eval_init(bh_ctx* c);

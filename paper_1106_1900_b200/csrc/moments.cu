@@ -120,6 +120,7 @@ __global__ void __launch_bounds__(128) k_moments(const DevScalars* __restrict__ 
             const uint32_t cb = c_cbegin[par], ce = c_cend[par];
             __threadfence();                                   // publish `cur` before counting in
             if (atomicAdd(c_arrive + par, 1u) != ce - cb - 1u) break;
+            c_arrive[par] = 0u;                                // ready for the next pass (bh_refresh_moments runs without k_emit_cells)
             __threadfence();                                   // all children are published; do not read them early
             node_moments(m, mom64, box, cb, ce);
             mom_store(m, mom64, box, par);

@@ -209,7 +209,8 @@ __global__ void __launch_bounds__(kWalkThreads, 2) k_walk_fused(DevScalars* sc, 
                                                                 const float4* __restrict__ pos, const float4* __restrict__ trec,
                                                                 const uint2* __restrict__ tlink, const float* __restrict__ box, const float4* __restrict__ erec,
                                                                 const uint32_t* __restrict__ g_begin, float eps2, float4* __restrict__ acc_out,
-                                                                uint32_t* __restrict__ g_npc, uint32_t* __restrict__ g_npp) {
+                                                                uint32_t* __restrict__ g_npc, uint32_t* __restrict__ g_npp,
+                                                                const uint8_t* __restrict__ g_active) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WarpShared* ws = reinterpret_cast<WarpShared*>(smem_raw) + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
@@ -221,6 +222,10 @@ __global__ void __launch_bounds__(kWalkThreads, 2) k_walk_fused(DevScalars* sc, 
         i = __shfl_sync(0xFFFFFFFFu, i, 0);
         if (i >= count) break;
         const uint32_t g = all ? i : deferred[i];
+        if (all && g_active && !__ldg(g_active + g)) {   // not in this walk's subset (the list path filters before deferring)
+            if (lane == 0) { g_npc[g] = 0u; g_npp[g] = 0u; }
+            continue;
+        }
         const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
         walk_group<kMac>(ws, lane, g, gb, ge, pos, trec, tlink, box, erec, eps2, acc_out, g_npc, g_npp, sc);
         __syncwarp();
@@ -340,10 +345,12 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
     const size_t smem = sizeof(WarpShared) * kWalkWarps;
     if (c->mac_kind == kMacMinDist)
         BH_LAUNCH(c, k_walk_fused<kMacMinDist>, c->sm_count * 2, kWalkThreads, smem, s, c->ws.sc, c->ws.ctl, fused_only ? 1 : 0, c->ws.deferred,
-                  c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.erec, c->ws.g_begin, eps * eps, c->ws.acc, c->ws.g_npc, c->ws.g_npp);
+                  c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.erec, c->ws.g_begin, eps * eps, c->ws.acc, c->ws.g_npc, c->ws.g_npp,
+                  c->active ? c->ws.gflag : nullptr);
     else
         BH_LAUNCH(c, k_walk_fused<kMacEq1>, c->sm_count * 2, kWalkThreads, smem, s, c->ws.sc, c->ws.ctl, fused_only ? 1 : 0, c->ws.deferred,
-                  c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.erec, c->ws.g_begin, eps * eps, c->ws.acc, c->ws.g_npc, c->ws.g_npp);
+                  c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.erec, c->ws.g_begin, eps * eps, c->ws.acc, c->ws.g_npc, c->ws.g_npp,
+                  c->active ? c->ws.gflag : nullptr);
     if (c->timing) cudaEventRecord(c->ev[10], s);
     return BH_OK;
 }

@@ -278,7 +278,7 @@ __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(Wa
         g = __shfl_sync(0xFFFFFFFFu, g, 0);
         if (g >= g1) break;
         const uint32_t pcoff = __ldg(g_pcoff + g);
-        if (pcoff == kNone) continue;          // deferred to the fused kernel
+        if (pcoff >= kSkip) continue;          // deferred to the fused kernel (kNone) or not in this walk's subset (kSkip)
         const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
         const int ng = (int)(ge - gb), npc = (int)__ldg(g_npc + g), npp = (int)__ldg(g_lpp + g);
         const uint32_t* lpc = lists + pcoff;

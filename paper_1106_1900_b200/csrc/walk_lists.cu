@@ -206,7 +206,8 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
                                                                 const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
                                                                 const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
                                                                 const uint32_t* __restrict__ g_begin, uint32_t* __restrict__ lists,
-                                                                uint32_t region_base, uint32_t region_entries, uint32_t chunk_entries) {
+                                                                uint32_t region_base, uint32_t region_entries, uint32_t chunk_entries,
+                                                                const uint8_t* __restrict__ g_active) {
     __shared__ ListWarpShared s_ws[kListWarps];
     __shared__ uint32_t s_chunk, s_taken;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -228,6 +229,10 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
             i = __shfl_sync(0xFFFFFFFFu, i, 0);
             if (i >= nchunk) break;
             const uint32_t g = base + i;
+            if (g_active && !__ldg(g_active + g)) {      // block time-steps: not in this walk's subset
+                if (lane == 0) { o.g_pcoff[g] = kSkip; o.g_npc[g] = 0u; o.g_npp[g] = 0u; }
+                continue;
+            }
             const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
             // a fresh chunk if this one will probably not do; a second try in a fresh chunk if it did not; a group that does
             // not fit a whole chunk (or finds the region used up) goes to the fused kernel instead
@@ -294,11 +299,31 @@ int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t region_base, uint32
     WalkListOut o = walk_list_out(c);
     if (c->mac_kind == kMacMinDist) {
         BH_LAUNCH(c, k_walk_lists<kMacMinDist>, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
-                  c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries);
+                  c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries,
+                  c->active ? c->ws.gflag : nullptr);
         return BH_OK;
     }
     BH_LAUNCH(c, k_walk_lists<kMacEq1>, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
-              c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries);
+              c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries,
+                  c->active ? c->ws.gflag : nullptr);
+    return BH_OK;
+}
+
+// Groups that hold at least one active particle (block time-steps): g_active[g] = any(active[gb .. ge)).
+__global__ void __launch_bounds__(256) k_group_active(const DevScalars* __restrict__ sc, const uint32_t* __restrict__ g_begin,
+                                                      const uint8_t* __restrict__ active, uint8_t* __restrict__ g_active) {
+    const uint32_t G = sc->n_groups;
+    for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < G; g += gridDim.x * blockDim.x) {
+        uint8_t any = 0;
+        for (uint32_t i = g_begin[g]; i < g_begin[g + 1]; ++i) any |= active[i];
+        g_active[g] = any ? 1 : 0;
+    }
+}
+
+int stage_group_active(bh_ctx* c, const uint8_t* d_active, cudaStream_t s) {
+    // ws.gflag is free after the build (it marks group starts per particle for S5 only): it now holds one flag per group
+    const int grid = (int)std::min<int64_t>(div_up(c->n, 256), (int64_t)c->sm_count * 8);
+    BH_LAUNCH(c, k_group_active, grid, 256, 0, s, c->ws.sc, c->ws.g_begin, d_active, c->ws.gflag);
     return BH_OK;
 }
 
