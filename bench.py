@@ -207,9 +207,14 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     cfg, n = _workload(args)
-    pm, vel, prm = _make_inputs(cfg, n, rank)
+    sharded = args.sharded and world > 1     # one problem, the walk shared by the ranks (strong scaling); default: replicas
+    pm, vel, prm = _make_inputs(cfg, n, 0 if sharded else rank)
     theta, eps, dt = args.theta or prm["theta"], prm["eps"], prm["dt"]
-    bh = BarnesHut(n, max_cells=args.max_cells, list_entries=args.list_entries, walk_waves=args.walk_waves)
+    if sharded:
+        from paper_1106_1900_b200 import ShardedBarnesHut
+        bh = ShardedBarnesHut(n, max_cells=args.max_cells, list_entries=args.list_entries, walk_waves=args.walk_waves)
+    else:
+        bh = BarnesHut(n, max_cells=args.max_cells, list_entries=args.list_entries, walk_waves=args.walk_waves)
     bh.set_particles(pm, vel)
     bh.set_mac(args.mac)
     bh.tree_build()
@@ -247,13 +252,13 @@ def run_ours(args):
     s1 = bh.sync_status()
     ms = sum(a.elapsed_time(b) for a, b in evs)
     ms_total = max_over_ranks(ms, world, dev)
-    value = job_throughput(world, n, args.steps, ms_total * 1e-3)
+    value = job_throughput(1 if sharded else world, n, args.steps, ms_total * 1e-3)
 
     # ---- block time-step ingredients, rank 0 reports: moments refreshed on
     #      the existing cells against a full rebuild, and the walk of the groups with an active particle (a dense core
     #      holding `--active-fraction` of the particles) against the walk of all groups
     block = None
-    if args.active_fraction > 0.0:
+    if args.active_fraction > 0.0 and not sharded:
         t = bh.export_tree()
         r = torch.linalg.vector_norm(t["pos_mass"][:, :3], dim=1)
         active = (r <= torch.quantile(r[:: max(1, n // 1_000_000)], args.active_fraction)).to(torch.uint8).contiguous()
@@ -308,7 +313,7 @@ def run_ours(args):
         host_step()
     barrier()
     e2e_s = max_over_ranks(max(time.perf_counter() - t0, 1e-9), world, dev)
-    e2e_value = job_throughput(world, n, e2e_steps, e2e_s)
+    e2e_value = job_throughput(1 if sharded else world, n, e2e_steps, e2e_s)
 
     if rank != 0:
         if world > 1:
@@ -362,13 +367,14 @@ def run_ours(args):
     line = {
         "metric": "particles/sec per full step (build+walk+integrate)", "value": value, "unit": "particles/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
-        "higher_is_better": True, "scaling": "weak",
+        "higher_is_better": True, "scaling": "strong" if sharded else "weak",
         "vs_baseline": value / PAPER_PARTICLES_PER_S if (cfg == "c2" and abs(theta - 0.75) < 1e-6 and world == 1) else None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{cfg}: Plummer sphere n={n}" if cfg in ("c1", "c2") else f"{cfg}: n={n}",
                    "theta": theta, "eps": eps, "dt": dt, "nleaf": 16, "ncrit": 64, "mac": "min_distance" if args.mac else "eq1", "rebuild_every_step": True,
                    "l2": f"{L2_FLUSH_BYTES >> 20} MiB buffer written between timed steps (outside the event pairs)",
-                   "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no collective)",
+                   "parallelism": "single GPU" if world == 1 else (f"{world} ranks share the walk of one problem: redundant build, one all-reduce of acc_pot per step"
+                                                                     if sharded else f"{world} independent replicas (no collective)"),
                    "cells": int(s1.n_cells), "groups": int(s1.n_groups), "levels": int(s1.n_levels),
                    "pp_per_particle": s1.sum_pp / n, "pc_per_particle": s1.sum_pc / n, "mac_tests_per_group": s1.sum_mac / max(1, s1.n_groups)},
         "clocks": clocks,
@@ -403,6 +409,9 @@ def main():
     ap.add_argument("--walk-waves", dest="walk_waves", type=int, default=0, help="k > 1: pipelined walk over at least k waves (0: default)")
     ap.add_argument("--active-fraction", dest="active_fraction", type=float, default=0.05,
                     help="block time-step leg: fraction of the particles (the densest core) that is active; 0 skips the leg")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1 only: one problem, every rank builds the tree and walks its share of the groups, one all-reduce per step "
+                         "(strong scaling); default: N independent replicas (weak scaling)")
     ap.add_argument("--mac", type=int, default=0, choices=[0, 1], help="0: Eq.1 (the metric's configuration); 1: minimum-distance MAC (PAPER.md:129)")
     ap.add_argument("--ref-groups", dest="ref_groups", type=int, default=None)
     ap.add_argument("--no-cpu", dest="no_cpu", action="store_true")

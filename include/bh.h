@@ -154,7 +154,8 @@ int bh_set_mac(bh_ctx* ctx, int mac);
 int bh_leapfrog_step(bh_ctx* ctx, float theta, float eps, float dt, void* stream);
 
 /* S9 on its own (L105), the kick-drift form of the same leapfrog: v += a * dt_kick; x += v * dt_drift, with the
- * accelerations of the last bh_compute_forces.  Invalidates tree and forces (the particles moved). */
+ * accelerations of the last bh_compute_forces.  Invalidates tree and forces (the particles moved) -- unless dt_drift is
+ * exactly 0: a pure kick leaves positions, tree and forces as they are (x = fmaf(v, 0, x) = x). */
 int bh_kick_drift(bh_ctx* ctx, float dt_kick, float dt_drift, void* stream);
 
 /* Synchronise `stream`, then report the deferred device status and the counters.  Returns the deferred status. */

@@ -252,6 +252,15 @@ class BarnesHut:
         t = self.workspace[off: off + nb].view(dtype)
         return t.view(shape) if shape is not None else t
 
+    def acc_view(self) -> torch.Tensor:
+        """float32[n,4] view of the acc_pot array in the workspace (no copy, no synchronisation)."""
+        v = BhTreeView()
+        # bh_export_tree would enqueue the export kernel; the acc array sits at a fixed place of the workspace, so ask once
+        if getattr(self, "_acc_ptr", None) is None:
+            self._check(self.lib.bh_export_tree(self.h, C.byref(v), self._stream()), "bh_export_tree")
+            self._acc_ptr = v.acc_pot
+        return self._view(self._acc_ptr, self.n * 4, torch.float32, (self.n, 4))
+
     def export_tree(self) -> dict:
         """Canonical arrays of bh_tree_view as torch tensors that alias the workspace (synchronises)."""
         v = BhTreeView()

@@ -278,7 +278,7 @@ int bh_kick_drift(bh_ctx* c, float dt_kick, float dt_drift, void* stream) {
     BH_CUDA(c, cudaSetDevice(c->device));
     int rc = stage_kick_drift(c, dt_kick, dt_drift, s);
     if (rc != BH_OK) return rc;
-    c->have_tree = c->have_forces = false;      // the topology (cells, groups) stays: bh_refresh_moments can revive the tree
+    if (dt_drift != 0.0f) c->have_tree = c->have_forces = false;   // the particles moved; the topology (cells, groups) stays: bh_refresh_moments can revive the tree
     return BH_OK;
 }
 

@@ -307,8 +307,8 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
     if (!fused_only) {
         const int W = (int)nwaves;
         const uint32_t half = (uint32_t)std::min<int64_t>(c->list_entries / 2, (int64_t)1 << 30);
-        // one block of eight warps per ~128 particles (~7 groups); alone on the device: up to 5 resident blocks per SM
-        const int grid_alone = (int)std::max<int64_t>(1, std::min<int64_t>(div_up(wave_particles, 128), (int64_t)c->sm_count * 5));
+        // one block of eight warps per ~128 particles (~7 groups); alone on the device: 4 resident blocks per SM
+        const int grid_alone = (int)std::max<int64_t>(1, std::min<int64_t>(div_up(wave_particles, 128), (int64_t)c->sm_count * 4));
         const int grid_beside = (int)std::max<int64_t>(1, std::min<int64_t>(div_up(wave_particles, 128), (int64_t)c->sm_count * kPipeListBlocks));
         if (!pipelined || W == 1) {
             // one wave after the other on the caller's stream; every wave has the whole list buffer and the whole device

@@ -49,6 +49,52 @@ def test_two_ranks_gloo(tmp_path):
     assert outs[0]["value"] == 2 * 2048 * 4 / 20e-3                                                 # whole-job aggregate
 
 
+SHARD_WORKER = textwrap.dedent("""
+    import json, os, sys
+    sys.path.insert(0, %r)
+    import numpy as np, torch
+    import torch.distributed as dist
+    import bh_inputs, oracle
+    from paper_1106_1900_b200.sharded import keep_own_rows, share_bounds, share_mask
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    dist.init_process_group("gloo")
+    n = 3000
+    pm, vel, prm = bh_inputs.make("c1", n=n, seed=71)             # the SAME particles on every rank
+    st = oracle.tree_build(pm, vel)
+    t = st.tree
+    mask = share_mask(n, world, rank, "cpu").numpy()
+    sel = np.array([g for g in range(t.ngroups) if mask[t.gbegin[g]: t.gbegin[g] + t.gcount[g]].any()], np.int64)
+    oracle.compute_forces(st, prm["theta"], prm["eps"], sel=sel)   # this rank's share of the walk (the oracle stands in for the GPU)
+    acc = torch.from_numpy(np.nan_to_num(st.accpot))
+    keep_own_rows(acc, n, world, rank)
+    dist.all_reduce(acc, op=dist.ReduceOp.SUM)                     # the one exchange of a step
+    full = oracle.compute_forces(oracle.tree_build(pm, vel), prm["theta"], prm["eps"]).accpot
+    out = dict(rank=rank, groups=int(sel.size), all_groups=int(t.ngroups), equal=bool(np.array_equal(acc.numpy(), full)),
+               bounds=share_bounds(n, world))
+    print("RANKOUT " + json.dumps(out), flush=True)
+    dist.barrier()
+    dist.destroy_process_group()
+""") % ROOT
+
+
+def test_group_sharded_walk_two_ranks_gloo(tmp_path):
+    """Host logic of the sharded walk (shares, own rows, one all-reduce) with the oracle as the force provider."""
+    script = tmp_path / "shard_worker.py"
+    script.write_text(SHARD_WORKER)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", "29733", str(script)]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    import json
+    import re
+    outs = sorted((json.loads(m) for m in re.findall(r"RANKOUT (\{[^{}]*\})", r.stdout)), key=lambda o: o["rank"])
+    assert [o["rank"] for o in outs] == [0, 1]
+    assert all(o["equal"] for o in outs)                                   # every rank ends with every force, bit for bit
+    G = outs[0]["all_groups"]
+    assert G <= outs[0]["groups"] + outs[1]["groups"] <= G + 1             # at most the straddling group is walked twice
+    assert outs[0]["bounds"] == [0, 1500, 3000]
+
+
 def test_reference_arm_runs_on_rank0_only():
     env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
