@@ -272,8 +272,9 @@ int walk_destroy(bh_ctx* c) {
 }
 
 // Expected list entries per particle (cells + particles per group / group size), from the measured c2 figures
-// (80 at theta = 0.75, 189 at theta = 0.5) and the theta^-3 growth of the opened volume; only sizes the waves.
-static double list_entries_per_particle(float theta) { return 32.0 / ((double)theta * theta * theta) + 16.0; }
+// (80 at theta = 0.75, 189 at theta = 0.5; c5: 334 at theta = 0.4) and the theta^-3 growth of the opened volume; only
+// sizes the waves (with a factor 1.5 on top; a group that still finds no room goes to the fused kernel).
+static double list_entries_per_particle(float theta) { return 24.0 / ((double)theta * theta * theta) + 16.0; }
 
 constexpr int kPipeEvalBlocks = 3;    // evaluation blocks per SM while a list walk runs beside them (12 warps x 128 registers)
 constexpr int kPipeListBlocks = 1;    // ... which leaves registers and shared memory for this many list blocks per SM
