@@ -261,7 +261,7 @@ __device__ __forceinline__ int choose_r2(int ng) {
     return 1;
 }
 
-__global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(WalkCtl* __restrict__ ctl, int wave, const float4* __restrict__ pos,
+__global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(const DevScalars* __restrict__ sc, WalkCtl* __restrict__ ctl, int wave, const float4* __restrict__ pos,
                                                                const float4* __restrict__ erec, const uint32_t* __restrict__ g_begin,
                                                                const uint32_t* __restrict__ lists, const uint32_t* __restrict__ g_pcoff,
                                                                const uint32_t* __restrict__ g_npc, const uint32_t* __restrict__ g_ppoff,
@@ -272,15 +272,26 @@ __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(Wa
     const uint32_t g0 = ctl->wave_g[wave], g1 = ctl->wave_g[wave + 1];
     const Consts k = make_consts(eps2);
     if (threadIdx.x == 0) atomicMin(&ctl->t_start[1][wave], global_ns());
+    // three sweeps over the wave's groups with one counter: first the groups with more than 3 times the average work
+    // (targets x list entries), then those above 1.5 times, then the rest -- the long groups start early and the kernel
+    // ends on short ones (the order in which groups are evaluated does not touch their sums)
+    const uint32_t G = g1 - g0;
+    const unsigned long long total = sc->sum_pc + sc->sum_pp;                 // interactions listed so far (all waves up to this one)
+    const unsigned long long mean = total / max(sc->n_groups, 1u);
     for (;;) {
-        uint32_t g = 0;
-        if (lane == 0) g = g0 + atomicAdd(&ctl->eval_next[wave], 1u);
-        g = __shfl_sync(0xFFFFFFFFu, g, 0);
-        if (g >= g1) break;
+        uint32_t i = 0;
+        if (lane == 0) i = atomicAdd(&ctl->eval_next[wave], 1u);
+        i = __shfl_sync(0xFFFFFFFFu, i, 0);
+        if (i >= 3u * G) break;
+        const uint32_t sweep = i >= 2u * G ? 2u : i >= G ? 1u : 0u;
+        const uint32_t g = g0 + (i - sweep * G);
         const uint32_t pcoff = __ldg(g_pcoff + g);
         if (pcoff >= kSkip) continue;          // deferred to the fused kernel (kNone) or not in this walk's subset (kSkip)
         const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
         const int ng = (int)(ge - gb), npc = (int)__ldg(g_npc + g), npp = (int)__ldg(g_lpp + g);
+        const unsigned long long work = (unsigned long long)ng * (unsigned long long)(npc + npp);
+        const uint32_t cls = 2ull * work > 6ull * mean ? 0u : 2ull * work > 3ull * mean ? 1u : 2u;
+        if (cls != sweep) continue;            // another sweep's
         const uint32_t* lpc = lists + pcoff;
         const uint32_t* lpp = lists + __ldg(g_ppoff + g);
         switch (choose_r2(ng)) {
@@ -303,7 +314,7 @@ int walk_eval_init(bh_ctx* c) {
 int stage_walk_eval(bh_ctx* c, int wave, float eps, int blocks_per_sm, cudaStream_t s) {
     const size_t smem = sizeof(EvalShared) * kEvalWarps;
     const int grid = c->sm_count * std::min(blocks_per_sm, kEvalBlocksPerSM);
-    BH_LAUNCH(c, k_walk_eval, grid, kEvalThreads, smem, s, c->ws.ctl, wave, c->ws.pos[c->cur], c->ws.erec, c->ws.g_begin, c->ws.lists,
+    BH_LAUNCH(c, k_walk_eval, grid, kEvalThreads, smem, s, c->ws.sc, c->ws.ctl, wave, c->ws.pos[c->cur], c->ws.erec, c->ws.g_begin, c->ws.lists,
               c->ws.g_pcoff, c->ws.g_npc, c->ws.g_ppoff, c->ws.g_lpp, eps * eps, c->ws.acc);
     return BH_OK;
 }
