@@ -7,9 +7,10 @@
 //   k_walk_fused                         S7 + S8 of the groups whose lists did not fit   (this file; normally none)
 // A "wave" is a contiguous range of particles (hence of groups) sized on the host so that its lists are expected to fit
 // the list buffer of the workspace; nothing is read back, so the whole sequence can be captured into a CUDA graph.  A
-// group whose lists do not fit its warp's arena is deferred by k_walk_lists and handled here instead: one warp per group,
-// frontier LIFO, accepted cells and leaf particles staged in shared-memory rings of 64 entries and swept every 32
-// (PAPER.md:85), the evaluation code shared with walk_eval.cu.  Capacity therefore bounds memory, never the result.
+// group whose lists fit neither a chunk of the list region nor what is left of it is deferred by k_walk_lists and handled
+// here instead (the round-1 one-kernel walk): one warp per group, frontier LIFO, accepted cells and leaf particles staged
+// in shared-memory rings of 64 entries and swept every 32 with the slot evaluation of walk_common.cuh.
+// Capacity therefore bounds memory, never the result.
 #include <algorithm>
 #include <cmath>
 #include "walk_common.cuh"

@@ -1,13 +1,15 @@
-// walk_common.cuh -- S8 force evaluation shared by the walk kernels (walk_eval.cu: list-driven; walk.cu: fused fallback).
+// walk_common.cuh -- what the walk kernels share: packed-fp32 helpers, the group box, the MAC tests (Eq.1 and the
+// minimum-distance variant), and the ring / slot force evaluation of the fused fallback kernel (walk.cu).  The
+// list-driven evaluation kernel (walk_eval.cu) has its own, later layout: two targets per 64-bit register.
 //
-// Evaluation layout (what differs from the paper's one-thread-per-particle sweep, and why):
+// Evaluation layout of the fused kernel (what differs from the paper's one-thread-per-particle sweep):
 //   (1) Lane use.  A group holds n <= 64 targets (mean ~19), so "one target per lane" idles ~half of the warp.  The
 //       paper's remedy is up to 4 threads per particle (L81, L97); here it is taken to its end: n is rounded up to a
 //       multiple of 4 and split in binary, 64 | 32 + 16 + 8 + 4 -> "slots" of T = 2^K targets.  In a slot a lane serves
 //       TWO targets, (l mod T/2) and (l mod T/2) + T/2, and sub-list (l div T/2): the 64 / T sub-lists interleave the ring
 //       entries, and a butterfly of shuffles adds the sub-list sums at the end of the group (>= 93 % useful lanes).
-//   (2) FP32 rate.  On sm_100a scalar FFMA issues at half rate; the full 128 lanes/clk/SM needs the packed f32x2 forms
-//       (FFMA2/FMUL2/FADD2, measured 71.8 vs 37-45 TFLOP/s).  The rings therefore store PAIRS of entries interleaved
+//   (2) FP32 rate.  The packed f32x2 forms (FFMA2/FMUL2/FADD2) get nearer to the 128 lanes/clk/SM than scalar FFMA
+//       (measured 71.8 vs 37-45 TFLOP/s; both are bounded by register-file bandwidth).  The rings therefore store PAIRS of entries interleaved
 //       (x0, x1, y0, y1, ...), one LDS.128 yields two packed operands, and each lane evaluates two list entries per
 //       instruction for each of its targets.
 //   (3) Shared-memory delivery.  An LDS.128 moves 512 B into the register file whether or not the lanes share the address,
