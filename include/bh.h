@@ -115,7 +115,10 @@ int bh_destroy(bh_ctx* ctx);
 
 /* Copy n particles into the workspace (cudaMemcpyAsync on `stream`; pointers may be host or device memory, host
  * memory should be pinned for the copy to be asynchronous).  vel may be NULL (zeros); id may be NULL (0..n-1).
- * Invalidates tree and forces. */
+ * Invalidates tree and forces.  The velocity and id copies run on an internal stream beside S0-S2 of the next
+ * bh_tree_build (which only need positions) and are joined by an event before anything reads them; under stream
+ * capture every copy stays on `stream`.  All source buffers must stay valid until the work enqueued on `stream` by the
+ * next bh_tree_build / bh_get_particles (or a synchronisation after it) has completed. */
 int bh_set_particles(bh_ctx* ctx, int64_t n, const float* pos_mass, const float* vel, const uint32_t* id, void* stream);
 
 /* Copy the current (key-sorted) state out; any pointer may be NULL; host or device destinations. */

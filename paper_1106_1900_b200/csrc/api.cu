@@ -105,6 +105,14 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
 
 using namespace bh;
 
+// Make `s` wait for the side-stream half of the last bh_set_particles (velocities, ids, zeroed accelerations).
+static int join_copies(bh_ctx* c, cudaStream_t s) {
+    if (!c->copies_pending) return BH_OK;
+    BH_CUDA(c, cudaStreamWaitEvent(s, c->ev_join, 0));
+    c->copies_pending = false;
+    return BH_OK;
+}
+
 extern "C" {
 
 size_t bh_workspace_bytes(int64_t n_max, const bh_config* cfg) {
@@ -173,11 +181,26 @@ int bh_set_particles(bh_ctx* c, int64_t n, const float* pos_mass, const float* v
     c->cur = 0;
     c->have_particles = c->have_topology = c->have_tree = c->have_forces = false;
     BH_CUDA(c, cudaMemcpyAsync(c->ws.pos[0], pos_mass, sizeof(float4) * (size_t)n, cudaMemcpyDefault, s));
-    if (vel) BH_CUDA(c, cudaMemcpyAsync(c->ws.vel[0], vel, sizeof(float4) * (size_t)n, cudaMemcpyDefault, s));
-    else BH_CUDA(c, cudaMemsetAsync(c->ws.vel[0], 0, sizeof(float4) * (size_t)n, s));
-    if (id) BH_CUDA(c, cudaMemcpyAsync(c->ws.idb[0], id, sizeof(uint32_t) * (size_t)n, cudaMemcpyDefault, s));
-    else { int rc = stage_iota(c, c->ws.idb[0], n, s); if (rc != BH_OK) return rc; }
-    BH_CUDA(c, cudaMemsetAsync(c->ws.acc, 0, sizeof(float4) * (size_t)n, s));
+    // S0-S2 need the positions only: velocities, ids and the zeroed accelerations arrive on an internal stream beside them
+    // and are joined (event) before the first stage that touches them (S3) or any call that reads them.  Not under
+    // stream capture: there everything stays on the caller's stream.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s, &cap) != cudaSuccess) { (void)cudaGetLastError(); cap = cudaStreamCaptureStatusActive; }
+    cudaStream_t side = s;
+    if (cap == cudaStreamCaptureStatusNone) {
+        side = c->s_lists;
+        BH_CUDA(c, cudaEventRecord(c->ev_fork, s));                // after whatever used the old arrays on the caller's stream
+        BH_CUDA(c, cudaStreamWaitEvent(side, c->ev_fork, 0));
+    }
+    if (vel) BH_CUDA(c, cudaMemcpyAsync(c->ws.vel[0], vel, sizeof(float4) * (size_t)n, cudaMemcpyDefault, side));
+    else BH_CUDA(c, cudaMemsetAsync(c->ws.vel[0], 0, sizeof(float4) * (size_t)n, side));
+    if (id) BH_CUDA(c, cudaMemcpyAsync(c->ws.idb[0], id, sizeof(uint32_t) * (size_t)n, cudaMemcpyDefault, side));
+    else { int rc = stage_iota(c, c->ws.idb[0], n, side); if (rc != BH_OK) return rc; }
+    BH_CUDA(c, cudaMemsetAsync(c->ws.acc, 0, sizeof(float4) * (size_t)n, side));
+    if (side != s) {
+        BH_CUDA(c, cudaEventRecord(c->ev_join, side));
+        c->copies_pending = true;
+    }
     c->have_particles = true;
     return BH_OK;
 }
@@ -187,6 +210,7 @@ int bh_get_particles(bh_ctx* c, float* pos_mass, float* vel, float* acc_pot, uin
     if (!c->have_particles) return BH_ERR_STATE;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     BH_CUDA(c, cudaSetDevice(c->device));
+    { int rcj = join_copies(c, s); if (rcj != BH_OK) return rcj; }
     const size_t n = (size_t)c->n;
     if (pos_mass) BH_CUDA(c, cudaMemcpyAsync(pos_mass, c->ws.pos[c->cur], sizeof(float4) * n, cudaMemcpyDefault, s));
     if (vel) BH_CUDA(c, cudaMemcpyAsync(vel, c->ws.vel[c->cur], sizeof(float4) * n, cudaMemcpyDefault, s));
@@ -207,6 +231,7 @@ int bh_tree_build(bh_ctx* c, void* stream) {
     if (c->timing) cudaEventRecord(c->ev[2], s);
     if ((rc = stage_sort(c, s)) != BH_OK) return rc;
     if (c->timing) cudaEventRecord(c->ev[3], s);
+    if ((rc = join_copies(c, s)) != BH_OK) return rc;          // S3 is the first stage that reads velocities and ids
     if ((rc = stage_reorder(c, s)) != BH_OK) return rc;
     if (c->timing) cudaEventRecord(c->ev[4], s);
     if ((rc = stage_cells(c, s)) != BH_OK) return rc;

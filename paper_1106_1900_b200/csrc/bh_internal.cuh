@@ -148,6 +148,7 @@ struct bh_ctx {
     int64_t sort_tiles, tree_tiles, scan_sum_cap;
     bool timing;
     cudaEvent_t ev[13];     // [0..10] stage boundaries; [11], [12]: after the list walk / the evaluation of a one-wave walk
+    bool copies_pending;    // bh_set_particles left copies on s_lists; ev_join marks their end (api.cu: join_copies)
     bool walk_split_timed;  // the last walk was one wave: ev[11], ev[12] are valid
     // walk pipeline (walk.cu): the list walk of wave w + 1 runs beside the evaluation of wave w on internal streams
     cudaStream_t s_lists, s_eval2;
