@@ -4,9 +4,10 @@
 // device counter.  What differs from the paper's one-thread-per-particle sweep, and why:
 //   (1) FP32 rate.  On sm_100a the register file delivers two 32-bit words per lane and cycle, so a three-operand FFMA
 //       cannot issue every cycle; the packed forms FFMA2 / FMUL2 / FADD2 with a broadcast scalar operand need fewer words
-//       per flop and come closest to the 128 FP32 lanes/clk/SM.  A 64-bit register here holds TWO TARGETS (particles of the group); the list entry is
-//       a scalar operand that the packed instructions broadcast to both halves (the `.F32` operand form of the SASS), so
-//       the records are used exactly as they sit in memory: no pairing of entries, no transposition, no padding entry.
+//       per flop and come closest to the 128 FP32 lanes/clk/SM.  A 64-bit register here holds TWO
+//       TARGETS (particles of the group); the list entry is a scalar operand that the packed instructions broadcast to
+//       both halves (the `.F32` operand form of the SASS), so the records are used exactly as they sit in memory: no
+//       pairing of entries, no transposition, no padding entry.
 //   (2) Lane use.  A group holds ng <= 64 targets (mean ~19; work-weighted mean ~27).  A lane serves R = 2, 4 or 6
 //       targets (R/2 packed registers per coordinate); L = ceil(ng / R) lanes cover the group, and the warp is split into
 //       S = floor(32 / L) such teams, each sweeping every S-th entry of the list ("up to 4 threads per particle",
