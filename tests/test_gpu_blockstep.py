@@ -20,18 +20,20 @@ def BH():
 
 
 def _moved_state(BH, n, seed, dt, **cfg):
-    """GPU: build, forces, kick-drift, refresh.  Oracle: the SAME topology (built from the original positions), moments and
-    group boxes recomputed from the positions the GPU holds after the drift."""
+    """GPU: build, forces, drift (kick 0: the new positions depend on the inputs only), refresh.  Oracle: the SAME topology
+    (built from the original positions), positions drifted by the oracle itself (O11: x = fmaf(v, dt, x), bit-identical
+    to the GPU's, which is checked), moments and group boxes recomputed from them."""
     pm, vel, prm = bh_inputs.make("c1", n=n, seed=seed)
     bh = BH(n, **cfg)
     g0 = gpu_tree(bh, pm, vel, prm["theta"], prm["eps"])
-    bh.kick_drift(dt, dt)
+    bh.kick_drift(0.0, dt)
     bh.refresh_moments()
     st = oracle.tree_build(pm, vel)
-    moved = np.empty((n, 4), np.float32)
-    bh.get_particles(pos_mass=moved)
+    moved = oracle.drift(st.pos, st.vel, np.float32(dt))
+    got = np.empty((n, 4), np.float32)
+    bh.get_particles(pos_mass=got)
     torch.cuda.synchronize()
-    assert np.array_equal(moved[:, 3], st.pos[:, 3]) and not np.array_equal(moved[:, :3], st.pos[:, :3])
+    assert np.array_equal(got, moved) and not np.array_equal(moved[:, :3], st.pos[:, :3])
     oracle.moments(st.tree, moved)
     st.pos = moved
     return bh, g0, st, prm
