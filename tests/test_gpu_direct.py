@@ -78,6 +78,7 @@ def test_acceleration_error_experiment():
     bh = BarnesHut(8192)
     bh.set_particles(pm, vel); bh.tree_build(); bh.compute_forces(0.5, 0.0)
     t = bh.export_tree()
-    ps = t["pos_mass"].cpu().numpy()
+    ps = oracle.tree_build(pm, vel).pos                     # the oracle's own sorted particles (the GPU's, bit for bit)
+    assert np.array_equal(t["pos_mass"].cpu().numpy(), ps)
     err = accuracy.relative_error(t["acc_pot"].cpu().numpy(), oracle.direct(ps, 0.0))
     assert abs(accuracy.exceeded_by(err, 0.5) - med[1]) < 1e-6 * med[1] + 1e-12

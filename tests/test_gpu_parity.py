@@ -248,7 +248,9 @@ def test_theta_to_zero_is_the_direct_sum(BH):
     pm, vel, _ = bh_inputs.make("c1", n=1500)
     bh = BH(1500)
     g = gpu_tree(bh, pm, vel, 1e-6, 0.01)
-    d = oracle.direct(g["pos_mass"], 0.01)
+    ps = oracle.tree_build(pm, vel).pos                     # the oracle's own sorted particles ...
+    assert np.array_equal(g["pos_mass"], ps)                # ... which are the GPU's, bit for bit
+    d = oracle.direct(ps, 0.01)
     a = g["acc_pot"].astype(np.float64)
     err = np.linalg.norm(a[:, :3] - d[:, :3], axis=1) / np.linalg.norm(d[:, :3], axis=1)
     assert np.sqrt(np.mean(err ** 2)) < 1e-5 and err.max() < 1e-4
