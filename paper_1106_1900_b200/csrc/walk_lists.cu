@@ -273,6 +273,7 @@ __global__ void k_walk_prepare(DevScalars* sc, WalkCtl* ctl, const uint32_t* __r
         uint32_t lo = 0, hi = G;           // lower_bound of t * wave_particles in g_begin[0..G)
         const unsigned long long target = (unsigned long long)t * wave_particles;
         if (t == nwaves) lo = G;
+        else if (t == 0) lo = 0;           // (no search for the common one-wave walk)
         else if (t == 0) lo = 0;
         else
             while (lo < hi) {
