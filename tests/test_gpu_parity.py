@@ -255,3 +255,27 @@ def test_theta_to_zero_is_the_direct_sum(BH):
     err = np.linalg.norm(a[:, :3] - d[:, :3], axis=1) / np.linalg.norm(d[:, :3], axis=1)
     assert np.sqrt(np.mean(err ** 2)) < 1e-5 and err.max() < 1e-4
     assert np.all(g["group_npc"] + g["group_npp"] == 1500)
+
+
+def test_stage_timing_and_walk_timeline(BH):
+    """The profiling aids of the boundary: per-stage CUDA-event times and the device timeline of the walk."""
+    pm, vel, prm = bh_inputs.make("c1", n=40000, seed=73)
+    for waves in (0, 3):
+        bh = BH(40000, walk_waves=waves)
+        bh.set_particles(pm, vel)
+        bh.set_stage_timing(True)
+        bh.tree_build()
+        bh.compute_forces(prm["theta"], prm["eps"])
+        ms = bh.stage_ms()
+        assert set(ms) == {"bbox", "keys", "sort", "reorder", "cells", "groups", "moments", "record", "walk", "lists", "eval"}
+        assert all(v >= 0.0 for v in ms.values()) and ms["walk"] > 0.0 and ms["sort"] > 0.0
+        tl = bh.walk_timeline()
+        if waves == 0:
+            assert ms["lists"] > 0.0 and ms["eval"] > 0.0 and ms["lists"] + ms["eval"] <= ms["walk"] * 1.001
+            assert len(tl) == 1
+        else:
+            assert ms["lists"] == 0.0 and ms["eval"] == 0.0          # the kernels of a pipelined walk overlap: no split
+            assert len(tl) == 3
+        for ls, le, es, ee in tl:
+            assert 0 <= ls <= le and es <= ee and le <= ee           # a wave is evaluated after it has been listed
+        bh.close()
