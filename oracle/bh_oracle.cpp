@@ -19,7 +19,9 @@
 // independent dilate, numpy stable argsort, a second tree construction (the paper's literal
 // per-level mask/flag loop, tests/level_loop_tree.py), structural tree invariants, direct-sum root
 // moments, the parallel-axis identity, closed-form two-mass quadrupole, (s/R)^3 convergence,
-// brute force O(N^2), theta -> 0, analytic Plummer potential, two-body orbit, reversibility.
+// brute force O(N^2), theta -> 0, analytic Plummer potential, two-body orbit, reversibility;
+// Eq.1's l, delta, r_open: hand-built cells with closed-form values and a target one ulp on either side of the
+// threshold, plus a numpy-float32 restatement over every cell and a root-to-leaf walk with it.
 // Parity unpinned against the paper: magnitudes of the interaction counts (Fig.6 inset is an image).
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).

@@ -333,3 +333,85 @@ def test_mindist_mac_limits_and_accuracy():
     l = (st.tree.box[:, 3:] - st.tree.box[:, :3]).max(axis=1).astype(np.float32)
     r = (l / np.float32(0.75)).astype(np.float32)
     assert np.array_equal(st.mac[:, 2], (r * r).astype(np.float32))
+
+
+# ---------------------------------------------------------------- Eq.1 (Fig.5): the VALUE of l, delta, r_open
+def _two_particle_cell_case(B, mB, xt_x, theta=0.5):
+    """A = (0,0,0) with mass 1 and B with mass mB form one leaf (nleaf = ncrit = 2); the target T sits alone in another
+    cell, level with the leaf's centre of mass in y and z, so that d(group box, com) = T.x - com.x.  Returns
+    (mac row of the leaf {A, B}, n_pc of T's group, n_pp of T's group)."""
+    com = np.array(B[:3]) * mB / (1.0 + mB)
+    pm = np.array([[0, 0, 0, 1.0], [B[0], B[1], B[2], mB], [xt_x, com[1], com[2], 1.0]], np.float32)
+    st = oracle.tree_build(pm, nleaf=2, ncrit=2)
+    t = st.tree
+    assert t.ncells == 3 and t.ngroups == 2 and list(t.pcount) == [3, 2, 1] and list(t.gcount) == [2, 1]
+    oracle.compute_forces(st, theta=theta, eps=0.0)
+    return st.mac[1], int(st.npc[1]), int(st.npp[1])
+
+
+def test_eq1_opening_radius_closed_form_and_flip_at_the_threshold():
+    """Hand-built cells whose l, delta and r_open are exact binary fractions known in closed form (Eq.1: d > l/theta + delta,
+    l = cell size, delta = |geometric centre - centre of mass|), and a target one ulp on either side of
+    the threshold.  A wrong delta (halved, dropped, measured from a box corner), a wrong sign or a wrong l fails here."""
+    f = np.float32
+    # (1) on an axis: box [0,1], l = 1, centre 0.5, com = 0.75, delta = 0.25; theta = 0.5: r_open = 2.25, r2_open = 5.0625
+    mac, npc, npp = _two_particle_cell_case((1, 0, 0), 3.0, 3.0)           # d = 3 - 0.75 = 2.25 exactly: NOT accepted (strict, A16)
+    assert tuple(mac) == (f(1.0), f(0.25), f(5.0625))
+    assert (npc, npp) == (0, 3)                                             # leaf {A,B} opened (2) + own leaf (1)
+    mac, npc, npp = _two_particle_cell_case((1, 0, 0), 3.0, np.nextafter(f(3.0), f(4.0)))
+    assert tuple(mac) == (f(1.0), f(0.25), f(5.0625)) and (npc, npp) == (1, 1)    # one ulp further: accepted
+    # (2) off-axis offset: B = (2,2,1), masses 1:3 -> box [0,2]x[0,2]x[0,1], l = 2, centre (1,1,.5), com = (1.5,1.5,.75),
+    #     u = (.5,.5,.25), delta = sqrt(.5625) = .75; theta = 0.5: r_open = 4.75, r2_open = 22.5625; threshold T.x = 6.25
+    mac, npc, npp = _two_particle_cell_case((2, 2, 1), 3.0, 6.25)
+    assert tuple(mac) == (f(2.0), f(0.75), f(22.5625)) and (npc, npp) == (0, 3)
+    mac, npc, npp = _two_particle_cell_case((2, 2, 1), 3.0, np.nextafter(f(6.25), f(7.0)))
+    assert (npc, npp) == (1, 1)
+    # (3) equal masses: com = centre, delta = 0 exactly: r_open = l / theta alone (theta = 0.25: 4, r2 = 16; threshold 4.5)
+    mac, npc, npp = _two_particle_cell_case((1, 0, 0), 1.0, 4.5, theta=0.25)
+    assert tuple(mac) == (f(1.0), f(0.0), f(16.0)) and (npc, npp) == (0, 3)
+    mac, npc, npp = _two_particle_cell_case((1, 0, 0), 1.0, np.nextafter(f(4.5), f(5.0)), theta=0.25)
+    assert (npc, npp) == (1, 1)
+
+
+def _eq1_accept_np(gbox, com, r2open):
+    """O9 restated in numpy float32: per-axis distance from the group's box to the centre of mass, d2 by fused multiply-adds."""
+    f = np.float32
+    d = np.maximum(np.maximum(gbox[:3] - com, com - gbox[3:]), f(0)).astype(np.float32)
+    d2 = f(np.float64(d[0]) * np.float64(d[0]))                      # one rounding: the product of two floats is exact in double
+    d2 = f(np.float64(d[1]) * np.float64(d[1]) + np.float64(d2))     # fmaf: exact product + addend, one rounding
+    d2 = f(np.float64(d[2]) * np.float64(d[2]) + np.float64(d2))
+    return d2 > r2open
+
+
+def test_eq1_mac_columns_and_lists_equal_a_walk_written_from_the_definition():
+    """The Eq.1 twin of the minimum-distance pin: l, delta, r2_open of EVERY cell from the tight box and the fp32 centre of
+    mass in numpy float32 (array_equal on all three columns), and the lists of a root-to-leaf walk with that test."""
+    st, _ = _state("c1", 3000)
+    t = st.tree
+    theta = np.float32(0.6)
+    r = oracle.walk_forces(t, st.pos, theta=float(theta), eps=0.01, sel=[0], forces=False)
+    mac = r["mac"]
+    com = t.mom64[:, 1:4].astype(np.float32)
+    bmin, bmax = t.box[:, :3], t.box[:, 3:]
+    l = (bmax - bmin).astype(np.float32).max(axis=1)
+    gc = (np.float32(0.5) * (bmin + bmax).astype(np.float32)).astype(np.float32)
+    u = (com - gc).astype(np.float32)
+    uu = (u * u).astype(np.float32)
+    s2 = ((uu[:, 0] + uu[:, 1]).astype(np.float32) + uu[:, 2]).astype(np.float32)
+    delta = np.sqrt(s2).astype(np.float32)
+    ropen = ((l / theta).astype(np.float32) + delta).astype(np.float32)
+    assert np.array_equal(mac[:, 0], l) and np.array_equal(mac[:, 1], delta)
+    assert np.array_equal(mac[:, 2], (ropen * ropen).astype(np.float32))
+    assert np.count_nonzero(delta) > 0.5 * t.ncells                 # the offset term is exercised by every cell with more than one particle
+    for g in range(0, t.ngroups, 7):
+        r = oracle.walk_forces(t, st.pos, theta=float(theta), eps=0.01, sel=[g], forces=False, want_lists=True)
+        cells, leaves, todo = [], [], [0]
+        while todo:
+            c = todo.pop()
+            if _eq1_accept_np(t.gbox[g], com[c], mac[c, 2]):
+                cells.append(c)
+            elif t.nchild[c] == 0:
+                leaves.append(c)
+            else:
+                todo.extend(range(t.child_begin[c], t.child_begin[c] + t.nchild[c]))
+        assert sorted(cells) == sorted(r["cells"].tolist()) and sorted(leaves) == sorted(r["leaves"].tolist())
