@@ -55,6 +55,8 @@ typedef struct bh_config {
     int32_t walk_waves; /* 0 (default): as few waves of groups as the list buffer allows (normally 1), one after the other;
                          * k > 1: at least k waves, run as a pipeline (list walk of wave w + 1 beside the evaluation of
                          * wave w on internal streams); 0..255 */
+    int32_t front_mode; /* 0 (default): S0-S3 in one cooperative launch whenever every sort tile is resident at once
+                         * (n <= 4096 x 2 x SMs, 1.2 M on B200); 1: always one launch per step and sort pass (any n) */
 } bh_config;
 
 typedef struct bh_ctx bh_ctx;

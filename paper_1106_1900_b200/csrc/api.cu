@@ -21,8 +21,8 @@ struct Carver {
 };
 
 struct Geometry {
-    int64_t n_max, max_cells, sort_tiles, tree_tiles, scan_sum_cap, list_entries;
-    int32_t nleaf, ncrit, walk_mode, walk_waves;
+    int64_t n_max, max_cells, sort_tiles, tree_tiles, list_entries;
+    int32_t nleaf, ncrit, walk_mode, walk_waves, front_mode;
 };
 
 static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
@@ -42,10 +42,10 @@ static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
     if (g->walk_mode < 0 || g->walk_mode > 1) return false;
     g->walk_waves = cfg ? cfg->walk_waves : 0;
     if (g->walk_waves < 0 || g->walk_waves > kMaxWaves) return false;
+    g->front_mode = cfg ? cfg->front_mode : 0;
+    if (g->front_mode < 0 || g->front_mode > 1) return false;
     g->sort_tiles = div_up(n_max, kSortTile);
     g->tree_tiles = div_up(n_max + 1, kTreeTile);
-    const int64_t biggest_scan = std::max<int64_t>(std::max<int64_t>((int64_t)kRadix * g->sort_tiles, (int64_t)kLevels * g->tree_tiles), n_max);
-    g->scan_sum_cap = div_up(biggest_scan, kScanTile) + 1;
     return true;
 }
 
@@ -58,11 +58,18 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     for (int k = 0; k < 2; ++k) { o.pos[k] = c.take<float4>(n); o.vel[k] = c.take<float4>(n); o.idb[k] = c.take<uint32_t>(n); }
     o.acc = c.take<float4>(n);
     for (int k = 0; k < 2; ++k) { o.key[k] = c.take<uint64_t>(n); o.val[k] = c.take<uint32_t>(n); }
-    o.fl = c.take<uint8_t>(n + 1);
-    o.dep = c.take<uint8_t>(n);
+    // control words that must be zero between launches (one memset in bh_create): kept together
+    o.front_gsum = c.take<uint32_t>((size_t)kSortPasses * kFrontGroupCap * kRadix + 8);
+    o.front_ctl = o.front_gsum ? o.front_gsum + (size_t)kSortPasses * kFrontGroupCap * kRadix : nullptr;
+    o.front_bar = o.front_ctl;
+    o.tree_done = o.front_ctl ? o.front_ctl + 2 : nullptr;
+    o.mom_done = o.front_ctl ? o.front_ctl + 3 : nullptr;
+    o.front_part = c.take<float>(8 * (size_t)g.sort_tiles);
+    o.front_matrix = c.take<uint32_t>((size_t)kRadix * (size_t)std::min<int64_t>(g.sort_tiles, kFrontTileCap));
+    o.fl = c.take<uint8_t>(n + 8);      // (k_bounds stores four boundaries per word: padded)
+    o.dep = c.take<uint8_t>(n + 8);
+    o.gl = c.take<uint8_t>(n + 8);
     o.gflag = c.take<uint8_t>(n);
-    o.gcell_at = c.take<uint32_t>(n);
-    o.gscan = c.take<uint32_t>(n);
     o.g_begin = c.take<uint32_t>(n + 1);
     o.g_cell = c.take<uint32_t>(n);
     o.g_npc = c.take<uint32_t>(n);
@@ -70,15 +77,11 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     o.sort_ghist = c.take<uint32_t>((size_t)kSortPasses * kRadix + kSortPasses + (size_t)kSortPasses * kRadix * g.sort_tiles);
     o.sort_ticket = o.sort_ghist ? o.sort_ghist + kSortPasses * kRadix : nullptr;
     o.sort_status = o.sort_ghist ? o.sort_ticket + kSortPasses : nullptr;
-    o.scan_sums = c.take<uint32_t>((size_t)g.scan_sum_cap);
-    o.tile_cnt = c.take<uint32_t>((size_t)kLevels * g.tree_tiles);
-    o.tile_base = c.take<uint32_t>((size_t)kLevels * g.tree_tiles);
-    o.c_pbegin = c.take<uint32_t>(C);
-    o.c_pend = c.take<uint32_t>(C);
-    o.c_cbegin = c.take<uint32_t>(C);
-    o.c_cend = c.take<uint32_t>(C);
+    o.tile_cnt = c.take<uint32_t>((size_t)kTreeRows * g.tree_tiles);
+    o.row_total = c.take<uint32_t>(kTreeRows);
+    o.mom_span = c.take<uint32_t>((size_t)kLevels * kMomBlockCap);
+    o.c_topo = c.take<uint4>(C);
     o.c_parent = c.take<uint32_t>(C);
-    o.c_arrive = c.take<uint32_t>(C);
     o.mom64 = c.take<double>(10 * C);
     o.box = c.take<float>(6 * C);
     o.trec = c.take<float4>(C);
@@ -92,6 +95,7 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     o.deferred = c.take<uint32_t>(n);
     o.e_level = c.take<int32_t>(C);
     o.e_prefix = c.take<uint64_t>(C);
+    o.e_pbegin = c.take<uint32_t>(C);
     o.e_pcount = c.take<uint32_t>(C);
     o.e_cbegin = c.take<int32_t>(C);
     o.e_nchild = c.take<int32_t>(C);
@@ -146,7 +150,7 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
     c->walk_waves = g.walk_waves;
     c->sort_tiles = g.sort_tiles;
     c->tree_tiles = g.tree_tiles;
-    c->scan_sum_cap = g.scan_sum_cap;
+    c->front_enabled = g.front_mode == 0;
     carve(g, static_cast<unsigned char*>(d_workspace), &c->ws);
     int rc = BH_OK;
     do {
@@ -154,6 +158,9 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
         int sms = 0;
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
         c->sm_count = sms;
+        if (cudaMemset(c->ws.sc, 0, sizeof(DevScalars)) != cudaSuccess) { rc = BH_ERR_CUDA; break; }   // status = BH_OK before the first build
+        if (cudaMemset(c->ws.front_gsum, 0, sizeof(uint32_t) * ((size_t)kSortPasses * kFrontGroupCap * kRadix + 8)) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
+        if (front_init(c) != BH_OK || moments_init(c) != BH_OK) { rc = BH_ERR_CUDA; break; }
         if (walk_init(c) != BH_OK || sort_init(c) != BH_OK) { rc = BH_ERR_CUDA; break; }
         for (int k = 0; k < 13; ++k)
             if (cudaEventCreate(&c->ev[k]) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
@@ -180,6 +187,7 @@ int bh_set_particles(bh_ctx* c, int64_t n, const float* pos_mass, const float* v
     c->n = n;
     c->cur = 0;
     c->have_particles = c->have_topology = c->have_tree = c->have_forces = false;
+    c->acc_in_order = true;                                   // zeroed below, in the callers' order
     BH_CUDA(c, cudaMemcpyAsync(c->ws.pos[0], pos_mass, sizeof(float4) * (size_t)n, cudaMemcpyDefault, s));
     // S0-S2 need the positions only: velocities, ids and the zeroed accelerations arrive on an internal stream beside them
     // and are joined (event) before the first stage that touches them (S3) or any call that reads them.  Not under
@@ -208,6 +216,7 @@ int bh_set_particles(bh_ctx* c, int64_t n, const float* pos_mass, const float* v
 int bh_get_particles(bh_ctx* c, float* pos_mass, float* vel, float* acc_pot, uint32_t* id, void* stream) {
     if (!c) return BH_ERR_INVALID_ARG;
     if (!c->have_particles) return BH_ERR_STATE;
+    if (acc_pot && !c->acc_in_order) return BH_ERR_STATE;    // the particles were re-sorted (bh_tree_build) after the last forces
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     BH_CUDA(c, cudaSetDevice(c->device));
     { int rcj = join_copies(c, s); if (rcj != BH_OK) return rcj; }
@@ -225,20 +234,32 @@ int bh_tree_build(bh_ctx* c, void* stream) {
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     BH_CUDA(c, cudaSetDevice(c->device));
     c->have_topology = c->have_tree = c->have_forces = false;
+    c->acc_in_order = false;                                  // S3 permutes pos / vel / id; acc_pot follows at the next forces
     int rc;
     if (c->timing) cudaEventRecord(c->ev[0], s);
-    if ((rc = stage_bbox_keys(c, s)) != BH_OK) return rc;      // records ev[1] between bbox and keys
-    if (c->timing) cudaEventRecord(c->ev[2], s);
-    if ((rc = stage_sort(c, s)) != BH_OK) return rc;
-    if (c->timing) cudaEventRecord(c->ev[3], s);
-    if ((rc = join_copies(c, s)) != BH_OK) return rc;          // S3 is the first stage that reads velocities and ids
-    if ((rc = stage_reorder(c, s)) != BH_OK) return rc;
+    if (front_fits(c)) {
+        // S0-S3 in one cooperative launch (front.cu); reported as "sort".  While velocities / ids of bh_set_particles are
+        // still arriving on the side stream, S3 stays a launch of its own behind the join.
+        const bool fuse = !c->copies_pending;
+        if (c->timing) { cudaEventRecord(c->ev[1], s); cudaEventRecord(c->ev[2], s); }
+        if ((rc = stage_front(c, fuse, s)) != BH_OK) return rc;
+        if (c->timing) cudaEventRecord(c->ev[3], s);
+        if (!fuse) {
+            if ((rc = join_copies(c, s)) != BH_OK) return rc;
+            if ((rc = stage_reorder(c, s)) != BH_OK) return rc;
+        }
+    } else {
+        if ((rc = stage_bbox_keys(c, s)) != BH_OK) return rc;      // records ev[1] between bbox and keys
+        if (c->timing) cudaEventRecord(c->ev[2], s);
+        if ((rc = stage_sort(c, s)) != BH_OK) return rc;
+        if (c->timing) cudaEventRecord(c->ev[3], s);
+        if ((rc = join_copies(c, s)) != BH_OK) return rc;          // S3 is the first stage that reads velocities and ids
+        if ((rc = stage_reorder(c, s)) != BH_OK) return rc;
+    }
     if (c->timing) cudaEventRecord(c->ev[4], s);
-    if ((rc = stage_cells(c, s)) != BH_OK) return rc;
-    if (c->timing) cudaEventRecord(c->ev[5], s);
-    if ((rc = stage_groups(c, s)) != BH_OK) return rc;
+    if ((rc = stage_cells(c, s)) != BH_OK) return rc;             // S4 + S5; records ev[5] between k_bounds and k_emit
     if (c->timing) cudaEventRecord(c->ev[6], s);
-    if ((rc = stage_moments(c, s)) != BH_OK) return rc;
+    if ((rc = stage_moments(c, c->theta_last, s)) != BH_OK) return rc;   // S6; with the fp32 records when theta is known
     if (c->timing) cudaEventRecord(c->ev[7], s);
     c->have_topology = c->have_tree = true;
     return BH_OK;
@@ -250,7 +271,7 @@ int bh_refresh_moments(bh_ctx* c, void* stream) {
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     BH_CUDA(c, cudaSetDevice(c->device));
     c->have_forces = false;
-    int rc = stage_moments(c, s);
+    int rc = stage_moments(c, c->theta_last, s);
     if (rc != BH_OK) return rc;
     c->have_tree = true;
     return BH_OK;
@@ -269,6 +290,7 @@ static int compute_forces_impl(bh_ctx* c, float theta, float eps, const uint8_t*
     if (rc != BH_OK) return rc;
     c->theta_last = theta;
     c->have_forces = true;
+    c->acc_in_order = true;    // (after an active-subset walk the rows of the other groups keep what they held)
     return BH_OK;
 }
 
@@ -289,6 +311,7 @@ int bh_leapfrog_step(bh_ctx* c, float theta, float eps, float dt, void* stream) 
     BH_CUDA(c, cudaSetDevice(c->device));
     const float h = 0.5f * dt;
     int rc;
+    c->theta_last = theta;                                    // S6 writes the fp32 records for this theta in the same pass
     if ((rc = stage_kick_drift(c, h, dt, s)) != BH_OK) return rc;
     if ((rc = bh_tree_build(c, stream)) != BH_OK) return rc;
     if ((rc = bh_compute_forces(c, theta, eps, stream)) != BH_OK) return rc;
@@ -316,7 +339,7 @@ int bh_sync_status(bh_ctx* c, void* stream, bh_stats* out) {
     BH_CUDA(c, cudaStreamSynchronize(s));
     if (out) {
         std::memset(out, 0, sizeof(*out));
-        out->status = c->have_tree ? h.status : BH_OK;
+        out->status = h.status;
         out->n = c->n;
         out->launches = c->launches;
         if (c->have_tree) {
@@ -332,7 +355,7 @@ int bh_sync_status(bh_ctx* c, void* stream, bh_stats* out) {
             out->sum_mac = (int64_t)h.sum_mac;
         }
     }
-    return c->have_tree ? h.status : BH_OK;
+    return h.status;
 }
 
 int bh_export_tree(bh_ctx* c, bh_tree_view* v, void* stream) {
@@ -352,7 +375,7 @@ int bh_export_tree(bh_ctx* c, bh_tree_view* v, void* stream) {
     v->level_offset = c->ws.sc->level_offset;
     v->cell_level = w.e_level;
     v->cell_prefix = w.e_prefix;
-    v->cell_pbegin = w.c_pbegin;
+    v->cell_pbegin = w.e_pbegin;
     v->cell_pcount = w.e_pcount;
     v->cell_child_begin = w.e_cbegin;
     v->cell_nchild = w.e_nchild;

@@ -23,14 +23,13 @@ constexpr int kSortThreads = 256;
 constexpr int kSortItemsPerThread = 16;
 constexpr int kSortTile = kSortThreads * kSortItemsPerThread;   // 4096 keys per block
 
-// ---- scan geometry
-constexpr int kScanThreads = 256;
-constexpr int kScanItems = 8;
-constexpr int kScanTile = kScanThreads * kScanItems;            // 2048 entries per block
-
-// ---- tree geometry (S4): one boundary per thread
-constexpr int kTreeTile = 256;
-constexpr int kHaloMax = 64;           // nleaf <= 64
+// ---- tree geometry (S4, S5): one boundary per thread
+constexpr int kTreeTile = 1024;
+constexpr int kHaloMax = 64;           // nleaf, ncrit <= 64
+constexpr int kTreeRows = kLevels + 1; // per-tile counts of starts: cells of level 0..20, then groups
+constexpr int kFrontTileCap = 1024;    // most sort tiles k_front can ever have resident (bounds its digit-count matrix)
+constexpr int kFrontGroupCap = kFrontTileCap / 16;   // groups of 16 tiles
+constexpr int kMomBlockCap = 160;      // most blocks of k_moments (one per SM; bounds the shared memory of k_moments_span)
 
 // ---- walk (S7, S8): waves of groups whose interaction lists share the list buffer
 constexpr int kMaxWaves = 255;
@@ -66,6 +65,12 @@ struct WalkCtl {
     unsigned long long t_end[2][kMaxWaves + 1];
 };
 
+__device__ __forceinline__ uint32_t ld_relaxed_u32(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
 __device__ __forceinline__ unsigned long long global_ns() {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
@@ -83,9 +88,8 @@ struct Ws {
     uint32_t* val[2];
     uint8_t* fl;          // [n+1] first level at which boundary i starts a new run (0..21)
     uint8_t* dep;         // [n]   level of the leaf holding particle i
-    uint8_t* gflag;       // [n]   1 where a group starts
-    uint32_t* gcell_at;   // [n]   cell of the group starting here
-    uint32_t* gscan;      // [n]   exclusive scan of gflag
+    uint8_t* gl;          // [n]   level of the cell of the group that starts at particle i (0xFF: no group starts here)
+    uint8_t* gflag;       // [n]   per GROUP: 1 if the group takes part in an active-subset walk (bh_compute_forces_active)
     uint32_t* g_begin;    // [n+1]
     uint32_t* g_cell;     // [n]
     uint32_t* g_npc;      // [n]
@@ -93,15 +97,18 @@ struct Ws {
     uint32_t* sort_ghist;  // [kSortPasses][kRadix] keys per digit value, all passes (counted by k_keys)
     uint32_t* sort_ticket; // [kSortPasses] tile tickets                       (contiguous with sort_ghist and
     uint32_t* sort_status; // [kSortPasses][sortTiles][kRadix] look-back words  sort_status: one memset)
-    uint32_t* scan_sums;  // partial sums of the generic scan
-    uint32_t* tile_cnt;   // [kLevels * treeTiles]
-    uint32_t* tile_base;  // same
-    uint32_t* c_pbegin;   // [max_cells]
-    uint32_t* c_pend;
-    uint32_t* c_cbegin;   // first child (0 for a leaf)
-    uint32_t* c_cend;     // one past the last child (0 for a leaf)
+    uint32_t* tile_cnt;   // [kTreeRows][treeTiles] starts per tile; after k_bounds: exclusive scan of every row over the tiles
+    uint32_t* row_total;  // [kTreeRows] cells per level, groups
+    uint32_t* tree_done;  // [1] blocks of k_bounds that have finished (returns to 0)
+    uint32_t* mom_span;   // [kLevels][momentBlocks] cell of each level that straddles the end of a block's particle range (kNone: none)
+    uint32_t* mom_done;   // [1] blocks of k_moments that have finished (returns to 0)
+    float* front_part;    // [sortTiles][8] per-tile box of k_front
+    uint32_t* front_matrix; // [frontTiles][kRadix] per-tile digit counts of the current pass
+    uint32_t* front_gsum;   // [kSortPasses][kFrontGroupCap][kRadix] digit counts per pass and group of 16 tiles (zero between launches)
+    uint32_t* front_ctl;    // control words that are zero between launches: front_bar[2], tree_done, mom_done
+    uint32_t* front_bar;    // [2] grid barrier of k_front: arrivals, generation
+    uint4* c_topo;        // [max_cells] (first particle, end particle, first child, end child); children (0, 0) for a leaf
     uint32_t* c_parent;
-    uint32_t* c_arrive;   // [max_cells] children that have published their moments (S6)
     double* mom64;        // [max_cells][10]
     float* box;           // [max_cells][6]
     float4* trec;         // [max_cells] walk record: (com, r2open)
@@ -116,6 +123,7 @@ struct Ws {
     // export (canonical arrays of bh_tree_view)
     int32_t* e_level;
     uint64_t* e_prefix;
+    uint32_t* e_pbegin;
     uint32_t* e_pcount;
     int32_t* e_cbegin;
     int32_t* e_nchild;
@@ -136,6 +144,7 @@ struct bh_ctx {
     int cur;               // which of pos[2]/vel[2]/idb[2] holds the live state
     int sorted;            // which of key[2]/val[2] holds the sorted keys / perm
     bool have_particles, have_topology, have_tree, have_forces;   // topology: cells + groups; tree: topology + current moments
+    bool acc_in_order;     // ws.acc is in the order of the current particle arrays (false between a re-sort and the next full forces)
     const uint8_t* active;   // per-particle flags of bh_compute_forces_active during that call (nullptr: every group)
     int64_t launches;
     int last_cuda;
@@ -145,7 +154,12 @@ struct bh_ctx {
     int walk_waves;
     int mac_kind;          // 0: Eq.1, 1: minimum distance (bh_set_mac)
     bh::Ws ws;
-    int64_t sort_tiles, tree_tiles, scan_sum_cap;
+    int64_t sort_tiles, tree_tiles;
+    int64_t front_max_tiles;   // sort tiles that are resident at once in a cooperative launch of k_front (0: not available)
+    bool front_enabled;        // bh_config.front_mode != 1
+    bool rec_valid;            // trec / tlink / erec hold the current tree for (rec_theta, rec_mac)
+    float rec_theta;
+    int rec_mac;
     bool timing;
     cudaEvent_t ev[13];     // [0..10] stage boundaries; [11], [12]: after the list walk / the evaluation of a one-wave walk
     bool copies_pending;    // bh_set_particles left copies on s_lists; ev_join marks their end (api.cu: join_copies)
@@ -180,13 +194,16 @@ namespace bh {
 static inline int64_t div_up(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // stage entry points (each only enqueues kernels on `s`)
+int front_init(bh_ctx* c);
+int moments_init(bh_ctx* c);
+bool front_fits(const bh_ctx* c);
+int stage_front(bh_ctx* c, bool fuse_reorder, cudaStream_t s);   // S0-S2 (+ S3) in one cooperative launch (front.cu)
 int stage_bbox_keys(bh_ctx* c, cudaStream_t s);       // S0, S1
 int stage_sort(bh_ctx* c, cudaStream_t s);            // S2
 int stage_reorder(bh_ctx* c, cudaStream_t s);         // S3
-int stage_cells(bh_ctx* c, cudaStream_t s);           // S4
-int stage_groups(bh_ctx* c, cudaStream_t s);          // S5
-int stage_moments(bh_ctx* c, cudaStream_t s);         // S6
-int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s);          // S6: fp32 walk record + r2open(theta)
+int stage_cells(bh_ctx* c, cudaStream_t s);           // S4 + S5
+int stage_moments(bh_ctx* c, float theta, cudaStream_t s);              // S6 (+ the fp32 records when theta > 0)
+int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s);          // S6: fp32 walk record + r2open(theta) alone
 int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s);   // S7, S8
 int stage_group_active(bh_ctx* c, const uint8_t* d_active, cudaStream_t s);   // groups with an active particle -> ws.gflag[g]
 int walk_init(bh_ctx* c);
@@ -202,14 +219,10 @@ struct WalkListOut {       // what k_walk_lists writes
 WalkListOut walk_list_out(bh_ctx* c);
 int stage_walk_prepare(bh_ctx* c, int nwaves, uint32_t wave_particles, cudaStream_t s);
 int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t region_base, uint32_t region_entries, cudaStream_t s);   // S7
-int stage_walk_eval(bh_ctx* c, int wave, float eps, int blocks_per_sm, cudaStream_t s);                           // S8
+int stage_walk_eval(bh_ctx* c, int wave, float eps, int blocks_per_sm, bool by_class, cudaStream_t s);                           // S8
 int stage_kick_drift(bh_ctx* c, float h, float dt, cudaStream_t s);  // S9
 int stage_kick(bh_ctx* c, float h, cudaStream_t s);                  // S9
 int stage_export(bh_ctx* c, cudaStream_t s);
 int stage_iota(bh_ctx* c, uint32_t* dst, int64_t n, cudaStream_t s);
-
-// generic exclusive scan (three kernels, no spinning): out[i] = sum_{j<i} in[j]; *total (device) = sum of all
-int scan_u32(bh_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, uint32_t* d_total, cudaStream_t s);
-int scan_u8(bh_ctx* c, const uint8_t* in, uint32_t* out, int64_t n, uint32_t* d_total, cudaStream_t s);
 
 }  // namespace bh

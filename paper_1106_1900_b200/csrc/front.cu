@@ -1,0 +1,441 @@
+// front.cu -- S0 domain box, S1 Morton keys, S2 stable LSD radix sort and S3 reorder in ONE cooperative launch, for
+// inputs whose sort tiles are all resident on the device at once (n <= 4096 x 2 x SMs: 1.2 M particles on B200).
+// PAPER.md:374-392 (keys), PAPER.md:350-370 (split / radix sort), PAPER.md:174 ("moving").
+//
+// Why: at 1 M particles the whole front end moves ~0.3 GB that sits in the 126 MB L2; the round-1 sequence of 14
+// launches (box, domain, keys, 8 sort passes with a decoupled look-back each, reorder) spent its time in launch gaps and
+// in the look-back chain, not in bandwidth.  Here one block owns one tile of 4096 particles for the whole kernel:
+//   * the box is reduced per tile and combined by every block after a grid barrier (no atomics, no reset launch);
+//   * the keys are made in registers and go straight into the first sort pass (the unsorted keys are never written);
+//   * a pass = rank the tile (one ballot per digit bit, as in keys_sort.cu), publish the tile's digit counts as a row
+//     of a [tiles][256] matrix (+ a reduction into the pass's global digit histogram), GRID BARRIER, sum the rows of
+//     the earlier tiles (all co-resident: no look-back chain), exchange through shared memory, scatter, GRID BARRIER;
+//   * the last phase gathers positions, velocities and ids by the permutation.
+// The barrier is a sense-reversing counter pair in the workspace (cooperative launch guarantees co-residency).
+// Values other blocks wrote during this launch are read with ld.global.cg: L1 may hold lines from earlier passes.
+// Result: identical to keys_sort.cu (stable LSD order is unique), which still serves larger inputs.
+#include <algorithm>
+#include <cstdio>
+#include "bh_internal.cuh"
+
+#ifdef BH_TIMELINE
+// working aid (-DBH_TIMELINE builds only): %globaltimer stamps of this file's kernel, read back by bh_debug_front
+__device__ unsigned long long g_bh_dbg[1024];
+extern "C" int bh_debug_front(unsigned long long* host1024) { return (int)cudaMemcpyFromSymbol(host1024, g_bh_dbg, sizeof(unsigned long long) * 1024); }
+#endif
+
+namespace bh {
+
+constexpr int kFrontThreads = 512;
+constexpr int kFrontWarps = kFrontThreads / 32;                 // 16
+constexpr int kFrontItems = kSortTile / kFrontThreads;          // 8 keys per thread
+constexpr uint32_t kBarSpinLimit = 1u << 24;
+
+struct FrontArgs {
+    const float4* pos_in;
+    const float4* vel_in;
+    const uint32_t* id_in;
+    float4* pos_out;
+    float4* vel_out;
+    uint32_t* id_out;
+    int n;
+    int fuse_reorder;
+    uint64_t* key0;
+    uint64_t* key1;
+    uint32_t* val0;
+    uint32_t* val1;
+    DevScalars* sc;
+    float* part;         // [tiles][8]   per-tile box: min xyz, max xyz, bad flag
+    uint32_t* matrix;    // [tiles][256] digit counts of every tile in the current pass
+    uint32_t* gsum;      // [8][groups][256] digit counts per pass and group of 16 tiles; zero on entry, zeroed again on exit
+    uint32_t* bar;       // [2]          barrier: arrivals, generation
+};
+
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// All blocks of the (cooperative) grid meet here.  bar[0] counts the arrivals of every barrier but the last (barrier k is
+// passed at k x blocks arrivals); the last barrier of the launch counts on bar[1], which only ever grows (`b0` = its value
+// when this block started, read before any block can arrive there), so that block 0 can put bar[0] back to zero for the
+// next launch once everybody is known to have left it.
+__device__ __forceinline__ void grid_barrier(uint32_t* bar, uint32_t target, DevScalars* sc) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();                                   // release what this block wrote
+        atomicAdd(bar, 1u);
+        uint32_t spins = 0;
+        while (ld_acquire_u32(bar) < target)
+            if (++spins > kBarSpinLimit) { atomicMin(&sc->status, (int)BH_ERR_CUDA); break; }   // never hang the device
+        __threadfence();
+    }
+    __syncthreads();
+}
+__device__ __forceinline__ void grid_barrier_last(uint32_t* bar, uint32_t b0, uint32_t nblocks, DevScalars* sc) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(bar + 1, 1u);
+        uint32_t spins = 0;
+        while (ld_acquire_u32(bar + 1) - b0 < nblocks)
+            if (++spins > kBarSpinLimit) { atomicMin(&sc->status, (int)BH_ERR_CUDA); break; }
+        if (blockIdx.x == 0) atomicExch(bar, 0u);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+__device__ __forceinline__ uint64_t dilate20f(uint32_t v) {
+    uint64_t x = v & 0xFFFFFu;
+    x = (x | (x << 32)) & 0x001F00000000FFFFull;
+    x = (x | (x << 16)) & 0x001F0000FF0000FFull;
+    x = (x | (x << 8)) & 0x100F00F00F00F00Full;
+    x = (x | (x << 4)) & 0x10C30C30C30C30C3ull;
+    x = (x | (x << 2)) & 0x1249249249249249ull;
+    return x;
+}
+
+// (x - lo) * 2^sh truncated and clamped to 20 bits.  The subtraction is the only rounding (O2): `scale` = 2^sh exactly
+// when sh is in the normal range (the product of a float and a power of two is exact unless it underflows, and then it is
+// < 1 either way); otherwise ldexpf.  cvt.rzi.u32.f32 truncates, sends negatives and NaN to 0 and saturates.
+__device__ __forceinline__ uint32_t grid_coordf(float x, float lo, int sh, float scale) {
+    const float d = __fsub_rn(x, lo);
+    const float s = scale != 0.0f ? __fmul_rn(d, scale) : ldexpf(d, sh);
+    return min(__float2uint_rz(s), (1u << kKeyBits) - 1u);
+}
+
+// exclusive prefix of v over the first 256 threads of a 512-thread block (threads >= 256 pass 0); every thread gets
+// the prefix of its own index
+__device__ __forceinline__ uint32_t block_excl_scan512(uint32_t v, uint32_t* wsum /*[16]*/) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    uint32_t base = 0;
+#pragma unroll
+    for (int k = 0; k < kFrontWarps; ++k) {
+        const uint32_t s = wsum[k];
+        if (k < w) base += s;
+    }
+    __syncthreads();
+    return base + inc - v;
+}
+
+__global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
+    extern __shared__ __align__(16) unsigned char xch[];
+    uint64_t* skey = reinterpret_cast<uint64_t*>(xch);
+    uint32_t* sval = reinterpret_cast<uint32_t*>(xch + kSortTile * 8);
+    __shared__ uint16_t wcnt[kFrontWarps][kRadix];
+    __shared__ uint32_t gbase[kRadix], lbase[kRadix], ex2[2][kRadix], tot2[2][kRadix];
+    __shared__ uint32_t wsum[kFrontWarps];
+    __shared__ float redf[kFrontWarps][8];
+    __shared__ float s_lo[3];
+    __shared__ int s_sh;
+
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const uint32_t tile = blockIdx.x, T = gridDim.x, G = (T + 15u) >> 4;
+    const int n = a.n;
+    const int wbase = (int)tile * kSortTile + w * (kFrontItems * 32);   // warp w owns a contiguous run: order = (warp, iteration, lane)
+    const uint32_t lt = (1u << lane) - 1u;
+    uint32_t b0 = 0, nbar = 0;                             // barrier bookkeeping (thread 0)
+    if (tid == 0) b0 = ld_acquire_u32(a.bar + 1);
+#ifdef BH_TIMELINE
+    int ntl = 0;
+#define TL() do { if (tid == 0 && (tile == 0 || tile == T - 1) && ntl < 120) g_bh_dbg[(tile == 0 ? 0 : 128) + ntl++] = global_ns(); } while (0)
+#else
+#define TL() do {} while (0)
+#endif
+    TL();
+
+    // ---------------------------------------------------------------- S0: box of this tile
+    {
+        float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
+        int bad = 0;
+#pragma unroll
+        for (int it = 0; it < kFrontItems; ++it) {
+            const int i = wbase + it * 32 + lane;
+            if (i < n) {
+                const float4 p = a.pos_in[i];
+                bad |= !(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(p.w) && p.w > 0.0f);
+                mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
+                mn[1] = fminf(mn[1], p.y); mx[1] = fmaxf(mx[1], p.y);
+                mn[2] = fminf(mn[2], p.z); mx[2] = fmaxf(mx[2], p.z);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                mn[k] = fminf(mn[k], __shfl_xor_sync(0xFFFFFFFFu, mn[k], o));
+                mx[k] = fmaxf(mx[k], __shfl_xor_sync(0xFFFFFFFFu, mx[k], o));
+            }
+            bad |= __shfl_xor_sync(0xFFFFFFFFu, bad, o);
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { redf[w][k] = mn[k]; redf[w][3 + k] = mx[k]; }
+            redf[w][6] = bad ? 1.0f : 0.0f;
+        }
+        __syncthreads();
+        if (tid < 7) {
+            float v = redf[0][tid];
+            for (int ww = 1; ww < kFrontWarps; ++ww) v = tid < 3 ? fminf(v, redf[ww][tid]) : fmaxf(v, redf[ww][tid]);
+            a.part[(size_t)tile * 8 + tid] = v;
+        }
+    }
+    TL();
+    grid_barrier(a.bar, ++nbar * T, a.sc);
+    TL();
+
+    // ---------------------------------------------------------------- domain (every block, redundantly): DESIGN.md O1
+    {
+        float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
+        float bad = 0.0f;
+        for (uint32_t t = tid; t < T; t += kFrontThreads) {
+            const float4 p0 = __ldcg(reinterpret_cast<const float4*>(a.part + (size_t)t * 8));
+            const float4 p1 = __ldcg(reinterpret_cast<const float4*>(a.part + (size_t)t * 8 + 4));
+            mn[0] = fminf(mn[0], p0.x); mn[1] = fminf(mn[1], p0.y); mn[2] = fminf(mn[2], p0.z);
+            mx[0] = fmaxf(mx[0], p0.w); mx[1] = fmaxf(mx[1], p1.x); mx[2] = fmaxf(mx[2], p1.y);
+            bad = fmaxf(bad, p1.z);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                mn[k] = fminf(mn[k], __shfl_xor_sync(0xFFFFFFFFu, mn[k], o));
+                mx[k] = fmaxf(mx[k], __shfl_xor_sync(0xFFFFFFFFu, mx[k], o));
+            }
+            bad = fmaxf(bad, __shfl_xor_sync(0xFFFFFFFFu, bad, o));
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { redf[w][k] = mn[k]; redf[w][3 + k] = mx[k]; }
+            redf[w][6] = bad;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            float lo[3], hi[3], anybad = 0.0f;
+            for (int k = 0; k < 3; ++k) { lo[k] = redf[0][k]; hi[k] = redf[0][3 + k]; }
+            for (int ww = 0; ww < kFrontWarps; ++ww) {
+                for (int k = 0; k < 3; ++k) { lo[k] = fminf(lo[k], redf[ww][k]); hi[k] = fmaxf(hi[k], redf[ww][3 + k]); }
+                anybad = fmaxf(anybad, redf[ww][6]);
+            }
+            float ext = 0.0f;
+            for (int k = 0; k < 3; ++k) ext = fmaxf(ext, __fsub_rn(hi[k], lo[k]));
+            int status = anybad > 0.0f ? (int)BH_ERR_NONFINITE : (int)BH_OK;
+            if (!isfinite(ext)) { status = (int)BH_ERR_NONFINITE; ext = 1.0f; }
+            if (ext == 0.0f) ext = 1.0f;
+            int e = 0;
+            (void)frexpf(ext, &e);                         // cube side 2^e: the smallest power of two strictly above the extent
+            for (int k = 0; k < 3; ++k) s_lo[k] = lo[k];
+            s_sh = kKeyBits - e;
+            if (tile == 0) {
+                for (int k = 0; k < 3; ++k) { a.sc->lo[k] = lo[k]; a.sc->hi[k] = hi[k]; }
+                a.sc->dom_e = e;
+                a.sc->status = status;
+                a.sc->n_cells = 0; a.sc->n_groups = 0; a.sc->n_levels = 0;
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---------------------------------------------------------------- S1: keys, in registers
+    uint64_t k[kFrontItems];
+    uint32_t v[kFrontItems];
+    {
+        const float lox = s_lo[0], loy = s_lo[1], loz = s_lo[2];
+        const int sh = s_sh;
+        const float scale = (sh >= -126 && sh <= 127) ? __int_as_float((127 + sh) << 23) : 0.0f;
+#pragma unroll
+        for (int it = 0; it < kFrontItems; ++it) {
+            const int i = wbase + it * 32 + lane;
+            k[it] = 0ull;
+            v[it] = (uint32_t)i;
+            if (i < n) {
+                const float4 p = a.pos_in[i];
+                k[it] = (dilate20f(grid_coordf(p.x, lox, sh, scale)) << 2) | (dilate20f(grid_coordf(p.y, loy, sh, scale)) << 1) | dilate20f(grid_coordf(p.z, loz, sh, scale));
+            }
+        }
+    }
+
+    TL();
+    // ---------------------------------------------------------------- S2: 8 passes of 8 bits
+    const int cnt_tile = min(kSortTile, n - (int)tile * kSortTile);
+#pragma unroll 1
+    for (int pass = 0; pass < kSortPasses; ++pass) {
+        const int shift = pass * kRadixBits;
+        const uint64_t* kin = (pass & 1) ? a.key0 : a.key1;      // pass p reads what pass p - 1 wrote: buffer (p - 1) & 1
+        const uint32_t* vin = (pass & 1) ? a.val0 : a.val1;
+        uint64_t* kout = (pass & 1) ? a.key1 : a.key0;
+        uint32_t* vout = (pass & 1) ? a.val1 : a.val0;
+        if (pass > 0) {
+#pragma unroll
+            for (int it = 0; it < kFrontItems; ++it) {
+                const int i = wbase + it * 32 + lane;
+                const bool ok = i < n;
+                k[it] = ok ? __ldcg(kin + i) : 0ull;
+                v[it] = ok ? __ldcg(vin + i) : 0u;
+            }
+        }
+        for (int j = tid; j < kFrontWarps * kRadix / 2; j += kFrontThreads) reinterpret_cast<uint32_t*>(&wcnt[0][0])[j] = 0u;
+        __syncthreads();
+        TL();
+        uint32_t rank[kFrontItems];
+#pragma unroll
+        for (int it = 0; it < kFrontItems; ++it) {
+            const int i = wbase + it * 32 + lane;
+            const bool ok = i < n;
+            const uint32_t d = (uint32_t)(k[it] >> shift) & (kRadix - 1);
+            uint32_t peers = __ballot_sync(0xFFFFFFFFu, ok);
+            if (!ok) peers = ~peers;
+#pragma unroll
+            for (int b = 0; b < kRadixBits; ++b) {
+                const bool bit = (d >> b) & 1u;
+                const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
+                peers &= bit ? m : ~m;
+            }
+            const uint32_t before = __popc(peers & lt);
+            uint32_t old = 0;
+            if (ok) old = wcnt[w][d];
+            __syncwarp();
+            if (ok && before == 0) wcnt[w][d] = (uint16_t)(old + __popc(peers));
+            __syncwarp();
+            rank[it] = old + before;
+        }
+        __syncthreads();
+        TL();
+        // digit = tid (first 256 threads): exclusive prefix over the warps, the tile's count; publish it
+        uint32_t tcount = 0;
+        if (tid < kRadix) {
+#pragma unroll
+            for (int ww = 0; ww < kFrontWarps; ++ww) {
+                const uint32_t t = wcnt[ww][tid];
+                wcnt[ww][tid] = (uint16_t)tcount;
+                tcount += t;
+            }
+            a.matrix[(size_t)tile * kRadix + tid] = tcount;
+            if (tcount) atomicAdd(a.gsum + ((size_t)pass * kFrontGroupCap + (tile >> 4)) * kRadix + tid, tcount);
+        }
+        TL();
+        grid_barrier(a.bar, ++nbar * T, a.sc);
+        TL();
+        // keys of this digit in the whole input (-> first output slot of the digit) and in the earlier tiles: the sums of the
+        // groups of 16 tiles + the rows of the earlier tiles of this tile's own group; split between the two halves of the block
+        {
+            const int d = tid & (kRadix - 1), h = tid >> 8;
+            const uint32_t* gs = a.gsum + (size_t)pass * kFrontGroupCap * kRadix + d;
+            const uint32_t myg = tile >> 4;
+            uint32_t tot = 0, ex = 0;
+#pragma unroll 8
+            for (uint32_t g = h; g < G; g += 2) {
+                const uint32_t x = __ldcg(gs + (size_t)g * kRadix);
+                tot += x;
+                if (g < myg) ex += x;
+            }
+#pragma unroll 8
+            for (uint32_t t = (myg << 4) + h; t < tile; t += 2) ex += __ldcg(a.matrix + (size_t)t * kRadix + d);
+            ex2[h][d] = ex;
+            tot2[h][d] = tot;
+        }
+        __syncthreads();
+        const uint32_t gh = tid < kRadix ? tot2[0][tid] + tot2[1][tid] : 0u;
+        const uint32_t dbase = block_excl_scan512(gh, wsum);                  // first output slot of digit d
+        const uint32_t dstart = block_excl_scan512(tcount, wsum);             // first slot of digit d inside the tile, sorted by digit
+        if (tid < kRadix) {
+            gbase[tid] = dbase + ex2[0][tid] + ex2[1][tid] - dstart;          // output slot = gbase[digit] + slot inside the sorted tile
+            lbase[tid] = dstart;
+        }
+        __syncthreads();
+        TL();
+        // exchange through shared memory: the tile leaves sorted by digit, so every digit's run is written contiguously
+#pragma unroll
+        for (int it = 0; it < kFrontItems; ++it) {
+            const int i = wbase + it * 32 + lane;
+            if (i < n) {
+                const uint32_t dg = (uint32_t)(k[it] >> shift) & (kRadix - 1);
+                const uint32_t lp = lbase[dg] + wcnt[w][dg] + rank[it];
+                skey[lp] = k[it];
+                sval[lp] = v[it];
+            }
+        }
+        __syncthreads();
+        TL();
+#pragma unroll 4
+        for (int lp = tid; lp < cnt_tile; lp += kFrontThreads) {
+            const uint64_t kk = skey[lp];
+            const uint32_t dst = gbase[(uint32_t)(kk >> shift) & (kRadix - 1)] + (uint32_t)lp;
+            kout[dst] = kk;
+            vout[dst] = sval[lp];
+        }
+        TL();
+        if (pass + 1 < kSortPasses) grid_barrier(a.bar, ++nbar * T, a.sc);
+        else grid_barrier_last(a.bar, b0, T, a.sc);
+        TL();
+        if (tile < G && tid < kRadix) a.gsum[((size_t)pass * kFrontGroupCap + tile) * kRadix + tid] = 0u;   // everyone has read it: zero for the next launch
+    }
+
+    // ---------------------------------------------------------------- S3: gather by the permutation (sorted keys / perm are in buffer 1)
+    if (a.fuse_reorder) {
+#pragma unroll 2
+        for (int it = 0; it < kFrontItems; ++it) {
+            const int j = wbase + it * 32 + lane;
+            if (j < n) {
+                const uint32_t src = __ldcg(a.val1 + j);
+                a.pos_out[j] = a.pos_in[src];
+                a.vel_out[j] = a.vel_in[src];
+                a.id_out[j] = a.id_in[src];
+            }
+        }
+    }
+    TL();
+#ifdef BH_TIMELINE
+    if (tid == 0 && (tile == 0 || tile == T - 1)) g_bh_dbg[(tile == 0 ? 0 : 128) + 127] = (unsigned long long)ntl;
+#endif
+}
+
+int front_init(bh_ctx* c) {
+    BH_CUDA(c, cudaFuncSetAttribute(k_front, cudaFuncAttributeMaxDynamicSharedMemorySize, kSortTile * 12));
+    int per_sm = 0;
+    BH_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_front, kFrontThreads, kSortTile * 12));
+    int coop = 0;
+    BH_CUDA(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device));
+    c->front_max_tiles = coop ? std::min<int64_t>((int64_t)per_sm * c->sm_count, kFrontTileCap) : 0;
+    return BH_OK;
+}
+
+bool front_fits(const bh_ctx* c) { return c->front_enabled && div_up(c->n, kSortTile) <= c->front_max_tiles; }
+
+// S0-S2 (and S3 unless velocities / ids are still arriving on the side stream) in one cooperative launch.
+int stage_front(bh_ctx* c, bool fuse_reorder, cudaStream_t s) {
+    const int n = (int)c->n;
+    const int tiles = (int)div_up(n, kSortTile);
+    const int a0 = c->cur, b0 = c->cur ^ 1;
+    FrontArgs a;
+    a.pos_in = c->ws.pos[a0]; a.vel_in = c->ws.vel[a0]; a.id_in = c->ws.idb[a0];
+    a.pos_out = c->ws.pos[b0]; a.vel_out = c->ws.vel[b0]; a.id_out = c->ws.idb[b0];
+    a.n = n;
+    a.fuse_reorder = fuse_reorder ? 1 : 0;
+    a.key0 = c->ws.key[0]; a.key1 = c->ws.key[1];
+    a.val0 = c->ws.val[0]; a.val1 = c->ws.val[1];
+    a.sc = c->ws.sc;
+    a.part = c->ws.front_part;
+    a.matrix = c->ws.front_matrix;
+    a.gsum = c->ws.front_gsum;
+    a.bar = c->ws.front_bar;
+    void* args[] = {(void*)&a};
+    cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_front, dim3(tiles), dim3(kFrontThreads), args, (size_t)kSortTile * 12, s);
+    c->launches += 1;
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return BH_ERR_CUDA; }
+    c->sorted = 1;                 // pass 7 wrote buffer 1
+    if (fuse_reorder) c->cur = b0;
+    return BH_OK;
+}
+
+}  // namespace bh

@@ -1,4 +1,5 @@
-// keys_sort.cu -- S0 domain box, S1 Morton keys, S2 stable LSD radix sort, S3 reorder, generic scan.
+// keys_sort.cu -- S0 domain box, S1 Morton keys, S2 stable LSD radix sort, S3 reorder: one kernel per step, for inputs of
+// any size (inputs whose sort tiles are all resident at once take the single cooperative launch of front.cu instead).
 // PAPER.md:374-392 (Appendix B: keys), PAPER.md:350-370 (Appendix A: scan, split, radix sort), PAPER.md:174 ("moving").
 #include <algorithm>
 #include "bh_internal.cuh"
@@ -130,11 +131,7 @@ __global__ void k_iota(uint32_t* dst, int n) {
     if (i < n) dst[i] = (uint32_t)i;
 }
 
-// ------------------------------------------------------------------------------------------ generic scan
-// Three kernels, no inter-block waiting: (A) per-tile sums, (B) one block scans the sums, (C) per-tile scan + offset.
-template <typename T>
-__device__ __forceinline__ uint32_t load_as_u32(const T* p, int64_t i) { return (uint32_t)p[i]; }
-
+// ------------------------------------------------------------------------------------------ block scan
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total) {
     // 256 threads; returns the exclusive prefix of v over the block
     __shared__ uint32_t wsum[8];
@@ -157,73 +154,6 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* t
     __syncthreads();
     *total = tot;
     return base + inc - v;
-}
-
-template <typename T>
-__global__ void __launch_bounds__(kScanThreads) k_scan_reduce(const T* __restrict__ in, int64_t n, uint32_t* __restrict__ sums) {
-    const int64_t base = (int64_t)blockIdx.x * kScanTile;
-    uint32_t s = 0;
-#pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
-        const int64_t i = base + k * kScanThreads + threadIdx.x;
-        if (i < n) s += load_as_u32(in, i);
-    }
-    uint32_t tot;
-    (void)block_exclusive_scan(s, &tot);
-    if (threadIdx.x == 0) sums[blockIdx.x] = tot;
-}
-
-__global__ void __launch_bounds__(kScanThreads) k_scan_sums(uint32_t* sums, int64_t m, uint32_t* d_total) {
-    // exclusive scan of sums[0..m) in place by one block; chunks of 256 with a running carry
-    uint32_t carry = 0;
-    for (int64_t b = 0; b < m; b += kScanThreads) {
-        const int64_t i = b + threadIdx.x;
-        const uint32_t v = (i < m) ? sums[i] : 0u;
-        uint32_t tot;
-        const uint32_t ex = block_exclusive_scan(v, &tot);
-        if (i < m) sums[i] = carry + ex;
-        carry += tot;
-    }
-    if (threadIdx.x == 0 && d_total) *d_total = carry;
-}
-
-template <typename T>
-__global__ void __launch_bounds__(kScanThreads) k_scan_apply(const T* __restrict__ in, int64_t n, const uint32_t* __restrict__ sums,
-                                                             uint32_t* __restrict__ out) {
-    // thread t owns kScanItems CONSECUTIVE entries, so the block scan of per-thread sums gives the order
-    const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
-    uint32_t v[kScanItems];
-    uint32_t s = 0;
-#pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
-        const int64_t i = base + k;
-        v[k] = (i < n) ? load_as_u32(in, i) : 0u;
-        s += v[k];
-    }
-    uint32_t tot;
-    uint32_t ex = block_exclusive_scan(s, &tot) + sums[blockIdx.x];
-#pragma unroll
-    for (int k = 0; k < kScanItems; ++k) {
-        const int64_t i = base + k;
-        if (i < n) out[i] = ex;
-        ex += v[k];
-    }
-}
-
-template <typename T>
-static int scan_impl(bh_ctx* c, const T* in, uint32_t* out, int64_t n, uint32_t* d_total, cudaStream_t s) {
-    const int64_t tiles = div_up(n, kScanTile);
-    if (tiles > c->scan_sum_cap) return BH_ERR_WORKSPACE;
-    BH_LAUNCH(c, k_scan_reduce<T>, (unsigned)tiles, kScanThreads, 0, s, in, n, c->ws.scan_sums);
-    BH_LAUNCH(c, k_scan_sums, 1, kScanThreads, 0, s, c->ws.scan_sums, tiles, d_total);
-    BH_LAUNCH(c, k_scan_apply<T>, (unsigned)tiles, kScanThreads, 0, s, in, n, c->ws.scan_sums, out);
-    return BH_OK;
-}
-int scan_u32(bh_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, uint32_t* d_total, cudaStream_t s) {
-    return scan_impl<uint32_t>(c, in, out, n, d_total, s);
-}
-int scan_u8(bh_ctx* c, const uint8_t* in, uint32_t* out, int64_t n, uint32_t* d_total, cudaStream_t s) {
-    return scan_impl<uint8_t>(c, in, out, n, d_total, s);
 }
 
 // ------------------------------------------------------------------------------------------ S2

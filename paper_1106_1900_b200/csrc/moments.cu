@@ -1,48 +1,129 @@
 // moments.cu -- S6: monopole + quadrupole moments and tight boxes, bottom-up, in binary64 with a fixed operation
-// order ("performed in double precision ... converted back to single precision"; Fig.4), then the
-// fp32 walk record with the opening radius of Eq.1.
+// order ("performed in double precision ... converted back to single precision"; Fig.4), and the
+// fp32 walk / evaluation records with the opening radius of Eq.1.
 // Every fp64 operation is an explicit round-to-nearest intrinsic so that no multiply-add is ever fused: the fp32
 // roundings of these values feed the MAC, and a one-ulp difference would flip an opening decision somewhere.
+//
+// The paper goes level by level, one launch per level (~20 dependent launches, nearly all tiny).  Here ONE launch:
+//   * a block owns a contiguous range of P particles and with it every cell that lies entirely inside the range.  It
+//     computes its leaves (one thread each, particles in ascending order) and then its nodes level by level from the
+//     deepest one, separated by __syncthreads only: a node's children lie inside the same range.  A node is computed by
+//     EIGHT LANES, one child each: the lanes load their child at once, and the sums run over the children in ascending
+//     order through shuffles -- the same sequence of roundings as a sequential loop (bit-identical);
+//   * the cells that straddle a range boundary (at most one per level and block) are left to the block that finishes
+//     last, which computes them level by level in the same way: their children are either owned cells (all published
+//     by then: read from L2) or straddling cells of the level below, which that block keeps in shared memory -- the
+//     dependent chain over the levels of the tree never leaves the SM.
+// No thread ever waits for another block.  Cells of the same level are numbered in ascending first particle, so the
+// owned cells of a block are one index range per level, read off the per-tile scans of tree.cu.
+// The fp32 records (what the walk tests and what the force loop consumes) are written in the same pass when the caller
+// knows theta (bh_leapfrog_step, or the theta of the last bh_compute_forces as a hint); k_cell_record writes them alone
+// when theta changes on an existing tree.
 #include <algorithm>
+#include <cstdio>
 #include "bh_internal.cuh"
+
+#ifdef BH_TIMELINE
+// working aid (-DBH_TIMELINE builds only): %globaltimer stamps of this file's kernel, read back by bh_debug_moments
+__device__ unsigned long long g_bh_dbg[1024];
+extern "C" int bh_debug_moments(unsigned long long* host1024) { return (int)cudaMemcpyFromSymbol(host1024, g_bh_dbg, sizeof(unsigned long long) * 1024); }
+#endif
 
 namespace bh {
 
 struct Mom {
-    double M, S[3], com[3], Q[6];
+    double M, com[3], Q[6];
     float bmin[3], bmax[3];
 };
 
-__device__ __forceinline__ void mom_store(const Mom& m, double* __restrict__ mom64, float* __restrict__ box, uint32_t c) {
-    double* o = mom64 + 10 * (size_t)c;
-    o[0] = m.M; o[1] = m.com[0]; o[2] = m.com[1]; o[3] = m.com[2];
-#pragma unroll
-    for (int k = 0; k < 6; ++k) o[4 + k] = m.Q[k];
-    float* b = box + 6 * (size_t)c;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) { b[k] = m.bmin[k]; b[3 + k] = m.bmax[k]; }
+struct RecOut {
+    float4* trec;
+    uint2* tlink;
+    float4* erec;
+    float theta;
+    int mac_kind;
+    int enabled;
+};
+
+// fp32 records of one cell: trec = (com, r2open), tlink = (first child | first particle, count | leaf << 31),
+// erec (48 B) = (com, M) (Qm_xx, Qm_yy, Qm_zz, Qm_xy) (Qm_xz, Qm_yz, -T/2, -3T/2), Qm = -3 Q, T = trace Q;
+// Eq.1: l = longest side of the tight box (A14), delta = |com - box centre|, r2open = (l / theta + delta)^2; the
+// minimum-distance MAC (A28): r2open = (l / theta)^2.  All in single fp32 operations (O8).
+struct Rec { float4 t; uint2 link; float4 e0, e1, e2; };
+__device__ __forceinline__ Rec make_record(const Mom& m, float theta, int mac_kind, uint32_t pb, uint32_t pe, uint32_t cb, uint32_t ce) {
+    Rec r;
+    const float M = (float)m.M;
+    const float cx = (float)m.com[0], cy = (float)m.com[1], cz = (float)m.com[2];
+    float l = fmaxf(fmaxf(__fsub_rn(m.bmax[0], m.bmin[0]), __fsub_rn(m.bmax[1], m.bmin[1])), __fsub_rn(m.bmax[2], m.bmin[2]));
+    l = fmaxf(l, 0.0f);
+    const float ux = __fsub_rn(cx, __fmul_rn(0.5f, __fadd_rn(m.bmin[0], m.bmax[0])));
+    const float uy = __fsub_rn(cy, __fmul_rn(0.5f, __fadd_rn(m.bmin[1], m.bmax[1])));
+    const float uz = __fsub_rn(cz, __fmul_rn(0.5f, __fadd_rn(m.bmin[2], m.bmax[2])));
+    const float s2 = __fadd_rn(__fadd_rn(__fmul_rn(ux, ux), __fmul_rn(uy, uy)), __fmul_rn(uz, uz));
+    const float delta = __fsqrt_rn(s2);
+    const float ropen = mac_kind == 1 ? __fdiv_rn(l, theta) : __fadd_rn(__fdiv_rn(l, theta), delta);   // A28 / Eq.1
+    const float r2open = __fmul_rn(ropen, ropen);
+    const bool leaf = (ce == cb);
+    r.link.x = leaf ? pb : cb;
+    r.link.y = leaf ? ((pe - pb) | 0x80000000u) : (ce - cb);
+    const float qxx = (float)m.Q[0], qyy = (float)m.Q[1], qzz = (float)m.Q[2], qxy = (float)m.Q[3], qxz = (float)m.Q[4], qyz = (float)m.Q[5];
+    const float T = __fadd_rn(__fadd_rn(qxx, qyy), qzz);
+    r.t = make_float4(cx, cy, cz, r2open);
+    r.e0 = make_float4(cx, cy, cz, M);
+    r.e1 = make_float4(__fmul_rn(-3.0f, qxx), __fmul_rn(-3.0f, qyy), __fmul_rn(-3.0f, qzz), __fmul_rn(-3.0f, qxy));
+    r.e2 = make_float4(__fmul_rn(-3.0f, qxz), __fmul_rn(-3.0f, qyz), __fmul_rn(-0.5f, T), __fmul_rn(-1.5f, T));
+    return r;
+}
+
+__device__ __forceinline__ void mom_store(const Mom& m, double* mom64, float* box, uint32_t c) {
+    double2* o = reinterpret_cast<double2*>(mom64 + 10 * (size_t)c);
+    o[0] = make_double2(m.M, m.com[0]);
+    o[1] = make_double2(m.com[1], m.com[2]);
+    o[2] = make_double2(m.Q[0], m.Q[1]);
+    o[3] = make_double2(m.Q[2], m.Q[3]);
+    o[4] = make_double2(m.Q[4], m.Q[5]);
+    float2* b = reinterpret_cast<float2*>(box + 6 * (size_t)c);
+    b[0] = make_float2(m.bmin[0], m.bmin[1]);
+    b[1] = make_float2(m.bmin[2], m.bmax[0]);
+    b[2] = make_float2(m.bmax[1], m.bmax[2]);
+}
+
+__device__ __forceinline__ void rec_store(const Rec& r, const RecOut& o, uint32_t c) {
+    o.trec[c] = r.t;
+    o.tlink[c] = r.link;
+    o.erec[3 * (size_t)c] = r.e0;
+    o.erec[3 * (size_t)c + 1] = r.e1;
+    o.erec[3 * (size_t)c + 2] = r.e2;
 }
 
 // Leaf: M = sum m; S = sum m x; com = S / M; Q_jk = sum (m r_j) r_k, r = x - com; particles in ascending order.
 __device__ __forceinline__ void leaf_moments(Mom& m, const float4* __restrict__ pos, uint32_t b, uint32_t e) {
+    double S[3] = {0.0, 0.0, 0.0};
     m.M = 0.0;
 #pragma unroll
-    for (int k = 0; k < 3; ++k) { m.S[k] = 0.0; m.bmin[k] = INFINITY; m.bmax[k] = -INFINITY; }
+    for (int k = 0; k < 3; ++k) { m.bmin[k] = INFINITY; m.bmax[k] = -INFINITY; }
 #pragma unroll
     for (int k = 0; k < 6; ++k) m.Q[k] = 0.0;
-    for (uint32_t i = b; i < e; ++i) {
-        const float4 p = __ldg(pos + i);
-        const double w = (double)p.w;
-        m.M = __dadd_rn(m.M, w);
-        m.S[0] = __dadd_rn(m.S[0], __dmul_rn(w, (double)p.x));
-        m.S[1] = __dadd_rn(m.S[1], __dmul_rn(w, (double)p.y));
-        m.S[2] = __dadd_rn(m.S[2], __dmul_rn(w, (double)p.z));
-        m.bmin[0] = fminf(m.bmin[0], p.x); m.bmax[0] = fmaxf(m.bmax[0], p.x);
-        m.bmin[1] = fminf(m.bmin[1], p.y); m.bmax[1] = fmaxf(m.bmax[1], p.y);
-        m.bmin[2] = fminf(m.bmin[2], p.z); m.bmax[2] = fmaxf(m.bmax[2], p.z);
+    for (uint32_t i0 = b; i0 < e; i0 += 4) {                  // four loads in flight; the sums stay in ascending particle order
+        float4 q[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) q[u] = __ldg(pos + min(i0 + u, e - 1));
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (i0 + u >= e) break;
+            const float4 p = q[u];
+            const double w = (double)p.w;
+            m.M = __dadd_rn(m.M, w);
+            S[0] = __dadd_rn(S[0], __dmul_rn(w, (double)p.x));
+            S[1] = __dadd_rn(S[1], __dmul_rn(w, (double)p.y));
+            S[2] = __dadd_rn(S[2], __dmul_rn(w, (double)p.z));
+            m.bmin[0] = fminf(m.bmin[0], p.x); m.bmax[0] = fmaxf(m.bmax[0], p.x);
+            m.bmin[1] = fminf(m.bmin[1], p.y); m.bmax[1] = fmaxf(m.bmax[1], p.y);
+            m.bmin[2] = fminf(m.bmin[2], p.z); m.bmax[2] = fmaxf(m.bmax[2], p.z);
+        }
     }
 #pragma unroll
-    for (int k = 0; k < 3; ++k) m.com[k] = __ddiv_rn(m.S[k], m.M);
+    for (int k = 0; k < 3; ++k) m.com[k] = __ddiv_rn(S[k], m.M);
     for (uint32_t i = b; i < e; ++i) {
         const float4 p = __ldg(pos + i);
         const double w = (double)p.w;
@@ -59,127 +140,342 @@ __device__ __forceinline__ void leaf_moments(Mom& m, const float4* __restrict__ 
     }
 }
 
+#ifdef BH_TIMELINE
+#define TLM() do { if (tid == 0 && ntl < 48) tl[ntl++] = global_ns(); } while (0)
+#else
+#define TLM() do {} while (0)
+#endif
+
+// What a parent reads of a child.
+struct Child {
+    double M, c[3], Q[6];
+    float bn[3], bx[3];
+};
+__device__ __forceinline__ void child_clear(Child& ch) {
+    ch.M = 0.0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { ch.c[k] = 0.0; ch.bn[k] = INFINITY; ch.bx[k] = -INFINITY; }
+#pragma unroll
+    for (int k = 0; k < 6; ++k) ch.Q[k] = 0.0;
+}
+// from the cell arrays, written earlier in this launch or the one before (possibly by another block): read from L2 (ld.global.cg)
+__device__ __forceinline__ void child_load_global(Child& ch, const double* mom64, const float* box, uint32_t c) {
+    const double2* mc = reinterpret_cast<const double2*>(mom64 + 10 * (size_t)c);
+    const float2* bc = reinterpret_cast<const float2*>(box + 6 * (size_t)c);
+    const double2 a0 = __ldcg(mc), a1 = __ldcg(mc + 1), a2 = __ldcg(mc + 2), a3 = __ldcg(mc + 3), a4 = __ldcg(mc + 4);
+    const float2 b0 = __ldcg(bc), b1 = __ldcg(bc + 1), b2 = __ldcg(bc + 2);
+    ch.M = a0.x; ch.c[0] = a0.y; ch.c[1] = a1.x; ch.c[2] = a1.y;
+    ch.Q[0] = a2.x; ch.Q[1] = a2.y; ch.Q[2] = a3.x; ch.Q[3] = a3.y; ch.Q[4] = a4.x; ch.Q[5] = a4.y;
+    ch.bn[0] = b0.x; ch.bn[1] = b0.y; ch.bn[2] = b1.x; ch.bx[0] = b1.y; ch.bx[1] = b2.x; ch.bx[2] = b2.y;
+}
+// the shared-memory copy of a straddling node (k_moments_span): 10 doubles, 6 floats
+struct __align__(16) SpanCell { double m[10]; float b[6]; float pad[2]; };
+__device__ __forceinline__ void child_load_shared(Child& ch, const SpanCell& sc) {
+    ch.M = sc.m[0]; ch.c[0] = sc.m[1]; ch.c[1] = sc.m[2]; ch.c[2] = sc.m[3];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) ch.Q[k] = sc.m[4 + k];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { ch.bn[k] = sc.b[k]; ch.bx[k] = sc.b[3 + k]; }
+}
+
+// Scratch of one lane group (eight lanes = one node): the children's terms, transposed through shared memory so that lane q
+// sums quantity q over the children in ascending order.
+struct NodeScratch { double a[8][4]; double q[8][6]; double p[8][6]; };     // (M, M cx, M cy, M cz), Q_c, (M d_j) d_k
+
 // Node: M = sum M_c; S = sum M_c com_c; com = S / M; Q_jk = sum_c ((Q + Q_c,jk) + (M_c d_j) d_k), d = com_c - com; children
-// in ascending order.  The children were written by other threads of this launch: read them from L2 (ld.global.cg).
-__device__ __forceinline__ void node_moments(Mom& m, const double* mom64, const float* box, uint32_t cb, uint32_t ce) {
-    m.M = 0.0;
+// in ascending order -- the same sequence of roundings as a sequential loop over the children.  Eight consecutive lanes
+// (sub = 0..7) hold one child each in `ch` (cleared where sub >= nch; nch = 0: the lane group has no node).  Products are
+// formed by the child's lane (one rounding each); the sums run in lane q < 4 (M, S) and lane q < 6 (Q) over scratch rows
+// 0..nch-1.  On return every lane holds the whole result in `m`.
+__device__ __forceinline__ void node_moments8(Mom& m, const Child& ch, int nch, int sub, NodeScratch& sx) {
+    float bn[3], bx[3];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) { m.S[k] = 0.0; m.bmin[k] = INFINITY; m.bmax[k] = -INFINITY; }
+    for (int k = 0; k < 3; ++k) { bn[k] = ch.bn[k]; bx[k] = ch.bx[k]; }
 #pragma unroll
-    for (int k = 0; k < 6; ++k) m.Q[k] = 0.0;
-    for (uint32_t k2 = cb; k2 < ce; ++k2) {
-        const double* mc = mom64 + 10 * (size_t)k2;
-        const float* bc = box + 6 * (size_t)k2;
-        const double Mc = __ldcg(mc);
-        m.M = __dadd_rn(m.M, Mc);
+    for (int o = 4; o > 0; o >>= 1)          // box: min / max are exact in any order
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            m.S[k] = __dadd_rn(m.S[k], __dmul_rn(Mc, __ldcg(mc + 1 + k)));
-            m.bmin[k] = fminf(m.bmin[k], __ldcg(bc + k));
-            m.bmax[k] = fmaxf(m.bmax[k], __ldcg(bc + 3 + k));
+            bn[k] = fminf(bn[k], __shfl_xor_sync(0xFFFFFFFFu, bn[k], o, 8));
+            bx[k] = fmaxf(bx[k], __shfl_xor_sync(0xFFFFFFFFu, bx[k], o, 8));
         }
-    }
 #pragma unroll
-    for (int k = 0; k < 3; ++k) m.com[k] = __ddiv_rn(m.S[k], m.M);
-    for (uint32_t k2 = cb; k2 < ce; ++k2) {
-        const double* mc = mom64 + 10 * (size_t)k2;
-        const double Mc = __ldcg(mc);
-        const double dx = __dsub_rn(__ldcg(mc + 1), m.com[0]);
-        const double dy = __dsub_rn(__ldcg(mc + 2), m.com[1]);
-        const double dz = __dsub_rn(__ldcg(mc + 3), m.com[2]);
-        const double tx = __dmul_rn(Mc, dx), ty = __dmul_rn(Mc, dy), tz = __dmul_rn(Mc, dz);
-        m.Q[0] = __dadd_rn(__dadd_rn(m.Q[0], __ldcg(mc + 4)), __dmul_rn(tx, dx));
-        m.Q[1] = __dadd_rn(__dadd_rn(m.Q[1], __ldcg(mc + 5)), __dmul_rn(ty, dy));
-        m.Q[2] = __dadd_rn(__dadd_rn(m.Q[2], __ldcg(mc + 6)), __dmul_rn(tz, dz));
-        m.Q[3] = __dadd_rn(__dadd_rn(m.Q[3], __ldcg(mc + 7)), __dmul_rn(tx, dy));
-        m.Q[4] = __dadd_rn(__dadd_rn(m.Q[4], __ldcg(mc + 8)), __dmul_rn(tx, dz));
-        m.Q[5] = __dadd_rn(__dadd_rn(m.Q[5], __ldcg(mc + 9)), __dmul_rn(ty, dz));
-    }
+    for (int k = 0; k < 3; ++k) { m.bmin[k] = bn[k]; m.bmax[k] = bx[k]; }
+    sx.a[sub][0] = ch.M;
+    sx.a[sub][1] = __dmul_rn(ch.M, ch.c[0]);
+    sx.a[sub][2] = __dmul_rn(ch.M, ch.c[1]);
+    sx.a[sub][3] = __dmul_rn(ch.M, ch.c[2]);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) sx.q[sub][k] = ch.Q[k];
+    __syncwarp();
+    double acc = 0.0;
+    if (sub < 4)
+        for (int k = 0; k < nch; ++k) acc = __dadd_rn(acc, sx.a[k][sub]);
+    const double M = __shfl_sync(0xFFFFFFFFu, acc, 0, 8);
+    double com = 0.0;
+    if (sub >= 1 && sub < 4 && nch > 0) com = __ddiv_rn(acc, M);
+    m.M = M;
+    m.com[0] = __shfl_sync(0xFFFFFFFFu, com, 1, 8);
+    m.com[1] = __shfl_sync(0xFFFFFFFFu, com, 2, 8);
+    m.com[2] = __shfl_sync(0xFFFFFFFFu, com, 3, 8);
+    const double dx = __dsub_rn(ch.c[0], m.com[0]), dy = __dsub_rn(ch.c[1], m.com[1]), dz = __dsub_rn(ch.c[2], m.com[2]);
+    const double tx = __dmul_rn(ch.M, dx), ty = __dmul_rn(ch.M, dy), tz = __dmul_rn(ch.M, dz);
+    sx.p[sub][0] = __dmul_rn(tx, dx); sx.p[sub][1] = __dmul_rn(ty, dy); sx.p[sub][2] = __dmul_rn(tz, dz);
+    sx.p[sub][3] = __dmul_rn(tx, dy); sx.p[sub][4] = __dmul_rn(tx, dz); sx.p[sub][5] = __dmul_rn(ty, dz);
+    __syncwarp();
+    double Q = 0.0;
+    if (sub < 6)
+        for (int k = 0; k < nch; ++k) Q = __dadd_rn(__dadd_rn(Q, sx.q[k][sub]), sx.p[k][sub]);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) m.Q[k] = __shfl_sync(0xFFFFFFFFu, Q, k, 8);
+    __syncwarp();                            // the scratch may be rewritten
 }
 
-// The whole bottom-up pass in ONE launch (the paper goes level by level: one launch per level, ~20
-// dependent launches that are nearly all empty).  A thread computes a leaf, publishes it (store, fence) and counts itself
-// in at the parent (c_arrive, zeroed by k_emit_cells); whoever arrives last at a node finds all of its children
-// published, computes the node and climbs on.  Nobody waits, so the launch cannot deadlock; every node is still computed
-// from its children in ascending order, so the values are bit-identical to the level-by-level pass.
-__global__ void __launch_bounds__(128) k_moments(const DevScalars* __restrict__ sc, const float4* __restrict__ pos,
-                                                 const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
-                                                 const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
-                                                 const uint32_t* __restrict__ c_parent, uint32_t* __restrict__ c_arrive,
-                                                 double* mom64, float* box) {
-    const uint32_t nc = sc->n_cells;
-    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
-        if (c_cend[c] != c_cbegin[c]) continue;   // node: computed by its last child
+constexpr int kMomThreads = 1024;
+constexpr int kMomGroups = kMomThreads / 8;      // nodes in flight per block step
+constexpr int kMomMaxBlocks = kMomBlockCap;      // straddling nodes per level (at most one per block)
+constexpr int kSpanThreads = 512;
+constexpr int kSpanGroups = kSpanThreads / 8;
+
+struct SpanShared {
+    NodeScratch sx[kSpanGroups];
+    SpanCell cell[2][kMomMaxBlocks];             // straddling nodes of the level being computed / the level below
+    uint32_t list[kLevels][kMomMaxBlocks];       // the straddling nodes of every level: cell indices, ascending
+    uint4 topo[kLevels][kMomMaxBlocks];          // ... and their topology
+    uint32_t cnt[kLevels + 1];
+};
+
+// The owned nodes [lo, hi) of one level: eight lanes per node, the next node's topology is requested before the current
+// node's children are summed.
+__device__ __forceinline__ void node_pass(uint32_t lo, uint32_t hi, const uint4* __restrict__ topo, double* mom64, float* box, const RecOut& ro,
+                                          NodeScratch* sx) {
+    const int tid = threadIdx.x, grp = tid >> 3, sub = tid & 7;
+    const uint32_t cnt = hi - lo;
+    uint4 tp = make_uint4(0u, 0u, 0u, 0u);
+    if ((uint32_t)grp < cnt) tp = __ldg(topo + lo + grp);
+    for (uint32_t q0 = 0; q0 < cnt; q0 += kMomGroups) {
+        const uint32_t q = q0 + grp;
+        const uint4 t = tp;
+        if (q + kMomGroups < cnt) tp = __ldg(topo + lo + q + kMomGroups);
+        const bool node = q < cnt && t.w != t.z;
+        if (!__any_sync(0xFFFFFFFFu, node)) continue;                 // (warp-uniform) none of this warp's four cells is a node
+        const int nch = node ? (int)(t.w - t.z) : 0;
+        Child ch;
+        child_clear(ch);
+        if (sub < nch) child_load_global(ch, mom64, box, t.z + sub);
         Mom m;
-        leaf_moments(m, pos, c_pbegin[c], c_pend[c]);
-        mom_store(m, mom64, box, c);
-        uint32_t cur = c;
-        for (;;) {
-            const uint32_t par = c_parent[cur];
-            if (par == kNone) break;
-            const uint32_t cb = c_cbegin[par], ce = c_cend[par];
-            __threadfence();                                   // publish `cur` before counting in
-            if (atomicAdd(c_arrive + par, 1u) != ce - cb - 1u) break;
-            c_arrive[par] = 0u;                                // ready for the next pass (bh_refresh_moments runs without k_emit_cells)
-            __threadfence();                                   // all children are published; do not read them early
-            node_moments(m, mom64, box, cb, ce);
-            mom_store(m, mom64, box, par);
-            cur = par;
+        node_moments8(m, ch, nch, sub, sx[grp]);
+        if (node) {
+            const uint32_t c = lo + q;
+            if (sub == 0) mom_store(m, mom64, box, c);
+            if (ro.enabled && sub == 1) rec_store(make_record(m, ro.theta, ro.mac_kind, t.x, t.y, t.z, t.w), ro, c);
         }
     }
 }
 
-// fp32 records per cell: what the walk tests (trec: com, r2open; tlink: first child / particle, count | leaf << 31) and what
-// the force loop consumes (erec, 48 B: (com, M) (Qm_xx, Qm_yy, Qm_zz, Qm_xy) (Qm_xz, Qm_yz, nTh, n3Th)),
-// with the opening radius of Eq.1:  l = longest side of the tight box (A14),
-// delta = |com - box centre|, r2open = (l / theta + delta)^2, all in single fp32 operations (O8).
-__global__ void __launch_bounds__(256) k_cell_record(const DevScalars* __restrict__ sc, float theta, int mac_kind,
-                                                     const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
-                                                     const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
-                                                     const double* __restrict__ mom64, const float* __restrict__ box,
-                                                     float4* __restrict__ trec, uint2* __restrict__ tlink, float4* __restrict__ erec) {
+// Leaves that START inside the block's particle range (a leaf that reaches into the next range is still computed here:
+// it depends on nothing but the particles) and the nodes that lie entirely inside it.
+__global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __restrict__ sc, const float4* __restrict__ pos, int n, int P, int tiles,
+                                                            const uint32_t* __restrict__ tile_base, const uint4* __restrict__ topo,
+                                                            double* mom64, float* box, uint32_t* span, const RecOut ro) {
+    extern __shared__ __align__(16) unsigned char mom_smem[];
+    NodeScratch* sx = reinterpret_cast<NodeScratch*>(mom_smem);
+    __shared__ uint32_t s_lo[kLevels], s_hi[kLevels], s_hin[kLevels], s_pre[kLevels + 1];
+    const int tid = threadIdx.x;
+    const uint32_t b = blockIdx.x, nb = gridDim.x;
+    const int nlev = (int)sc->n_levels;                       // 0: capacity overflow, the tree is empty
+#ifdef BH_TIMELINE
+    unsigned long long tl[48]; int ntl = 0;
+#endif
+    TLM();
+    // ---- the cells that start inside this block's particle range [b P, (b + 1) P): one index range per level
+    if (tid < kLevels) {
+        const int L = tid;
+        uint32_t lo = 0, hi = 0, hin = 0, sp = kNone;
+        if (L < nlev) {
+            const uint32_t off = sc->level_offset[L];
+            const int64_t tb0 = (int64_t)b * P / kTreeTile, tb1 = (int64_t)(b + 1) * P / kTreeTile;
+            lo = off + tile_base[(size_t)L * tiles + tb0];
+            hi = tb1 < tiles ? off + tile_base[(size_t)L * tiles + tb1] : sc->level_offset[L + 1];
+            hin = hi;
+            if (hi > lo) {
+                const uint4 t = topo[hi - 1];
+                if ((int64_t)t.y > (int64_t)(b + 1) * P && t.w != t.z) { sp = hi - 1; hin = hi - 1; }   // the last one is a node that straddles the boundary
+            }
+        }
+        s_lo[L] = lo; s_hi[L] = hi; s_hin[L] = hin;
+        span[(size_t)L * nb + b] = sp;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t run = 0;
+        for (int L = 0; L < kLevels; ++L) { s_pre[L] = run; run += s_hi[L] - s_lo[L]; }
+        s_pre[kLevels] = run;
+    }
+    __syncthreads();
+    TLM();
+    // ---- leaves: one thread each
+    const uint32_t total = s_pre[kLevels];
+    for (uint32_t f = tid; f < total; f += kMomThreads) {
+        int L = 0;
+#pragma unroll
+        for (int k = 1; k < kLevels; ++k) L += (f >= s_pre[k]) ? 1 : 0;       // s_pre is non-decreasing
+        const uint32_t c = s_lo[L] + (f - s_pre[L]);
+        const uint4 t = __ldg(topo + c);
+        if (t.w != t.z) continue;
+        Mom m;
+        leaf_moments(m, pos, t.x, t.y);
+        mom_store(m, mom64, box, c);
+        if (ro.enabled) rec_store(make_record(m, ro.theta, ro.mac_kind, t.x, t.y, t.z, t.w), ro, c);
+    }
+    __syncthreads();
+    TLM();
+    // ---- owned nodes, deepest level first
+    for (int L = nlev - 2; L >= 0; --L) {
+        if (s_hin[L] == s_lo[L]) continue;                    // (uniform over the block)
+        node_pass(s_lo[L], s_hin[L], topo, mom64, box, ro, sx);
+        __syncthreads();
+    }
+    TLM();
+#ifdef BH_TIMELINE
+    if (tid == 0 && b == nb / 2) { for (int q = 0; q < ntl; ++q) g_bh_dbg[256 + q] = tl[q]; g_bh_dbg[256 + 127] = ntl; }
+#endif
+}
+
+// The straddling nodes, level by level from the deepest one, by ONE block that keeps them in shared memory: a child that
+// straddles a boundary itself was computed one level ago (shared memory), any other child is a cell of k_moments (L2).
+__global__ void __launch_bounds__(kSpanThreads, 1) k_moments_span(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo,
+                                                                  double* mom64, float* box, const uint32_t* __restrict__ span, uint32_t nb, const RecOut ro) {
+    extern __shared__ __align__(16) unsigned char mom_smem[];
+    SpanShared& sh = *reinterpret_cast<SpanShared*>(mom_smem);
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int nlev = (int)sc->n_levels;
+#ifdef BH_TIMELINE
+    unsigned long long tl[48]; int ntl = 0;
+#endif
+    TLM();
+    const int grp = tid >> 3, sub = tid & 7;
+    // the straddling nodes of every level, in ascending order (= block order), and their topology: warp w takes levels w, w + 16, ...
+    for (int L = tid >> 5; L < nlev; L += kSpanThreads / 32) {
+        uint32_t run = 0;
+        for (uint32_t b0 = 0; b0 < nb; b0 += 32) {
+            uint32_t sp = kNone;
+            if (b0 + lane < nb) sp = __ldg(span + (size_t)L * nb + b0 + lane);
+            const uint32_t bal = __ballot_sync(0xFFFFFFFFu, sp != kNone);
+            if (sp != kNone) {
+                const uint32_t at = run + __popc(bal & ((1u << lane) - 1u));
+                sh.list[L][at] = sp;
+                sh.topo[L][at] = __ldg(topo + sp);
+            }
+            run += __popc(bal);
+        }
+        if (lane == 0) sh.cnt[L] = run;
+    }
+    if (tid == 0) sh.cnt[nlev] = 0;
+    __syncthreads();
+    TLM();
+    for (int L = nlev - 1; L >= 0; --L) {
+        const int cur = L & 1, below = cur ^ 1;
+        const uint32_t cnt = sh.cnt[L], cntb = sh.cnt[L + 1];
+        const uint32_t* listb = sh.list[L + 1 < kLevels ? L + 1 : L];
+        for (uint32_t q0 = 0; q0 < cnt; q0 += kSpanGroups) {
+            const uint32_t q = q0 + grp;
+            if ((q & ~3u) >= cnt) continue;                            // (warp-uniform) no node for this warp's four groups
+            const bool have = q < cnt;
+            uint32_t c = 0;
+            uint4 t = make_uint4(0u, 0u, 0u, 0u);
+            if (have) { c = sh.list[L][q]; t = sh.topo[L][q]; }
+            const int nch = have ? (int)(t.w - t.z) : 0;
+            Child ch;
+            child_clear(ch);
+            if (sub < nch) {
+                const uint32_t cc = t.z + sub;
+                int lo2 = 0, hi2 = (int)cntb;
+                while (lo2 < hi2) {
+                    const int mid = (lo2 + hi2) >> 1;
+                    if (listb[mid] < cc) lo2 = mid + 1; else hi2 = mid;
+                }
+                if (lo2 < (int)cntb && listb[lo2] == cc) child_load_shared(ch, sh.cell[below][lo2]);
+                else child_load_global(ch, mom64, box, cc);
+            }
+            Mom m;
+            node_moments8(m, ch, nch, sub, sh.sx[grp]);
+            if (have) {
+                if (sub == 0) {
+                    mom_store(m, mom64, box, c);
+                    SpanCell& o = sh.cell[cur][q];
+                    o.m[0] = m.M; o.m[1] = m.com[0]; o.m[2] = m.com[1]; o.m[3] = m.com[2];
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) o.m[4 + k] = m.Q[k];
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) { o.b[k] = m.bmin[k]; o.b[3 + k] = m.bmax[k]; }
+                }
+                if (ro.enabled && sub == 1) rec_store(make_record(m, ro.theta, ro.mac_kind, t.x, t.y, t.z, t.w), ro, c);
+            }
+        }
+        __syncthreads();
+        TLM();
+    }
+#ifdef BH_TIMELINE
+    if (tid == 0) { for (int q = 0; q < ntl; ++q) g_bh_dbg[384 + q] = tl[q]; g_bh_dbg[384 + 127] = ntl; }
+#endif
+}
+
+// fp32 records alone (theta or the MAC changed on an existing tree).
+__global__ void __launch_bounds__(256) k_cell_record(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo,
+                                                     const double* __restrict__ mom64, const float* __restrict__ box, const RecOut ro) {
     const uint32_t nc = sc->n_cells;
     for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
-        const double* m = mom64 + 10 * (size_t)c;
-        const float* b = box + 6 * (size_t)c;
-        const float M = (float)m[0];
-        const float cx = (float)m[1], cy = (float)m[2], cz = (float)m[3];
-        float l = fmaxf(fmaxf(__fsub_rn(b[3], b[0]), __fsub_rn(b[4], b[1])), __fsub_rn(b[5], b[2]));
-        l = fmaxf(l, 0.0f);
-        const float ux = __fsub_rn(cx, __fmul_rn(0.5f, __fadd_rn(b[0], b[3])));
-        const float uy = __fsub_rn(cy, __fmul_rn(0.5f, __fadd_rn(b[1], b[4])));
-        const float uz = __fsub_rn(cz, __fmul_rn(0.5f, __fadd_rn(b[2], b[5])));
-        const float s2 = __fadd_rn(__fadd_rn(__fmul_rn(ux, ux), __fmul_rn(uy, uy)), __fmul_rn(uz, uz));
-        const float delta = __fsqrt_rn(s2);
-        const float ropen = mac_kind == 1 ? __fdiv_rn(l, theta) : __fadd_rn(__fdiv_rn(l, theta), delta);   // A28 / Eq.1
-        const float r2open = __fmul_rn(ropen, ropen);
-        const uint32_t cb = c_cbegin[c], ce = c_cend[c];
-        const bool leaf = (ce == cb);
-        uint2 link;
-        link.x = leaf ? c_pbegin[c] : cb;
-        link.y = leaf ? ((c_pend[c] - c_pbegin[c]) | 0x80000000u) : (ce - cb);
-        // evaluation record, pre-scaled once: Qm = -3 Q, nTh = -T/2, n3Th = -3T/2 (T = trace of Q)
-        const float qxx = (float)m[4], qyy = (float)m[5], qzz = (float)m[6], qxy = (float)m[7], qxz = (float)m[8], qyz = (float)m[9];
-        const float T = (qxx + qyy) + qzz;
-        trec[c] = make_float4(cx, cy, cz, r2open);
-        tlink[c] = link;
-        erec[3 * (size_t)c] = make_float4(cx, cy, cz, M);
-        erec[3 * (size_t)c + 1] = make_float4(-3.0f * qxx, -3.0f * qyy, -3.0f * qzz, -3.0f * qxy);
-        erec[3 * (size_t)c + 2] = make_float4(-3.0f * qxz, -3.0f * qyz, -0.5f * T, -1.5f * T);
+        const double* s = mom64 + 10 * (size_t)c;
+        const float* bb = box + 6 * (size_t)c;
+        Mom m;
+        m.M = s[0]; m.com[0] = s[1]; m.com[1] = s[2]; m.com[2] = s[3];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) m.Q[k] = s[4 + k];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { m.bmin[k] = bb[k]; m.bmax[k] = bb[3 + k]; }
+        const uint4 t = topo[c];
+        rec_store(make_record(m, ro.theta, ro.mac_kind, t.x, t.y, t.z, t.w), ro, c);
     }
 }
 
-int stage_moments(bh_ctx* c, cudaStream_t s) {
-    const int grid = (int)std::min<int64_t>(div_up(std::min<int64_t>(c->max_cells, c->n + c->n / 2 + 1), 128), (int64_t)c->sm_count * 16);
-    BH_LAUNCH(c, k_moments, grid, 128, 0, s, c->ws.sc, c->ws.pos[c->cur], c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin,
-              c->ws.c_cend, c->ws.c_parent, c->ws.c_arrive, c->ws.mom64, c->ws.box);
+static RecOut rec_out(bh_ctx* c, float theta, bool enabled) {
+    RecOut ro;
+    ro.trec = c->ws.trec; ro.tlink = c->ws.tlink; ro.erec = c->ws.erec;
+    ro.theta = theta; ro.mac_kind = c->mac_kind; ro.enabled = enabled ? 1 : 0;
+    return ro;
+}
+
+int moments_init(bh_ctx* c) {
+    BH_CUDA(c, cudaFuncSetAttribute(k_moments_span, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SpanShared)));
+    BH_CUDA(c, cudaFuncSetAttribute(k_moments, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(NodeScratch) * kMomGroups)));
+    return BH_OK;
+}
+
+// theta > 0: the fp32 records are written in the same pass (c->rec_theta / rec_mac remember for which criterion).
+int stage_moments(bh_ctx* c, float theta, cudaStream_t s) {
+    const int64_t n = c->n;
+    // particles per block: a multiple of the tree tile; one block per SM (one wave), at most kMomMaxBlocks blocks
+    const int64_t nb_target = std::min<int64_t>(c->sm_count, kMomMaxBlocks);
+    const int64_t P = div_up(div_up(n + 1, nb_target), kTreeTile) * kTreeTile;
+    const int nb = (int)div_up(n + 1, P);
+    const int tiles = (int)div_up(n + 1, kTreeTile);
+    const bool rec = theta > 0.0f;
+    BH_LAUNCH(c, k_moments, nb, kMomThreads, sizeof(NodeScratch) * kMomGroups, s, c->ws.sc, c->ws.pos[c->cur], (int)n, (int)P, tiles, c->ws.tile_cnt, c->ws.c_topo,
+              c->ws.mom64, c->ws.box, c->ws.mom_span, rec_out(c, theta, rec));
+    BH_LAUNCH(c, k_moments_span, 1, kSpanThreads, sizeof(SpanShared), s, c->ws.sc, c->ws.c_topo, c->ws.mom64, c->ws.box,
+              c->ws.mom_span, (uint32_t)nb, rec_out(c, theta, rec));
+    c->rec_valid = rec;
+    c->rec_theta = theta;
+    c->rec_mac = c->mac_kind;
     return BH_OK;
 }
 
 int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s) {
     const int grid = (int)std::min<int64_t>(div_up(c->max_cells, 256), (int64_t)c->sm_count * 16);
-    BH_LAUNCH(c, k_cell_record, grid, 256, 0, s, c->ws.sc, theta, c->mac_kind, c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin, c->ws.c_cend,
-              c->ws.mom64, c->ws.box, c->ws.trec, c->ws.tlink, c->ws.erec);
+    BH_LAUNCH(c, k_cell_record, grid, 256, 0, s, c->ws.sc, c->ws.c_topo, c->ws.mom64, c->ws.box, rec_out(c, theta, true));
+    c->rec_valid = true;
+    c->rec_theta = theta;
+    c->rec_mac = c->mac_kind;
     return BH_OK;
 }
 

@@ -1,193 +1,281 @@
 // tree.cu -- S4 sparse octree (cells + links) and S5 groups.
 // PAPER.md:63-65 (Fig.1-2) defines the tree level by level: mask keys, group equal prefixes of unflagged particles,
-// <= nleaf -> leaf.  That tree is a pure function of the sorted keys, and this file builds the identical arrays in
-// one streaming pass instead of ~20 dependent mask/compact rounds:
-//   cl(i)  = number of leading levels on which key[i-1] and key[i] agree  (XOR + count-leading-zeros),
-//   fl(i)  = cl(i) + 1 = first level at which particle i starts a new run     (fl(0) = fl(n) = 0; identical keys: 21),
+// <= nleaf -> leaf; PAPER.md:75 takes the groups from the tree cells (<= ncrit particles).  Both are pure functions of
+// the sorted keys, and this file builds the identical arrays in TWO launches instead of ~20 dependent mask/compact
+// rounds plus a link kernel:
+//   cl(a, b) = number of leading levels on which two keys agree  (XOR + count-leading-zeros),
+//   fl(i)  = cl(key[i-1], key[i]) + 1 = first level at which particle i starts a new run   (fl(0) = fl(n) = 0),
 //   dep(i) = level of the leaf holding i = min(1 + max_{s in [i-nleaf, i]} cl(key[s], key[s+nleaf]), 20)
-//            (a level-L run through i holds > nleaf particles iff some window of nleaf+1 sorted keys around i agrees on L levels).
+//            (a level-L run through i holds > nleaf particles iff some window of nleaf+1 sorted keys around i agrees on L levels),
+//   glv(i) = 1 + max_{s in [i-ncrit, i]} cl(key[s], key[s+ncrit]) = the highest level at which i's run holds <= ncrit particles.
 // A cell of level L starts at boundary i iff fl(i) <= L <= dep(i) and ends at boundary j iff fl(j) <= L <= dep(j-1).
-// Numbering (level-major, ascending first particle) = exclusive scan of the per-(level, tile) start counts.
+// A group starts at i iff a cell of level glv(i) starts there (glv <= dep: the group is that cell, A12), or -- a leaf that
+// holds more than ncrit particles (level-20 overflow, or nleaf > ncrit) -- iff i is a multiple of ncrit past the leaf's
+// first particle (found by a binary search over the sorted keys).
+// k_bounds computes fl, dep, the group marks and the per-(row, tile) counts of starts (rows: levels 0..20, then groups);
+// the LAST block to finish scans every row over the tiles (no extra launch).  k_emit numbers the cells level-major in
+// ascending first particle (= the exclusive scans) and writes begin / end / first child / child end / parent, the groups,
+// and the tree's scalars.  No atomics touch the topology: the result is deterministic.
 #include <algorithm>
 #include "bh_internal.cuh"
 
 namespace bh {
 
-__device__ __forceinline__ int common_level(uint64_t a, uint64_t b) {
+constexpr int kTreeThreads = 256;                  // a block handles a tile of kTreeTile = 1024 boundaries
+constexpr int kTreeWarps = kTreeThreads / 32;
+constexpr int kTreePer = kTreeTile / kTreeThreads; // 4
+constexpr int kWin = kTreeTile + 2 * kHaloMax;     // keys a tile looks at: [t0 - 64, t0 + 1024 + 64)
+
+// cl for 60-bit keys: (clz - 4) / 3, the division as a multiplication (exact for 0..60)
+__device__ __forceinline__ int common_level_fast(uint64_t a, uint64_t b) {
     const uint64_t x = a ^ b;
     if (x == 0) return kMaxLevel;
-    const int msb = 63 - __clzll((long long)x);
-    return (59 - msb) / 3;
+    return ((__clzll((long long)x) - 4) * 43) >> 7;
 }
 
-// fl, dep and the per-(level, tile) counts of cell starts.  One boundary per thread; boundaries 0..n.
-__global__ void __launch_bounds__(kTreeTile) k_bounds_count(const uint64_t* __restrict__ key, int n, int nleaf, int tiles,
-                                                            uint8_t* __restrict__ fl, uint8_t* __restrict__ dep,
-                                                            uint32_t* __restrict__ tile_cnt) {
-    __shared__ uint64_t skey[kTreeTile + 2 * kHaloMax];
-    __shared__ int8_t sw[kTreeTile + kHaloMax];
-    __shared__ uint32_t scnt[kLevels];
+// max of the int8 table t over [first, last] (inclusive; first > last: -1): bytes up to a word boundary, whole words, bytes
+__device__ __forceinline__ int range_max(const int8_t* t, int first, int last) {
+    int m = -1;
+    int x = first;
+    for (; x <= last && (x & 3); ++x) m = max(m, (int)t[x]);
+    uint32_t wm = 0x80808080u;
+    for (; x + 3 <= last; x += 4) wm = __vmaxs4(wm, *reinterpret_cast<const uint32_t*>(t + x));
+    for (; x <= last; ++x) m = max(m, (int)t[x]);
+    m = max(m, max(max((int)(int8_t)(wm & 0xFF), (int)(int8_t)((wm >> 8) & 0xFF)), max((int)(int8_t)((wm >> 16) & 0xFF), (int)(int8_t)(wm >> 24))));
+    return m;
+}
+
+// Window maxima of four consecutive positions: out[b] = max t[j0 + b - w .. j0 + b], b = 0..3 (w >= 0).
+__device__ __forceinline__ void window_max4(const int8_t* t, int j0, int w, int out[4]) {
+    if (w < 3) {
+#pragma unroll
+        for (int b = 0; b < 4; ++b) out[b] = range_max(t, j0 + b - w, j0 + b);
+        return;
+    }
+    const int common = range_max(t, j0 + 3 - w, j0);                 // shared by all four windows
+    const int l0 = t[j0 - w], l1 = t[j0 + 1 - w], l2 = t[j0 + 2 - w];
+    const int r1 = t[j0 + 1], r2 = t[j0 + 2], r3 = t[j0 + 3];
+    out[0] = max(common, max(l0, max(l1, l2)));
+    out[1] = max(common, max(max(l1, l2), r1));
+    out[2] = max(common, max(l2, max(r1, r2)));
+    out[3] = max(common, max(r1, max(r2, r3)));
+}
+
+__global__ void __launch_bounds__(kTreeThreads) k_bounds(const uint64_t* __restrict__ key, int n, int nleaf, int ncrit, int tiles,
+                                                         uint8_t* __restrict__ fl, uint8_t* __restrict__ dep, uint8_t* __restrict__ gl,
+                                                         uint32_t* tile_cnt, uint32_t* row_total, uint32_t* done) {
+    __shared__ uint64_t skey[kWin];
+    __shared__ __align__(4) int8_t ta[kWin + 8], tb[kWin + 8];   // cl(key[s], key[s + nleaf]) and cl(key[s], key[s + ncrit]), s = g0 + index
+    __shared__ uint32_t scnt[kTreeRows];
+    __shared__ uint32_t s_last;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int t0 = blockIdx.x * kTreeTile;
     const int g0 = t0 - kHaloMax;                       // global index of skey[0]
-    for (int j = threadIdx.x; j < kTreeTile + 2 * kHaloMax; j += kTreeTile) {
+    for (int j = tid; j < kWin; j += kTreeThreads) {
         const int gi = g0 + j;
         skey[j] = (gi >= 0 && gi < n) ? key[gi] : 0ull;
     }
-    if (threadIdx.x < kLevels) scnt[threadIdx.x] = 0;
+    if (tid < kTreeRows) scnt[tid] = 0u;
     __syncthreads();
-    // sw[j] = cl(key[s], key[s+nleaf]) for s = g0 + j (window of nleaf+1 keys), -1 where the window leaves [0, n)
-    for (int j = threadIdx.x; j < kTreeTile + kHaloMax; j += kTreeTile) {
+    for (int j = tid; j < kWin; j += kTreeThreads) {     // -1 where the window leaves [0, n) (or the part of the table a tile needs)
         const int s = g0 + j;
-        int w = -1;
-        if (s >= 0 && s + nleaf < n) w = common_level(skey[j], skey[j + nleaf]);
-        sw[j] = (int8_t)w;
+        int a = -1, b = -1;
+        if (s >= 0 && s + nleaf < n && j + nleaf < kWin) a = common_level_fast(skey[j], skey[j + nleaf]);
+        if (s >= 0 && s + ncrit < n && j + ncrit < kWin) b = common_level_fast(skey[j], skey[j + ncrit]);
+        ta[j] = (int8_t)a;
+        tb[j] = (int8_t)b;
     }
     __syncthreads();
-    const int i = t0 + threadIdx.x;
-    if (i <= n) {
-        const int j = threadIdx.x + kHaloMax;
-        int myfl = 0;
-        if (i > 0 && i < n) myfl = common_level(skey[j - 1], skey[j]) + 1;
-        fl[i] = (uint8_t)myfl;
-        if (i < n) {
-            int m = -1;
-            for (int k = 0; k <= nleaf; ++k) m = max(m, (int)sw[j - k]);
-            const int d = min(m + 1, kMaxLevel);
-            dep[i] = (uint8_t)d;
-            for (int L = myfl; L <= d; ++L) atomicAdd(&scnt[L], 1u);
+    // ---- four consecutive boundaries per thread
+    const int i0 = t0 + kTreePer * tid, j0 = kTreePer * tid + kHaloMax;
+    int wl[4], wc[4];
+    window_max4(ta, j0, nleaf, wl);
+    window_max4(tb, j0, ncrit, wc);
+    uint32_t pfl = 0, pdep = 0, pgl = 0;                 // four bytes each
+#pragma unroll
+    for (int b = 0; b < kTreePer; ++b) {
+        const int i = i0 + b, j = j0 + b;
+        int myfl = 0, d = 0, glev = 0xFF;
+        if (i <= n) {
+            if (i > 0 && i < n) myfl = common_level_fast(skey[j - 1], skey[j]) + 1;
+            if (i < n) {
+                d = min(wl[b] + 1, kMaxLevel);
+                const int gv = wc[b] + 1;
+                bool gstart;
+                int gcell_level = gv;
+                if (gv <= d) {
+                    gstart = myfl <= gv;                                     // the group is the level-gv cell, which starts here
+                } else {                                                      // a leaf with more than ncrit particles: chunks of ncrit
+                    gcell_level = d;
+                    const int sh = 60 - 3 * d;
+                    const uint64_t target = (skey[j] >> sh) << sh;            // smallest key of the leaf's key range
+                    int lo = 0, hi = i;                                       // first particle of the leaf = lower_bound(target)
+                    while (lo < hi) {
+                        const int mid = (lo + hi) >> 1;
+                        if (__ldg(key + mid) < target) lo = mid + 1; else hi = mid;
+                    }
+                    gstart = ((i - lo) % ncrit) == 0;
+                }
+                if (gstart) { glev = gcell_level; atomicAdd(&scnt[kLevels], 1u); }
+                for (int L = myfl; L <= d; ++L) atomicAdd(&scnt[L], 1u);       // cells that start here (0.24 per particle)
+            }
         }
+        pfl |= (uint32_t)myfl << (8 * b);
+        pdep |= (uint32_t)d << (8 * b);
+        pgl |= (uint32_t)glev << (8 * b);
+    }
+    if (i0 <= n) {                                       // the arrays are padded to whole words
+        *reinterpret_cast<uint32_t*>(fl + i0) = pfl;
+        *reinterpret_cast<uint32_t*>(dep + i0) = pdep;
+        *reinterpret_cast<uint32_t*>(gl + i0) = pgl;
     }
     __syncthreads();
-    if (threadIdx.x < kLevels) tile_cnt[(size_t)threadIdx.x * tiles + blockIdx.x] = scnt[threadIdx.x];
-}
-
-__global__ void k_tree_finalize(const uint32_t* __restrict__ tile_base, int tiles, const uint32_t* __restrict__ d_total,
-                                uint32_t max_cells, DevScalars* sc) {
-    const int t = threadIdx.x;
-    __shared__ uint32_t lo[kLevels + 1];
-    if (t < kLevels) lo[t] = tile_base[(size_t)t * tiles];
-    if (t == kLevels) lo[t] = *d_total;
+    if (tid < kTreeRows) tile_cnt[(size_t)tid * tiles + blockIdx.x] = scnt[tid];
+    // ---- the last block to get here scans every row over the tiles (exclusive, in place) and leaves the row totals
     __syncthreads();
-    // more cells than the workspace holds: report it and publish an EMPTY tree, so that every later stage is a no-op
-    const bool overflow = lo[kLevels] > max_cells;
-    if (t <= kLevels) sc->level_offset[t] = overflow ? 0u : lo[t];
-    if (t == 0) {
-        int nl = 0;
-        for (int L = 0; L < kLevels; ++L) if (lo[L + 1] > lo[L]) nl = L + 1;
-        sc->n_cells = overflow ? 0u : lo[kLevels];
-        sc->n_levels = overflow ? 0u : (uint32_t)nl;
-        if (overflow) atomicMin(&sc->status, (int)BH_ERR_CAPACITY);
+    if (tid == 0) {
+        __threadfence();
+        const uint32_t old = atomicAdd(done, 1u);
+        s_last = (old == (uint32_t)tiles - 1u) ? 1u : 0u;
+        if (s_last) { atomicExch(done, 0u); __threadfence(); }
+    }
+    __syncthreads();
+    if (!s_last) return;
+    for (int r = w; r < kTreeRows; r += kTreeWarps) {    // a warp per row; 32 x 32 entries requested at once
+        uint32_t* row = tile_cnt + (size_t)r * tiles;
+        uint32_t carry = 0;
+        for (int base = 0; base < tiles; base += 1024) {
+            uint32_t x[32];
+#pragma unroll
+            for (int q = 0; q < 32; ++q) {
+                const int t = base + 32 * q + lane;
+                x[q] = t < tiles ? __ldcg(row + t) : 0u;
+            }
+#pragma unroll
+            for (int q = 0; q < 32; ++q) {
+                if (base + 32 * q >= tiles) break;
+                uint32_t inc = x[q];
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+                    if (lane >= o) inc += u;
+                }
+                const int t = base + 32 * q + lane;
+                if (t < tiles) row[t] = carry + inc - x[q];
+                carry += __shfl_sync(0xFFFFFFFFu, inc, 31);
+            }
+        }
+        if (lane == 0) row_total[r] = carry;
     }
 }
 
-// Emit the cell arrays.  S[L] = global index a level-L cell starting at this boundary would get.
-__global__ void __launch_bounds__(kTreeTile) k_emit_cells(const uint8_t* __restrict__ fl, const uint8_t* __restrict__ dep, int n, int tiles,
-                                                          const uint32_t* __restrict__ tile_base, uint32_t max_cells,
-                                                          uint32_t* __restrict__ c_pbegin, uint32_t* __restrict__ c_pend,
-                                                          uint32_t* __restrict__ c_cbegin, uint32_t* __restrict__ c_cend,
-                                                          uint32_t* __restrict__ c_parent, uint32_t* __restrict__ c_arrive) {
-    constexpr int kWarps = kTreeTile / 32;
-    __shared__ uint32_t wc[kLevels][kWarps];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+// Emit the cell arrays and the groups.  A level-L cell that starts at boundary i gets the index
+//   S(L, i) = level_offset[L] + (level-L starts in earlier tiles) + (level-L starts before i in this tile),
+// the last term from one ballot per level and warp.  Starts are sparse (0.24 per particle), so every thread only walks
+// the levels at which a cell really starts or ends at its boundary.
+__global__ void __launch_bounds__(kTreeThreads) k_emit(const uint8_t* __restrict__ fl, const uint8_t* __restrict__ dep, const uint8_t* __restrict__ gl,
+                                                       int n, int tiles, const uint32_t* __restrict__ tile_base, const uint32_t* __restrict__ row_total,
+                                                       uint32_t max_cells, uint4* __restrict__ c_topo, uint32_t* __restrict__ c_parent,
+                                                       uint32_t* __restrict__ g_begin, uint32_t* __restrict__ g_cell, DevScalars* sc) {
+    __shared__ uint32_t bal[kTreeWarps][kTreeRows];      // ballots of the current 256 boundaries: who starts a cell of level L / a group
+    __shared__ uint32_t wpre[kTreeWarps][kTreeRows];     // starts in the earlier warps of this round + everything before (the running base)
+    __shared__ uint32_t base[kTreeRows];
+    __shared__ uint32_t s_overflow;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const uint32_t lt = (1u << lane) - 1u;
-    const int i = blockIdx.x * kTreeTile + threadIdx.x;
-    int myfl = 255, mydep = -1, prevdep = -1;
-    if (i <= n) {
-        myfl = fl[i];
-        if (i < n) mydep = dep[i];
-        if (i > 0) prevdep = dep[i - 1];
-    }
-    uint32_t S[kLevels + 1];
-#pragma unroll
-    for (int L = 0; L < kLevels; ++L) {
-        const bool st = (myfl <= L) && (L <= mydep);
-        const uint32_t b = __ballot_sync(0xFFFFFFFFu, st);
-        S[L] = __popc(b & lt);
-        if (lane == 0) wc[L][w] = __popc(b);
-    }
-    S[kLevels] = 0;
-    __syncthreads();
-    if (threadIdx.x < kLevels) {
-        uint32_t run = tile_base[(size_t)threadIdx.x * tiles + blockIdx.x];
-#pragma unroll
-        for (int ww = 0; ww < kWarps; ++ww) {
-            const uint32_t t = wc[threadIdx.x][ww];
-            wc[threadIdx.x][ww] = run;
+    if (tid == 0) {
+        // level offsets from the row totals (level-major numbering); more cells than the workspace holds: report it and
+        // publish an EMPTY tree, so that every later stage is a no-op
+        uint32_t off[kLevels + 1];
+        uint32_t run = 0;
+        int nl = 0;
+        for (int L = 0; L < kLevels; ++L) {
+            off[L] = run;
+            const uint32_t t = row_total[L];
+            if (t) nl = L + 1;
             run += t;
         }
+        off[kLevels] = run;
+        const bool overflow = run > max_cells;
+        s_overflow = overflow ? 1u : 0u;
+        for (int L = 0; L < kLevels; ++L) base[L] = off[L] + tile_base[(size_t)L * tiles + blockIdx.x];
+        base[kLevels] = tile_base[(size_t)kLevels * tiles + blockIdx.x];       // groups are numbered from 0
+        if (blockIdx.x == 0) {
+            for (int L = 0; L <= kLevels; ++L) sc->level_offset[L] = overflow ? 0u : off[L];
+            sc->n_cells = overflow ? 0u : run;
+            sc->n_levels = overflow ? 0u : (uint32_t)nl;
+            sc->n_groups = overflow ? 0u : row_total[kLevels];
+            if (overflow) atomicMin(&sc->status, (int)BH_ERR_CAPACITY);
+            else g_begin[row_total[kLevels]] = (uint32_t)n;           // sentinel
+        }
     }
     __syncthreads();
+    if (s_overflow) return;
+    auto S = [&](int L) { return wpre[w][L] + (uint32_t)__popc(bal[w][L] & lt); };
+    for (int r = 0; r < kTreePer; ++r) {
+        const int i = blockIdx.x * kTreeTile + r * kTreeThreads + tid;
+        int myfl = 255, mydep = -1, prevdep = -1, mygl = 255;
+        if (i <= n) {
+            myfl = fl[i];
+            if (i < n) { mydep = dep[i]; mygl = gl[i]; }
+            if (i > 0) prevdep = dep[i - 1];
+        }
+        uint32_t mine = 0;
 #pragma unroll
-    for (int L = 0; L < kLevels; ++L) S[L] += wc[L][w];
-    if (i > n) return;
+        for (int L = 0; L < kLevels; ++L) {
+            const uint32_t b = __ballot_sync(0xFFFFFFFFu, (myfl <= L) && (L <= mydep));
+            if (lane == L) mine = b;
+        }
+        {
+            const uint32_t b = __ballot_sync(0xFFFFFFFFu, mygl != 255);
+            if (lane == kLevels) mine = b;
+        }
+        if (lane < kTreeRows) bal[w][lane] = mine;
+        __syncthreads();
+        if (tid < kTreeRows) {
+            uint32_t run = base[tid];
 #pragma unroll
-    for (int L = 0; L < kLevels; ++L) {
-        if (myfl <= L && L <= mydep) {           // a level-L cell starts here
-            const uint32_t c = S[L];
-            if (c < max_cells) {
-                c_pbegin[c] = (uint32_t)i;
-                const bool leaf = (L == mydep);
-                c_cbegin[c] = leaf ? 0u : S[L + 1];
-                if (leaf) c_cend[c] = 0u;
-                uint32_t par = kNone;
-                if (L > 0) par = (myfl <= L - 1) ? S[L - 1] : S[L - 1] - 1u;
-                c_parent[c] = par;
-                c_arrive[c] = 0u;                // children counted in by k_moments
+            for (int ww = 0; ww < kTreeWarps; ++ww) {
+                wpre[ww][tid] = run;
+                run += __popc(bal[ww][tid]);
+            }
+            base[tid] = run;
+        }
+        __syncthreads();
+        if (i <= n) {
+            const int top = max(mydep, prevdep);
+            for (int L = myfl; L <= top; ++L) {
+                const uint32_t sL = S(L);
+                if (L <= mydep) {                        // a level-L cell starts here
+                    uint32_t* t = reinterpret_cast<uint32_t*>(c_topo + sL);      // (first particle, end particle, first child, end child)
+                    t[0] = (uint32_t)i;
+                    const bool leaf = (L == mydep);
+                    t[2] = leaf ? 0u : S(L + 1);
+                    if (leaf) t[3] = 0u;
+                    uint32_t par = kNone;
+                    if (L > 0) par = (myfl <= L - 1) ? S(L - 1) : S(L - 1) - 1u;
+                    c_parent[sL] = par;
+                }
+                if (i > 0 && L <= prevdep) {             // a level-L cell ends here
+                    uint32_t* t = reinterpret_cast<uint32_t*>(c_topo + (sL - 1u));
+                    t[1] = (uint32_t)i;
+                    if (L < prevdep) t[3] = S(L + 1);
+                }
+            }
+            if (mygl != 255) {                           // the group's cell (a chunk of an over-full leaf: that leaf)
+                const uint32_t g = S(kLevels);
+                g_begin[g] = (uint32_t)i;
+                g_cell[g] = (myfl <= mygl) ? S(mygl) : S(mygl) - 1u;
             }
         }
-        if (i > 0 && myfl <= L && L <= prevdep) {   // a level-L cell ends here
-            const uint32_t c = S[L] - 1u;
-            if (c < max_cells) {
-                c_pend[c] = (uint32_t)i;
-                if (L < prevdep) c_cend[c] = S[L + 1];
-            }
-        }
+        __syncthreads();                                 // bal / wpre are rewritten by the next round
     }
-}
-
-// ------------------------------------------------------------------------------------------ S5
-// groups are tree cells with <= ncrit particles; here the highest such cells (A12), in particle order.
-__global__ void __launch_bounds__(256) k_group_mark(const DevScalars* __restrict__ sc, int ncrit,
-                                                    const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
-                                                    const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
-                                                    const uint32_t* __restrict__ c_parent,
-                                                    uint8_t* __restrict__ gflag, uint32_t* __restrict__ gcell_at) {
-    const uint32_t nc = sc->n_cells;
-    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
-        const uint32_t b = c_pbegin[c], cnt = c_pend[c] - b;
-        const uint32_t par = c_parent[c];
-        const bool parent_big = (par == kNone) || (c_pend[par] - c_pbegin[par] > (uint32_t)ncrit);
-        if (!parent_big) continue;
-        if (cnt <= (uint32_t)ncrit) {
-            gflag[b] = 1;
-            gcell_at[b] = c;
-        } else if (c_cend[c] == c_cbegin[c]) {     // overflow leaf at the deepest level: chunks of ncrit
-            for (uint32_t o = 0; o < cnt; o += ncrit) {
-                gflag[b + o] = 1;
-                gcell_at[b + o] = c;
-            }
-        }
-    }
-}
-
-__global__ void __launch_bounds__(256) k_group_write(const uint8_t* __restrict__ gflag, const uint32_t* __restrict__ gscan,
-                                                     const uint32_t* __restrict__ gcell_at, int n,
-                                                     uint32_t* __restrict__ g_begin, uint32_t* __restrict__ g_cell, DevScalars* sc) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n && gflag[i]) {
-        const uint32_t g = gscan[i];
-        g_begin[g] = (uint32_t)i;
-        g_cell[g] = gcell_at[i];
-    }
-    if (i == n) g_begin[sc->n_groups] = (uint32_t)n;   // sentinel; n_groups was written by the scan
 }
 
 // ------------------------------------------------------------------------------------------ export
 __global__ void __launch_bounds__(256) k_export(const DevScalars* __restrict__ sc, const uint64_t* __restrict__ key,
-                                                const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
-                                                const uint32_t* __restrict__ c_cbegin, const uint32_t* __restrict__ c_cend,
-                                                const uint32_t* __restrict__ c_parent, const float4* __restrict__ trec, const double* __restrict__ mom64,
-                                                int32_t* __restrict__ e_level, uint64_t* __restrict__ e_prefix, uint32_t* __restrict__ e_pcount,
+                                                const uint4* __restrict__ c_topo, const uint32_t* __restrict__ c_parent, const float4* __restrict__ trec, const double* __restrict__ mom64,
+                                                int32_t* __restrict__ e_level, uint64_t* __restrict__ e_prefix, uint32_t* __restrict__ e_pbegin, uint32_t* __restrict__ e_pcount,
                                                 int32_t* __restrict__ e_cbegin, int32_t* __restrict__ e_nchild, int32_t* __restrict__ e_parent,
                                                 float* __restrict__ e_mom32, float* __restrict__ e_r2open) {
     const uint32_t nc = sc->n_cells;
@@ -195,16 +283,18 @@ __global__ void __launch_bounds__(256) k_export(const DevScalars* __restrict__ s
         int L = 0;
         while (L < kMaxLevel && c >= sc->level_offset[L + 1]) ++L;
         e_level[c] = L;
-        const uint32_t b = c_pbegin[c];
+        const uint4 t = c_topo[c];
+        const uint32_t b = t.x;
         e_prefix[c] = (L == 0) ? 0ull : (key[b] >> (60 - 3 * L));
-        e_pcount[c] = c_pend[c] - b;
-        const uint32_t cb = c_cbegin[c], ce = c_cend[c];
+        e_pbegin[c] = b;
+        e_pcount[c] = t.y - b;
+        const uint32_t cb = t.z, ce = t.w;
         e_cbegin[c] = (ce == cb) ? -1 : (int32_t)cb;
         e_nchild[c] = (int32_t)(ce - cb);
         e_parent[c] = (c_parent[c] == kNone) ? -1 : (int32_t)c_parent[c];
         float* m = e_mom32 + 10 * (size_t)c;
 #pragma unroll
-        for (int k = 0; k < 10; ++k) m[k] = (float)mom64[10 * (size_t)c + k];   // the fp32 roundings the walk record is built from
+        for (int k = 0; k < 10; ++k) m[k] = (float)mom64[10 * (size_t)c + k];   // the fp32 roundings (the walk's own records: bh_tree_view.cell_trec / cell_erec)
         e_r2open[c] = trec[c].w;
     }
 }
@@ -214,32 +304,18 @@ int stage_cells(bh_ctx* c, cudaStream_t s) {
     const int n = (int)c->n;
     const int tiles = (int)div_up((int64_t)n + 1, kTreeTile);
     const uint64_t* key = c->ws.key[c->sorted];
-    BH_LAUNCH(c, k_bounds_count, tiles, kTreeTile, 0, s, key, n, (int)c->nleaf, tiles, c->ws.fl, c->ws.dep, c->ws.tile_cnt);
-    int rc = scan_u32(c, c->ws.tile_cnt, c->ws.tile_base, (int64_t)kLevels * tiles, &c->ws.sc->n_cells, s);
-    if (rc != BH_OK) return rc;
-    BH_LAUNCH(c, k_tree_finalize, 1, 32, 0, s, c->ws.tile_base, tiles, &c->ws.sc->n_cells, (uint32_t)c->max_cells, c->ws.sc);
-    BH_LAUNCH(c, k_emit_cells, tiles, kTreeTile, 0, s, c->ws.fl, c->ws.dep, n, tiles, c->ws.tile_base, (uint32_t)c->max_cells,
-              c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin, c->ws.c_cend, c->ws.c_parent, c->ws.c_arrive);
-    return BH_OK;
-}
-
-int stage_groups(bh_ctx* c, cudaStream_t s) {
-    const int n = (int)c->n;
-    BH_CUDA(c, cudaMemsetAsync(c->ws.gflag, 0, (size_t)n, s));
-    const int grid = (int)std::min<int64_t>(div_up(c->max_cells, 256), (int64_t)c->sm_count * 16);
-    BH_LAUNCH(c, k_group_mark, grid, 256, 0, s, c->ws.sc, (int)c->ncrit, c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin,
-              c->ws.c_cend, c->ws.c_parent, c->ws.gflag, c->ws.gcell_at);
-    int rc = scan_u8(c, c->ws.gflag, c->ws.gscan, n, &c->ws.sc->n_groups, s);
-    if (rc != BH_OK) return rc;
-    BH_LAUNCH(c, k_group_write, (unsigned)div_up((int64_t)n + 1, 256), 256, 0, s, c->ws.gflag, c->ws.gscan, c->ws.gcell_at, n,
-              c->ws.g_begin, c->ws.g_cell, c->ws.sc);
+    BH_LAUNCH(c, k_bounds, tiles, kTreeThreads, 0, s, key, n, (int)c->nleaf, (int)c->ncrit, tiles, c->ws.fl, c->ws.dep, c->ws.gl, c->ws.tile_cnt,
+              c->ws.row_total, c->ws.tree_done);
+    if (c->timing) cudaEventRecord(c->ev[5], s);
+    BH_LAUNCH(c, k_emit, tiles, kTreeThreads, 0, s, c->ws.fl, c->ws.dep, c->ws.gl, n, tiles, c->ws.tile_cnt, c->ws.row_total, (uint32_t)c->max_cells,
+              c->ws.c_topo, c->ws.c_parent, c->ws.g_begin, c->ws.g_cell, c->ws.sc);
     return BH_OK;
 }
 
 int stage_export(bh_ctx* c, cudaStream_t s) {
     const int grid = (int)std::min<int64_t>(div_up(c->max_cells, 256), (int64_t)c->sm_count * 16);
-    BH_LAUNCH(c, k_export, grid, 256, 0, s, c->ws.sc, c->ws.key[c->sorted], c->ws.c_pbegin, c->ws.c_pend, c->ws.c_cbegin,
-              c->ws.c_cend, c->ws.c_parent, c->ws.trec, c->ws.mom64, c->ws.e_level, c->ws.e_prefix, c->ws.e_pcount, c->ws.e_cbegin,
+    BH_LAUNCH(c, k_export, grid, 256, 0, s, c->ws.sc, c->ws.key[c->sorted], c->ws.c_topo, c->ws.c_parent, c->ws.trec, c->ws.mom64,
+              c->ws.e_level, c->ws.e_prefix, c->ws.e_pbegin, c->ws.e_pcount, c->ws.e_cbegin,
               c->ws.e_nchild, c->ws.e_parent, c->ws.e_mom32, c->ws.e_r2open);
     return BH_OK;
 }

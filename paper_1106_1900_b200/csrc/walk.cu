@@ -292,7 +292,8 @@ constexpr int kPipeListBlocks = 1;    // ... which leaves registers and shared m
 // (~5800 warp instructions per group), so beside the evaluation it starves.  Hence opt-in.
 int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
     if (c->timing) cudaEventRecord(c->ev[8], s);
-    int rc = stage_cell_record(c, theta, s);
+    int rc = BH_OK;
+    if (!(c->rec_valid && c->rec_theta == theta && c->rec_mac == c->mac_kind)) rc = stage_cell_record(c, theta, s);   // else: written by S6
     if (rc != BH_OK) return rc;
     if (c->timing) cudaEventRecord(c->ev[9], s);
     const bool fused_only = c->walk_mode == 1;
@@ -318,7 +319,7 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
             for (int w = 0; w < W; ++w) {
                 if ((rc = stage_walk_lists(c, w, grid_alone, 0u, whole, s)) != BH_OK) return rc;
                 if (W == 1 && c->timing) cudaEventRecord(c->ev[11], s);
-                if ((rc = stage_walk_eval(c, w, eps, 99, s)) != BH_OK) return rc;
+                if ((rc = stage_walk_eval(c, w, eps, 99, true, s)) != BH_OK) return rc;
                 if (W == 1 && c->timing) cudaEventRecord(c->ev[12], s);
             }
             c->walk_split_timed = c->timing && W == 1;
@@ -336,7 +337,7 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
                 // evaluation of wave w
                 cudaStream_t se = (w & 1) ? s2 : s;
                 BH_CUDA(c, cudaStreamWaitEvent(se, c->ev_lists[w], 0));
-                if ((rc = stage_walk_eval(c, w, eps, (w + 1 < W) ? kPipeEvalBlocks : 99, se)) != BH_OK) return rc;
+                if ((rc = stage_walk_eval(c, w, eps, (w + 1 < W) ? kPipeEvalBlocks : 99, false, se)) != BH_OK) return rc;
                 BH_CUDA(c, cudaEventRecord(c->ev_eval[w], se));
             }
             // join: the caller's stream continues after every evaluation (and with them every list walk)

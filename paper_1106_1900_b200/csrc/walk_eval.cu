@@ -267,7 +267,7 @@ __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(co
                                                                const float4* __restrict__ erec, const uint32_t* __restrict__ g_begin,
                                                                const uint32_t* __restrict__ lists, const uint32_t* __restrict__ g_pcoff,
                                                                const uint32_t* __restrict__ g_npc, const uint32_t* __restrict__ g_ppoff,
-                                                               const uint32_t* __restrict__ g_lpp, float eps2, float4* __restrict__ acc_out) {
+                                                               const uint32_t* __restrict__ g_lpp, float eps2, float4* __restrict__ acc_out, int by_class) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     EvalShared* ws = reinterpret_cast<EvalShared*>(smem_raw) + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
@@ -276,15 +276,18 @@ __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(co
     if (threadIdx.x == 0) atomicMin(&ctl->t_start[1][wave], global_ns());
     // three sweeps over the wave's groups with one counter: first the groups with more than 3 times the average work
     // (targets x list entries), then those above 1.5 times, then the rest -- the long groups start early and the kernel
-    // ends on short ones (the order in which groups are evaluated does not touch their sums)
+    // ends on short ones (the order in which groups are evaluated does not touch their sums).  The class of a group must
+    // be the same for every warp that looks at it, so `by_class` is only set when nothing adds to the interaction sums
+    // while this kernel runs (one wave after the other); beside a concurrent list walk (pipelined waves) there is one sweep.
     const uint32_t G = g1 - g0;
+    const uint32_t nsweeps = by_class ? 3u : 1u;
     const unsigned long long total = sc->sum_pc + sc->sum_pp;                 // interactions listed so far (all waves up to this one)
     const unsigned long long mean = total / max(sc->n_groups, 1u);
     for (;;) {
         uint32_t i = 0;
         if (lane == 0) i = atomicAdd(&ctl->eval_next[wave], 1u);
         i = __shfl_sync(0xFFFFFFFFu, i, 0);
-        if (i >= 3u * G) break;
+        if (i >= nsweeps * G) break;
         const uint32_t sweep = i >= 2u * G ? 2u : i >= G ? 1u : 0u;
         const uint32_t g = g0 + (i - sweep * G);
         const uint32_t pcoff = __ldg(g_pcoff + g);
@@ -292,7 +295,7 @@ __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(co
         const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
         const int ng = (int)(ge - gb), npc = (int)__ldg(g_npc + g), npp = (int)__ldg(g_lpp + g);
         const unsigned long long work = (unsigned long long)ng * (unsigned long long)(npc + npp);
-        const uint32_t cls = 2ull * work > 6ull * mean ? 0u : 2ull * work > 3ull * mean ? 1u : 2u;
+        const uint32_t cls = !by_class ? 0u : 2ull * work > 6ull * mean ? 0u : 2ull * work > 3ull * mean ? 1u : 2u;
         if (cls != sweep) continue;            // another sweep's
         const uint32_t* lpc = lists + pcoff;
         const uint32_t* lpp = lists + __ldg(g_ppoff + g);
@@ -313,11 +316,11 @@ int walk_eval_init(bh_ctx* c) {
     return walk_lists_init(c);
 }
 
-int stage_walk_eval(bh_ctx* c, int wave, float eps, int blocks_per_sm, cudaStream_t s) {
+int stage_walk_eval(bh_ctx* c, int wave, float eps, int blocks_per_sm, bool by_class, cudaStream_t s) {
     const size_t smem = sizeof(EvalShared) * kEvalWarps;
     const int grid = c->sm_count * std::min(blocks_per_sm, kEvalBlocksPerSM);
     BH_LAUNCH(c, k_walk_eval, grid, kEvalThreads, smem, s, c->ws.sc, c->ws.ctl, wave, c->ws.pos[c->cur], c->ws.erec, c->ws.g_begin, c->ws.lists,
-              c->ws.g_pcoff, c->ws.g_npc, c->ws.g_ppoff, c->ws.g_lpp, eps * eps, c->ws.acc);
+              c->ws.g_pcoff, c->ws.g_npc, c->ws.g_ppoff, c->ws.g_lpp, eps * eps, c->ws.acc, by_class ? 1 : 0);
     return BH_OK;
 }
 

@@ -75,7 +75,7 @@ template <int kMac>
 __device__ __forceinline__ bool list_group(ListWarpShared* ws, const int lane, const uint32_t g, const uint32_t gb, const uint32_t ge,
                                            const float4* __restrict__ pos, const float4* __restrict__ trec, const uint2* __restrict__ tlink,
                                            const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
-                                           const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
+                                           const uint4* __restrict__ c_topo,
                                            uint32_t* __restrict__ lists, ListArena& ar, WalkListOut o, WalkSums& sums) {
     const uint32_t lt = (1u << lane) - 1u;
     const int ng = (int)(ge - gb);
@@ -84,7 +84,8 @@ __device__ __forceinline__ bool list_group(ListWarpShared* ws, const int lane, c
     float mn[3], mx[3];
     {
         const uint32_t gc = __ldg(g_cell + g);
-        if (__ldg(c_pend + gc) - __ldg(c_pbegin + gc) == (uint32_t)ng) {
+        const uint2 pr = __ldg(reinterpret_cast<const uint2*>(c_topo + gc));     // (first particle, end particle) of the group's cell
+        if (pr.y - pr.x == (uint32_t)ng) {
             const float* b = box + 6 * (size_t)gc;
             mn[0] = __ldg(b); mn[1] = __ldg(b + 1); mn[2] = __ldg(b + 2);
             mx[0] = __ldg(b + 3); mx[1] = __ldg(b + 4); mx[2] = __ldg(b + 5);
@@ -191,10 +192,12 @@ __device__ __forceinline__ bool list_group(ListWarpShared* ws, const int lane, c
 // A chunk of the wave's list region for this warp (bump allocation from a device cursor).  False when the region is used up.
 __device__ __forceinline__ bool alloc_chunk(WalkCtl* ctl, int wave, int lane, uint32_t region_base, uint32_t region_entries,
                                             uint32_t chunk_entries, ListArena& ar) {
-    uint32_t off = 0;
-    if (lane == 0) off = atomicAdd(&ctl->arena_next[wave], chunk_entries);
+    // the cursor saturates: once the region is used up nobody adds to it any more, so it can never wrap around and hand
+    // out a chunk twice however many groups still ask
+    uint32_t off = region_entries;
+    if (lane == 0 && ld_relaxed_u32(&ctl->arena_next[wave]) < region_entries) off = atomicAdd(&ctl->arena_next[wave], chunk_entries);
     off = __shfl_sync(0xFFFFFFFFu, off, 0);
-    if (off > region_entries || region_entries - off < chunk_entries) { ar.pc_top = ar.pp_bot = 0u; return false; }
+    if (off >= region_entries || region_entries - off < chunk_entries) { ar.pc_top = ar.pp_bot = 0u; return false; }
     ar.pc_top = region_base + off;
     ar.pp_bot = ar.pc_top + chunk_entries;
     return true;
@@ -204,7 +207,7 @@ template <int kMac>
 __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, int wave, const float4* __restrict__ pos,
                                                                 const float4* __restrict__ trec, const uint2* __restrict__ tlink,
                                                                 const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
-                                                                const uint32_t* __restrict__ c_pbegin, const uint32_t* __restrict__ c_pend,
+                                                                const uint4* __restrict__ c_topo,
                                                                 const uint32_t* __restrict__ g_begin, uint32_t* __restrict__ lists,
                                                                 uint32_t region_base, uint32_t region_entries, uint32_t chunk_entries,
                                                                 const uint8_t* __restrict__ g_active) {
@@ -242,10 +245,10 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
                 alloc_chunk(o.ctl, wave, lane, region_base, region_entries, chunk_entries, ar);
             }
             const uint32_t before = ar.pp_bot - ar.pc_top;
-            bool ok = before != 0u && list_group<kMac>(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
+            bool ok = before != 0u && list_group<kMac>(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_topo, lists, ar, o, sums);
             if (!ok && !fresh && alloc_chunk(o.ctl, wave, lane, region_base, region_entries, chunk_entries, ar)) {
                 const uint32_t b2 = ar.pp_bot - ar.pc_top;
-                ok = list_group<kMac>(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_pbegin, c_pend, lists, ar, o, sums);
+                ok = list_group<kMac>(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_topo, lists, ar, o, sums);
                 if (ok) last_total = b2 - (ar.pp_bot - ar.pc_top);
             } else if (ok) {
                 last_total = before - (ar.pp_bot - ar.pc_top);
@@ -274,7 +277,6 @@ __global__ void k_walk_prepare(DevScalars* sc, WalkCtl* ctl, const uint32_t* __r
         const unsigned long long target = (unsigned long long)t * wave_particles;
         if (t == nwaves) lo = G;
         else if (t == 0) lo = 0;           // (no search for the common one-wave walk)
-        else if (t == 0) lo = 0;
         else
             while (lo < hi) {
                 const uint32_t mid = (lo + hi) >> 1;
@@ -301,12 +303,12 @@ int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t region_base, uint32
     WalkListOut o = walk_list_out(c);
     if (c->mac_kind == kMacMinDist) {
         BH_LAUNCH(c, k_walk_lists<kMacMinDist>, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
-                  c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries,
+                  c->ws.c_topo, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries,
                   c->active ? c->ws.gflag : nullptr);
         return BH_OK;
     }
     BH_LAUNCH(c, k_walk_lists<kMacEq1>, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
-              c->ws.c_pbegin, c->ws.c_pend, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries,
+              c->ws.c_topo, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries,
                   c->active ? c->ws.gflag : nullptr);
     return BH_OK;
 }
