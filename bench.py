@@ -224,11 +224,18 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     bh.set_stage_timing(True)
 
+    use_graph = not args.no_graph and not sharded
+    if use_graph:
+        bh.step_graph_build(theta, eps, dt)  # bh_leapfrog_step captured once; a timed step is one graph launch
+
     def one_step(ev0=None, ev1=None):
         flush.fill_(1)                       # evict the previous step's working set from L2 (not timed)
         if ev0 is not None:
             ev0.record(stream)
-        bh.leapfrog_step(theta, eps, dt)
+        if use_graph:
+            bh.step_graph_launch()
+        else:
+            bh.leapfrog_step(theta, eps, dt)
         if ev1 is not None:
             ev1.record(stream)
 
@@ -372,6 +379,7 @@ def run_ours(args):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{cfg}: Plummer sphere n={n}" if cfg in ("c1", "c2") else f"{cfg}: n={n}",
                    "theta": theta, "eps": eps, "dt": dt, "nleaf": 16, "ncrit": 64, "mac": "min_distance" if args.mac else "eq1", "rebuild_every_step": True,
+                   "step": "bh_step_graph_launch (bh_leapfrog_step captured into a CUDA graph)" if use_graph else "bh_leapfrog_step",
                    "l2": f"{L2_FLUSH_BYTES >> 20} MiB buffer written between timed steps (outside the event pairs)",
                    "parallelism": "single GPU" if world == 1 else (f"{world} ranks share the walk of one problem: redundant build, one all-reduce of acc_pot per step"
                                                                      if sharded else f"{world} independent replicas (no collective)"),
@@ -416,6 +424,7 @@ def main():
     ap.add_argument("--ref-groups", dest="ref_groups", type=int, default=None)
     ap.add_argument("--no-cpu", dest="no_cpu", action="store_true")
     ap.add_argument("--no-e2e", dest="no_e2e", action="store_true", help="skip the host-buffer leg (for profiling runs)")
+    ap.add_argument("--no-graph", dest="no_graph", action="store_true", help="time plain bh_leapfrog_step launches instead of the captured step")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                      # timing rule: at least 3 warm-up steps

@@ -158,6 +158,16 @@ int bh_set_mac(bh_ctx* ctx, int mac);
 /* S9 around S0-S8 (L105): v += a dt/2; x += v dt; tree_build; compute_forces; v += a dt/2.  Needs valid forces. */
 int bh_leapfrog_step(bh_ctx* ctx, float theta, float eps, float dt, void* stream);
 
+/* The same step as ONE graph launch.  bh_step_graph_build captures bh_leapfrog_step(theta, eps, dt) on `stream` into CUDA
+ * graphs owned by the ctx (nothing runs; the particle arrays ping-pong between two buffer sets, so the step is captured once
+ * for either parity) and bh_step_graph_launch replays the one that matches the current state: the result is that of
+ * bh_leapfrog_step bit for bit, without the per-kernel launch gaps (~12 launches per step).  Needs valid forces, like
+ * bh_leapfrog_step.  The graphs stay valid until bh_set_particles with another n, bh_set_mac or bh_destroy; the list-walk
+ * geometry (waves) is the one chosen at capture.  Stage timing (bh_set_stage_timing) enabled at capture time is recorded
+ * by the replays as well.  Returns BH_ERR_STATE without forces or without a captured step. */
+int bh_step_graph_build(bh_ctx* ctx, float theta, float eps, float dt, void* stream);
+int bh_step_graph_launch(bh_ctx* ctx, void* stream);
+
 /* S9 on its own (L105), the kick-drift form of the same leapfrog: v += a * dt_kick; x += v * dt_drift, with the
  * accelerations of the last bh_compute_forces.  Invalidates tree and forces (the particles moved) -- unless dt_drift is
  * exactly 0: a pure kick leaves positions, tree and forces as they are (x = fmaf(v, 0, x) = x). */

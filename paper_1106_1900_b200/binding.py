@@ -20,7 +20,8 @@ STATUS = {0: "BH_OK", -1: "BH_ERR_INVALID_ARG", -2: "BH_ERR_WORKSPACE", -3: "BH_
 
 # every symbol include/bh.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", "bh_get_particles", "bh_tree_build",
-           "bh_compute_forces", "bh_refresh_moments", "bh_compute_forces_active", "bh_set_mac", "bh_leapfrog_step", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
+           "bh_compute_forces", "bh_refresh_moments", "bh_compute_forces_active", "bh_set_mac", "bh_leapfrog_step", "bh_step_graph_build",
+           "bh_step_graph_launch", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
            "bh_get_stage_ms", "bh_get_walk_timeline", "bh_direct_forces", "bh_last_cuda_error", "bh_status_string"]
 
 
@@ -78,6 +79,10 @@ def load_library():
     lib.bh_set_mac.restype = C.c_int
     lib.bh_leapfrog_step.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_void_p]
     lib.bh_kick_drift.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p]
+    lib.bh_step_graph_build.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_void_p]
+    lib.bh_step_graph_build.restype = C.c_int
+    lib.bh_step_graph_launch.argtypes = [C.c_void_p, C.c_void_p]
+    lib.bh_step_graph_launch.restype = C.c_int
     lib.bh_sync_status.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(BhStats)]
     lib.bh_export_tree.argtypes = [C.c_void_p, C.POINTER(BhTreeView), C.c_void_p]
     lib.bh_set_stage_timing.argtypes = [C.c_void_p, C.c_int]
@@ -215,6 +220,14 @@ class BarnesHut:
 
     def leapfrog_step(self, theta: float, eps: float, dt: float):
         self._check(self.lib.bh_leapfrog_step(self.h, theta, eps, dt, self._stream()), "bh_leapfrog_step")
+
+    def step_graph_build(self, theta: float, eps: float, dt: float):
+        """Capture bh_leapfrog_step(theta, eps, dt) into CUDA graphs owned by the context (nothing runs)."""
+        self._check(self.lib.bh_step_graph_build(self.h, theta, eps, dt, self._stream()), "bh_step_graph_build")
+
+    def step_graph_launch(self):
+        """One captured step: bh_leapfrog_step as a single graph launch."""
+        self._check(self.lib.bh_step_graph_launch(self.h, self._stream()), "bh_step_graph_launch")
 
     def kick_drift(self, dt_kick: float, dt_drift: float):
         self._check(self.lib.bh_kick_drift(self.h, dt_kick, dt_drift, self._stream()), "bh_kick_drift")

@@ -64,8 +64,8 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     o.front_bar = o.front_ctl;
     o.tree_done = o.front_ctl ? o.front_ctl + 2 : nullptr;
     o.mom_done = o.front_ctl ? o.front_ctl + 3 : nullptr;
-    o.front_part = c.take<float>(8 * (size_t)g.sort_tiles);
-    o.front_matrix = c.take<uint32_t>((size_t)kRadix * (size_t)std::min<int64_t>(g.sort_tiles, kFrontTileCap));
+    o.front_part = c.take<float>(8 * (size_t)kFrontTileCap);
+    o.front_matrix = c.take<uint32_t>((size_t)kRadix * (size_t)kFrontTileCap);
     o.fl = c.take<uint8_t>(n + 8);      // (k_bounds stores four boundaries per word: padded)
     o.dep = c.take<uint8_t>(n + 8);
     o.gl = c.take<uint8_t>(n + 8);
@@ -108,6 +108,12 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
 }  // namespace bh
 
 using namespace bh;
+
+static void drop_step_graph(bh_ctx* c) {
+    for (int k = 0; k < 2; ++k)
+        if (c->step_graph[k]) { cudaGraphExecDestroy(c->step_graph[k]); c->step_graph[k] = nullptr; }
+    c->step_graph_valid = false;
+}
 
 // Make `s` wait for the side-stream half of the last bh_set_particles (velocities, ids, zeroed accelerations).
 static int join_copies(bh_ctx* c, cudaStream_t s) {
@@ -175,6 +181,7 @@ int bh_destroy(bh_ctx* c) {
     cudaSetDevice(c->device);
     for (int k = 0; k < 13; ++k)
         if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+    drop_step_graph(c);
     walk_destroy(c);
     delete c;
     return BH_OK;
@@ -184,6 +191,7 @@ int bh_set_particles(bh_ctx* c, int64_t n, const float* pos_mass, const float* v
     if (!c || !pos_mass || n < 1 || n > c->n_max) return BH_ERR_INVALID_ARG;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     BH_CUDA(c, cudaSetDevice(c->device));
+    if (c->step_graph_valid && n != c->n) drop_step_graph(c);   // captured for the old particle count
     c->n = n;
     c->cur = 0;
     c->have_particles = c->have_topology = c->have_tree = c->have_forces = false;
@@ -236,31 +244,31 @@ int bh_tree_build(bh_ctx* c, void* stream) {
     c->have_topology = c->have_tree = c->have_forces = false;
     c->acc_in_order = false;                                  // S3 permutes pos / vel / id; acc_pot follows at the next forces
     int rc;
-    if (c->timing) cudaEventRecord(c->ev[0], s);
+    if (c->timing) stage_mark(c, 0, s);
     if (front_fits(c)) {
         // S0-S3 in one cooperative launch (front.cu); reported as "sort".  While velocities / ids of bh_set_particles are
         // still arriving on the side stream, S3 stays a launch of its own behind the join.
         const bool fuse = !c->copies_pending;
-        if (c->timing) { cudaEventRecord(c->ev[1], s); cudaEventRecord(c->ev[2], s); }
+        if (c->timing) { stage_mark(c, 1, s); stage_mark(c, 2, s); }
         if ((rc = stage_front(c, fuse, s)) != BH_OK) return rc;
-        if (c->timing) cudaEventRecord(c->ev[3], s);
+        if (c->timing) stage_mark(c, 3, s);
         if (!fuse) {
             if ((rc = join_copies(c, s)) != BH_OK) return rc;
             if ((rc = stage_reorder(c, s)) != BH_OK) return rc;
         }
     } else {
         if ((rc = stage_bbox_keys(c, s)) != BH_OK) return rc;      // records ev[1] between bbox and keys
-        if (c->timing) cudaEventRecord(c->ev[2], s);
+        if (c->timing) stage_mark(c, 2, s);
         if ((rc = stage_sort(c, s)) != BH_OK) return rc;
-        if (c->timing) cudaEventRecord(c->ev[3], s);
+        if (c->timing) stage_mark(c, 3, s);
         if ((rc = join_copies(c, s)) != BH_OK) return rc;          // S3 is the first stage that reads velocities and ids
         if ((rc = stage_reorder(c, s)) != BH_OK) return rc;
     }
-    if (c->timing) cudaEventRecord(c->ev[4], s);
+    if (c->timing) stage_mark(c, 4, s);
     if ((rc = stage_cells(c, s)) != BH_OK) return rc;             // S4 + S5; records ev[5] between k_bounds and k_emit
-    if (c->timing) cudaEventRecord(c->ev[6], s);
+    if (c->timing) stage_mark(c, 6, s);
     if ((rc = stage_moments(c, c->theta_last, s)) != BH_OK) return rc;   // S6; with the fp32 records when theta is known
-    if (c->timing) cudaEventRecord(c->ev[7], s);
+    if (c->timing) stage_mark(c, 7, s);
     c->have_topology = c->have_tree = true;
     return BH_OK;
 }
@@ -316,6 +324,55 @@ int bh_leapfrog_step(bh_ctx* c, float theta, float eps, float dt, void* stream) 
     if ((rc = bh_tree_build(c, stream)) != BH_OK) return rc;
     if ((rc = bh_compute_forces(c, theta, eps, stream)) != BH_OK) return rc;
     if ((rc = stage_kick(c, h, s)) != BH_OK) return rc;
+    return BH_OK;
+}
+
+int bh_step_graph_build(bh_ctx* c, float theta, float eps, float dt, void* stream) {
+    if (!c || !std::isfinite(dt) || !(theta > 0.0f) || !std::isfinite(theta) || !(eps >= 0.0f) || !std::isfinite(eps))
+        return BH_ERR_INVALID_ARG;
+    if (!c->have_forces || c->copies_pending) return BH_ERR_STATE;
+    (void)stream;                                             // nothing runs here; the capture uses an internal stream (the legacy
+    cudaStream_t s = c->s_lists;                              // default stream cannot be captured) and the graph is replayed on the caller's
+    BH_CUDA(c, cudaSetDevice(c->device));
+    drop_step_graph(c);
+    // The particle arrays ping-pong (S3 gathers from one set into the other), so a step is captured once for either
+    // parity; capturing only records the launches, nothing runs, and after the second capture the host-side state is back
+    // where it started.
+    const int64_t launches0 = c->launches;
+    int rc = BH_OK;
+    for (int k = 0; k < 2 && rc == BH_OK; ++k) {
+        const int parity = c->cur;
+        cudaGraph_t g = nullptr;
+        BH_CUDA(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeRelaxed));
+        c->capturing = true;
+        rc = bh_leapfrog_step(c, theta, eps, dt, static_cast<void*>(s));
+        c->capturing = false;
+        const cudaError_t e = cudaStreamEndCapture(s, &g);
+        if (rc == BH_OK && e != cudaSuccess) { c->last_cuda = (int)e; rc = BH_ERR_CUDA; }
+        if (rc == BH_OK) {
+            const cudaError_t e2 = cudaGraphInstantiate(&c->step_graph[parity], g, 0);
+            if (e2 != cudaSuccess) { c->last_cuda = (int)e2; rc = BH_ERR_CUDA; }
+        }
+        if (g) cudaGraphDestroy(g);
+    }
+    c->graph_launches = (c->launches - launches0) / 2;
+    c->launches = launches0;
+    if (rc != BH_OK) { (void)cudaGetLastError(); drop_step_graph(c); return rc; }
+    c->graph_theta = theta; c->graph_eps = eps; c->graph_dt = dt;
+    c->step_graph_valid = true;
+    return BH_OK;
+}
+
+int bh_step_graph_launch(bh_ctx* c, void* stream) {
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->step_graph_valid || !c->have_forces || c->copies_pending) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    BH_CUDA(c, cudaGraphLaunch(c->step_graph[c->cur], s));
+    // the host-side bookkeeping of bh_leapfrog_step
+    c->cur ^= 1;
+    c->theta_last = c->graph_theta;
+    c->launches += c->graph_launches;
     return BH_OK;
 }
 
@@ -393,8 +450,10 @@ int bh_export_tree(bh_ctx* c, bh_tree_view* v, void* stream) {
 
 int bh_set_mac(bh_ctx* c, int mac) {
     if (!c || (mac != BH_MAC_EQ1 && mac != BH_MAC_MIN_DISTANCE)) return BH_ERR_INVALID_ARG;
+    if (mac == c->mac_kind) return BH_OK;
     c->mac_kind = mac;
     c->have_forces = false;
+    drop_step_graph(c);
     return BH_OK;
 }
 

@@ -161,6 +161,11 @@ struct bh_ctx {
     float rec_theta;
     int rec_mac;
     bool timing;
+    bool capturing;        // inside bh_step_graph_build
+    cudaGraphExec_t step_graph[2];   // bh_leapfrog_step captured for either parity of the particle ping-pong buffers (api.cu)
+    bool step_graph_valid;
+    float graph_theta, graph_eps, graph_dt;
+    int64_t graph_launches;          // kernels in one captured step
     cudaEvent_t ev[13];     // [0..10] stage boundaries; [11], [12]: after the list walk / the evaluation of a one-wave walk
     bool copies_pending;    // bh_set_particles left copies on s_lists; ev_join marks their end (api.cu: join_copies)
     bool walk_split_timed;  // the last walk was one wave: ev[11], ev[12] are valid
@@ -192,6 +197,13 @@ namespace bh {
     } while (0)
 
 static inline int64_t div_up(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// Stage-boundary event k on stream s.  While the step is being captured into a graph (bh_step_graph_build) the record
+// becomes an external event node, so the stage times of a replayed graph can be read like those of plain launches.
+static inline void stage_mark(bh_ctx* c, int k, cudaStream_t s) {
+    if (c->capturing) cudaEventRecordWithFlags(c->ev[k], s, cudaEventRecordExternal);
+    else cudaEventRecord(c->ev[k], s);
+}
 
 // stage entry points (each only enqueues kernels on `s`)
 int front_init(bh_ctx* c);

@@ -39,6 +39,7 @@ struct FrontArgs {
     float4* vel_out;
     uint32_t* id_out;
     int n;
+    int tile_n;          // keys per tile (block): a multiple of 512, <= kSortTile; the tiles are spread evenly over the SMs
     int fuse_reorder;
     uint64_t* key0;
     uint64_t* key1;
@@ -142,7 +143,8 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const uint32_t tile = blockIdx.x, T = gridDim.x, G = (T + 15u) >> 4;
     const int n = a.n;
-    const int wbase = (int)tile * kSortTile + w * (kFrontItems * 32);   // warp w owns a contiguous run: order = (warp, iteration, lane)
+    const int pw = a.tile_n / kFrontWarps;                                // keys per warp (a multiple of 32)
+    const int wbase = (int)tile * a.tile_n + w * pw;                      // warp w owns a contiguous run: order = (warp, iteration, lane)
     const uint32_t lt = (1u << lane) - 1u;
     uint32_t b0 = 0, nbar = 0;                             // barrier bookkeeping (thread 0)
     if (tid == 0) b0 = ld_acquire_u32(a.bar + 1);
@@ -161,7 +163,7 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
 #pragma unroll
         for (int it = 0; it < kFrontItems; ++it) {
             const int i = wbase + it * 32 + lane;
-            if (i < n) {
+            if (it * 32 < pw && i < n) {
                 const float4 p = a.pos_in[i];
                 bad |= !(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(p.w) && p.w > 0.0f);
                 mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
@@ -258,7 +260,7 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
             const int i = wbase + it * 32 + lane;
             k[it] = 0ull;
             v[it] = (uint32_t)i;
-            if (i < n) {
+            if (it * 32 < pw && i < n) {
                 const float4 p = a.pos_in[i];
                 k[it] = (dilate20f(grid_coordf(p.x, lox, sh, scale)) << 2) | (dilate20f(grid_coordf(p.y, loy, sh, scale)) << 1) | dilate20f(grid_coordf(p.z, loz, sh, scale));
             }
@@ -267,7 +269,7 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
 
     TL();
     // ---------------------------------------------------------------- S2: 8 passes of 8 bits
-    const int cnt_tile = min(kSortTile, n - (int)tile * kSortTile);
+    const int cnt_tile = min(a.tile_n, n - (int)tile * a.tile_n);
 #pragma unroll 1
     for (int pass = 0; pass < kSortPasses; ++pass) {
         const int shift = pass * kRadixBits;
@@ -279,7 +281,7 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
 #pragma unroll
             for (int it = 0; it < kFrontItems; ++it) {
                 const int i = wbase + it * 32 + lane;
-                const bool ok = i < n;
+                const bool ok = it * 32 < pw && i < n;
                 k[it] = ok ? __ldcg(kin + i) : 0ull;
                 v[it] = ok ? __ldcg(vin + i) : 0u;
             }
@@ -290,6 +292,7 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
         uint32_t rank[kFrontItems];
 #pragma unroll
         for (int it = 0; it < kFrontItems; ++it) {
+            if (it * 32 >= pw) { rank[it] = 0u; continue; }                // (warp-uniform)
             const int i = wbase + it * 32 + lane;
             const bool ok = i < n;
             const uint32_t d = (uint32_t)(k[it] >> shift) & (kRadix - 1);
@@ -323,6 +326,7 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
             a.matrix[(size_t)tile * kRadix + tid] = tcount;
             if (tcount) atomicAdd(a.gsum + ((size_t)pass * kFrontGroupCap + (tile >> 4)) * kRadix + tid, tcount);
         }
+        const uint32_t dstart = block_excl_scan512(tcount, wsum);             // first slot of digit d inside the tile, sorted by digit
         TL();
         grid_barrier(a.bar, ++nbar * T, a.sc);
         TL();
@@ -347,7 +351,6 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
         __syncthreads();
         const uint32_t gh = tid < kRadix ? tot2[0][tid] + tot2[1][tid] : 0u;
         const uint32_t dbase = block_excl_scan512(gh, wsum);                  // first output slot of digit d
-        const uint32_t dstart = block_excl_scan512(tcount, wsum);             // first slot of digit d inside the tile, sorted by digit
         if (tid < kRadix) {
             gbase[tid] = dbase + ex2[0][tid] + ex2[1][tid] - dstart;          // output slot = gbase[digit] + slot inside the sorted tile
             lbase[tid] = dstart;
@@ -358,7 +361,7 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
 #pragma unroll
         for (int it = 0; it < kFrontItems; ++it) {
             const int i = wbase + it * 32 + lane;
-            if (i < n) {
+            if (it * 32 < pw && i < n) {
                 const uint32_t dg = (uint32_t)(k[it] >> shift) & (kRadix - 1);
                 const uint32_t lp = lbase[dg] + wcnt[w][dg] + rank[it];
                 skey[lp] = k[it];
@@ -386,7 +389,7 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
 #pragma unroll 2
         for (int it = 0; it < kFrontItems; ++it) {
             const int j = wbase + it * 32 + lane;
-            if (j < n) {
+            if (it * 32 < pw && j < n) {
                 const uint32_t src = __ldcg(a.val1 + j);
                 a.pos_out[j] = a.pos_in[src];
                 a.vel_out[j] = a.vel_in[src];
@@ -412,15 +415,23 @@ int front_init(bh_ctx* c) {
 
 bool front_fits(const bh_ctx* c) { return c->front_enabled && div_up(c->n, kSortTile) <= c->front_max_tiles; }
 
+// Keys per tile: the input spread evenly over every resident block slot (two per SM), in multiples of 512.
+static int front_tile(const bh_ctx* c) {
+    const int64_t t = div_up(div_up(c->n, c->front_max_tiles), 512) * 512;
+    return (int)std::min<int64_t>(std::max<int64_t>(t, 512), kSortTile);
+}
+
 // S0-S2 (and S3 unless velocities / ids are still arriving on the side stream) in one cooperative launch.
 int stage_front(bh_ctx* c, bool fuse_reorder, cudaStream_t s) {
     const int n = (int)c->n;
-    const int tiles = (int)div_up(n, kSortTile);
+    const int tile_n = front_tile(c);
+    const int tiles = (int)div_up(n, tile_n);
     const int a0 = c->cur, b0 = c->cur ^ 1;
     FrontArgs a;
     a.pos_in = c->ws.pos[a0]; a.vel_in = c->ws.vel[a0]; a.id_in = c->ws.idb[a0];
     a.pos_out = c->ws.pos[b0]; a.vel_out = c->ws.vel[b0]; a.id_out = c->ws.idb[b0];
     a.n = n;
+    a.tile_n = tile_n;
     a.fuse_reorder = fuse_reorder ? 1 : 0;
     a.key0 = c->ws.key[0]; a.key1 = c->ws.key[1];
     a.val0 = c->ws.val[0]; a.val1 = c->ws.val[1];

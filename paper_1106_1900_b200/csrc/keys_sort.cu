@@ -324,7 +324,7 @@ int stage_bbox_keys(bh_ctx* c, cudaStream_t s) {
     const int grid = (int)std::min<int64_t>(div_up(n, 256 * 4), (int64_t)c->sm_count * 8);
     BH_LAUNCH(c, k_bbox, grid, 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc);
     BH_LAUNCH(c, k_domain, 1, 32, 0, s, c->ws.sc);
-    if (c->timing) cudaEventRecord(c->ev[1], s);
+    if (c->timing) stage_mark(c, 1, s);
     const int kgrid = (int)std::min<int64_t>(div_up(n, 256), (int64_t)c->sm_count * 8);
     BH_LAUNCH(c, k_keys, kgrid, 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc, c->ws.key[0], c->ws.val[0], c->ws.sort_ghist);
     return BH_OK;

@@ -97,7 +97,9 @@ __device__ __forceinline__ void rec_store(const Rec& r, const RecOut& o, uint32_
 }
 
 // Leaf: M = sum m; S = sum m x; com = S / M; Q_jk = sum (m r_j) r_k, r = x - com; particles in ascending order.
-__device__ __forceinline__ void leaf_moments(Mom& m, const float4* __restrict__ pos, uint32_t b, uint32_t e) {
+// `ld(i)` returns particle i (from the block's shared-memory copy where it has one).
+template <typename Loader>
+__device__ __forceinline__ void leaf_moments(Mom& m, Loader ld, uint32_t b, uint32_t e) {
     double S[3] = {0.0, 0.0, 0.0};
     m.M = 0.0;
 #pragma unroll
@@ -107,7 +109,7 @@ __device__ __forceinline__ void leaf_moments(Mom& m, const float4* __restrict__ 
     for (uint32_t i0 = b; i0 < e; i0 += 4) {                  // four loads in flight; the sums stay in ascending particle order
         float4 q[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) q[u] = __ldg(pos + min(i0 + u, e - 1));
+        for (int u = 0; u < 4; ++u) q[u] = ld(min(i0 + u, e - 1));
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             if (i0 + u >= e) break;
@@ -125,7 +127,7 @@ __device__ __forceinline__ void leaf_moments(Mom& m, const float4* __restrict__ 
 #pragma unroll
     for (int k = 0; k < 3; ++k) m.com[k] = __ddiv_rn(S[k], m.M);
     for (uint32_t i = b; i < e; ++i) {
-        const float4 p = __ldg(pos + i);
+        const float4 p = ld(i);
         const double w = (double)p.w;
         const double rx = __dsub_rn((double)p.x, m.com[0]);
         const double ry = __dsub_rn((double)p.y, m.com[1]);
@@ -232,6 +234,7 @@ __device__ __forceinline__ void node_moments8(Mom& m, const Child& ch, int nch, 
 
 constexpr int kMomThreads = 1024;
 constexpr int kMomGroups = kMomThreads / 8;      // nodes in flight per block step
+constexpr int kMomStage = 8192;                  // particles a block can stage in the shared memory of its node scratch
 constexpr int kMomMaxBlocks = kMomBlockCap;      // straddling nodes per level (at most one per block)
 constexpr int kSpanThreads = 512;
 constexpr int kSpanGroups = kSpanThreads / 8;
@@ -313,6 +316,13 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
     }
     __syncthreads();
     TLM();
+    // ---- the block's particles, once, coalesced, into shared memory (the node scratch is not in use yet) when they fit
+    float4* spos = reinterpret_cast<float4*>(mom_smem);
+    const uint32_t p0 = b * (uint32_t)P;
+    const uint32_t staged = P <= kMomStage ? min((uint32_t)P, (uint32_t)n - min((uint32_t)n, p0)) : 0u;
+    for (uint32_t i = tid; i < staged; i += kMomThreads) spos[i] = __ldg(pos + p0 + i);
+    __syncthreads();
+    auto ld = [&](uint32_t i) -> float4 { return (i - p0 < staged) ? spos[i - p0] : __ldg(pos + i); };
     // ---- leaves: one thread each
     const uint32_t total = s_pre[kLevels];
     for (uint32_t f = tid; f < total; f += kMomThreads) {
@@ -323,7 +333,7 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
         const uint4 t = __ldg(topo + c);
         if (t.w != t.z) continue;
         Mom m;
-        leaf_moments(m, pos, t.x, t.y);
+        leaf_moments(m, ld, t.x, t.y);
         mom_store(m, mom64, box, c);
         if (ro.enabled) rec_store(make_record(m, ro.theta, ro.mac_kind, t.x, t.y, t.z, t.w), ro, c);
     }
@@ -377,16 +387,13 @@ __global__ void __launch_bounds__(kSpanThreads, 1) k_moments_span(const DevScala
         const int cur = L & 1, below = cur ^ 1;
         const uint32_t cnt = sh.cnt[L], cntb = sh.cnt[L + 1];
         const uint32_t* listb = sh.list[L + 1 < kLevels ? L + 1 : L];
-        for (uint32_t q0 = 0; q0 < cnt; q0 += kSpanGroups) {
-            const uint32_t q = q0 + grp;
-            if ((q & ~3u) >= cnt) continue;                            // (warp-uniform) no node for this warp's four groups
-            const bool have = q < cnt;
-            uint32_t c = 0;
-            uint4 t = make_uint4(0u, 0u, 0u, 0u);
-            if (have) { c = sh.list[L][q]; t = sh.topo[L][q]; }
-            const int nch = have ? (int)(t.w - t.z) : 0;
-            Child ch;
+        // the children of round r + 1 are requested before round r is summed
+        auto fetch = [&](uint32_t q, Child& ch, uint4& t) {
             child_clear(ch);
+            t = make_uint4(0u, 0u, 0u, 0u);
+            if (q >= cnt) return;
+            t = sh.topo[L][q];
+            const int nch = (int)(t.w - t.z);
             if (sub < nch) {
                 const uint32_t cc = t.z + sub;
                 int lo2 = 0, hi2 = (int)cntb;
@@ -397,6 +404,19 @@ __global__ void __launch_bounds__(kSpanThreads, 1) k_moments_span(const DevScala
                 if (lo2 < (int)cntb && listb[lo2] == cc) child_load_shared(ch, sh.cell[below][lo2]);
                 else child_load_global(ch, mom64, box, cc);
             }
+        };
+        Child chn;
+        uint4 tn;
+        fetch((uint32_t)grp, chn, tn);
+        for (uint32_t q0 = 0; q0 < cnt; q0 += kSpanGroups) {
+            const uint32_t q = q0 + grp;
+            if ((q & ~3u) >= cnt) break;                               // (warp-uniform) no node left for this warp's four groups
+            const Child ch = chn;
+            const uint4 t = tn;
+            fetch(q + kSpanGroups, chn, tn);
+            const bool have = q < cnt;
+            const int nch = have ? (int)(t.w - t.z) : 0;
+            const uint32_t c = have ? sh.list[L][q] : 0u;
             Mom m;
             node_moments8(m, ch, nch, sub, sh.sx[grp]);
             if (have) {

@@ -61,14 +61,15 @@ __device__ __forceinline__ void window_max4(const int8_t* t, int j0, int w, int 
     out[3] = max(common, max(r1, max(r2, r3)));
 }
 
-__global__ void __launch_bounds__(kTreeThreads) k_bounds(const uint64_t* __restrict__ key, int n, int nleaf, int ncrit, int tiles,
+template <int kNleaf, int kNcrit>      // compile-time leaf / group sizes (0: the run-time arguments)
+__global__ void __launch_bounds__(kTreeThreads) k_bounds(const uint64_t* __restrict__ key, int n, int nleaf_rt, int ncrit_rt, int tiles,
                                                          uint8_t* __restrict__ fl, uint8_t* __restrict__ dep, uint8_t* __restrict__ gl,
-                                                         uint32_t* tile_cnt, uint32_t* row_total, uint32_t* done) {
+                                                         uint32_t* tile_cnt) {
     __shared__ uint64_t skey[kWin];
     __shared__ __align__(4) int8_t ta[kWin + 8], tb[kWin + 8];   // cl(key[s], key[s + nleaf]) and cl(key[s], key[s + ncrit]), s = g0 + index
     __shared__ uint32_t scnt[kTreeRows];
-    __shared__ uint32_t s_last;
-    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int nleaf = kNleaf ? kNleaf : nleaf_rt, ncrit = kNcrit ? kNcrit : ncrit_rt;
+    const int tid = threadIdx.x;
     const int t0 = blockIdx.x * kTreeTile;
     const int g0 = t0 - kHaloMax;                       // global index of skey[0]
     for (int j = tid; j < kWin; j += kTreeThreads) {
@@ -131,39 +132,43 @@ __global__ void __launch_bounds__(kTreeThreads) k_bounds(const uint64_t* __restr
     }
     __syncthreads();
     if (tid < kTreeRows) tile_cnt[(size_t)tid * tiles + blockIdx.x] = scnt[tid];
-    // ---- the last block to get here scans every row over the tiles (exclusive, in place) and leaves the row totals
-    __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        const uint32_t old = atomicAdd(done, 1u);
-        s_last = (old == (uint32_t)tiles - 1u) ? 1u : 0u;
-        if (s_last) { atomicExch(done, 0u); __threadfence(); }
-    }
-    __syncthreads();
-    if (!s_last) return;
-    for (int r = w; r < kTreeRows; r += kTreeWarps) {    // a warp per row; 32 x 32 entries requested at once
+}
+
+// Exclusive scan of every row of tile_cnt over the tiles, in place, and the row totals: one warp (one block, so that every
+// row has an SM's load / store path to itself) per row; a lane scans a contiguous run of the row, all loads in flight at once.
+__global__ void __launch_bounds__(32) k_scan_rows(uint32_t* tile_cnt, uint32_t* row_total, int tiles) {
+    const int lane = threadIdx.x, r = blockIdx.x;
+    {
         uint32_t* row = tile_cnt + (size_t)r * tiles;
         uint32_t carry = 0;
-        for (int base = 0; base < tiles; base += 1024) {
-            uint32_t x[32];
+        for (int base = 0; base < tiles; base += 32 * 40) {
+            const int per = min(40, (min(tiles - base, 32 * 40) + 31) / 32);   // entries per lane in this stretch
+            const int first = base + lane * per;
+            uint32_t x[40];
 #pragma unroll
-            for (int q = 0; q < 32; ++q) {
-                const int t = base + 32 * q + lane;
-                x[q] = t < tiles ? __ldcg(row + t) : 0u;
+            for (int q = 0; q < 40; ++q) {                       // every load is requested before any is used
+                const int t = min(first + q, tiles - 1);
+                x[q] = __ldcg(row + t);
             }
+            uint32_t sum = 0;
 #pragma unroll
-            for (int q = 0; q < 32; ++q) {
-                if (base + 32 * q >= tiles) break;
-                uint32_t inc = x[q];
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, inc, o);
-                    if (lane >= o) inc += u;
-                }
-                const int t = base + 32 * q + lane;
-                if (t < tiles) row[t] = carry + inc - x[q];
-                carry += __shfl_sync(0xFFFFFFFFu, inc, 31);
+            for (int q = 0; q < 40; ++q) {
+                if (!(q < per && first + q < tiles)) x[q] = 0u;
+                sum += x[q];
             }
+            uint32_t inc = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+                if (lane >= o) inc += u;
+            }
+            uint32_t run = carry + inc - sum;
+#pragma unroll
+            for (int q = 0; q < 40; ++q) {
+                if (q < per && first + q < tiles) row[first + q] = run;
+                run += x[q];
+            }
+            carry += __shfl_sync(0xFFFFFFFFu, inc, 31);
         }
         if (lane == 0) row_total[r] = carry;
     }
@@ -183,30 +188,34 @@ __global__ void __launch_bounds__(kTreeThreads) k_emit(const uint8_t* __restrict
     __shared__ uint32_t s_overflow;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const uint32_t lt = (1u << lane) - 1u;
-    if (tid == 0) {
+    if (w == 0) {
         // level offsets from the row totals (level-major numbering); more cells than the workspace holds: report it and
         // publish an EMPTY tree, so that every later stage is a no-op
-        uint32_t off[kLevels + 1];
-        uint32_t run = 0;
-        int nl = 0;
-        for (int L = 0; L < kLevels; ++L) {
-            off[L] = run;
-            const uint32_t t = row_total[L];
-            if (t) nl = L + 1;
-            run += t;
+        const uint32_t tot = lane < kTreeRows ? row_total[lane] : 0u;
+        const uint32_t tb = lane < kTreeRows ? tile_base[(size_t)lane * tiles + blockIdx.x] : 0u;
+        const uint32_t cells = lane < kLevels ? tot : 0u;
+        uint32_t inc = cells;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+            if (lane >= o) inc += u;
         }
-        off[kLevels] = run;
-        const bool overflow = run > max_cells;
-        s_overflow = overflow ? 1u : 0u;
-        for (int L = 0; L < kLevels; ++L) base[L] = off[L] + tile_base[(size_t)L * tiles + blockIdx.x];
-        base[kLevels] = tile_base[(size_t)kLevels * tiles + blockIdx.x];       // groups are numbered from 0
+        const uint32_t off = inc - cells;                              // lane L: first cell of level L; lane kLevels: all cells
+        const uint32_t ncell = __shfl_sync(0xFFFFFFFFu, inc, 31);
+        const uint32_t levels = __ballot_sync(0xFFFFFFFFu, cells != 0u);
+        const uint32_t ngroups = __shfl_sync(0xFFFFFFFFu, tot, kLevels);
+        const bool overflow = ncell > max_cells;
+        if (lane == 0) s_overflow = overflow ? 1u : 0u;
+        if (lane < kTreeRows) base[lane] = (lane < kLevels ? off : 0u) + tb;   // groups are numbered from 0
         if (blockIdx.x == 0) {
-            for (int L = 0; L <= kLevels; ++L) sc->level_offset[L] = overflow ? 0u : off[L];
-            sc->n_cells = overflow ? 0u : run;
-            sc->n_levels = overflow ? 0u : (uint32_t)nl;
-            sc->n_groups = overflow ? 0u : row_total[kLevels];
-            if (overflow) atomicMin(&sc->status, (int)BH_ERR_CAPACITY);
-            else g_begin[row_total[kLevels]] = (uint32_t)n;           // sentinel
+            if (lane <= kLevels) sc->level_offset[lane] = overflow ? 0u : off;
+            if (lane == 0) {
+                sc->n_cells = overflow ? 0u : ncell;
+                sc->n_levels = overflow ? 0u : (uint32_t)(32 - __clz(levels));
+                sc->n_groups = overflow ? 0u : ngroups;
+                if (overflow) atomicMin(&sc->status, (int)BH_ERR_CAPACITY);
+                else g_begin[ngroups] = (uint32_t)n;                   // sentinel
+            }
         }
     }
     __syncthreads();
@@ -304,9 +313,12 @@ int stage_cells(bh_ctx* c, cudaStream_t s) {
     const int n = (int)c->n;
     const int tiles = (int)div_up((int64_t)n + 1, kTreeTile);
     const uint64_t* key = c->ws.key[c->sorted];
-    BH_LAUNCH(c, k_bounds, tiles, kTreeThreads, 0, s, key, n, (int)c->nleaf, (int)c->ncrit, tiles, c->ws.fl, c->ws.dep, c->ws.gl, c->ws.tile_cnt,
-              c->ws.row_total, c->ws.tree_done);
-    if (c->timing) cudaEventRecord(c->ev[5], s);
+    if (c->nleaf == 16 && c->ncrit == 64)
+        BH_LAUNCH(c, (k_bounds<16, 64>), tiles, kTreeThreads, 0, s, key, n, 16, 64, tiles, c->ws.fl, c->ws.dep, c->ws.gl, c->ws.tile_cnt);
+    else
+        BH_LAUNCH(c, (k_bounds<0, 0>), tiles, kTreeThreads, 0, s, key, n, (int)c->nleaf, (int)c->ncrit, tiles, c->ws.fl, c->ws.dep, c->ws.gl, c->ws.tile_cnt);
+    BH_LAUNCH(c, k_scan_rows, kTreeRows, 32, 0, s, c->ws.tile_cnt, c->ws.row_total, tiles);
+    if (c->timing) stage_mark(c, 5, s);
     BH_LAUNCH(c, k_emit, tiles, kTreeThreads, 0, s, c->ws.fl, c->ws.dep, c->ws.gl, n, tiles, c->ws.tile_cnt, c->ws.row_total, (uint32_t)c->max_cells,
               c->ws.c_topo, c->ws.c_parent, c->ws.g_begin, c->ws.g_cell, c->ws.sc);
     return BH_OK;

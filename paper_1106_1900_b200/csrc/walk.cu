@@ -291,11 +291,11 @@ constexpr int kPipeListBlocks = 1;    // ... which leaves registers and shared m
 // 8 list warps per SM take 2.96 ms (8 waves) against 2.38 ms for one wave: the list walk is bound by instruction issue
 // (~5800 warp instructions per group), so beside the evaluation it starves.  Hence opt-in.
 int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
-    if (c->timing) cudaEventRecord(c->ev[8], s);
+    if (c->timing) stage_mark(c, 8, s);
     int rc = BH_OK;
     if (!(c->rec_valid && c->rec_theta == theta && c->rec_mac == c->mac_kind)) rc = stage_cell_record(c, theta, s);   // else: written by S6
     if (rc != BH_OK) return rc;
-    if (c->timing) cudaEventRecord(c->ev[9], s);
+    if (c->timing) stage_mark(c, 9, s);
     const bool fused_only = c->walk_mode == 1;
     c->walk_split_timed = false;
     // ---- waves: each must fit the list buffer (pipelined: half of it) 1.5 times over
@@ -318,9 +318,9 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
             const uint32_t whole = (uint32_t)std::min<int64_t>(c->list_entries, (int64_t)1 << 30);
             for (int w = 0; w < W; ++w) {
                 if ((rc = stage_walk_lists(c, w, grid_alone, 0u, whole, s)) != BH_OK) return rc;
-                if (W == 1 && c->timing) cudaEventRecord(c->ev[11], s);
+                if (W == 1 && c->timing) stage_mark(c, 11, s);
                 if ((rc = stage_walk_eval(c, w, eps, 99, true, s)) != BH_OK) return rc;
-                if (W == 1 && c->timing) cudaEventRecord(c->ev[12], s);
+                if (W == 1 && c->timing) stage_mark(c, 12, s);
             }
             c->walk_split_timed = c->timing && W == 1;
         } else {
@@ -354,7 +354,7 @@ int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s) {
         BH_LAUNCH(c, k_walk_fused<kMacEq1>, c->sm_count * 2, kWalkThreads, smem, s, c->ws.sc, c->ws.ctl, fused_only ? 1 : 0, c->ws.deferred,
                   c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.erec, c->ws.g_begin, eps * eps, c->ws.acc, c->ws.g_npc, c->ws.g_npp,
                   c->active ? c->ws.gflag : nullptr);
-    if (c->timing) cudaEventRecord(c->ev[10], s);
+    if (c->timing) stage_mark(c, 10, s);
     return BH_OK;
 }
 
