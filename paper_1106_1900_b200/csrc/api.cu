@@ -62,8 +62,6 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     o.front_gsum = c.take<uint32_t>((size_t)kSortPasses * kFrontGroupCap * kRadix + 8);
     o.front_ctl = o.front_gsum ? o.front_gsum + (size_t)kSortPasses * kFrontGroupCap * kRadix : nullptr;
     o.front_bar = o.front_ctl;
-    o.tree_done = o.front_ctl ? o.front_ctl + 2 : nullptr;
-    o.mom_done = o.front_ctl ? o.front_ctl + 3 : nullptr;
     o.front_part = c.take<float>(8 * (size_t)kFrontTileCap);
     o.front_matrix = c.take<uint32_t>((size_t)kRadix * (size_t)kFrontTileCap);
     o.fl = c.take<uint8_t>(n + 8);      // (k_bounds stores four boundaries per word: padded)

@@ -99,13 +99,11 @@ struct Ws {
     uint32_t* sort_status; // [kSortPasses][sortTiles][kRadix] look-back words  sort_status: one memset)
     uint32_t* tile_cnt;   // [kTreeRows][treeTiles] starts per tile; after k_bounds: exclusive scan of every row over the tiles
     uint32_t* row_total;  // [kTreeRows] cells per level, groups
-    uint32_t* tree_done;  // [1] blocks of k_bounds that have finished (returns to 0)
     uint32_t* mom_span;   // [kLevels][momentBlocks] cell of each level that straddles the end of a block's particle range (kNone: none)
-    uint32_t* mom_done;   // [1] blocks of k_moments that have finished (returns to 0)
     float* front_part;    // [sortTiles][8] per-tile box of k_front
     uint32_t* front_matrix; // [frontTiles][kRadix] per-tile digit counts of the current pass
     uint32_t* front_gsum;   // [kSortPasses][kFrontGroupCap][kRadix] digit counts per pass and group of 16 tiles (zero between launches)
-    uint32_t* front_ctl;    // control words that are zero between launches: front_bar[2], tree_done, mom_done
+    uint32_t* front_ctl;    // control words that are zero between launches: front_bar[2]
     uint32_t* front_bar;    // [2] grid barrier of k_front: arrivals, generation
     uint4* c_topo;        // [max_cells] (first particle, end particle, first child, end child); children (0, 0) for a leaf
     uint32_t* c_parent;

@@ -21,7 +21,10 @@
 // when theta changes on an existing tree.
 #include <algorithm>
 #include <cstdio>
+#include <cooperative_groups.h>
 #include "bh_internal.cuh"
+
+namespace cg = cooperative_groups;
 
 #ifdef BH_TIMELINE
 // working aid (-DBH_TIMELINE builds only): %globaltimer stamps of this file's kernel, read back by bh_debug_moments
@@ -236,12 +239,14 @@ constexpr int kMomThreads = 1024;
 constexpr int kMomGroups = kMomThreads / 8;      // nodes in flight per block step
 constexpr int kMomStage = 8192;                  // particles a block can stage in the shared memory of its node scratch
 constexpr int kMomMaxBlocks = kMomBlockCap;      // straddling nodes per level (at most one per block)
-constexpr int kSpanThreads = 512;
+constexpr int kSpanCtas = 8;                     // CTAs of the cluster that computes the straddling nodes
+constexpr int kSpanThreads = 256;
 constexpr int kSpanGroups = kSpanThreads / 8;
+constexpr int kSpanSlots = (kMomMaxBlocks + kSpanCtas - 1) / kSpanCtas;
 
 struct SpanShared {
     NodeScratch sx[kSpanGroups];
-    SpanCell cell[2][kMomMaxBlocks];             // straddling nodes of the level being computed / the level below
+    SpanCell cell[2][kSpanSlots];                // this CTA's straddling nodes of the level being computed / the level below
     uint32_t list[kLevels][kMomMaxBlocks];       // the straddling nodes of every level: cell indices, ascending
     uint4 topo[kLevels][kMomMaxBlocks];          // ... and their topology
     uint32_t cnt[kLevels + 1];
@@ -351,12 +356,19 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
 #endif
 }
 
-// The straddling nodes, level by level from the deepest one, by ONE block that keeps them in shared memory: a child that
-// straddles a boundary itself was computed one level ago (shared memory), any other child is a cell of k_moments (L2).
-__global__ void __launch_bounds__(kSpanThreads, 1) k_moments_span(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo,
-                                                                  double* mom64, float* box, const uint32_t* __restrict__ span, uint32_t nb, const RecOut ro) {
+// The straddling nodes, level by level from the deepest one, by ONE THREAD-BLOCK CLUSTER of eight CTAs that keeps them in
+// (distributed) shared memory: node q of a level belongs to CTA q mod 8, which stores the result in its own shared memory
+// (and in the cell arrays); a child that straddles a boundary itself was computed one level ago and is read from the shared
+// memory of the CTA that owns it (DSMEM), any other child is a cell of k_moments (L2).  cluster.sync() separates the
+// levels, so the dependent chain over the levels of the tree never goes through global memory, and the fp64 work of a
+// level is spread over eight SMs.
+__global__ void __cluster_dims__(kSpanCtas, 1, 1) __launch_bounds__(kSpanThreads, 1)
+k_moments_span(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo, double* mom64, float* box,
+               const uint32_t* __restrict__ span, uint32_t nb, const RecOut ro) {
     extern __shared__ __align__(16) unsigned char mom_smem[];
     SpanShared& sh = *reinterpret_cast<SpanShared*>(mom_smem);
+    cg::cluster_group cluster = cg::this_cluster();
+    const uint32_t rank = cluster.block_rank();
     const int tid = threadIdx.x, lane = tid & 31;
     const int nlev = (int)sc->n_levels;
 #ifdef BH_TIMELINE
@@ -364,7 +376,8 @@ __global__ void __launch_bounds__(kSpanThreads, 1) k_moments_span(const DevScala
 #endif
     TLM();
     const int grp = tid >> 3, sub = tid & 7;
-    // the straddling nodes of every level, in ascending order (= block order), and their topology: warp w takes levels w, w + 16, ...
+    // the straddling nodes of every level, in ascending order (= block order), and their topology (every CTA builds the
+    // same lists): warp w takes levels w, w + 8, ...
     for (int L = tid >> 5; L < nlev; L += kSpanThreads / 32) {
         uint32_t run = 0;
         for (uint32_t b0 = 0; b0 < nb; b0 += 32) {
@@ -387,13 +400,30 @@ __global__ void __launch_bounds__(kSpanThreads, 1) k_moments_span(const DevScala
         const int cur = L & 1, below = cur ^ 1;
         const uint32_t cnt = sh.cnt[L], cntb = sh.cnt[L + 1];
         const uint32_t* listb = sh.list[L + 1 < kLevels ? L + 1 : L];
-        // the children of round r + 1 are requested before round r is summed
-        auto fetch = [&](uint32_t q, Child& ch, uint4& t) {
+        // this CTA's nodes: q = rank + kSpanCtas * local, local = 0, 1, ...; lane group `grp` takes local = grp, grp + kSpanGroups, ...
+        // The stores to the cell arrays of a node are issued AFTER the cluster barrier has been signalled: the peers only
+        // need the shared-memory copy, and the barrier's release would otherwise wait for the global stores.
+        bool pend = false;
+        Mom pm;
+        uint4 pt = make_uint4(0u, 0u, 0u, 0u);
+        uint32_t pc = 0;
+        auto flush = [&]() {
+            if (!pend) return;
+            if (sub == 0) mom_store(pm, mom64, box, pc);
+            if (ro.enabled && sub == 1) rec_store(make_record(pm, ro.theta, ro.mac_kind, pt.x, pt.y, pt.z, pt.w), ro, pc);
+            pend = false;
+        };
+        for (uint32_t l0 = 0; rank + kSpanCtas * l0 < cnt; l0 += kSpanGroups) {
+            const uint32_t local = l0 + grp, q = rank + kSpanCtas * local;
+            if (rank + kSpanCtas * (local & ~3u) >= cnt) break;        // (warp-uniform) no node left for this warp's four groups
+            flush();
+            const bool have = q < cnt;
+            uint32_t c = 0;
+            uint4 t = make_uint4(0u, 0u, 0u, 0u);
+            if (have) { c = sh.list[L][q]; t = sh.topo[L][q]; }
+            const int nch = have ? (int)(t.w - t.z) : 0;
+            Child ch;
             child_clear(ch);
-            t = make_uint4(0u, 0u, 0u, 0u);
-            if (q >= cnt) return;
-            t = sh.topo[L][q];
-            const int nch = (int)(t.w - t.z);
             if (sub < nch) {
                 const uint32_t cc = t.z + sub;
                 int lo2 = 0, hi2 = (int)cntb;
@@ -401,42 +431,34 @@ __global__ void __launch_bounds__(kSpanThreads, 1) k_moments_span(const DevScala
                     const int mid = (lo2 + hi2) >> 1;
                     if (listb[mid] < cc) lo2 = mid + 1; else hi2 = mid;
                 }
-                if (lo2 < (int)cntb && listb[lo2] == cc) child_load_shared(ch, sh.cell[below][lo2]);
-                else child_load_global(ch, mom64, box, cc);
+                if (lo2 < (int)cntb && listb[lo2] == cc) {              // computed one level ago by CTA lo2 mod 8, kept in its slot lo2 / 8
+                    const SpanCell* remote = cluster.map_shared_rank(&sh.cell[below][lo2 / kSpanCtas], lo2 % kSpanCtas);
+                    child_load_shared(ch, *remote);
+                } else {
+                    child_load_global(ch, mom64, box, cc);
+                }
             }
-        };
-        Child chn;
-        uint4 tn;
-        fetch((uint32_t)grp, chn, tn);
-        for (uint32_t q0 = 0; q0 < cnt; q0 += kSpanGroups) {
-            const uint32_t q = q0 + grp;
-            if ((q & ~3u) >= cnt) break;                               // (warp-uniform) no node left for this warp's four groups
-            const Child ch = chn;
-            const uint4 t = tn;
-            fetch(q + kSpanGroups, chn, tn);
-            const bool have = q < cnt;
-            const int nch = have ? (int)(t.w - t.z) : 0;
-            const uint32_t c = have ? sh.list[L][q] : 0u;
             Mom m;
             node_moments8(m, ch, nch, sub, sh.sx[grp]);
             if (have) {
                 if (sub == 0) {
-                    mom_store(m, mom64, box, c);
-                    SpanCell& o = sh.cell[cur][q];
+                    SpanCell& o = sh.cell[cur][local];
                     o.m[0] = m.M; o.m[1] = m.com[0]; o.m[2] = m.com[1]; o.m[3] = m.com[2];
 #pragma unroll
                     for (int k = 0; k < 6; ++k) o.m[4 + k] = m.Q[k];
 #pragma unroll
                     for (int k = 0; k < 3; ++k) { o.b[k] = m.bmin[k]; o.b[3 + k] = m.bmax[k]; }
                 }
-                if (ro.enabled && sub == 1) rec_store(make_record(m, ro.theta, ro.mac_kind, t.x, t.y, t.z, t.w), ro, c);
+                pend = true; pm = m; pt = t; pc = c;
             }
         }
-        __syncthreads();
+        cluster.barrier_arrive();                                      // this CTA's part of the level is in its shared memory
+        flush();
+        cluster.barrier_wait();                                        // ... and so is everybody else's
         TLM();
     }
 #ifdef BH_TIMELINE
-    if (tid == 0) { for (int q = 0; q < ntl; ++q) g_bh_dbg[384 + q] = tl[q]; g_bh_dbg[384 + 127] = ntl; }
+    if (tid == 0 && rank == 0) { for (int q = 0; q < ntl; ++q) g_bh_dbg[384 + q] = tl[q]; g_bh_dbg[384 + 127] = ntl; }
 #endif
 }
 
@@ -482,7 +504,7 @@ int stage_moments(bh_ctx* c, float theta, cudaStream_t s) {
     const bool rec = theta > 0.0f;
     BH_LAUNCH(c, k_moments, nb, kMomThreads, sizeof(NodeScratch) * kMomGroups, s, c->ws.sc, c->ws.pos[c->cur], (int)n, (int)P, tiles, c->ws.tile_cnt, c->ws.c_topo,
               c->ws.mom64, c->ws.box, c->ws.mom_span, rec_out(c, theta, rec));
-    BH_LAUNCH(c, k_moments_span, 1, kSpanThreads, sizeof(SpanShared), s, c->ws.sc, c->ws.c_topo, c->ws.mom64, c->ws.box,
+    BH_LAUNCH(c, k_moments_span, kSpanCtas, kSpanThreads, sizeof(SpanShared), s, c->ws.sc, c->ws.c_topo, c->ws.mom64, c->ws.box,
               c->ws.mom_span, (uint32_t)nb, rec_out(c, theta, rec));
     c->rec_valid = rec;
     c->rec_theta = theta;
