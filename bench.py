@@ -32,7 +32,8 @@ if ROOT not in sys.path:
 import bh_inputs  # noqa: E402
 
 PAPER_PARTICLES_PER_S = 2.8e6      # GTX480, Plummer N = 2^20, theta = 0.75
-FLOP_PP, FLOP_PC = 20, 64          # DESIGN.md flop convention (FMA = 2, rsqrt = 1)
+FLOP_PP, FLOP_PC = 20, 64          # DESIGN.md flop convention A25: the O10 formulas counted with FMA = 2, rsqrt = 1
+FLOP_PC_EXECUTED = 56              # what the pre-scaled p-c body of k_walk_eval executes: 3 add + 22 fma + 8 mul + 1 rsqrt
 L2_FLUSH_BYTES = 256 << 20
 
 
@@ -336,16 +337,29 @@ def run_ours(args):
     eval_ms = stage_acc.get("eval", 0.0) / args.steps              # k_walk_eval alone (0 if the walk ran as several waves)
     lists_ms = stage_acc.get("lists", 0.0) / args.steps
     flops = FLOP_PP * s1.sum_pp + FLOP_PC * s1.sum_pc              # of the last step's walk
+    flops_exec = FLOP_PP * s1.sum_pp + FLOP_PC_EXECUTED * s1.sum_pc
     kernel_ms = eval_ms if eval_ms > 0.0 else walk_ms
     achieved = flops / (kernel_ms * 1e-3) / 1e12
+    # measured FP32 peak: register-resident multiply-add chains on every SM (bh_probe_fp32), this run, this box
+    from paper_1106_1900_b200 import probe_fp32
+    probe = probe_fp32(dev)
+    peak_measured = max(probe[k] for k in ("ffma", "ffma2", "ffma2_shared_operand", "ffma2_broadcast_scalar"))
     prof = os.path.join(ROOT, "profiles", "walk_traffic.json")
     traffic = json.load(open(prof)).get("dram_bytes_per_launch") if os.path.exists(prof) else None
     build_ms = sum(stage_acc[k] for k in ("bbox", "keys", "sort", "reorder", "cells", "groups", "moments", "record")) / args.steps
     roofline = {"bound": "alu", "kernel": "k_walk_eval" if eval_ms > 0.0 else "k_walk_lists + k_walk_eval (pipelined waves)",
                 "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops, "traffic": traffic,
+                "traffic_source": "profiles/walk_traffic.json: dram bytes of one launch from an ncu --set full capture of this kernel (cold L2); not measured in this run",
+                "peak_measured": peak_measured, "frac_of_measured": achieved / peak_measured,
+                "peak_measured_kind": "best multiply-add chain of bh_probe_fp32 in this run (probe_fp32 lists them: scalar fma, packed fma with three "
+                                      "register operands / a shared operand / a broadcast scalar; pc_body, pp_body: the force bodies alone)",
+                "probe_fp32": probe,
+                "achieved_executed": flops_exec / (kernel_ms * 1e-3) / 1e12, "frac_executed": flops_exec / (kernel_ms * 1e-3) / 1e12 / peak_tflops,
+                "walk_frac_executed": flops_exec / (walk_ms * 1e-3) / 1e12 / peak_tflops,
+                "flops_executed_what": "20 per p-p, 56 per p-c: the operations the pre-scaled p-c body really executes (the 64 of the convention counts the O10 formula)",
                 "peak_kind": f"148 SMs x 128 FP32 lanes x 2 flop x sm_max_mhz ({peak_kind} clock {sm_max:.0f} MHz), DESIGN.md",
-                "flop_convention": "20 per p-p, 64 per p-c (FMA=2, rsqrt=1); useful interactions only",
+                "flop_convention": "20 per p-p, 64 per p-c: DESIGN.md A25, the O10 formulas counted with FMA = 2, rsqrt = 1; useful interactions only",
                 "kernel_ms": kernel_ms, "lists_ms": lists_ms, "walk_ms": walk_ms,
                 "walk_frac": flops / (walk_ms * 1e-3) / 1e12 / peak_tflops,
                 "walk_frac_what": "the same flops over S7 + S8 together (list walk + evaluation), the figure north_star's 50 % target is read against",
@@ -435,10 +449,21 @@ def main():
     ap.add_argument("--ref-groups", dest="ref_groups", type=int, default=None)
     ap.add_argument("--no-cpu", dest="no_cpu", action="store_true")
     ap.add_argument("--no-e2e", dest="no_e2e", action="store_true", help="skip the host-buffer leg (for profiling runs)")
+    ap.add_argument("--probe-fp32", dest="probe_fp32", action="store_true", help="only run the FP32 issue-rate probes (bh_probe_fp32) and print them")
     ap.add_argument("--no-graph", dest="no_graph", action="store_true", help="time plain bh_leapfrog_step launches instead of the captured step")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                      # timing rule: at least 3 warm-up steps
+    if args.probe_fp32:
+        import torch
+        from paper_1106_1900_b200 import probe_fp32
+        torch.cuda.set_device(0)
+        props = torch.cuda.get_device_properties(0)
+        peaks, kind = _peaks()
+        nominal = props.multi_processor_count * 128 * 2 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12
+        print(json.dumps({"probe_fp32": probe_fp32(), "unit": "TFLOP/s", "nominal": nominal, "gpu": props.name, "sms": props.multi_processor_count,
+                          "what": "bh_probe_fp32: 512 threads x SMs, register-resident chains (include/bh.h); pc_body / pp_body in the 20 / 64 convention"}))
+        return
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -201,6 +201,17 @@ int bh_get_walk_timeline(bh_ctx* ctx, void* stream, int64_t* ns, int capacity_wa
  * `stream`; both pointers are borrowed.  Not on the per-step path.  Returns BH_OK, BH_ERR_INVALID_ARG or BH_ERR_CUDA. */
 int bh_direct_forces(const float* d_pos_mass, int64_t n, float eps, int64_t t0, int64_t t1, double* d_acc_pot, void* stream);
 
+/* FP32 issue-rate probes ("a register-resident FFMA-chain probe"); a measurement aid, not on the
+ * per-step path.  Runs one kernel on every SM of the current device (512 threads per block: four warps per scheduler,
+ * the occupancy of the evaluation kernel) on the legacy default stream, synchronises, and returns the achieved rate.
+ *   kind 0: scalar fma, three distinct 32-bit register operands        1: packed fma.rn.f32x2, three distinct 64-bit operands
+ *   kind 2: packed, one operand shared by consecutive instructions     3: packed, a 32-bit scalar broadcast to both halves
+ *   kind 4: the particle-cell body of S8 on entries in shared memory   5: the particle-particle body
+ * *tflops: 2 flop per multiply-add lane (kinds 0-3); kinds 4, 5 in the 20 / 64 flop convention of DESIGN.md (A25), with
+ * the flops the code really executes (56 per particle-cell interaction) in *tflops_executed (may be NULL).
+ * d_scratch: device memory, at least 4 * (SMs * 512 + 4096) bytes, borrowed.  No ctx needed. */
+int bh_probe_fp32(int kind, void* d_scratch, size_t scratch_bytes, double* tflops, double* tflops_executed);
+
 int bh_last_cuda_error(const bh_ctx* ctx);
 const char* bh_status_string(int status);
 

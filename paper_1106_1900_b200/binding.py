@@ -22,7 +22,7 @@ STATUS = {0: "BH_OK", -1: "BH_ERR_INVALID_ARG", -2: "BH_ERR_WORKSPACE", -3: "BH_
 SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", "bh_get_particles", "bh_tree_build",
            "bh_compute_forces", "bh_refresh_moments", "bh_compute_forces_active", "bh_set_mac", "bh_leapfrog_step", "bh_step_graph_build",
            "bh_step_graph_launch", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
-           "bh_get_stage_ms", "bh_get_walk_timeline", "bh_direct_forces", "bh_last_cuda_error", "bh_status_string"]
+           "bh_get_stage_ms", "bh_get_walk_timeline", "bh_direct_forces", "bh_probe_fp32", "bh_last_cuda_error", "bh_status_string"]
 
 
 class BhConfig(C.Structure):
@@ -91,6 +91,8 @@ def load_library():
     lib.bh_get_walk_timeline.restype = C.c_int
     lib.bh_direct_forces.argtypes = [C.c_void_p, C.c_int64, C.c_float, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
     lib.bh_direct_forces.restype = C.c_int
+    lib.bh_probe_fp32.argtypes = [C.c_int, C.c_void_p, C.c_size_t, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.bh_probe_fp32.restype = C.c_int
     lib.bh_last_cuda_error.argtypes = [C.c_void_p]
     lib.bh_status_string.restype = C.c_char_p
     lib.bh_status_string.argtypes = [C.c_int]
@@ -122,6 +124,29 @@ def direct_forces(pos_mass: torch.Tensor, eps: float, t0: int = 0, t1: int | Non
                                          C.c_void_p(torch.cuda.current_stream(pos_mass.device).cuda_stream))
     if rc != BH_OK:
         raise BhError(rc, "bh_direct_forces")
+    return out
+
+
+PROBE_KINDS = {"ffma": 0, "ffma2": 1, "ffma2_shared_operand": 2, "ffma2_broadcast_scalar": 3, "pc_body": 4, "pp_body": 5}
+
+
+def probe_fp32(device=None) -> dict:
+    """bh_probe_fp32 for every kind: {name: TFLOP/s} (+ "<body>_executed" for the force bodies).  Synchronises."""
+    lib = load_library()
+    dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    scratch = torch.empty(sms * 512 + 4096, dtype=torch.float32, device=dev)
+    torch.cuda.synchronize(dev)
+    out = {}
+    with torch.cuda.device(dev):
+        for name, kind in PROBE_KINDS.items():
+            a, b = C.c_double(0.0), C.c_double(0.0)
+            rc = lib.bh_probe_fp32(kind, scratch.data_ptr(), scratch.numel() * 4, C.byref(a), C.byref(b))
+            if rc != BH_OK:
+                raise BhError(rc, "bh_probe_fp32")
+            out[name] = a.value
+            if kind >= 4:
+                out[name + "_executed"] = b.value
     return out
 
 

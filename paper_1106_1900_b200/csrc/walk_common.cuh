@@ -64,6 +64,56 @@ __device__ __forceinline__ Consts make_consts(float eps2) {
 
 struct Acc2 { f2 ax, ay, az, p; };
 
+// ---- the force bodies of the list evaluation (walk_eval.cu; also timed on their own by probe.cu)
+__device__ __forceinline__ f2 bc(float s) { return pk(s, s); }   // ptxas folds this into the broadcast operand form
+
+// One p-c entry on one packed pair of targets.  Record: v0 = (com, M), v1 = (Qm_xx, Qm_yy, Qm_zz, Qm_xy),
+// v2 = (Qm_xz, Qm_yz, nTh, n3Th) with Qm = -3 Q, nTh = -T/2, n3Th = -3T/2.  rho^2 = |dr|^2 + eps^2, u = 1/rho^2,
+// q = Qm dr, w = dr.q:   -phi += (1/rho) (M + u (nTh - w u / 2)),   a += (1/rho^5) (q + dr (M rho^2 + n3Th - 5 w u / 2)).
+__device__ __forceinline__ void pc_bc(const float4& v0, const float4& v1, const float4& v2, f2 ntx, f2 nty, f2 ntz, const Consts& k, Acc2& a) {
+    const f2 dx = add2(bc(v0.x), ntx), dy = add2(bc(v0.y), nty), dz = add2(bc(v0.z), ntz);
+    const f2 r2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, k.e2)));
+    const f2 ri = rsqrt2(r2);
+    const f2 u = mul2(ri, ri), uu = mul2(u, u), ri5 = mul2(ri, uu);
+    const f2 qx = fma2(bc(v1.x), dx, fma2(bc(v1.w), dy, mul2(bc(v2.x), dz)));
+    const f2 qy = fma2(bc(v1.w), dx, fma2(bc(v1.y), dy, mul2(bc(v2.y), dz)));
+    const f2 qz = fma2(bc(v2.x), dx, fma2(bc(v2.y), dy, mul2(bc(v1.z), dz)));
+    const f2 w = fma2(dx, qx, fma2(dy, qy, mul2(dz, qz)));
+    const f2 wu = mul2(w, u);
+    a.p = fma2(ri, fma2(u, fma2(wu, k.mhalf, bc(v2.z)), bc(v0.w)), a.p);
+    const f2 c = fma2(bc(v0.w), r2, fma2(wu, k.m2p5, bc(v2.w)));
+    a.ax = fma2(fma2(dx, c, qx), ri5, a.ax);
+    a.ay = fma2(fma2(dy, c, qy), ri5, a.ay);
+    a.az = fma2(fma2(dz, c, qz), ri5, a.az);
+}
+
+// One p-p entry on one packed pair of targets tA, tA + 1.  kSelf: the entry is particle `e` of the group itself: skip
+// e == target (A19) and the shadow targets >= ng (they sit ON a real particle: r = 0 would give 0 * inf when eps = 0).
+template <bool kSelf>
+__device__ __forceinline__ void pp_bc(const float4& v, f2 ntx, f2 nty, f2 ntz, const Consts& k, Acc2& a, int e, int tA, int ng) {
+    const f2 dx = add2(bc(v.x), ntx), dy = add2(bc(v.y), nty), dz = add2(bc(v.z), ntz);
+    const f2 r2 = fma2(dx, dx, fma2(dy, dy, fma2(dz, dz, k.e2)));
+    f2 ri;
+    if (kSelf) {
+        float lo, hi;
+        upk(r2, lo, hi);
+        lo = (e == tA || tA >= ng) ? 0.0f : rsqrt_approx(lo);
+        hi = (e == tA + 1 || tA + 1 >= ng) ? 0.0f : rsqrt_approx(hi);
+        ri = pk(lo, hi);
+    } else {
+        ri = rsqrt2(r2);
+    }
+    const f2 ri2 = mul2(ri, ri);
+    const f2 mr = mul2(bc(v.w), ri);
+    const f2 mr3 = mul2(mr, ri2);
+    a.p = add2(a.p, mr);
+    a.ax = fma2(dx, mr3, a.ax);
+    a.ay = fma2(dy, mr3, a.ay);
+    a.az = fma2(dz, mr3, a.az);
+}
+
+
+
 // One pair of p-c entries on one target.  With rho^2 = |dr|^2 + eps^2, u = 1/rho^2, q = Qm dr = -3 Q dr, w = dr.q:
 //   -phi += (1/rho)   (M + u (nTh - w u / 2))
 //   a    += (1/rho^5) (q + dr (M rho^2 + n3Th - 5 w u / 2))

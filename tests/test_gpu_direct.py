@@ -82,3 +82,24 @@ def test_acceleration_error_experiment():
     assert np.array_equal(t["pos_mass"].cpu().numpy(), ps)
     err = accuracy.relative_error(t["acc_pot"].cpu().numpy(), oracle.direct(ps, 0.0))
     assert abs(accuracy.exceeded_by(err, 0.5) - med[1]) < 1e-6 * med[1] + 1e-12
+
+
+def test_fp32_probes_report_sane_rates():
+    import torch
+    """bh_probe_fp32 (SURVEY.md 8(d)): every kind runs, is positive and below the nominal FP32 peak; argument errors."""
+    import ctypes as C
+    import __graft_entry__ as g
+    g.build()
+    from paper_1106_1900_b200 import load_library, probe_fp32
+    p = probe_fp32()
+    props = torch.cuda.get_device_properties(0)
+    nominal = props.multi_processor_count * 128 * 2 * 2.1e9 / 1e12      # generous clock bound
+    assert set(p) == {"ffma", "ffma2", "ffma2_shared_operand", "ffma2_broadcast_scalar", "pc_body", "pc_body_executed", "pp_body", "pp_body_executed"}
+    for k, v in p.items():
+        assert 1.0 < v < nominal, (k, v)
+    assert p["pc_body_executed"] < p["pc_body"] and abs(p["pc_body_executed"] / p["pc_body"] - 56 / 64) < 1e-9
+    lib = load_library()
+    x = C.c_double()
+    s = torch.empty(16, dtype=torch.float32, device="cuda")
+    assert lib.bh_probe_fp32(0, s.data_ptr(), 64, C.byref(x), None) == -2          # scratch too small
+    assert lib.bh_probe_fp32(9, s.data_ptr(), 64, C.byref(x), None) == -1
