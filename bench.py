@@ -187,6 +187,36 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# ------------------------------------------------------------------------------------------------ ranks
+def spawn_ranks(n: int) -> int:
+    """Re-run this command line under torch.distributed.run with one rank per GPU of this node (what the driver does itself
+    when it launches N > 1; a bare `python bench.py --gpus N` must not silently measure one GPU)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n), "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.run(cmd).returncode
+
+
+def dry_run_ranks():
+    import torch
+    import torch.distributed as dist
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    cuda = torch.cuda.is_available()
+    if world > 1:
+        if cuda:
+            torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+        dist.init_process_group("nccl" if cuda else "gloo")
+    t = max_over_ranks(float(rank + 1), world, torch.device("cuda") if cuda else None)
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "n_gpus": world, "max_over_ranks": t, "backend": ("nccl" if cuda else "gloo") if world > 1 else None}))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 # ------------------------------------------------------------------------------------------------ the CUDA path
 def run_ours(args):
     import torch
@@ -420,6 +450,8 @@ def run_ours(args):
         "build_hbm": build_hbm,
         "wall_s_timed_region": wall,
         "block_step": block,
+        "sharded": ({"bounds": bh.bounds, "flops_per_rank_last_step": bh.last_work, "balance": "by the previous step's 20 n_pp + 64 n_pc per group"}
+                    if sharded else None),
         "cpu_baseline": cpu,
         "paper_context": "2.8 M particles/s on a GTX480, Plummer N=2^20, theta=0.75 (PAPER.md:182, 256)",
     }
@@ -451,7 +483,13 @@ def main():
     ap.add_argument("--no-e2e", dest="no_e2e", action="store_true", help="skip the host-buffer leg (for profiling runs)")
     ap.add_argument("--probe-fp32", dest="probe_fp32", action="store_true", help="only run the FP32 issue-rate probes (bh_probe_fp32) and print them")
     ap.add_argument("--no-graph", dest="no_graph", action="store_true", help="time plain bh_leapfrog_step launches instead of the captured step")
+    ap.add_argument("--dry-run-ranks", dest="dry_run_ranks", action="store_true",
+                    help="only start the ranks, join them in a process group (nccl on GPUs, gloo without) and let rank 0 report the world size")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and (args.impl == "ours" or args.dry_run_ranks):
+        sys.exit(spawn_ranks(args.gpus))     # `python bench.py --gpus N` starts its own N ranks (one per GPU)
+    if args.dry_run_ranks:
+        return dry_run_ranks()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                      # timing rule: at least 3 warm-up steps
     if args.probe_fp32:

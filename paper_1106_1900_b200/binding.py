@@ -299,6 +299,18 @@ class BarnesHut:
             self._acc_ptr = v.acc_pot
         return self._view(self._acc_ptr, self.n * 4, torch.float32, (self.n, 4))
 
+    def group_views(self):
+        """(group_begin int32[G+1], group_npc int32[G], group_npp int32[G]) as views of the workspace; synchronises (the group
+        count lives on the device).  No export kernel is launched."""
+        if getattr(self, "_group_ptrs", None) is None:
+            v = BhTreeView()
+            self._check(self.lib.bh_export_tree(self.h, C.byref(v), self._stream()), "bh_export_tree")
+            self._group_ptrs = (v.group_begin, v.group_npc, v.group_npp)
+        ng = int(self.sync_status().n_groups)
+        pb, pc, pp = self._group_ptrs
+        i32 = torch.int32
+        return self._view(pb, ng + 1, i32), self._view(pc, ng, i32), self._view(pp, ng, i32)
+
     def export_tree(self) -> dict:
         """Canonical arrays of bh_tree_view as torch tensors that alias the workspace (synchronises)."""
         v = BhTreeView()

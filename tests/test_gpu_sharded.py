@@ -62,3 +62,73 @@ def test_shares_add_up_to_the_walk_of_all_groups(mod, world):
     assert G <= walked <= G + world - 1                                   # only groups that straddle a boundary are walked twice
     b = mod.share_bounds(n, world)
     assert b[0] == 0 and b[-1] == n and all(x < y for x, y in zip(b, b[1:]))
+
+
+TWO_RANK_WORKER = r"""
+import json, os, sys
+sys.path.insert(0, %r)
+sys.path.insert(0, os.path.join(%r, "tests"))
+import numpy as np, torch
+import torch.distributed as dist
+import bh_inputs, oracle
+from parity_common import check_forces, compare_counts, compare_tree, export_numpy
+from paper_1106_1900_b200 import ShardedBarnesHut
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+torch.cuda.set_device(0)                       # both ranks share the one GPU of the box; their kernels never wait for each other,
+dist.init_process_group("gloo")                # the exchange goes through gloo (NCCL refuses two ranks on one device)
+n = 20000
+pm, vel, prm = bh_inputs.make("c1", n=n, seed=79)
+theta, eps, dt = prm["theta"], prm["eps"], prm["dt"]
+bh = ShardedBarnesHut(n)
+assert bh.world == 2
+bh.set_particles(pm, vel)
+b0 = list(bh.bounds)                           # equal particle counts before the first evaluation
+bh.tree_build()
+bh.compute_forces(theta, eps)                  # world > 1: own share by bh_compute_forces_active, all-reduce of acc_pot, work all-reduce
+st = oracle.compute_forces(oracle.tree_build(pm, vel), theta, eps)
+g = export_numpy(bh)
+bad = compare_tree(g, st)
+mine = np.nonzero(g["group_npc"] + g["group_npp"] > 0)[0]      # the groups this rank walked
+compare_counts(g, st, sel=mine, problems=bad)
+assert not bad, bad
+e0 = check_forces(g, st)                       # EVERY particle's force is present on EVERY rank, within the tolerance of the oracle
+for step in range(2):
+    so = oracle.tree_build(g["pos_mass"].copy(), g["vel"].copy(), g["id"].view(np.uint32).copy())
+    so.accpot = g["acc_pot"].astype(np.float64)
+    s2 = oracle.leapfrog_step(so, theta, eps, dt)
+    bh.leapfrog_step(theta, eps, dt)
+    g = export_numpy(bh)
+    bad = compare_tree(g, s2, check_vel=False)
+    assert not bad, bad
+    check_forces(g, s2)
+torch.cuda.synchronize()
+out = dict(rank=rank, groups_walked=int(mine.size), groups=int(g["n_groups"]), acc_rms=e0["acc_rms"], bounds0=b0, bounds=list(bh.bounds),
+           work=bh.last_work, checksum=float(np.float64(g["acc_pot"]).sum()))
+print("RANKOUT " + json.dumps(out), flush=True)
+dist.barrier()
+dist.destroy_process_group()
+"""
+
+
+def test_two_ranks_share_the_walk_and_match_the_oracle(tmp_path):
+    """ShardedBarnesHut with world size 2 for real: two processes (on the one GPU), redundant build, each walks its share,
+    the all-reduce delivers every force to both; checked against the ORACLE per call, and the shares move to balance flops."""
+    import json
+    import os
+    import re
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "two_rank_worker.py"
+    script.write_text(TWO_RANK_WORKER % (root, root))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", "29741", str(script)]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=root)
+    assert r.returncode == 0, (r.stdout[-1500:], r.stderr[-3000:])
+    outs = sorted((json.loads(m) for m in re.findall(r"RANKOUT (\{.*?\})\n", r.stdout)), key=lambda o: o["rank"])
+    assert [o["rank"] for o in outs] == [0, 1]
+    G = outs[0]["groups"]
+    assert outs[0]["checksum"] == outs[1]["checksum"]                          # the ranks stay bit-identical
+    assert outs[0]["bounds0"] == [0, 10000, 20000] and outs[0]["bounds"] == outs[1]["bounds"] and outs[0]["bounds"][1] != 10000
+    w = outs[0]["work"]
+    assert max(w) / (sum(w) / 2) < 1.15, w                                     # balanced by the previous step's flops

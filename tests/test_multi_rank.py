@@ -107,3 +107,71 @@ def test_reference_arm_runs_on_rank0_only():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "particles/s"
+
+
+def test_bench_starts_its_own_ranks_without_torchrun():
+    """`python bench.py --gpus 2` with no launcher must create two ranks itself (dry run: process group + max-over-ranks only)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-run-ranks"], capture_output=True, text=True,
+                       timeout=300, env=env, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    import json
+    lines = [json.loads(x) for x in r.stdout.splitlines() if x.startswith("{")]
+    assert len(lines) == 1 and lines[0]["n_gpus"] == 2 and lines[0]["max_over_ranks"] == 2.0
+
+
+BALANCE_WORKER = textwrap.dedent("""
+    import json, os, sys
+    sys.path.insert(0, %r)
+    import numpy as np, torch
+    import torch.distributed as dist
+    import bh_inputs, oracle
+    from paper_1106_1900_b200.sharded import balanced_bounds, keep_own_rows, share_bounds, share_mask
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    dist.init_process_group("gloo")
+    n = 6000
+    pm, vel, prm = bh_inputs.make("c1", n=n, seed=73)
+    st = oracle.tree_build(pm, vel)
+    t = st.tree
+    full = oracle.compute_forces(oracle.tree_build(pm, vel), prm["theta"], prm["eps"])
+    work_all = t.gcount * (20 * full.npp + 64 * full.npc)
+    bounds = share_bounds(n, world)
+    imb = []
+    for it in range(2):                                             # equal counts first, then balanced by the measured work
+        mask = share_mask(n, world, rank, "cpu", bounds).numpy()
+        sel = np.array([g for g in range(t.ngroups) if mask[t.gbegin[g]: t.gbegin[g] + t.gcount[g]].any()], np.int64)
+        oracle.compute_forces(st, prm["theta"], prm["eps"], sel=sel)
+        acc = torch.from_numpy(np.nan_to_num(st.accpot))
+        keep_own_rows(acc, n, world, rank, bounds)
+        dist.all_reduce(acc, op=dist.ReduceOp.SUM)
+        work = torch.zeros(t.ngroups, dtype=torch.int64)
+        work[sel] = torch.from_numpy(t.gcount[sel] * (20 * st.npp[sel] + 64 * st.npc[sel]))
+        mine = float(work.sum())
+        dist.all_reduce(work, op=dist.ReduceOp.MAX)
+        per = torch.tensor([mine], dtype=torch.float64); allw = [torch.zeros(1, dtype=torch.float64) for _ in range(world)]
+        dist.all_gather(allw, per)
+        imb.append(max(float(x) for x in allw) * world / float(work.sum()))
+        equal = bool(np.array_equal(acc.numpy(), full.accpot))
+        bounds = balanced_bounds(torch.from_numpy(t.gbegin), work, n, world)
+    out = dict(rank=rank, imbalance=imb, equal=equal, bounds=bounds, work_ok=bool(np.array_equal(work.numpy(), work_all)))
+    print("RANKOUT " + json.dumps(out), flush=True)
+    dist.barrier()
+    dist.destroy_process_group()
+""") % ROOT
+
+
+def test_balanced_shares_two_ranks_gloo(tmp_path):
+    """Shares by the previous walk's flops per group: same forces, and the slowest rank's work drops."""
+    script = tmp_path / "balance_worker.py"
+    script.write_text(BALANCE_WORKER)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", "29735", str(script)]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    import json
+    import re
+    outs = sorted((json.loads(m) for m in re.findall(r"RANKOUT (\{.*?\})\n", r.stdout)), key=lambda o: o["rank"])
+    assert [o["rank"] for o in outs] == [0, 1]
+    assert all(o["equal"] and o["work_ok"] for o in outs)
+    assert outs[0]["bounds"] == outs[1]["bounds"] and outs[0]["bounds"][1] != 3000        # every rank derives the same, moved boundary
+    assert outs[0]["imbalance"][1] < outs[0]["imbalance"][0] and outs[0]["imbalance"][1] < 1.1, outs[0]["imbalance"]
