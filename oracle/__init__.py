@@ -266,3 +266,72 @@ def leapfrog_step(st: State, theta: float, eps: float, dt: float, nleaf: int = N
     compute_forces(s2, theta, eps)
     s2.vel = kick(s2.vel, s2.accpot.astype(np.float32), h)
     return s2
+
+
+# ---------------------------------------------------------------------------------------------- block time-steps (reading A29)
+@dataclass
+class BlockState:
+    """Key-sorted particle state of the block time-step scheme: (pos, vel, accb) of particle i hold at tick[i]."""
+    pos: np.ndarray      # float32[N,4]
+    vel: np.ndarray      # float32[N,4]
+    accb: np.ndarray     # float32[N,4]  held acceleration + potential (at the particle's own time)
+    ids: np.ndarray      # uint32[N]
+    tick: np.ndarray     # uint32[N]    time of the last update, in units of dt_max / 2^R
+    rung: np.ndarray     # uint8[N]     dt_i = dt_max / 2^rung
+    tree: Tree
+    len_scale: float
+    eta: float
+    dt_max: float
+    R: int
+    now: int = 0         # system time in ticks
+    active: np.ndarray = None
+    npc: np.ndarray = None
+    npp: np.ndarray = None
+
+
+def rungs(acc, active, len_scale, eta, dt_max, R, tick, out=None):
+    """A29 criterion: rung of the active particles (all if active is None) from their accelerations."""
+    a = np.ascontiguousarray(acc, np.float32)
+    n = a.shape[0]
+    out = np.zeros(n, np.uint8) if out is None else out
+    act = None if active is None else np.ascontiguousarray(active, np.uint8)
+    lib().orc_rungs(C.c_int64(n), _p(a), _p(act), C.c_float(len_scale), C.c_float(eta), C.c_float(dt_max), C.c_int32(R),
+                    C.c_uint32(tick), _p(out))
+    return out
+
+
+def block_init(st: State, len_scale: float, eta: float, dt_max: float, R: int) -> BlockState:
+    """All particles synchronised at tick 0 with the forces of `st`; rungs from the criterion."""
+    accb = np.ascontiguousarray(st.accpot, np.float64).astype(np.float32)
+    r = rungs(accb, None, len_scale, eta, dt_max, R, 0)
+    return BlockState(st.pos.copy(), st.vel.copy(), accb, st.ids.copy(), np.zeros(st.tree.n, np.uint32), r, st.tree,
+                      float(len_scale), float(eta), float(dt_max), int(R))
+
+
+def block_active(bs: BlockState):
+    """(tick_next, active uint8[N])."""
+    act = np.zeros(bs.tree.n, np.uint8)
+    lib().orc_block_active.restype = C.c_uint32
+    nxt = int(lib().orc_block_active(C.c_int64(bs.tree.n), _p(bs.tick), _p(bs.rung), C.c_int32(bs.R), _p(act)))
+    return nxt, act
+
+
+def block_step(bs: BlockState, theta: float, eps: float, acc_new=None) -> BlockState:
+    """One system step on the EXISTING cells and groups: active set, predictor, moments (+ group boxes) of the moved
+    particles, walk + forces of the groups with an active particle, corrector, new rungs.  acc_new (float32[N,4]): use
+    these accelerations instead of the oracle's own (per-call parity: the integer decisions then follow the same floats)."""
+    t = bs.tree
+    nxt, act = block_active(bs)
+    L = lib()
+    L.orc_block_predict(C.c_int64(t.n), _p(bs.pos), _p(bs.vel), _p(bs.accb), _p(act), _p(bs.rung), C.c_float(bs.dt_max))
+    moments(t, bs.pos)
+    sel = np.nonzero(np.add.reduceat(act.astype(np.int64), t.gbegin) > 0)[0].astype(np.int64)
+    r = walk_forces(t, bs.pos, theta, eps, sel=sel)
+    bs.npc, bs.npp = r["npc"], r["npp"]
+    new = np.nan_to_num(r["accpot"]).astype(np.float32) if acc_new is None else np.ascontiguousarray(acc_new, np.float32)
+    bs.acc_eval = r["accpot"]
+    L.orc_block_correct(C.c_int64(t.n), _p(bs.vel), _p(bs.accb), _p(new), _p(act), _p(bs.rung), C.c_float(bs.dt_max),
+                        C.c_uint32(nxt), _p(bs.tick))
+    rungs(bs.accb, act, bs.len_scale, bs.eta, bs.dt_max, bs.R, nxt, out=bs.rung)
+    bs.now, bs.active = nxt, act
+    return bs

@@ -13,7 +13,8 @@
 //   O5 reorder (L174) O6 sparse octree (L63, L65, Fig.1-2)  O7 groups (L75)
 //   O8 moments + boxes, binary64, fixed order (L109-115, L127, L266)
 //   O9 group walk with Eq.1 (L83, L87, L125)  O10 p-p / p-c forces, binary64 (L85, L109)
-//   O11 leapfrog (L105)   plus an O(N^2) binary64 direct sum (L131: theta -> 0 limit).
+//   O11 leapfrog (L105)   plus an O(N^2) binary64 direct sum (L131: theta -> 0 limit), and the block time-step
+//   scheme of L101 / L105 / L264-266 in the reading A29 (orc_rungs, orc_block_*).
 //
 // Pins (tests/ -m "not gpu"): dilate worked example L376, mask example L67, List 1 (L380-390) as an
 // independent dilate, numpy stable argsort, a second tree construction (the paper's literal
@@ -21,7 +22,9 @@
 // moments, the parallel-axis identity, closed-form two-mass quadrupole, (s/R)^3 convergence,
 // brute force O(N^2), theta -> 0, analytic Plummer potential, two-body orbit, reversibility;
 // Eq.1's l, delta, r_open: hand-built cells with closed-form values and a target one ulp on either side of the
-// threshold, plus a numpy-float32 restatement over every cell and a root-to-leaf walk with it.
+// threshold, plus a numpy-float32 restatement over every cell and a root-to-leaf walk with it; block time-steps: rung
+// closed forms and thresholds, commensurate times, the one-rung case against the shared-step leapfrog, second order on a
+// two-body orbit with unequal steps, energy over a macro-step.
 // Parity unpinned against the paper: magnitudes of the interaction counts (Fig.6 inset is an image).
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
@@ -436,6 +439,73 @@ void orc_kick(int64_t n, float* vel4, const float* acc4, float h) {
 void orc_drift(int64_t n, float* pos4, const float* vel4, float dt) {
     for (int64_t i = 0; i < n; ++i)
         for (int k = 0; k < 3; ++k) pos4[4 * i + k] = fmaf(vel4[4 * i + k], dt, pos4[4 * i + k]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Block time-steps (L45, L101 "time-step calculation ... on the GPU", L105 "... or on a subset of particles in case of
+// the block-time step regime", L264-266).  The paper names the ingredients and leaves the criterion open; reading A29
+// (DESIGN.md):  every particle i carries (x_i, v_i, a_i) at its own time t_i = tick_i * dt_max / 2^R and a step
+// dt_i = dt_max / 2^rung_i (a power-of-two fraction, so times stay commensurate).  One system step goes to
+// t_next = min_i (t_i + dt_i); the ACTIVE particles are those with t_i + dt_i = t_next.  Only they are predicted
+// (x_i += v_i dt_i + a_i dt_i^2 / 2, the leapfrog predictor of Hut et al. that L105 cites) and, after the accelerations
+// of the groups that hold them have been recomputed (moments refreshed on the existing cells, L266), corrected
+// (v_i += (a_i + a_new) dt_i / 2, "the velocities are corrected"); inactive particles stay where they were last updated.
+// All in float, single operations as written.
+
+// Time-step criterion (A29): tau = eta * sqrt(len / |a|), rung = the smallest r in [0, R] with dt_max / 2^r <= tau (R if
+// none); a particle may only move to a longer step at a time that is a multiple of it: rung >= R - ctz(tick) for tick > 0.
+// acc4: float[n][4]; only particles with active[i] != 0 get a new rung (active may be null: all).
+void orc_rungs(int64_t n, const float* acc4, const uint8_t* active, float len, float eta, float dt_max, int32_t R,
+               uint32_t tick, uint8_t* rung) {
+    int lowest = 0;                                      // longest step the current time allows
+    if (tick != 0) {
+        int z = 0;
+        while (((tick >> z) & 1u) == 0u) ++z;
+        lowest = R - z < 0 ? 0 : R - z;
+    }
+    for (int64_t i = 0; i < n; ++i) {
+        if (active && !active[i]) continue;
+        const float ax = acc4[4 * i], ay = acc4[4 * i + 1], az = acc4[4 * i + 2];
+        const float a2 = fmaf(az, az, fmaf(ay, ay, ax * ax));
+        const float amag = sqrtf(a2);
+        const float tau = eta * sqrtf(len / amag);       // |a| = 0: tau = +inf, the longest step
+        int r = 0;
+        while (r < R && !(ldexpf(dt_max, -r) <= tau)) ++r;
+        rung[i] = (uint8_t)(r < lowest ? lowest : r);
+    }
+}
+
+// tick_next = min_i (tick_i + 2^(R - rung_i)); active_i = (tick_i + 2^(R - rung_i) == tick_next).  Returns tick_next.
+uint32_t orc_block_active(int64_t n, const uint32_t* tick, const uint8_t* rung, int32_t R, uint8_t* active) {
+    uint32_t next = 0xFFFFFFFFu;
+    for (int64_t i = 0; i < n; ++i) next = std::min<uint32_t>(next, tick[i] + (1u << (R - rung[i])));
+    for (int64_t i = 0; i < n; ++i) active[i] = (tick[i] + (1u << (R - rung[i])) == next) ? 1 : 0;
+    return next;
+}
+
+// Predictor of the active particles (L105): h = dt_max / 2^rung; x = fmaf(a, (0.5f * h) * h, fmaf(v, h, x)).
+void orc_block_predict(int64_t n, float* pos4, const float* vel4, const float* acc4, const uint8_t* active, const uint8_t* rung,
+                       float dt_max) {
+    for (int64_t i = 0; i < n; ++i) {
+        if (!active[i]) continue;
+        const float h = ldexpf(dt_max, -(int)rung[i]);
+        const float hh = (0.5f * h) * h;
+        for (int k = 0; k < 3; ++k) pos4[4 * i + k] = fmaf(acc4[4 * i + k], hh, fmaf(vel4[4 * i + k], h, pos4[4 * i + k]));
+    }
+}
+
+// Corrector of the active particles (L105): v = fmaf(a_old + a_new, 0.5f * h, v); the held acceleration (and potential)
+// becomes the new one; tick_i = tick_next.
+void orc_block_correct(int64_t n, float* vel4, float* accb4, const float* accnew4, const uint8_t* active, const uint8_t* rung,
+                       float dt_max, uint32_t tick_next, uint32_t* tick) {
+    for (int64_t i = 0; i < n; ++i) {
+        if (!active[i]) continue;
+        const float h = ldexpf(dt_max, -(int)rung[i]);
+        const float hh = 0.5f * h;
+        for (int k = 0; k < 3; ++k) vel4[4 * i + k] = fmaf(accb4[4 * i + k] + accnew4[4 * i + k], hh, vel4[4 * i + k]);
+        for (int k = 0; k < 4; ++k) accb4[4 * i + k] = accnew4[4 * i + k];
+        tick[i] = tick_next;
+    }
 }
 
 }  // extern "C"
