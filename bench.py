@@ -297,14 +297,15 @@ def run_ours(args):
     #      holding `--active-fraction` of the particles) against the walk of all groups
     block = None
     if args.active_fraction > 0.0 and not sharded:
+        # (a) the two ingredients on a prescribed active set: a dense core holding `--active-fraction` of the particles
         t = bh.export_tree()
         r = torch.linalg.vector_norm(t["pos_mass"][:, :3], dim=1)
         active = (r <= torch.quantile(r[:: max(1, n // 1_000_000)], args.active_fraction)).to(torch.uint8).contiguous()
         cum = torch.cat([torch.zeros(1, dtype=torch.int64, device=dev), torch.cumsum(active.to(torch.int64), 0)])
         gb = t["group_begin"].to(torch.int64)
         n_active_groups = int(((cum[gb[1:]] - cum[gb[:-1]]) > 0).sum())
-        ea, eb, ec = (torch.cuda.Event(enable_timing=True) for _ in range(3))
-        t_ref, t_act = [], []
+        ea, eb, ec, ed = (torch.cuda.Event(enable_timing=True) for _ in range(4))
+        t_ref, t_part, t_act = [], [], []
         sub = dt / 16.0                      # a sub-step of the block hierarchy: the particles move by dt / 16 on the cells of a fresh build
         for _ in range(5):
             bh.tree_build()
@@ -314,17 +315,46 @@ def run_ours(args):
             ea.record(stream)
             bh.refresh_moments()
             eb.record(stream)
-            bh.compute_forces_active(theta, eps, active)
+            bh.refresh_moments_active(active)
             ec.record(stream)
+            bh.refresh_moments()             # (every particle moved in this set-up: the full refresh is the valid one)
+            bh.compute_forces_active(theta, eps, active)
+            ed.record(stream)
             torch.cuda.synchronize()
-            t_ref.append(ea.elapsed_time(eb)); t_act.append(eb.elapsed_time(ec))
+            t_ref.append(ea.elapsed_time(eb)); t_part.append(eb.elapsed_time(ec)); t_act.append(ec.elapsed_time(ed))
         sa = bh.sync_status()
         block = {"active_fraction": args.active_fraction, "active_particles": int(active.sum()), "active_groups": n_active_groups,
-                 "groups": int(sa.n_groups), "refresh_moments_ms": statistics.median(t_ref), "forces_active_ms": statistics.median(t_act),
-                 "sub_step": sub, "interactions_active": int(sa.sum_pc + sa.sum_pp),
-                 "what": "fresh build + forces (untimed), bh_kick_drift by dt/16 (untimed), then timed: bh_refresh_moments (S6 on the "
-                         "existing cells) and bh_compute_forces_active (S7 + S8 of the groups with an active particle); compare "
-                         "refresh_moments_ms with build_ms and forces_active_ms with stages_ms.walk + stages_ms.record"}
+                 "groups": int(sa.n_groups), "refresh_moments_ms": statistics.median(t_ref), "refresh_moments_active_ms": statistics.median(t_part),
+                 "refresh_plus_forces_active_ms": statistics.median(t_act), "sub_step": sub, "interactions_active": int(sa.sum_pc + sa.sum_pp),
+                 "what": "fresh build + forces (untimed), bh_kick_drift by dt/16 (untimed), then timed: bh_refresh_moments (S6 on all existing "
+                         "cells), bh_refresh_moments_active (only the cells above an active particle), and refresh + bh_compute_forces_active "
+                         "(S7 + S8 of the groups with an active particle); compare with build_ms and stages_ms.walk"}
+        # (b) the scheme itself (A29): one macro-step dt of individual power-of-two steps, rebuilding when the lists have grown
+        R, eta, growth = 4, 0.3, 1.10
+        bh.tree_build()
+        bh.compute_forces(theta, eps)
+        bh.block_init(eps, eta, dt, R)
+        rung0 = np.bincount(bh.block_state()["rung"], minlength=R + 1).tolist()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        steps = updated = rebuilds = 0
+        rebuild = False
+        while True:
+            bh.block_step(theta, eps, rebuild=rebuild)
+            bst = bh.block_state(arrays=False)["stats"]   # synchronises: the 48-byte read-back that decides about the rebuild
+            steps += 1; updated += int(bst.n_active); rebuilds += int(rebuild)
+            rebuild = bst.interactions_now > growth * bst.interactions_first
+            if int(bst.now_tick) >= 1 << R:
+                break
+        sec = time.perf_counter() - t0
+        block["scheme"] = {"max_rung": R, "eta": eta, "len_scale": eps, "dt_max": dt, "particles_per_rung_at_start": rung0, "block_steps": steps,
+                           "rebuilds": rebuilds, "rebuild_rule": f"interactions of the walked groups > {growth} x what they were when first walked on the cells",
+                           "particle_updates": updated, "mean_active_fraction": updated / (steps * n), "seconds": sec,
+                           "particle_updates_per_s": updated / sec, "ms_per_block_step": 1e3 * sec / steps,
+                           "shared_step_equivalent": "the same accuracy with one shared step needs 2^R full steps per macro-step",
+                           "updates_saved_vs_shared_smallest_step": (n * (1 << R)) / max(updated, 1)}
+        bh.set_particles(pm, vel)            # leave the context in the plain state for the legs below
+        bh.tree_build(); bh.compute_forces(theta, eps)
 
     # ---- e2e: the same step driven from HOST buffers through the C ABI (H2D and D2H inside the timed region)
     hp = torch.from_numpy(pm).pin_memory(); hv = torch.from_numpy(vel).pin_memory()

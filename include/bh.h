@@ -147,6 +147,44 @@ int bh_compute_forces(bh_ctx* ctx, float theta, float eps, void* stream);
 int bh_refresh_moments(bh_ctx* ctx, void* stream);
 int bh_compute_forces_active(bh_ctx* ctx, float theta, float eps, const uint8_t* d_active, void* stream);
 
+/* bh_refresh_moments restricted to "the multipole moments of tree-cells that have updated child particles" (L266): only
+ * the leaves that hold an active particle and their ancestors are recomputed (d_active as above); every other cell keeps
+ * the moments, box and records it holds, which are still exact if only active particles moved. */
+int bh_refresh_moments_active(bh_ctx* ctx, const uint8_t* d_active, void* stream);
+
+/* The block time-step scheme itself (L45, L101 "time-step calculation ... on the GPU", L105, L264-266; reading A29).
+ * Every particle i holds (x_i, v_i, a_i) at its own time t_i = tick_i * dt_max / 2^max_rung and steps by
+ * dt_i = dt_max / 2^rung_i, rung_i = the smallest r in [0, max_rung] with dt_max / 2^r <= eta * sqrt(len_scale / |a_i|)
+ * that keeps t_i a multiple of dt_i.
+ * bh_block_init: needs valid forces (bh_compute_forces); all particles at tick 0, rungs from the criterion.
+ * bh_block_step: one system step to t_next = min_i (t_i + dt_i).  The ACTIVE particles (t_i + dt_i = t_next) are predicted
+ *   (x += v dt + a dt^2 / 2), the moments of the cells above them refreshed on the existing cells (rebuild = 0; L266) or the
+ *   tree rebuilt from the current positions (rebuild != 0: S0-S6, the block state follows the sort), the groups that hold
+ *   them walked (L264), their velocities corrected (v += (a_old + a_new) dt / 2) and their next step chosen.  Inactive
+ *   particles are not touched.  Only enqueues work.
+ * bh_block_state: synchronises and reports (any pointer may be NULL; host or device destinations, key-sorted order):
+ *   tick, rung, the active flags of the last step, the held accelerations (float[n][4]).  interactions_now /
+ *   interactions_first = the list lengths of the groups walked in the last step, now and when each group was first walked
+ *   on the current cells: their ratio is the decline L266 speaks of ("the tree-cell size increases, which causes more
+ *   cells to be opened"); the caller rebuilds when it has grown too far. */
+typedef struct bh_block_config {
+    float len_scale;    /* length in the criterion (e.g. the softening eps), > 0 */
+    float eta;          /* accuracy parameter, > 0 */
+    float dt_max;       /* longest step, > 0 */
+    int32_t max_rung;   /* shortest step = dt_max / 2^max_rung; 0..20 */
+} bh_block_config;
+typedef struct bh_block_stats {
+    int64_t steps;                 /* block steps since bh_block_init */
+    int64_t steps_since_rebuild;
+    int64_t now_tick;              /* system time in ticks of dt_max / 2^max_rung */
+    int64_t n_active;              /* particles moved by the last step */
+    int64_t interactions_now;      /* sum over the groups walked in the last step of (n_pc + n_pp) */
+    int64_t interactions_first;    /* the same groups when each was first walked on the current cells */
+} bh_block_stats;
+int bh_block_init(bh_ctx* ctx, const bh_block_config* cfg, void* stream);
+int bh_block_step(bh_ctx* ctx, float theta, float eps, int rebuild, void* stream);
+int bh_block_state(bh_ctx* ctx, bh_block_stats* out, uint32_t* tick, uint8_t* rung, uint8_t* active, float* acc_held, void* stream);
+
 /* Which multipole acceptance criterion S7 uses from the next bh_compute_forces on (the tree need not be rebuilt).
  *   BH_MAC_EQ1 (default): Eq.1 (L125): d > l / theta + delta, d = distance between the group's box and the cell's centre of
  *     mass, l = longest side of the cell's tight box, delta = |centre of mass - box centre|.

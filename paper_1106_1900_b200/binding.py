@@ -20,7 +20,8 @@ STATUS = {0: "BH_OK", -1: "BH_ERR_INVALID_ARG", -2: "BH_ERR_WORKSPACE", -3: "BH_
 
 # every symbol include/bh.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", "bh_get_particles", "bh_tree_build",
-           "bh_compute_forces", "bh_refresh_moments", "bh_compute_forces_active", "bh_set_mac", "bh_leapfrog_step", "bh_step_graph_build",
+           "bh_compute_forces", "bh_refresh_moments", "bh_compute_forces_active", "bh_refresh_moments_active", "bh_block_init", "bh_block_step",
+           "bh_block_state", "bh_set_mac", "bh_leapfrog_step", "bh_step_graph_build",
            "bh_step_graph_launch", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
            "bh_get_stage_ms", "bh_get_walk_timeline", "bh_direct_forces", "bh_probe_fp32", "bh_last_cuda_error", "bh_status_string"]
 
@@ -35,6 +36,15 @@ class BhStats(C.Structure):
                 ("n_groups", C.c_int64), ("sum_pc", C.c_int64), ("sum_pp", C.c_int64), ("sum_mac", C.c_int64),
                 ("launches", C.c_int64), ("lo", C.c_float * 3), ("hi", C.c_float * 3), ("domain_exp", C.c_int32),
                 ("reserved", C.c_int32)]
+
+
+class BhBlockConfig(C.Structure):
+    _fields_ = [("len_scale", C.c_float), ("eta", C.c_float), ("dt_max", C.c_float), ("max_rung", C.c_int32)]
+
+
+class BhBlockStats(C.Structure):
+    _fields_ = [("steps", C.c_int64), ("steps_since_rebuild", C.c_int64), ("now_tick", C.c_int64), ("n_active", C.c_int64),
+                ("interactions_now", C.c_int64), ("interactions_first", C.c_int64)]
 
 
 _VIEW_FIELDS = ["pos_mass", "vel", "acc_pot", "id", "key", "perm", "level_offset", "cell_level", "cell_prefix",
@@ -75,6 +85,14 @@ def load_library():
     lib.bh_refresh_moments.restype = C.c_int
     lib.bh_compute_forces_active.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p]
     lib.bh_compute_forces_active.restype = C.c_int
+    lib.bh_refresh_moments_active.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.bh_refresh_moments_active.restype = C.c_int
+    lib.bh_block_init.argtypes = [C.c_void_p, C.POINTER(BhBlockConfig), C.c_void_p]
+    lib.bh_block_init.restype = C.c_int
+    lib.bh_block_step.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_int, C.c_void_p]
+    lib.bh_block_step.restype = C.c_int
+    lib.bh_block_state.argtypes = [C.c_void_p, C.POINTER(BhBlockStats), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.bh_block_state.restype = C.c_int
     lib.bh_set_mac.argtypes = [C.c_void_p, C.c_int]
     lib.bh_set_mac.restype = C.c_int
     lib.bh_leapfrog_step.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_void_p]
@@ -238,6 +256,36 @@ class BarnesHut:
             raise BhError(-1, "active must be a contiguous CUDA uint8[n] tensor")
         self._keep_active = active
         self._check(self.lib.bh_compute_forces_active(self.h, theta, eps, active.data_ptr(), self._stream()), "bh_compute_forces_active")
+
+    def refresh_moments_active(self, active: torch.Tensor):
+        """S6 only for the cells above an active particle; active: CUDA uint8[n] in the current sorted order."""
+        if not (active.is_cuda and active.dtype == torch.uint8 and active.is_contiguous() and active.numel() == self.n):
+            raise BhError(-1, "active must be a contiguous CUDA uint8[n] tensor")
+        self._keep_active = active
+        self._check(self.lib.bh_refresh_moments_active(self.h, active.data_ptr(), self._stream()), "bh_refresh_moments_active")
+
+    def block_init(self, len_scale: float, eta: float, dt_max: float, max_rung: int):
+        """Block time-steps (include/bh.h): all particles at tick 0 with the current forces, rungs from the criterion."""
+        cfg = BhBlockConfig(len_scale, eta, dt_max, max_rung)
+        self._check(self.lib.bh_block_init(self.h, C.byref(cfg), self._stream()), "bh_block_init")
+
+    def block_step(self, theta: float, eps: float, rebuild: bool = False):
+        """One system step of the block scheme: active set, predictor, moments (or rebuild), walk of the active groups, corrector."""
+        self._check(self.lib.bh_block_step(self.h, theta, eps, int(bool(rebuild)), self._stream()), "bh_block_step")
+
+    def block_state(self, arrays: bool = True) -> dict:
+        """bh_block_state: stats (+ tick uint32[n], rung uint8[n], active uint8[n], acc_held float32[n,4] as numpy); synchronises."""
+        st = BhBlockStats()
+        out = {}
+        if arrays:
+            n = self.n
+            out = dict(tick=np.empty(n, np.uint32), rung=np.empty(n, np.uint8), active=np.empty(n, np.uint8), acc_held=np.empty((n, 4), np.float32))
+            self._check(self.lib.bh_block_state(self.h, C.byref(st), _ptr(out["tick"]), _ptr(out["rung"]), _ptr(out["active"]),
+                                                _ptr(out["acc_held"]), self._stream()), "bh_block_state")
+        else:
+            self._check(self.lib.bh_block_state(self.h, C.byref(st), None, None, None, None, self._stream()), "bh_block_state")
+        out["stats"] = st
+        return out
 
     def set_mac(self, mac: int):
         """0: Eq.1 (default); 1: minimum-distance MAC."""

@@ -79,6 +79,7 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     o.row_total = c.take<uint32_t>(kTreeRows);
     o.mom_span = c.take<uint32_t>((size_t)kLevels * kMomBlockCap);
     o.c_topo = c.take<uint4>(C);
+    o.c_dirty = c.take<uint8_t>(C);
     o.c_parent = c.take<uint32_t>(C);
     o.mom64 = c.take<double>(10 * C);
     o.box = c.take<float>(6 * C);
@@ -86,6 +87,8 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     o.tlink = c.take<uint2>(C);
     o.erec = c.take<float4>(3 * C);
     o.ctl = c.take<WalkCtl>(1);
+    for (int k = 0; k < 2; ++k) { o.accb[k] = c.take<float4>(n); o.tick[k] = c.take<uint32_t>(n); o.rung[k] = c.take<uint8_t>(n); o.bactive[k] = c.take<uint8_t>(n); }
+    o.g_base = c.take<uint32_t>(n);
     o.lists = c.take<uint32_t>((size_t)g.list_entries);
     o.g_pcoff = c.take<uint32_t>(n);
     o.g_ppoff = c.take<uint32_t>(n);
@@ -193,6 +196,7 @@ int bh_set_particles(bh_ctx* c, int64_t n, const float* pos_mass, const float* v
     c->n = n;
     c->cur = 0;
     c->have_particles = c->have_topology = c->have_tree = c->have_forces = false;
+    c->block_on = false;
     c->acc_in_order = true;                                   // zeroed below, in the callers' order
     BH_CUDA(c, cudaMemcpyAsync(c->ws.pos[0], pos_mass, sizeof(float4) * (size_t)n, cudaMemcpyDefault, s));
     // S0-S2 need the positions only: velocities, ids and the zeroed accelerations arrive on an internal stream beside them
@@ -265,7 +269,7 @@ int bh_tree_build(bh_ctx* c, void* stream) {
     if (c->timing) stage_mark(c, 4, s);
     if ((rc = stage_cells(c, s)) != BH_OK) return rc;             // S4 + S5; records ev[5] between k_bounds and k_emit
     if (c->timing) stage_mark(c, 6, s);
-    if ((rc = stage_moments(c, c->theta_last, s)) != BH_OK) return rc;   // S6; with the fp32 records when theta is known
+    if ((rc = stage_moments(c, c->theta_last, nullptr, s)) != BH_OK) return rc;   // S6; with the fp32 records when theta is known
     if (c->timing) stage_mark(c, 7, s);
     c->have_topology = c->have_tree = true;
     return BH_OK;
@@ -277,7 +281,7 @@ int bh_refresh_moments(bh_ctx* c, void* stream) {
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     BH_CUDA(c, cudaSetDevice(c->device));
     c->have_forces = false;
-    int rc = stage_moments(c, c->theta_last, s);
+    int rc = stage_moments(c, c->theta_last, nullptr, s);
     if (rc != BH_OK) return rc;
     c->have_tree = true;
     return BH_OK;
@@ -307,6 +311,90 @@ int bh_compute_forces_active(bh_ctx* c, float theta, float eps, const uint8_t* d
     cudaPointerAttributes a;
     if (cudaPointerGetAttributes(&a, d_active) != cudaSuccess || a.type != cudaMemoryTypeDevice) { (void)cudaGetLastError(); return BH_ERR_INVALID_ARG; }
     return compute_forces_impl(c, theta, eps, d_active, stream);
+}
+
+int bh_refresh_moments_active(bh_ctx* c, const uint8_t* d_active, void* stream) {
+    if (!c || !d_active) return BH_ERR_INVALID_ARG;
+    if (!c->have_topology) return BH_ERR_STATE;
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, d_active) != cudaSuccess || a.type != cudaMemoryTypeDevice) { (void)cudaGetLastError(); return BH_ERR_INVALID_ARG; }
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    c->have_forces = false;
+    int rc = stage_moments(c, c->theta_last, d_active, s);
+    if (rc != BH_OK) return rc;
+    c->have_tree = true;
+    return BH_OK;
+}
+
+int bh_block_init(bh_ctx* c, const bh_block_config* cfg, void* stream) {
+    if (!c || !cfg || !(cfg->len_scale > 0.0f) || !std::isfinite(cfg->len_scale) || !(cfg->eta > 0.0f) || !std::isfinite(cfg->eta) ||
+        !(cfg->dt_max > 0.0f) || !std::isfinite(cfg->dt_max) || cfg->max_rung < 0 || cfg->max_rung > 20)
+        return BH_ERR_INVALID_ARG;
+    if (!c->have_forces) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    c->blk_len = cfg->len_scale; c->blk_eta = cfg->eta; c->blk_dt_max = cfg->dt_max; c->blk_R = cfg->max_rung;
+    c->blk_steps = 0;
+    c->blk_since_rebuild = 0;
+    int rc = stage_block_init(c, s);
+    if (rc != BH_OK) return rc;
+    c->block_on = true;
+    return BH_OK;
+}
+
+int bh_block_step(bh_ctx* c, float theta, float eps, int rebuild, void* stream) {
+    if (!c || !(theta > 0.0f) || !std::isfinite(theta) || !(eps >= 0.0f) || !std::isfinite(eps)) return BH_ERR_INVALID_ARG;
+    if (!c->block_on || !c->have_topology || c->copies_pending) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    int rc;
+    c->theta_last = theta;
+    if ((rc = stage_block_predict(c, s)) != BH_OK) return rc;
+    const uint8_t* act;
+    if (rebuild) {
+        // S0-S6 on the current positions (the active ones predicted); the block state then follows the sort
+        if ((rc = bh_tree_build(c, stream)) != BH_OK) return rc;
+        if ((rc = stage_block_permute(c, s)) != BH_OK) return rc;
+        c->blk_since_rebuild = 0;
+        act = c->ws.bactive[c->bcur];
+    } else {
+        act = c->ws.bactive[c->bcur];
+        c->have_forces = false;
+        if ((rc = stage_moments(c, theta, act, s)) != BH_OK) return rc;       // only the cells above an active particle (L266)
+        c->have_tree = true;
+    }
+    if ((rc = bh_compute_forces_active(c, theta, eps, act, stream)) != BH_OK) return rc;
+    if ((rc = stage_block_correct(c, s)) != BH_OK) return rc;
+    c->blk_steps += 1;
+    c->blk_since_rebuild += 1;
+    return BH_OK;
+}
+
+int bh_block_state(bh_ctx* c, bh_block_stats* out, uint32_t* tick, uint8_t* rung, uint8_t* active, float* acc_held, void* stream) {
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->block_on) return BH_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    const size_t n = (size_t)c->n;
+    const int b = c->bcur;
+    if (tick) BH_CUDA(c, cudaMemcpyAsync(tick, c->ws.tick[b], sizeof(uint32_t) * n, cudaMemcpyDefault, s));
+    if (rung) BH_CUDA(c, cudaMemcpyAsync(rung, c->ws.rung[b], n, cudaMemcpyDefault, s));
+    if (active) BH_CUDA(c, cudaMemcpyAsync(active, c->ws.bactive[b], n, cudaMemcpyDefault, s));
+    if (acc_held) BH_CUDA(c, cudaMemcpyAsync(acc_held, c->ws.accb[b], sizeof(float4) * n, cudaMemcpyDefault, s));
+    DevScalars h;
+    BH_CUDA(c, cudaMemcpyAsync(&h, c->ws.sc, sizeof(h), cudaMemcpyDeviceToHost, s));
+    BH_CUDA(c, cudaStreamSynchronize(s));
+    if (out) {
+        std::memset(out, 0, sizeof(*out));
+        out->steps = c->blk_steps;
+        out->steps_since_rebuild = c->blk_since_rebuild;
+        out->now_tick = c->blk_steps ? (int64_t)h.tick_next[(c->blk_steps - 1) & 1] : 0;
+        out->n_active = (int64_t)h.n_active;
+        out->interactions_now = (int64_t)h.deg_now;
+        out->interactions_first = (int64_t)h.deg_base;
+    }
+    return BH_OK;
 }
 
 int bh_leapfrog_step(bh_ctx* c, float theta, float eps, float dt, void* stream) {

@@ -50,6 +50,10 @@ struct DevScalars {
     unsigned long long sum_pc;
     unsigned long long sum_pp;
     unsigned long long sum_mac;
+    // block time-steps (blockstep.cu)
+    uint32_t tick_next[2];   // next system time, per step parity (the idle slot is reset to ~0)
+    uint32_t n_active;       // particles moved by the last block step
+    unsigned long long deg_now, deg_base;   // interactions of the groups walked in the last block step / when each was first walked on this tree
 };
 
 // Walk control block (device): wave boundaries in groups, work counters, the groups deferred to the fused kernel.
@@ -105,6 +109,7 @@ struct Ws {
     uint32_t* front_gsum;   // [kSortPasses][kFrontGroupCap][kRadix] digit counts per pass and group of 16 tiles (zero between launches)
     uint32_t* front_ctl;    // control words that are zero between launches: front_bar[2]
     uint32_t* front_bar;    // [2] grid barrier of k_front: arrivals, generation
+    uint8_t* c_dirty;     // [max_cells] partial refresh (block time-steps): the cell has an active particle below it
     uint4* c_topo;        // [max_cells] (first particle, end particle, first child, end child); children (0, 0) for a leaf
     uint32_t* c_parent;
     double* mom64;        // [max_cells][10]
@@ -113,6 +118,12 @@ struct Ws {
     uint2* tlink;         // [max_cells] walk record: (first child | first particle, count | leaf << 31)
     float4* erec;         // [max_cells][3] evaluation record: (com, M) (Qm_xx, Qm_yy, Qm_zz, Qm_xy) (Qm_xz, Qm_yz, -T/2, -3T/2), Qm = -3 Q
     WalkCtl* ctl;
+    // block time-steps: held accelerations, time of the last update (ticks of dt_max / 2^R), rung, active flags; [2]: ping-pong for a rebuild
+    float4* accb[2];
+    uint32_t* tick[2];
+    uint8_t* rung[2];
+    uint8_t* bactive[2];
+    uint32_t* g_base;     // [n] per group: interactions when it was first walked on this tree (0: not yet)
     uint32_t* lists;      // [list_entries] interaction lists: cell indices / particle indices
     uint32_t* g_pcoff;    // [n] first entry of the group's cell list (kNone: deferred to the fused kernel)
     uint32_t* g_ppoff;    // [n] first entry of the group's particle list
@@ -155,6 +166,13 @@ struct bh_ctx {
     int64_t sort_tiles, tree_tiles;
     int64_t front_max_tiles;   // sort tiles that are resident at once in a cooperative launch of k_front (0: not available)
     bool front_enabled;        // bh_config.front_mode != 1
+    // block time-steps
+    bool block_on;             // bh_block_init done on this particle set
+    int bcur;                  // which of accb / tick / rung / bactive is live
+    float blk_len, blk_eta, blk_dt_max;
+    int blk_R;
+    int64_t blk_steps;         // block steps since bh_block_init (parity of tick_next)
+    int64_t blk_since_rebuild; // block steps on the current cells
     bool rec_valid;            // trec / tlink / erec hold the current tree for (rec_theta, rec_mac)
     float rec_theta;
     int rec_mac;
@@ -212,7 +230,7 @@ int stage_bbox_keys(bh_ctx* c, cudaStream_t s);       // S0, S1
 int stage_sort(bh_ctx* c, cudaStream_t s);            // S2
 int stage_reorder(bh_ctx* c, cudaStream_t s);         // S3
 int stage_cells(bh_ctx* c, cudaStream_t s);           // S4 + S5
-int stage_moments(bh_ctx* c, float theta, cudaStream_t s);              // S6 (+ the fp32 records when theta > 0)
+int stage_moments(bh_ctx* c, float theta, const uint8_t* d_active, cudaStream_t s);   // S6 (+ the fp32 records when theta > 0); d_active: only the cells above an active particle
 int stage_cell_record(bh_ctx* c, float theta, cudaStream_t s);          // S6: fp32 walk record + r2open(theta) alone
 int stage_walk(bh_ctx* c, float theta, float eps, cudaStream_t s);   // S7, S8
 int stage_group_active(bh_ctx* c, const uint8_t* d_active, cudaStream_t s);   // groups with an active particle -> ws.gflag[g]
@@ -224,6 +242,12 @@ int walk_destroy(bh_ctx* c);
 struct WalkListOut {       // what k_walk_lists writes
     DevScalars* sc;
     WalkCtl* ctl;
+    // block time-steps: held accelerations, time of the last update (ticks of dt_max / 2^R), rung, active flags; [2]: ping-pong for a rebuild
+    float4* accb[2];
+    uint32_t* tick[2];
+    uint8_t* rung[2];
+    uint8_t* bactive[2];
+    uint32_t* g_base;     // [n] per group: interactions when it was first walked on this tree (0: not yet)
     uint32_t *g_pcoff, *g_ppoff, *g_lpp, *g_npc, *g_npp, *deferred;
 };
 WalkListOut walk_list_out(bh_ctx* c);
@@ -232,6 +256,10 @@ int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t region_base, uint32
 int stage_walk_eval(bh_ctx* c, int wave, float eps, int blocks_per_sm, bool by_class, cudaStream_t s);                           // S8
 int stage_kick_drift(bh_ctx* c, float h, float dt, cudaStream_t s);  // S9
 int stage_kick(bh_ctx* c, float h, cudaStream_t s);                  // S9
+int stage_block_init(bh_ctx* c, cudaStream_t s);
+int stage_block_predict(bh_ctx* c, cudaStream_t s);                   // next time, active set, predictor
+int stage_block_permute(bh_ctx* c, cudaStream_t s);                   // after a rebuild: the block state follows the sort
+int stage_block_correct(bh_ctx* c, cudaStream_t s);                   // corrector, new rungs, degradation sums
 int stage_export(bh_ctx* c, cudaStream_t s);
 int stage_iota(bh_ctx* c, uint32_t* dst, int64_t n, cudaStream_t s);
 

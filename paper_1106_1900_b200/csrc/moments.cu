@@ -255,7 +255,7 @@ struct SpanShared {
 // The owned nodes [lo, hi) of one level: eight lanes per node, the next node's topology is requested before the current
 // node's children are summed.
 __device__ __forceinline__ void node_pass(uint32_t lo, uint32_t hi, const uint4* __restrict__ topo, double* mom64, float* box, const RecOut& ro,
-                                          NodeScratch* sx) {
+                                          NodeScratch* sx, uint8_t* dirty, bool partial) {
     const int tid = threadIdx.x, grp = tid >> 3, sub = tid & 7;
     const uint32_t cnt = hi - lo;
     uint4 tp = make_uint4(0u, 0u, 0u, 0u);
@@ -264,8 +264,15 @@ __device__ __forceinline__ void node_pass(uint32_t lo, uint32_t hi, const uint4*
         const uint32_t q = q0 + grp;
         const uint4 t = tp;
         if (q + kMomGroups < cnt) tp = __ldg(topo + lo + q + kMomGroups);
-        const bool node = q < cnt && t.w != t.z;
-        if (!__any_sync(0xFFFFFFFFu, node)) continue;                 // (warp-uniform) none of this warp's four cells is a node
+        bool node = q < cnt && t.w != t.z;
+        if (partial) {                                                // a node whose children are all clean keeps what it holds
+            uint32_t d = 0;
+            if (node && (uint32_t)sub < t.w - t.z) d = __ldcg(dirty + t.z + sub);
+            d |= __shfl_xor_sync(0xFFFFFFFFu, d, 1, 8); d |= __shfl_xor_sync(0xFFFFFFFFu, d, 2, 8); d |= __shfl_xor_sync(0xFFFFFFFFu, d, 4, 8);
+            if (node && sub == 0) dirty[lo + q] = (uint8_t)(d ? 1 : 0);
+            node = node && d != 0;
+        }
+        if (!__any_sync(0xFFFFFFFFu, node)) continue;                 // (warp-uniform) none of this warp's four cells is a node to compute
         const int nch = node ? (int)(t.w - t.z) : 0;
         Child ch;
         child_clear(ch);
@@ -284,9 +291,11 @@ __device__ __forceinline__ void node_pass(uint32_t lo, uint32_t hi, const uint4*
 // it depends on nothing but the particles) and the nodes that lie entirely inside it.
 __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __restrict__ sc, const float4* __restrict__ pos, int n, int P, int tiles,
                                                             const uint32_t* __restrict__ tile_base, const uint4* __restrict__ topo,
-                                                            double* mom64, float* box, uint32_t* span, const RecOut ro) {
+                                                            double* mom64, float* box, uint32_t* span, const RecOut ro,
+                                                            const uint8_t* __restrict__ active, uint8_t* dirty) {
     extern __shared__ __align__(16) unsigned char mom_smem[];
     NodeScratch* sx = reinterpret_cast<NodeScratch*>(mom_smem);
+    const bool partial = active != nullptr;                   // block time-steps (L266): only cells with an updated particle below them
     __shared__ uint32_t s_lo[kLevels], s_hi[kLevels], s_hin[kLevels], s_pre[kLevels + 1];
     const int tid = threadIdx.x;
     const uint32_t b = blockIdx.x, nb = gridDim.x;
@@ -337,6 +346,12 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
         const uint32_t c = s_lo[L] + (f - s_pre[L]);
         const uint4 t = __ldg(topo + c);
         if (t.w != t.z) continue;
+        if (partial) {
+            uint32_t any = 0;
+            for (uint32_t i = t.x; i < t.y; ++i) any |= __ldg(active + i);
+            dirty[c] = (uint8_t)(any ? 1 : 0);
+            if (!any) continue;
+        }
         Mom m;
         leaf_moments(m, ld, t.x, t.y);
         mom_store(m, mom64, box, c);
@@ -347,7 +362,7 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
     // ---- owned nodes, deepest level first
     for (int L = nlev - 2; L >= 0; --L) {
         if (s_hin[L] == s_lo[L]) continue;                    // (uniform over the block)
-        node_pass(s_lo[L], s_hin[L], topo, mom64, box, ro, sx);
+        node_pass(s_lo[L], s_hin[L], topo, mom64, box, ro, sx, dirty, partial);
         __syncthreads();
     }
     TLM();
@@ -364,7 +379,7 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
 // level is spread over eight SMs.
 __global__ void __cluster_dims__(kSpanCtas, 1, 1) __launch_bounds__(kSpanThreads, 1)
 k_moments_span(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo, double* mom64, float* box,
-               const uint32_t* __restrict__ span, uint32_t nb, const RecOut ro) {
+               const uint32_t* __restrict__ span, uint32_t nb, const RecOut ro, uint8_t* dirty, int partial) {
     extern __shared__ __align__(16) unsigned char mom_smem[];
     SpanShared& sh = *reinterpret_cast<SpanShared*>(mom_smem);
     cg::cluster_group cluster = cg::this_cluster();
@@ -421,9 +436,19 @@ k_moments_span(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo
             uint32_t c = 0;
             uint4 t = make_uint4(0u, 0u, 0u, 0u);
             if (have) { c = sh.list[L][q]; t = sh.topo[L][q]; }
-            const int nch = have ? (int)(t.w - t.z) : 0;
+            int nch = have ? (int)(t.w - t.z) : 0;
+            bool clean = false;
+            if (partial) {                                              // all children clean: hand on what the cell arrays hold
+                uint32_t d = 0;
+                if (sub < nch) d = __ldcg(dirty + t.z + sub);
+                d |= __shfl_xor_sync(0xFFFFFFFFu, d, 1, 8); d |= __shfl_xor_sync(0xFFFFFFFFu, d, 2, 8); d |= __shfl_xor_sync(0xFFFFFFFFu, d, 4, 8);
+                if (have && sub == 0) dirty[c] = (uint8_t)(d ? 1 : 0);
+                clean = have && d == 0;
+                if (clean) nch = 0;
+            }
             Child ch;
             child_clear(ch);
+            if (clean && sub == 0) child_load_global(ch, mom64, box, c);   // (its own record, for the parent)
             if (sub < nch) {
                 const uint32_t cc = t.z + sub;
                 int lo2 = 0, hi2 = (int)cntb;
@@ -440,7 +465,16 @@ k_moments_span(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo
             }
             Mom m;
             node_moments8(m, ch, nch, sub, sh.sx[grp]);
-            if (have) {
+            if (clean) {
+                if (sub == 0) {
+                    SpanCell& o = sh.cell[cur][local];
+                    o.m[0] = ch.M; o.m[1] = ch.c[0]; o.m[2] = ch.c[1]; o.m[3] = ch.c[2];
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) o.m[4 + k] = ch.Q[k];
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) { o.b[k] = ch.bn[k]; o.b[3 + k] = ch.bx[k]; }
+                }
+            } else if (have) {
                 if (sub == 0) {
                     SpanCell& o = sh.cell[cur][local];
                     o.m[0] = m.M; o.m[1] = m.com[0]; o.m[2] = m.com[1]; o.m[3] = m.com[2];
@@ -494,7 +528,7 @@ int moments_init(bh_ctx* c) {
 }
 
 // theta > 0: the fp32 records are written in the same pass (c->rec_theta / rec_mac remember for which criterion).
-int stage_moments(bh_ctx* c, float theta, cudaStream_t s) {
+int stage_moments(bh_ctx* c, float theta, const uint8_t* d_active, cudaStream_t s) {
     const int64_t n = c->n;
     // particles per block: a multiple of the tree tile; one block per SM (one wave), at most kMomMaxBlocks blocks
     const int64_t nb_target = std::min<int64_t>(c->sm_count, kMomMaxBlocks);
@@ -503,9 +537,9 @@ int stage_moments(bh_ctx* c, float theta, cudaStream_t s) {
     const int tiles = (int)div_up(n + 1, kTreeTile);
     const bool rec = theta > 0.0f;
     BH_LAUNCH(c, k_moments, nb, kMomThreads, sizeof(NodeScratch) * kMomGroups, s, c->ws.sc, c->ws.pos[c->cur], (int)n, (int)P, tiles, c->ws.tile_cnt, c->ws.c_topo,
-              c->ws.mom64, c->ws.box, c->ws.mom_span, rec_out(c, theta, rec));
+              c->ws.mom64, c->ws.box, c->ws.mom_span, rec_out(c, theta, rec), d_active, c->ws.c_dirty);
     BH_LAUNCH(c, k_moments_span, kSpanCtas, kSpanThreads, sizeof(SpanShared), s, c->ws.sc, c->ws.c_topo, c->ws.mom64, c->ws.box,
-              c->ws.mom_span, (uint32_t)nb, rec_out(c, theta, rec));
+              c->ws.mom_span, (uint32_t)nb, rec_out(c, theta, rec), c->ws.c_dirty, d_active ? 1 : 0);
     c->rec_valid = rec;
     c->rec_theta = theta;
     c->rec_mac = c->mac_kind;

@@ -114,3 +114,125 @@ def test_call_order_and_arguments(BH):
     bh.set_particles(pm, vel)
     with pytest.raises(BhError):
         bh.refresh_moments()                                    # new particles: the old cells do not describe them
+
+
+# ------------------------------------------------------------------------------------------------ the scheme itself (A29)
+def _block_pair(BH, n, seed, R, eta, dt_max=1.0 / 16, theta=0.6, eps=0.02, **cfg):
+    """GPU context and oracle BlockState on the same particles, both initialised from the GPU's own fp32 forces."""
+    pm, vel, _ = bh_inputs.make("c1", n=n, seed=seed)
+    bh = BH(n, **cfg)
+    g = gpu_tree(bh, pm, vel, theta, eps)
+    bh.block_init(eps, eta, dt_max, R)
+    st = oracle.tree_build(pm, vel)
+    assert np.array_equal(st.pos, g["pos_mass"])
+    st.accpot = g["acc_pot"].astype(np.float64)           # the held accelerations are the GPU's fp32 values on both sides
+    bs = oracle.block_init(st, eps, eta, dt_max, R)
+    return bh, bs, theta, eps
+
+
+def _check_block_step(bh, bs, theta, eps, rebuild=False):
+    """One block step on both sides.  The oracle replays it from the same state, takes its integer decisions from the same
+    floats (the GPU's new accelerations), and everything but the forces must agree bit for bit."""
+    bh.block_step(theta, eps, rebuild=rebuild)
+    g = export_numpy(bh)
+    b = bh.block_state()
+    if rebuild:
+        # the oracle: active set + predictor on the old order, then a fresh tree of the moved particles; its block state follows its own sort
+        nxt, act = oracle.block_active(bs)
+        oracle.lib().orc_block_predict(oracle.C.c_int64(bs.tree.n), oracle._p(bs.pos), oracle._p(bs.vel), oracle._p(bs.accb), oracle._p(act),
+                                       oracle._p(bs.rung), oracle.C.c_float(bs.dt_max))
+        st = oracle.tree_build(bs.pos, bs.vel, bs.ids)
+        p = st.perm
+        bs.pos, bs.vel, bs.ids, bs.tree = st.pos, st.vel, st.ids, st.tree
+        bs.accb, bs.tick, bs.rung = bs.accb[p].copy(), bs.tick[p].copy(), bs.rung[p].copy()
+        act = act[p].copy()
+        assert np.array_equal(g["pos_mass"], bs.pos) and np.array_equal(g["id"].view(np.uint32), bs.ids)
+        t = bs.tree
+        sel = np.nonzero(np.add.reduceat(act.astype(np.int64), t.gbegin) > 0)[0].astype(np.int64)
+        r = oracle.walk_forces(t, bs.pos, theta, eps, sel=sel)
+        bs.npc, bs.npp, bs.acc_eval = r["npc"], r["npp"], r["accpot"]
+        oracle.lib().orc_block_correct(oracle.C.c_int64(t.n), oracle._p(bs.vel), oracle._p(bs.accb), oracle._p(np.ascontiguousarray(g["acc_pot"])),
+                                       oracle._p(act), oracle._p(bs.rung), oracle.C.c_float(bs.dt_max), oracle.C.c_uint32(nxt), oracle._p(bs.tick))
+        oracle.rungs(bs.accb, act, bs.len_scale, bs.eta, bs.dt_max, bs.R, nxt, out=bs.rung)
+        bs.now, bs.active = nxt, act
+    else:
+        bs = oracle.block_step(bs, theta, eps, acc_new=g["acc_pot"])
+    t = bs.tree
+    assert int(b["stats"].now_tick) == bs.now and int(b["stats"].n_active) == int(bs.active.sum())
+    assert np.array_equal(b["active"], bs.active)
+    assert np.array_equal(g["pos_mass"], bs.pos)                                  # predictor: bit-exact
+    assert np.array_equal(g["cell_mom64"], t.mom64) and np.array_equal(g["cell_box"], t.box)   # partial refresh == full recomputation
+    sel = np.nonzero(np.add.reduceat(bs.active.astype(np.int64), t.gbegin) > 0)[0]
+    st = oracle.State(bs.pos, bs.vel, bs.ids, None, None, None, 0, t, bs.npc, bs.npp, bs.acc_eval)
+    bad = compare_counts(g, st, sel=sel)
+    assert not bad, "\n".join(bad)
+    check_forces(g, st, sel=sel)
+    assert np.array_equal(g["vel"], bs.vel)                                       # corrector with the same new accelerations: bit-exact
+    assert np.array_equal(b["acc_held"], bs.accb) and np.array_equal(b["tick"], bs.tick) and np.array_equal(b["rung"], bs.rung)
+    return bs, b
+
+
+@pytest.mark.parametrize("n,R,eta,cfg", [(20000, 4, 0.2, {}), (4097, 3, 0.1, {}), (6000, 2, 0.3, dict(walk_mode=1)), (12000, 5, 0.15, dict(front_mode=1))])
+def test_block_steps_track_the_oracle(BH, n, R, eta, cfg):
+    bh, bs, theta, eps = _block_pair(BH, n, 83, R, eta, **cfg)
+    b0 = bh.block_state()
+    assert np.array_equal(b0["rung"], bs.rung) and len(set(bs.rung)) >= 2 and np.all(b0["tick"] == 0)
+    fractions = []
+    for step in range(6):
+        bs, b = _check_block_step(bh, bs, theta, eps)
+        fractions.append(int(b["stats"].n_active) / n)
+    assert min(fractions) < 0.8                                                   # steps move a subset only (L264)
+    assert b["stats"].interactions_now >= b["stats"].interactions_first > 0      # the cells only grow between rebuilds (L266)
+
+
+def test_block_step_with_a_rebuild(BH):
+    bh, bs, theta, eps = _block_pair(BH, 15000, 89, 3, 0.2)
+    for step in range(5):
+        bs, b = _check_block_step(bh, bs, theta, eps, rebuild=(step == 2))
+        assert int(b["stats"].steps_since_rebuild) == (step + 1 if step < 2 else step - 1)
+    assert b["stats"].interactions_first > 0
+
+
+def test_block_scheme_reaches_the_macro_step_and_conserves_energy(BH):
+    pm, vel, _ = bh_inputs.make("c1", n=8192, seed=97)
+    theta, eps, R = 0.4, 0.05, 3
+    bh = BH(8192)
+    g0 = gpu_tree(bh, pm, vel, theta, eps)
+    bh.block_init(eps, 0.1, 1.0 / 16, R)
+
+    def energy(g):
+        d = oracle.direct(g["pos_mass"], eps)
+        m = g["pos_mass"][:, 3].astype(np.float64)
+        return 0.5 * np.sum(m * np.sum(g["vel"][:, :3].astype(np.float64) ** 2, axis=1)) + 0.5 * np.sum(m * d[:, 3])
+
+    e0 = energy(g0)
+    steps = 0
+    while True:
+        bh.block_step(theta, eps)
+        steps += 1
+        if int(bh.block_state(arrays=False)["stats"].now_tick) >= 1 << R:
+            break
+    b = bh.block_state()
+    assert np.all(b["tick"] == 1 << R) and 2 <= steps <= 1 << R                 # everybody is synchronised at the end of the longest step
+    assert abs((energy(export_numpy(bh)) - e0) / e0) < 2e-4
+
+
+def test_block_call_order(BH):
+    from paper_1106_1900_b200 import BhError
+    pm, vel, prm = bh_inputs.make("c1", n=3000, seed=101)
+    bh = BH(3000)
+    bh.set_particles(pm, vel)
+    bh.tree_build()
+    with pytest.raises(BhError):
+        bh.block_init(0.01, 0.2, 1 / 16, 3)                 # no forces yet
+    with pytest.raises(BhError):
+        bh.block_step(0.5, 0.01)                            # not initialised
+    bh.compute_forces(0.5, 0.01)
+    for bad in ((0.0, 0.2, 1 / 16, 3), (0.01, 0.0, 1 / 16, 3), (0.01, 0.2, 0.0, 3), (0.01, 0.2, 1 / 16, 21)):
+        with pytest.raises(BhError):
+            bh.block_init(*bad)
+    bh.block_init(0.01, 0.2, 1 / 16, 3)
+    bh.block_step(0.5, 0.01)
+    bh.set_particles(pm, vel)
+    with pytest.raises(BhError):
+        bh.block_step(0.5, 0.01)                            # new particles: the block state is gone
