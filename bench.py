@@ -98,6 +98,15 @@ def _workload(args):
     return cfg, n
 
 
+WORKLOADS = {"c1": "Plummer sphere", "c2": "Plummer sphere", "c3": "uniform cube", "c4": "three-component galaxy (NFW halo + exponential disk + Hernquist bulge)",
+             "c5": "two colliding Plummer spheres"}
+
+
+def workload_name(cfg: str, n: int) -> str:
+    """The same string in both arms (ours / reference), so that the driver can see that they ran the same workload."""
+    return f"{cfg}: {WORKLOADS[cfg]} n={n}"
+
+
 def rank_seed(cfg: str, rank: int) -> int:
     """Every rank steps its own replica of the workload: same recipe, different seed."""
     return bh_inputs.SEEDS[cfg] + 1000 * rank
@@ -180,7 +189,7 @@ def run_reference(args):
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * n / v,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": v / PAPER_PARTICLES_PER_S if cfg == "c2" and abs(theta - 0.75) < 1e-6 else None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{cfg}: {n} particles, theta={theta}, eps={prm['eps']}, dt={prm['dt']}", "nleaf": 16, "ncrit": 64},
+            "config": {"workload": workload_name(cfg, n), "theta": theta, "eps": prm["eps"], "dt": prm["dt"], "nleaf": 16, "ncrit": 64},
             "cpu_baseline": {"value": v, "unit": "particles/s", "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
             "e2e": {"value": v, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -330,10 +339,10 @@ def run_ours(args):
                          "cells), bh_refresh_moments_active (only the cells above an active particle), and refresh + bh_compute_forces_active "
                          "(S7 + S8 of the groups with an active particle); compare with build_ms and stages_ms.walk"}
         # (b) the scheme itself (A29): one macro-step dt of individual power-of-two steps, rebuilding when the lists have grown
-        R, eta, growth = 4, 0.3, 1.10
+        R, eta, growth, dt_macro = 6, 0.3, 1.10, 16.0 * dt
         bh.tree_build()
         bh.compute_forces(theta, eps)
-        bh.block_init(eps, eta, dt, R)
+        bh.block_init(eps, eta, dt_macro, R)
         rung0 = np.bincount(bh.block_state()["rung"], minlength=R + 1).tolist()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
@@ -347,12 +356,12 @@ def run_ours(args):
             if int(bst.now_tick) >= 1 << R:
                 break
         sec = time.perf_counter() - t0
-        block["scheme"] = {"max_rung": R, "eta": eta, "len_scale": eps, "dt_max": dt, "particles_per_rung_at_start": rung0, "block_steps": steps,
+        block["scheme"] = {"max_rung": R, "eta": eta, "len_scale": eps, "dt_max": dt_macro, "particles_per_rung_at_start": rung0, "block_steps": steps,
                            "rebuilds": rebuilds, "rebuild_rule": f"interactions of the walked groups > {growth} x what they were when first walked on the cells",
                            "particle_updates": updated, "mean_active_fraction": updated / (steps * n), "seconds": sec,
                            "particle_updates_per_s": updated / sec, "ms_per_block_step": 1e3 * sec / steps,
-                           "shared_step_equivalent": "the same accuracy with one shared step needs 2^R full steps per macro-step",
-                           "updates_saved_vs_shared_smallest_step": (n * (1 << R)) / max(updated, 1)}
+                           "shared_step_equivalent": "one shared step as short as the shortest step in use would need 2^(deepest rung in use) full steps per macro-step",
+                           "updates_saved_vs_shared_smallest_step": (n * (1 << max(i for i, c in enumerate(rung0) if c))) / max(updated, 1)}
         bh.set_particles(pm, vel)            # leave the context in the plain state for the legs below
         bh.tree_build(); bh.compute_forces(theta, eps)
 
@@ -462,7 +471,7 @@ def run_ours(args):
         "higher_is_better": True, "scaling": "strong" if sharded else "weak",
         "vs_baseline": value / PAPER_PARTICLES_PER_S if (cfg == "c2" and abs(theta - 0.75) < 1e-6 and world == 1) else None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{cfg}: Plummer sphere n={n}" if cfg in ("c1", "c2") else f"{cfg}: n={n}",
+        "config": {"workload": workload_name(cfg, n),
                    "theta": theta, "eps": eps, "dt": dt, "nleaf": 16, "ncrit": 64, "mac": "min_distance" if args.mac else "eq1", "rebuild_every_step": True,
                    "step": "bh_step_graph_launch (bh_leapfrog_step captured into a CUDA graph)" if use_graph else "bh_leapfrog_step",
                    "l2": f"{L2_FLUSH_BYTES >> 20} MiB buffer written between timed steps (outside the event pairs)",

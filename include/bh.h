@@ -101,6 +101,9 @@ typedef struct bh_tree_view {
     const float*    cell_box;      /* float[C][6]: min xyz, max xyz (S6) */
     const float*    cell_mom32;    /* float[C][10]: the fp32 roundings used by the walk; valid after bh_compute_forces */
     const float*    cell_r2open;   /* float[C]: (l/theta + delta)^2 (Eq.1); valid after bh_compute_forces */
+    const float*    cell_trec;     /* float[C][4]: what a MAC test of the walk reads: (com xyz as fp32, r2open); valid after bh_compute_forces */
+    const float*    cell_erec;     /* float[C][12]: what an accepted cell costs the force loop (S8): (com xyz, M) (-3Qxx, -3Qyy, -3Qzz, -3Qxy)
+                                    * (-3Qxz, -3Qyz, -T/2, -3T/2), T = Qxx + Qyy + Qzz, every entry one fp32 operation on the fp32 roundings */
     const uint32_t* group_begin;   /* uint32[G+1]: first particle of each group; group_begin[G] = n (S5) */
     const uint32_t* group_cell;    /* uint32[G]: the cell a group comes from */
     const uint32_t* group_npc;     /* uint32[G]: accepted cells per group (S7); valid after bh_compute_forces */

@@ -49,7 +49,7 @@ class BhBlockStats(C.Structure):
 
 _VIEW_FIELDS = ["pos_mass", "vel", "acc_pot", "id", "key", "perm", "level_offset", "cell_level", "cell_prefix",
                 "cell_pbegin", "cell_pcount", "cell_child_begin", "cell_nchild", "cell_parent", "cell_mom64", "cell_box",
-                "cell_mom32", "cell_r2open", "group_begin", "group_cell", "group_npc", "group_npp"]
+                "cell_mom32", "cell_r2open", "cell_trec", "cell_erec", "group_begin", "group_cell", "group_npc", "group_npp"]
 
 
 class BhTreeView(C.Structure):
@@ -385,6 +385,8 @@ class BarnesHut:
         out["cell_box"] = self._view(v.cell_box, nc * 6, f32, (nc, 6))
         out["cell_mom32"] = self._view(v.cell_mom32, nc * 10, f32, (nc, 10))
         out["cell_r2open"] = self._view(v.cell_r2open, nc, f32)
+        out["cell_trec"] = self._view(v.cell_trec, nc * 4, f32, (nc, 4))
+        out["cell_erec"] = self._view(v.cell_erec, nc * 12, f32, (nc, 12))
         out["group_begin"] = self._view(v.group_begin, ng + 1, i32)
         out["group_cell"] = self._view(v.group_cell, ng, i32)
         out["group_npc"] = self._view(v.group_npc, ng, i32)

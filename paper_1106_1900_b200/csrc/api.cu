@@ -527,6 +527,8 @@ int bh_export_tree(bh_ctx* c, bh_tree_view* v, void* stream) {
     v->cell_box = w.box;
     v->cell_mom32 = w.e_mom32;
     v->cell_r2open = w.e_r2open;
+    v->cell_trec = reinterpret_cast<const float*>(w.trec);
+    v->cell_erec = reinterpret_cast<const float*>(w.erec);
     v->group_begin = w.g_begin;
     v->group_cell = w.g_cell;
     v->group_npc = w.g_npc;

@@ -334,8 +334,35 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
     float4* spos = reinterpret_cast<float4*>(mom_smem);
     const uint32_t p0 = b * (uint32_t)P;
     const uint32_t staged = P <= kMomStage ? min((uint32_t)P, (uint32_t)n - min((uint32_t)n, p0)) : 0u;
+#ifdef BH_NO_TMA
     for (uint32_t i = tid; i < staged; i += kMomThreads) spos[i] = __ldg(pos + p0 + i);
     __syncthreads();
+#else
+    // one contiguous run of up to 128 KB: a 1-D bulk copy (TMA, cp.async.bulk) issued by one thread and completed on an
+    // mbarrier, instead of seven 16-byte loads and stores per thread (A/B: -DBH_NO_TMA)
+    __shared__ __align__(8) unsigned long long s_bar;
+    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&s_bar);
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0 && staged) {
+        const uint32_t bytes = staged * 16u;
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+        for (uint32_t off = 0; off < bytes; off += 32768u) {
+            const uint32_t len = min(32768u, bytes - off);
+            const uint32_t dst = (uint32_t)__cvta_generic_to_shared(mom_smem + off);
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(dst), "l"(reinterpret_cast<const unsigned char*>(pos + p0) + off), "r"(len), "r"(bar) : "memory");
+        }
+    }
+    if (staged) {
+        uint32_t done = 0;
+        while (!done)
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(bar) : "memory");
+    }
+#endif
     auto ld = [&](uint32_t i) -> float4 { return (i - p0 < staged) ? spos[i - p0] : __ldg(pos + i); };
     // ---- leaves: one thread each
     const uint32_t total = s_pre[kLevels];

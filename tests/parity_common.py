@@ -75,6 +75,15 @@ def compare_tree(g, st, problems=None, check_vel=True):
     if st.mom32 is not None:
         eq("cell_mom32", g["cell_mom32"].view(np.uint32), st.mom32.view(np.uint32))
         eq("cell_r2open", g["cell_r2open"].view(np.uint32), np.ascontiguousarray(st.mac[:, 2]).view(np.uint32))
+        # the records the walk kernels really read (not a re-export): MAC record and evaluation record, from the oracle's fp32 moments
+        m = st.mom32
+        f = np.float32
+        T = ((m[:, 4] + m[:, 5]).astype(f) + m[:, 6]).astype(f)
+        trec = np.column_stack([m[:, 1], m[:, 2], m[:, 3], st.mac[:, 2]]).astype(f)
+        erec = np.column_stack([m[:, 1], m[:, 2], m[:, 3], m[:, 0], f(-3) * m[:, 4], f(-3) * m[:, 5], f(-3) * m[:, 6], f(-3) * m[:, 7],
+                                f(-3) * m[:, 8], f(-3) * m[:, 9], f(-0.5) * T, f(-1.5) * T]).astype(f)
+        eq("cell_trec", g["cell_trec"].view(np.uint32), np.ascontiguousarray(trec).view(np.uint32))
+        eq("cell_erec", g["cell_erec"].view(np.uint32), np.ascontiguousarray(erec).view(np.uint32))
     return bad
 
 

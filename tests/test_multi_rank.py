@@ -170,7 +170,7 @@ def test_balanced_shares_two_ranks_gloo(tmp_path):
     assert r.returncode == 0, r.stderr[-2000:]
     import json
     import re
-    outs = sorted((json.loads(m) for m in re.findall(r"RANKOUT (\{.*?\})\n", r.stdout)), key=lambda o: o["rank"])
+    outs = sorted((json.loads(m) for m in re.findall(r"RANKOUT (\{[^{}]*\})", r.stdout)), key=lambda o: o["rank"])
     assert [o["rank"] for o in outs] == [0, 1]
     assert all(o["equal"] and o["work_ok"] for o in outs)
     assert outs[0]["bounds"] == outs[1]["bounds"] and outs[0]["bounds"][1] != 3000        # every rank derives the same, moved boundary
