@@ -38,7 +38,9 @@ typedef enum bh_status {
     BH_ERR_INVALID_ARG = -1, /* null pointer, n <= 0, n > n_max, theta <= 0 or non-finite, eps < 0, non-finite dt, bad config */
     BH_ERR_WORKSPACE = -2,   /* workspace too small or not device memory */
     BH_ERR_STATE = -3,       /* forces before build, step before forces, build before particles */
-    BH_ERR_CUDA = -4,        /* a CUDA runtime call failed (bh_last_cuda_error gives the code) */
+    BH_ERR_CUDA = -4,        /* a CUDA runtime call failed (bh_last_cuda_error gives the code); also the deferred status when a
+                              * bounded device-side wait (grid barrier of the front end, look-back of a sort pass) ran out:
+                              * the kernels then finish without writing out of bounds, but the build is not valid */
     BH_ERR_NONFINITE = -5,   /* deferred: NaN/Inf position or mass <= 0 seen by S0 (A27) */
     BH_ERR_CAPACITY = -6     /* deferred: more cells than max_cells */
 } bh_status;
@@ -126,7 +128,9 @@ int bh_destroy(bh_ctx* ctx);
  * next bh_tree_build / bh_get_particles (or a synchronisation after it) has completed. */
 int bh_set_particles(bh_ctx* ctx, int64_t n, const float* pos_mass, const float* vel, const uint32_t* id, void* stream);
 
-/* Copy the current (key-sorted) state out; any pointer may be NULL; host or device destinations. */
+/* Copy the current (key-sorted) state out; any pointer may be NULL; host or device destinations.  BH_ERR_STATE when
+ * acc_pot is asked for between a bh_tree_build (which re-sorts the particles) and the next force evaluation: the stored
+ * accelerations would be in the previous order. */
 int bh_get_particles(bh_ctx* ctx, float* pos_mass, float* vel, float* acc_pot, uint32_t* id, void* stream);
 
 /* S0-S6: domain, keys, sort, reorder, octree, groups, fp64 moments and boxes (L55-65, L107-115).  theta-independent. */
@@ -220,10 +224,14 @@ int bh_sync_status(bh_ctx* ctx, void* stream, bh_stats* out);
 /* Fill `out` with device pointers to the canonical tree arrays (see bh_tree_view). */
 int bh_export_tree(bh_ctx* ctx, bh_tree_view* out, void* stream);
 
-/* Per-stage device times of the last bh_tree_build + bh_compute_forces, in ms, when enabled (adds event records,
- * do not enable under graph capture).  Order: bbox, keys, sort, reorder, cells, groups, moments, record (fp32 walk
- * records + opening radii), walk (S7 + S8: list walk, evaluation, fallback kernel), lists (k_walk_lists alone), eval
- * (k_walk_eval alone); the last two are 0 when the walk ran as a pipeline of several waves (the kernels overlap: see
+/* Per-stage device times of the last bh_tree_build + bh_compute_forces, in ms, when enabled (adds event records; a step
+ * captured by bh_step_graph_build while timing is enabled records them on every replay).  Order: bbox, keys, sort,
+ * reorder, cells, groups, moments, record, walk, lists, eval.  The stages are timed in the groups they are launched in:
+ * with the one-launch front end (front_mode 0, n <= 1.2 M) "sort" is the whole of S0-S3 (k_front) and bbox, keys, reorder
+ * read ~0; "cells" = k_bounds + k_scan_rows, "groups" = k_emit (cells and groups are emitted together); "moments" = S6
+ * including the fp32 walk records when theta is known at build time ("record" then reads ~0; otherwise it is
+ * k_cell_record); walk = S7 + S8 (list walk, evaluation, fallback kernel), lists = k_walk_lists alone, eval =
+ * k_walk_eval alone; the last two are 0 when the walk ran as a pipeline of several waves (the kernels overlap: see
  * bh_get_walk_timeline).  Synchronises. */
 int bh_set_stage_timing(bh_ctx* ctx, int enable);
 int bh_get_stage_ms(bh_ctx* ctx, float ms[11]);
