@@ -254,7 +254,7 @@ def run_ours(args):
         from paper_1106_1900_b200 import ShardedBarnesHut
         bh = ShardedBarnesHut(n, max_cells=args.max_cells, list_entries=args.list_entries, walk_waves=args.walk_waves)
     else:
-        bh = BarnesHut(n, max_cells=args.max_cells, list_entries=args.list_entries, walk_waves=args.walk_waves)
+        bh = BarnesHut(n, max_cells=args.max_cells, list_entries=args.list_entries, walk_waves=args.walk_waves, walk_private=int(args.walk_private))
     bh.set_particles(pm, vel)
     bh.set_mac(args.mac)
     bh.tree_build()
@@ -521,6 +521,7 @@ def main():
     ap.add_argument("--no-cpu", dest="no_cpu", action="store_true")
     ap.add_argument("--no-e2e", dest="no_e2e", action="store_true", help="skip the host-buffer leg (for profiling runs)")
     ap.add_argument("--probe-fp32", dest="probe_fp32", action="store_true", help="only run the FP32 issue-rate probes (bh_probe_fp32) and print them")
+    ap.add_argument("--walk-private", dest="walk_private", action="store_true", help="every group walks from the root on its own (no shared super-group walk)")
     ap.add_argument("--no-graph", dest="no_graph", action="store_true", help="time plain bh_leapfrog_step launches instead of the captured step")
     ap.add_argument("--dry-run-ranks", dest="dry_run_ranks", action="store_true",
                     help="only start the ranks, join them in a process group (nccl on GPUs, gloo without) and let rank 0 report the world size")

@@ -59,6 +59,10 @@ typedef struct bh_config {
                          * wave w on internal streams); 0..255 */
     int32_t front_mode; /* 0 (default): S0-S3 in one cooperative launch whenever every sort tile is resident at once
                          * (n <= 4096 x 2 x SMs, 1.2 M on B200); 1: always one launch per step and sort pass (any n) */
+    int32_t walk_private; /* 0 (default): the eight groups of a block share the common part of their walks (cells every one of
+                           * them accepts / opens, decided once against the union of their boxes; exact, see walk_lists.cu);
+                           * 1: every group walks from the root on its own.  Counts are identical; the order of the list
+                           * entries, and with it the last bits of the fp32 sums, differs between the two */
 } bh_config;
 
 typedef struct bh_ctx bh_ctx;

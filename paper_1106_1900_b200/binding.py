@@ -28,7 +28,7 @@ SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", 
 
 class BhConfig(C.Structure):
     _fields_ = [("nleaf", C.c_int32), ("ncrit", C.c_int32), ("max_cells", C.c_int64), ("list_entries", C.c_int64),
-                ("walk_mode", C.c_int32), ("walk_waves", C.c_int32), ("front_mode", C.c_int32)]
+                ("walk_mode", C.c_int32), ("walk_waves", C.c_int32), ("front_mode", C.c_int32), ("walk_private", C.c_int32)]
 
 
 class BhStats(C.Structure):
@@ -123,8 +123,8 @@ def load_library():
 
 
 def workspace_bytes(n_max: int, nleaf: int = 0, ncrit: int = 0, max_cells: int = 0, list_entries: int = 0, walk_mode: int = 0,
-                    walk_waves: int = 0, front_mode: int = 0) -> int:
-    cfg = BhConfig(nleaf, ncrit, max_cells, list_entries, walk_mode, walk_waves, front_mode)
+                    walk_waves: int = 0, front_mode: int = 0, walk_private: int = 0) -> int:
+    cfg = BhConfig(nleaf, ncrit, max_cells, list_entries, walk_mode, walk_waves, front_mode, walk_private)
     return int(load_library().bh_workspace_bytes(n_max, C.byref(cfg)))
 
 
@@ -186,12 +186,12 @@ class BarnesHut:
     """One Barnes-Hut context on one GPU: same calls as include/bh.h (bh_tree_build, bh_compute_forces, bh_leapfrog_step)."""
 
     def __init__(self, n_max: int, nleaf: int = 0, ncrit: int = 0, max_cells: int = 0, list_entries: int = 0, walk_mode: int = 0,
-                 walk_waves: int = 0, front_mode: int = 0, device=None):
+                 walk_waves: int = 0, front_mode: int = 0, walk_private: int = 0, device=None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1106_1900_b200 needs a CUDA device: there is no CPU fallback")
         self.lib = load_library()
         self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
-        cfg = BhConfig(nleaf, ncrit, max_cells, list_entries, walk_mode, walk_waves, front_mode)
+        cfg = BhConfig(nleaf, ncrit, max_cells, list_entries, walk_mode, walk_waves, front_mode, walk_private)
         nbytes = int(self.lib.bh_workspace_bytes(n_max, C.byref(cfg)))
         if nbytes == 0:
             raise BhError(-1, "bad n_max / config")

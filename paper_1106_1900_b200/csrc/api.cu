@@ -22,7 +22,7 @@ struct Carver {
 
 struct Geometry {
     int64_t n_max, max_cells, sort_tiles, tree_tiles, list_entries;
-    int32_t nleaf, ncrit, walk_mode, walk_waves, front_mode;
+    int32_t nleaf, ncrit, walk_mode, walk_waves, front_mode, walk_private;
 };
 
 static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
@@ -42,6 +42,8 @@ static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
     if (g->walk_mode < 0 || g->walk_mode > 1) return false;
     g->walk_waves = cfg ? cfg->walk_waves : 0;
     if (g->walk_waves < 0 || g->walk_waves > kMaxWaves) return false;
+    g->walk_private = cfg ? cfg->walk_private : 0;
+    if (g->walk_private < 0 || g->walk_private > 1) return false;
     g->front_mode = cfg ? cfg->front_mode : 0;
     if (g->front_mode < 0 || g->front_mode > 1) return false;
     g->sort_tiles = div_up(n_max, kSortTile);
@@ -158,6 +160,7 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
     c->sort_tiles = g.sort_tiles;
     c->tree_tiles = g.tree_tiles;
     c->front_enabled = g.front_mode == 0;
+    c->walk_share = g.walk_private ? 0 : 1;
     carve(g, static_cast<unsigned char*>(d_workspace), &c->ws);
     int rc = BH_OK;
     do {

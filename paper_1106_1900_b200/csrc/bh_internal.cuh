@@ -161,6 +161,7 @@ struct bh_ctx {
     int64_t list_entries;
     int walk_mode;
     int walk_waves;
+    int walk_share;        // 1: the groups of a block of eight share the common part of their walks (walk_lists.cu)
     int mac_kind;          // 0: Eq.1, 1: minimum distance (bh_set_mac)
     bh::Ws ws;
     int64_t sort_tiles, tree_tiles;

@@ -28,8 +28,14 @@ namespace bh {
 
 constexpr int kEvalWarps = 4;
 constexpr int kEvalThreads = kEvalWarps * 32;
-constexpr int kEvalBlocksPerSM = 4;          // 16 warps / SM at <= 128 registers
-constexpr int kBatch = 128;                  // list entries per batch
+#ifndef BH_EVAL_BLOCKS
+#define BH_EVAL_BLOCKS 4
+#endif
+constexpr int kEvalBlocksPerSM = BH_EVAL_BLOCKS;          // 4: 16 warps / SM at <= 128 registers
+#ifndef BH_EVAL_BATCH
+#define BH_EVAL_BATCH 128
+#endif
+constexpr int kBatch = BH_EVAL_BATCH;        // list entries per batch
 constexpr int kPerLane = kBatch / 32;        // entries a lane gathers per batch
 
 struct __align__(16) EvalShared {

@@ -71,103 +71,243 @@ __device__ __forceinline__ bool flush_leaves(const uint2* q, int k, int lane, ui
     return true;
 }
 
+// ---- the walk of a SUPER-GROUP: kSG consecutive groups share the part of the walk that is the same for all of them.
+// For the union box U of the groups (G inside U for every member G) the fp32 test of O9 is monotone: the per-axis distances
+// of G are >= those of U, and <= e_k = max(Umax_k - com_k, com_k - Umin_k); hence
+//     d2(U) >  r2open   =>  every member accepts the cell          (d2(G) >= d2(U), each operation rounds monotonically)
+//     D2(U) <= r2open   =>  no member accepts it: opened by all    (d2(G) <= D2(U) = fma chain over e_k)
+// and only the cells in between ("ambiguous") must be tested by every member on its own.  One warp walks the tree once
+// with these two tests: cells accepted by all -> shared cell list, leaves opened by all -> shared particle list (unless the
+// leaf holds particles of the super-group itself: own particles are cut out per member, A19), ambiguous cells -> frontier.
+// Every member then copies the shared lists into its own lists (4 bytes per entry against ~120 instructions per MAC
+// test and append) and continues the walk from the frontier with its own box.  The lists are sets, so the counts are
+// exactly those of O9; which groups form a super-group depends on the group index only, never on the active subset.
+#ifndef BH_SG
+#define BH_SG 8
+#endif
+constexpr int kSG = BH_SG;              // groups per super-group
+constexpr int kAmbCap = 384;
+struct SharedWalk {                     // the result of a shared walk: the two shared lists sit in the list region like a group's
+    uint32_t amb[kAmbCap];
+    uint32_t spc_off, n_spc, spp_off, n_spp, n_amb, leafsum, ok;
+};
+
+__device__ __forceinline__ void sg_classify(const float mn[3], const float mx[3], const float4& r, bool& acc_all, bool& open_all) {
+    const float ax = __fsub_rn(mn[0], r.x), bx = __fsub_rn(r.x, mx[0]);
+    const float ay = __fsub_rn(mn[1], r.y), by = __fsub_rn(r.y, mx[1]);
+    const float az = __fsub_rn(mn[2], r.z), bz = __fsub_rn(r.z, mx[2]);
+    const float dx = fmaxf(fmaxf(ax, bx), 0.0f), dy = fmaxf(fmaxf(ay, by), 0.0f), dz = fmaxf(fmaxf(az, bz), 0.0f);
+    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+    // e_k = max(Umax_k - com_k, com_k - Umin_k) = max(-bx, -ax): the same roundings, negated
+    const float ex = fmaxf(-bx, -ax), ey = fmaxf(-by, -ay), ez = fmaxf(-bz, -az);
+    const float D2 = __fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex)));
+    acc_all = d2 > r.w;
+    open_all = !(D2 > r.w);
+}
+
+// The shared walk of one super-group (one warp).  The shared lists are written into this warp's chunk of the list region
+// (cells upward from pc_top, particles downward from pp_bot, like a group's lists) and stay allocated; sw->ok = 0 when
+// they do not fit or the frontier overflows: the members then walk alone.
+__device__ __noinline__ void shared_walk(ListWarpShared* ws, SharedWalk* sw, const int lane, const float mn[3], const float mx[3],
+                                         const uint32_t sb, const uint32_t se, const float4* __restrict__ trec, const uint2* __restrict__ tlink,
+                                         uint32_t* __restrict__ lists, ListArena& ar, WalkSums& sums) {
+    const uint32_t lt = (1u << lane) - 1u;
+    const uint32_t pc0 = ar.pc_top, pp0 = ar.pp_bot;
+    uint32_t pc_top = pc0, pp_bot = pp0;
+    uint32_t n_amb = 0, leafsum = 0, nmac = 0;
+    bool ok = pp0 > pc0;
+    int sp = 1;
+    if (lane == 0) ws->stack[0] = make_uint2(0u, 1u);
+    __syncwarp();
+    while (sp > 0 && ok) {
+        int kpop = (kLStackCap - kLStackReserve - sp) / 7;
+        kpop = max(1, min(kpop, 4));
+        kpop = min(kpop, sp);
+        const int r = lane >> 3, c8 = lane & 7;
+        bool valid = false;
+        uint32_t cell = 0u;
+        if (r < kpop) {
+            const uint2 e = ws->stack[sp - 1 - r];
+            valid = (uint32_t)c8 < e.y;
+            cell = e.x + (uint32_t)c8;
+        }
+        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f);
+        uint2 lk = make_uint2(0u, 0u);
+        if (valid) { r0 = __ldg(trec + cell); lk = __ldg(tlink + cell); }
+        sp -= kpop;
+        __syncwarp();
+        bool acc_all = false, open_all = false;
+        sg_classify(mn, mx, r0, acc_all, open_all);
+        acc_all = acc_all && valid;
+        const bool isleaf = (lk.y >> 31) != 0u;
+        const uint32_t first = lk.x, cnt = lk.y & 0x7FFFFFFFu;
+        const bool opened_node = valid && !acc_all && open_all && !isleaf;
+        const bool opened_leaf = valid && !acc_all && open_all && isleaf && !(first < se && first + cnt > sb);   // no particle of the super-group in it
+        const bool amb = valid && !acc_all && !opened_node && !opened_leaf;
+        nmac += (uint32_t)__popc(__ballot_sync(0xFFFFFFFFu, valid));
+        const uint32_t amask = __ballot_sync(0xFFFFFFFFu, acc_all);
+        if (amask) {
+            if (pc_top + __popc(amask) > pp_bot) { ok = false; break; }
+            if (acc_all) lists[pc_top + __popc(amask & lt)] = cell;
+            pc_top += __popc(amask);
+        }
+        const uint32_t nmask = __ballot_sync(0xFFFFFFFFu, opened_node);
+        if (opened_node) ws->stack[sp + __popc(nmask & lt)] = lk;
+        sp += __popc(nmask);
+        const uint32_t bmask = __ballot_sync(0xFFFFFFFFu, amb);
+        if (bmask) {
+            if (n_amb + __popc(bmask) > kAmbCap) { ok = false; break; }
+            if (amb) sw->amb[n_amb + __popc(bmask & lt)] = cell;
+            n_amb += __popc(bmask);
+        }
+        const uint32_t lmask = __ballot_sync(0xFFFFFFFFu, opened_leaf);
+        if (lmask) {                                                     // the leaf's particles -> shared particle list
+            int total;
+            const int off = warp_excl_scan(opened_leaf ? (int)cnt : 0, lane, total);
+            if ((uint32_t)total > pp_bot - pc_top) { ok = false; break; }
+            pp_bot -= (uint32_t)total;
+            if (opened_leaf)
+                for (uint32_t t = 0; t < cnt; ++t) lists[pp_bot + off + t] = first + t;
+            leafsum += (uint32_t)total;
+        }
+        __syncwarp();
+    }
+    if (ok) { ar.pc_top = pc_top; ar.pp_bot = pp_bot; sums.mac += nmac; }     // the shared lists stay allocated
+    if (lane == 0) {
+        sw->spc_off = pc0; sw->n_spc = pc_top - pc0; sw->spp_off = pp_bot; sw->n_spp = pp0 - pp_bot;
+        sw->n_amb = n_amb; sw->leafsum = leafsum; sw->ok = ok ? 1u : 0u;
+    }
+    __syncwarp();
+}
+
+// The walk of one group; `sw` != nullptr: continue from the shared walk of its super-group instead of starting at the root.
 template <int kMac>
 __device__ __forceinline__ bool list_group(ListWarpShared* ws, const int lane, const uint32_t g, const uint32_t gb, const uint32_t ge,
-                                           const float4* __restrict__ pos, const float4* __restrict__ trec, const uint2* __restrict__ tlink,
-                                           const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
-                                           const uint4* __restrict__ c_topo,
+                                           const float mn[3], const float mx[3], const SharedWalk* sw,
+                                           const float4* __restrict__ trec, const uint2* __restrict__ tlink,
+                                           const float* __restrict__ box,
                                            uint32_t* __restrict__ lists, ListArena& ar, WalkListOut o, WalkSums& sums) {
     const uint32_t lt = (1u << lane) - 1u;
     const int ng = (int)(ge - gb);
-    // ---- group box (A13).  A group that is a whole cell has that cell's box (exact min / max of the same particles);
-    //      a chunk of a level-20 overflow leaf takes it from its particles.
-    float mn[3], mx[3];
-    {
-        const uint32_t gc = __ldg(g_cell + g);
-        const uint2 pr = __ldg(reinterpret_cast<const uint2*>(c_topo + gc));     // (first particle, end particle) of the group's cell
-        if (pr.y - pr.x == (uint32_t)ng) {
-            const float* b = box + 6 * (size_t)gc;
-            mn[0] = __ldg(b); mn[1] = __ldg(b + 1); mn[2] = __ldg(b + 2);
-            mx[0] = __ldg(b + 3); mx[1] = __ldg(b + 4); mx[2] = __ldg(b + 5);
-        } else {
-            group_box(pos, gb, ng, lane, nullptr, mn, mx);
-        }
-    }
-
     const uint32_t pc0 = ar.pc_top, pp0 = ar.pp_bot;
     uint32_t pc_top = pc0, pp_bot = pp0;
     uint32_t npp = 0, nmac = 0;
     bool fits = true;
-    int sp = 1, lq = 0;
-    if (lane == 0) ws->stack[0] = make_uint2(0u, 1u);   // the root (A17) as the only child of a virtual node
-    __syncwarp();
+    int sp = 0, lq = 0;
 
-    while (sp > 0 && fits) {
-        // pop up to 4 kSub nodes; lane = (node r of a sub-batch, child c8); all records are requested before any is used
-        int kpop = (kLStackCap - kLStackReserve - sp) / 7;
-        kpop = max(1, min(kpop, 4 * kSub));
-        kpop = min(kpop, sp);
-        const int r = lane >> 3, c8 = lane & 7;
-        bool valid[kSub];
-        uint32_t cell[kSub];
-        float4 r0[kSub];
-        uint2 lk[kSub];
-        CellBox cbx[kMac == kMacMinDist ? kSub : 1];
-#pragma unroll
-        for (int j = 0; j < kSub; ++j) {
-            valid[j] = false;
-            cell[j] = 0u;
-            const int idx = 4 * j + r;
-            if (idx < kpop) {
-                const uint2 e = ws->stack[sp - 1 - idx];
-                valid[j] = (uint32_t)c8 < e.y;
-                cell[j] = e.x + (uint32_t)c8;
+    // one test + append of a cell by every lane that holds one (cell, r0, lk valid where `valid`)
+    auto classify = [&](bool valid, uint32_t cell, const float4& r0, const uint2& lk, const CellBox& cbx) -> bool {
+        const bool accept = valid && (kMac == kMacMinDist ? mac_accept_box(mn, mx, cbx, r0.w) : mac_accept(mn, mx, r0));
+        const bool isleaf = valid && !accept && (lk.y >> 31) != 0u;
+        const bool isnode = valid && !accept && !isleaf;
+        nmac += (uint32_t)__popc(__ballot_sync(0xFFFFFFFFu, valid));
+        // ---- accepted cells -> cell list
+        const uint32_t amask = __ballot_sync(0xFFFFFFFFu, accept);
+        if (amask) {
+            const uint32_t na = (uint32_t)__popc(amask);
+            if (pc_top + na > pp_bot) return false;
+            if (accept) lists[pc_top + (uint32_t)__popc(amask & lt)] = cell;
+            pc_top += na;
+        }
+        // ---- opened nodes -> back onto the stack (the callers guarantee room for 32 entries)
+        const uint32_t nmask = __ballot_sync(0xFFFFFFFFu, isnode);
+        if (isnode) ws->stack[sp + __popc(nmask & lt)] = lk;
+        sp += __popc(nmask);
+        // ---- opened leaves -> queue; expanded 32 at a time
+        const uint32_t lmask = __ballot_sync(0xFFFFFFFFu, isleaf);
+        if (lmask) {
+            if (isleaf) ws->leafq[lq + __popc(lmask & lt)] = make_uint2(lk.x, lk.y & 0x7FFFFFFFu);
+            lq += __popc(lmask);
+            __syncwarp();
+            if (lq >= 32) {
+                lq -= 32;
+                if (!flush_leaves(ws->leafq + lq, 32, lane, gb, ge, lists, pc_top, pp_bot, npp)) return false;
             }
         }
+        return true;
+    };
+    // the stack of opened nodes, until it is empty
+    auto drain = [&]() {
+        while (sp > 0 && fits) {
+            // pop up to 4 kSub nodes; lane = (node r of a sub-batch, child c8); all records are requested before any is used
+            int kpop = (kLStackCap - kLStackReserve - sp) / 7;
+            kpop = max(1, min(kpop, 4 * kSub));
+            kpop = min(kpop, sp);
+            const int r = lane >> 3, c8 = lane & 7;
+            bool valid[kSub];
+            uint32_t cell[kSub];
+            float4 r0[kSub];
+            uint2 lk[kSub];
+            CellBox cbx[kMac == kMacMinDist ? kSub : 1];
 #pragma unroll
-        for (int j = 0; j < kSub; ++j) {
-            r0[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-            lk[j] = make_uint2(0u, 0u);
-            if (valid[j]) {
-                r0[j] = __ldg(trec + cell[j]);
-                lk[j] = __ldg(tlink + cell[j]);
-                if (kMac == kMacMinDist) cbx[j] = load_cell_box(box, cell[j]);
-            }
-        }
-        sp -= kpop;
-        __syncwarp();                 // every lane has read its stack entries: the slots may be overwritten
-#pragma unroll
-        for (int j = 0; j < kSub; ++j) {
-            if (4 * j >= kpop) break;
-            const bool accept = valid[j] && (kMac == kMacMinDist ? mac_accept_box(mn, mx, cbx[j], r0[j].w) : mac_accept(mn, mx, r0[j]));
-            const bool isleaf = valid[j] && !accept && (lk[j].y >> 31) != 0u;
-            const bool isnode = valid[j] && !accept && !isleaf;
-            nmac += (uint32_t)__popc(__ballot_sync(0xFFFFFFFFu, valid[j]));
-            // ---- accepted cells -> cell list
-            const uint32_t amask = __ballot_sync(0xFFFFFFFFu, accept);
-            if (amask) {
-                const uint32_t na = (uint32_t)__popc(amask);
-                if (pc_top + na > pp_bot) { fits = false; break; }
-                if (accept) lists[pc_top + (uint32_t)__popc(amask & lt)] = cell[j];
-                pc_top += na;
-            }
-            // ---- opened nodes -> back onto the stack (kpop <= (cap - reserve - sp) / 7 guarantees room for 8 per popped node)
-            const uint32_t nmask = __ballot_sync(0xFFFFFFFFu, isnode);
-            if (isnode) ws->stack[sp + __popc(nmask & lt)] = lk[j];
-            sp += __popc(nmask);
-            // ---- opened leaves -> queue; expanded 32 at a time
-            const uint32_t lmask = __ballot_sync(0xFFFFFFFFu, isleaf);
-            if (lmask) {
-                if (isleaf) ws->leafq[lq + __popc(lmask & lt)] = make_uint2(lk[j].x, lk[j].y & 0x7FFFFFFFu);
-                lq += __popc(lmask);
-                __syncwarp();
-                if (lq >= 32) {
-                    lq -= 32;
-                    if (!flush_leaves(ws->leafq + lq, 32, lane, gb, ge, lists, pc_top, pp_bot, npp)) { fits = false; break; }
+            for (int j = 0; j < kSub; ++j) {
+                valid[j] = false;
+                cell[j] = 0u;
+                const int idx = 4 * j + r;
+                if (idx < kpop) {
+                    const uint2 e = ws->stack[sp - 1 - idx];
+                    valid[j] = (uint32_t)c8 < e.y;
+                    cell[j] = e.x + (uint32_t)c8;
                 }
             }
+#pragma unroll
+            for (int j = 0; j < kSub; ++j) {
+                r0[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+                lk[j] = make_uint2(0u, 0u);
+                if (valid[j]) {
+                    r0[j] = __ldg(trec + cell[j]);
+                    lk[j] = __ldg(tlink + cell[j]);
+                    if (kMac == kMacMinDist) cbx[j] = load_cell_box(box, cell[j]);
+                }
+            }
+            sp -= kpop;
+            __syncwarp();                 // every lane has read its stack entries: the slots may be overwritten
+#pragma unroll
+            for (int j = 0; j < kSub; ++j) {
+                if (4 * j >= kpop) break;
+                if (!classify(valid[j], cell[j], r0[j], lk[j], cbx[kMac == kMacMinDist ? j : 0])) { fits = false; break; }
+            }
+            __syncwarp();
         }
+    };
+
+    if (sw == nullptr) {
+        sp = 1;
+        if (lane == 0) ws->stack[0] = make_uint2(0u, 1u);   // the root (A17) as the only child of a virtual node
         __syncwarp();
+        drain();
+    } else {
+        // what every member of the super-group has in common: copy it
+        const uint32_t nc = sw->n_spc, np = sw->n_spp;
+        if (pc_top + nc + np > pp_bot) fits = false;
+        if (fits) {
+            const uint32_t* src_c = lists + sw->spc_off;
+            const uint32_t* src_p = lists + sw->spp_off;
+#pragma unroll 4
+            for (uint32_t i = lane; i < nc; i += 32) lists[pc_top + i] = __ldcg(src_c + i);
+            pc_top += nc;
+            pp_bot -= np;
+#pragma unroll 4
+            for (uint32_t i = lane; i < np; i += 32) lists[pp_bot + i] = __ldcg(src_p + i);
+            npp = sw->leafsum;
+            // the ambiguous cells, 32 at a time, each followed by the walk below the nodes it opened
+            const uint32_t na = sw->n_amb;
+            for (uint32_t a0 = 0; a0 < na && fits; a0 += 32) {
+                const bool valid = a0 + lane < na;
+                const uint32_t cell = valid ? sw->amb[a0 + lane] : 0u;
+                float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f);
+                uint2 lk = make_uint2(0u, 0u);
+                CellBox cbx;
+                if (valid) {
+                    r0 = __ldg(trec + cell);
+                    lk = __ldg(tlink + cell);
+                    if (kMac == kMacMinDist) cbx = load_cell_box(box, cell);
+                }
+                if (!classify(valid, cell, r0, lk, cbx)) { fits = false; break; }
+                __syncwarp();
+                drain();
+            }
+        }
     }
     if (fits && lq > 0) fits = flush_leaves(ws->leafq, lq, lane, gb, ge, lists, pc_top, pp_bot, npp);
 
@@ -203,6 +343,26 @@ __device__ __forceinline__ bool alloc_chunk(WalkCtl* ctl, int wave, int lane, ui
     return true;
 }
 
+constexpr int kChunkSG = kListWarps;                                   // super-groups per chunk: one shared walk per warp
+constexpr int kShareChunk = kSG * kChunkSG;                             // 64 consecutive groups a block claims at a time
+constexpr size_t kListSmem = sizeof(ListWarpShared) * kListWarps + sizeof(SharedWalk) * kChunkSG;
+
+// The box of group g (A13).  A group that is a whole cell has that cell's box (exact min / max of the same particles); a
+// chunk of an over-full leaf takes it from its particles (all lanes take part).
+__device__ __forceinline__ void load_group_box(uint32_t g, uint32_t gb, uint32_t ge, int lane, const float4* __restrict__ pos,
+                                               const float* __restrict__ box, const uint32_t* __restrict__ g_cell,
+                                               const uint4* __restrict__ c_topo, float mn[3], float mx[3]) {
+    const uint32_t gc = __ldg(g_cell + g);
+    const uint2 pr = __ldg(reinterpret_cast<const uint2*>(c_topo + gc));     // (first particle, end particle) of the group's cell
+    if (pr.y - pr.x == ge - gb) {
+        const float* bb = box + 6 * (size_t)gc;
+        mn[0] = __ldg(bb); mn[1] = __ldg(bb + 1); mn[2] = __ldg(bb + 2);
+        mx[0] = __ldg(bb + 3); mx[1] = __ldg(bb + 4); mx[2] = __ldg(bb + 5);
+    } else {
+        group_box(pos, gb, (int)(ge - gb), lane, nullptr, mn, mx);
+    }
+}
+
 template <int kMac>
 __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, int wave, const float4* __restrict__ pos,
                                                                 const float4* __restrict__ trec, const uint2* __restrict__ tlink,
@@ -210,33 +370,83 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
                                                                 const uint4* __restrict__ c_topo,
                                                                 const uint32_t* __restrict__ g_begin, uint32_t* __restrict__ lists,
                                                                 uint32_t region_base, uint32_t region_entries, uint32_t chunk_entries,
-                                                                const uint8_t* __restrict__ g_active) {
-    __shared__ ListWarpShared s_ws[kListWarps];
-    __shared__ uint32_t s_chunk, s_taken;
+                                                                const uint8_t* __restrict__ g_active, int share) {
+    extern __shared__ __align__(16) unsigned char list_smem[];
+    ListWarpShared* s_ws = reinterpret_cast<ListWarpShared*>(list_smem);
+    SharedWalk* s_sw = reinterpret_cast<SharedWalk*>(list_smem + sizeof(ListWarpShared) * kListWarps);
+    __shared__ uint32_t s_chunk;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t g0 = o.ctl->wave_g[wave], g1 = o.ctl->wave_g[wave + 1];
     if (threadIdx.x == 0) atomicMin(&o.ctl->t_start[0][wave], global_ns());
     ListArena ar = {0u, 0u};           // this warp's current chunk of the list region: cell lists grow up, particle lists down
     uint32_t last_total = 0u;          // entries of the last group this warp listed: Morton neighbours need about as many
     WalkSums sums = {0ull, 0ull, 0ull};
+    const bool sharing = share && kMac == kMacEq1;
     for (;;) {
-        __syncthreads();               // everyone is done with the previous chunk's counters
-        if (threadIdx.x == 0) { s_chunk = atomicAdd(&o.ctl->list_next[wave], (uint32_t)kGroupChunk); s_taken = 0; }
+#ifdef BH_LIST_BLOCK_CHUNKS
+        __syncthreads();               // everyone is done with the previous chunk
+        if (threadIdx.x == 0) s_chunk = atomicAdd(&o.ctl->list_next[wave], (uint32_t)kShareChunk);
         __syncthreads();
         const uint32_t base = g0 + s_chunk;
         if (base >= g1) break;
-        const uint32_t nchunk = min((uint32_t)kGroupChunk, g1 - base);
-        for (;;) {
-            uint32_t i = 0;
-            if (lane == 0) i = atomicAdd(&s_taken, 1u);
-            i = __shfl_sync(0xFFFFFFFFu, i, 0);
-            if (i >= nchunk) break;
-            const uint32_t g = base + i;
+        const uint32_t nchunk = min((uint32_t)kShareChunk, g1 - base);
+        const uint32_t s0 = (uint32_t)warp * kSG;
+#else
+        // every warp claims its own super-group: no warp ever waits for another.  Task t covers a FIXED range of groups (the
+        // partition depends on the number of groups only, so the lists, and with them the order of the fp32 sums, do not
+        // depend on timing or on the active subset): eight groups per task over the first 70 % of the groups, four up to
+        // 93 %, then two -- small tasks at the end keep the tail of the kernel short.
+        uint32_t claim = 0;
+        if (lane == 0) claim = atomicAdd(&o.ctl->list_next[wave], 1u);
+        claim = __shfl_sync(0xFFFFFFFFu, claim, 0);
+        const uint32_t Gw = g1 - g0;
+        const uint32_t nA = (uint32_t)(0.70f * (float)Gw) / kSG, gA = nA * kSG;
+        const uint32_t szB = kSG >= 4 ? kSG / 2 : kSG;
+        const uint32_t nB = ((uint32_t)(0.93f * (float)Gw) > gA ? (uint32_t)(0.93f * (float)Gw) - gA : 0u) / szB, gB = gA + nB * szB;
+        const uint32_t szC = kSG >= 4 ? kSG / 4 : kSG;
+        uint32_t off, sz;
+        if (claim < nA) { off = claim * kSG; sz = kSG; }
+        else if (claim < nA + nB) { off = gA + (claim - nA) * szB; sz = szB; }
+        else { off = gB + (claim - nA - nB) * szC; sz = szC; }
+        if (off >= Gw) break;
+        const uint32_t base = g0 + off;
+        const uint32_t nchunk = min(sz, g1 - base);
+        const uint32_t s0 = 0u;
+#endif
+        // ---- warp w takes the super-group w of the chunk (groups base + kSG w ...): one shared walk, then its members one by
+        //      one from where the shared walk stopped.  No warp waits for another inside a chunk.
+        SharedWalk* sw = s_sw + warp;
+        const uint32_t nm = s0 < nchunk ? min((uint32_t)kSG, nchunk - s0) : 0u;
+        bool shared_ok = false;
+        if (sharing && nm >= 2u) {
+            bool any = false;
+            for (uint32_t m = 0; m < nm; ++m) any = any || !(g_active && !__ldg(g_active + base + s0 + m));
+            if (any) {
+                // the union box of EVERY member, active or not: the split must not depend on the subset that is walked
+                float un[3] = {INFINITY, INFINITY, INFINITY}, ux[3] = {-INFINITY, -INFINITY, -INFINITY};
+                for (uint32_t m = 0; m < nm; ++m) {
+                    const uint32_t g = base + s0 + m;
+                    float mn[3], mx[3];
+                    load_group_box(g, __ldg(g_begin + g), __ldg(g_begin + g + 1), lane, pos, box, g_cell, c_topo, mn, mx);
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) { un[k] = fminf(un[k], mn[k]); ux[k] = fmaxf(ux[k], mx[k]); }
+                }
+                const uint32_t sb = __ldg(g_begin + base + s0), se = __ldg(g_begin + base + s0 + nm);
+                if (ar.pp_bot - ar.pc_top < last_total + (last_total >> 1) + 256u) alloc_chunk(o.ctl, wave, lane, region_base, region_entries, chunk_entries, ar);
+                shared_walk(&s_ws[warp], sw, lane, un, ux, sb, se, trec, tlink, lists, ar, sums);
+                shared_ok = sw->ok != 0u;
+            }
+        }
+        for (uint32_t m = 0; m < nm; ++m) {
+            const uint32_t g = base + s0 + m;
             if (g_active && !__ldg(g_active + g)) {      // block time-steps: not in this walk's subset
                 if (lane == 0) { o.g_pcoff[g] = kSkip; o.g_npc[g] = 0u; o.g_npp[g] = 0u; }
                 continue;
             }
             const uint32_t gb = __ldg(g_begin + g), ge = __ldg(g_begin + g + 1);
+            float mn[3], mx[3];
+            load_group_box(g, gb, ge, lane, pos, box, g_cell, c_topo, mn, mx);
+            const SharedWalk* swp = shared_ok ? sw : nullptr;
             // a fresh chunk if this one will probably not do; a second try in a fresh chunk if it did not; a group that does
             // not fit a whole chunk (or finds the region used up) goes to the fused kernel instead
             bool fresh = false;
@@ -245,10 +455,10 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
                 alloc_chunk(o.ctl, wave, lane, region_base, region_entries, chunk_entries, ar);
             }
             const uint32_t before = ar.pp_bot - ar.pc_top;
-            bool ok = before != 0u && list_group<kMac>(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_topo, lists, ar, o, sums);
+            bool ok = before != 0u && list_group<kMac>(&s_ws[warp], lane, g, gb, ge, mn, mx, swp, trec, tlink, box, lists, ar, o, sums);
             if (!ok && !fresh && alloc_chunk(o.ctl, wave, lane, region_base, region_entries, chunk_entries, ar)) {
                 const uint32_t b2 = ar.pp_bot - ar.pc_top;
-                ok = list_group<kMac>(&s_ws[warp], lane, g, gb, ge, pos, trec, tlink, box, g_cell, c_topo, lists, ar, o, sums);
+                ok = list_group<kMac>(&s_ws[warp], lane, g, gb, ge, mn, mx, swp, trec, tlink, box, lists, ar, o, sums);
                 if (ok) last_total = b2 - (ar.pp_bot - ar.pc_top);
             } else if (ok) {
                 last_total = before - (ar.pp_bot - ar.pc_top);
@@ -261,7 +471,7 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
         }
     }
     if (threadIdx.x == 0) atomicMax(&o.ctl->t_end[0][wave], global_ns());
-    if (lane == 0 && sums.mac) {
+    if (lane == 0 && (sums.mac || sums.pc || sums.pp)) {
         atomicAdd(&o.sc->sum_pc, sums.pc);
         atomicAdd(&o.sc->sum_pp, sums.pp);
         atomicAdd(&o.sc->sum_mac, sums.mac);
@@ -302,14 +512,14 @@ int stage_walk_lists(bh_ctx* c, int wave, int grid, uint32_t region_base, uint32
     const uint32_t chunk_entries = std::min(std::max(std::min(share, 65536u), 4096u), region_entries);
     WalkListOut o = walk_list_out(c);
     if (c->mac_kind == kMacMinDist) {
-        BH_LAUNCH(c, k_walk_lists<kMacMinDist>, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
+        BH_LAUNCH(c, k_walk_lists<kMacMinDist>, grid, kListThreads, kListSmem, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
                   c->ws.c_topo, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries,
-                  c->active ? c->ws.gflag : nullptr);
+                  c->active ? c->ws.gflag : nullptr, c->walk_share);
         return BH_OK;
     }
-    BH_LAUNCH(c, k_walk_lists<kMacEq1>, grid, kListThreads, 0, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
+    BH_LAUNCH(c, k_walk_lists<kMacEq1>, grid, kListThreads, kListSmem, s, o, wave, c->ws.pos[c->cur], c->ws.trec, c->ws.tlink, c->ws.box, c->ws.g_cell,
               c->ws.c_topo, c->ws.g_begin, c->ws.lists, region_base, region_entries, chunk_entries,
-                  c->active ? c->ws.gflag : nullptr);
+                  c->active ? c->ws.gflag : nullptr, c->walk_share);
     return BH_OK;
 }
 
@@ -332,6 +542,8 @@ int stage_group_active(bh_ctx* c, const uint8_t* d_active, cudaStream_t s) {
 }
 
 int walk_lists_init(bh_ctx* c) {
+    BH_CUDA(c, cudaFuncSetAttribute(k_walk_lists<kMacEq1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kListSmem));
+    BH_CUDA(c, cudaFuncSetAttribute(k_walk_lists<kMacMinDist>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kListSmem));
     BH_CUDA(c, cudaFuncSetAttribute(k_walk_lists<kMacEq1>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
     BH_CUDA(c, cudaFuncSetAttribute(k_walk_lists<kMacMinDist>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxShared));
     return BH_OK;
