@@ -120,55 +120,71 @@ __device__ __noinline__ void shared_walk(ListWarpShared* ws, SharedWalk* sw, con
     if (lane == 0) ws->stack[0] = make_uint2(0u, 1u);
     __syncwarp();
     while (sp > 0 && ok) {
+        // pop up to 4 kSub nodes; lane = (node r of a sub-batch, child c8); all records are requested before any is used
         int kpop = (kLStackCap - kLStackReserve - sp) / 7;
-        kpop = max(1, min(kpop, 4));
+        kpop = max(1, min(kpop, 4 * kSub));
         kpop = min(kpop, sp);
         const int r = lane >> 3, c8 = lane & 7;
-        bool valid = false;
-        uint32_t cell = 0u;
-        if (r < kpop) {
-            const uint2 e = ws->stack[sp - 1 - r];
-            valid = (uint32_t)c8 < e.y;
-            cell = e.x + (uint32_t)c8;
+        bool valid[kSub];
+        uint32_t cell[kSub];
+        float4 r0[kSub];
+        uint2 lk[kSub];
+#pragma unroll
+        for (int j = 0; j < kSub; ++j) {
+            valid[j] = false;
+            cell[j] = 0u;
+            const int idx = 4 * j + r;
+            if (idx < kpop) {
+                const uint2 e = ws->stack[sp - 1 - idx];
+                valid[j] = (uint32_t)c8 < e.y;
+                cell[j] = e.x + (uint32_t)c8;
+            }
         }
-        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f);
-        uint2 lk = make_uint2(0u, 0u);
-        if (valid) { r0 = __ldg(trec + cell); lk = __ldg(tlink + cell); }
+#pragma unroll
+        for (int j = 0; j < kSub; ++j) {
+            r0[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+            lk[j] = make_uint2(0u, 0u);
+            if (valid[j]) { r0[j] = __ldg(trec + cell[j]); lk[j] = __ldg(tlink + cell[j]); }
+        }
         sp -= kpop;
         __syncwarp();
-        bool acc_all = false, open_all = false;
-        sg_classify(mn, mx, r0, acc_all, open_all);
-        acc_all = acc_all && valid;
-        const bool isleaf = (lk.y >> 31) != 0u;
-        const uint32_t first = lk.x, cnt = lk.y & 0x7FFFFFFFu;
-        const bool opened_node = valid && !acc_all && open_all && !isleaf;
-        const bool opened_leaf = valid && !acc_all && open_all && isleaf && !(first < se && first + cnt > sb);   // no particle of the super-group in it
-        const bool amb = valid && !acc_all && !opened_node && !opened_leaf;
-        nmac += (uint32_t)__popc(__ballot_sync(0xFFFFFFFFu, valid));
-        const uint32_t amask = __ballot_sync(0xFFFFFFFFu, acc_all);
-        if (amask) {
-            if (pc_top + __popc(amask) > pp_bot) { ok = false; break; }
-            if (acc_all) lists[pc_top + __popc(amask & lt)] = cell;
-            pc_top += __popc(amask);
-        }
-        const uint32_t nmask = __ballot_sync(0xFFFFFFFFu, opened_node);
-        if (opened_node) ws->stack[sp + __popc(nmask & lt)] = lk;
-        sp += __popc(nmask);
-        const uint32_t bmask = __ballot_sync(0xFFFFFFFFu, amb);
-        if (bmask) {
-            if (n_amb + __popc(bmask) > kAmbCap) { ok = false; break; }
-            if (amb) sw->amb[n_amb + __popc(bmask & lt)] = cell;
-            n_amb += __popc(bmask);
-        }
-        const uint32_t lmask = __ballot_sync(0xFFFFFFFFu, opened_leaf);
-        if (lmask) {                                                     // the leaf's particles -> shared particle list
-            int total;
-            const int off = warp_excl_scan(opened_leaf ? (int)cnt : 0, lane, total);
-            if ((uint32_t)total > pp_bot - pc_top) { ok = false; break; }
-            pp_bot -= (uint32_t)total;
-            if (opened_leaf)
-                for (uint32_t t = 0; t < cnt; ++t) lists[pp_bot + off + t] = first + t;
-            leafsum += (uint32_t)total;
+#pragma unroll
+        for (int j = 0; j < kSub; ++j) {
+            if (4 * j >= kpop) break;
+            bool acc_all = false, open_all = false;
+            sg_classify(mn, mx, r0[j], acc_all, open_all);
+            acc_all = acc_all && valid[j];
+            const bool isleaf = (lk[j].y >> 31) != 0u;
+            const uint32_t first = lk[j].x, cnt = lk[j].y & 0x7FFFFFFFu;
+            const bool opened_node = valid[j] && !acc_all && open_all && !isleaf;
+            const bool opened_leaf = valid[j] && !acc_all && open_all && isleaf && !(first < se && first + cnt > sb);   // no particle of the super-group in it
+            const bool amb = valid[j] && !acc_all && !opened_node && !opened_leaf;
+            nmac += (uint32_t)__popc(__ballot_sync(0xFFFFFFFFu, valid[j]));
+            const uint32_t amask = __ballot_sync(0xFFFFFFFFu, acc_all);
+            if (amask) {
+                if (pc_top + __popc(amask) > pp_bot) { ok = false; break; }
+                if (acc_all) lists[pc_top + __popc(amask & lt)] = cell[j];
+                pc_top += __popc(amask);
+            }
+            const uint32_t nmask = __ballot_sync(0xFFFFFFFFu, opened_node);
+            if (opened_node) ws->stack[sp + __popc(nmask & lt)] = lk[j];
+            sp += __popc(nmask);
+            const uint32_t bmask = __ballot_sync(0xFFFFFFFFu, amb);
+            if (bmask) {
+                if (n_amb + __popc(bmask) > kAmbCap) { ok = false; break; }
+                if (amb) sw->amb[n_amb + __popc(bmask & lt)] = cell[j];
+                n_amb += __popc(bmask);
+            }
+            const uint32_t lmask = __ballot_sync(0xFFFFFFFFu, opened_leaf);
+            if (lmask) {                                                     // the leaf's particles -> shared particle list
+                int total;
+                const int off = warp_excl_scan(opened_leaf ? (int)cnt : 0, lane, total);
+                if ((uint32_t)total > pp_bot - pc_top) { ok = false; break; }
+                pp_bot -= (uint32_t)total;
+                if (opened_leaf)
+                    for (uint32_t t = 0; t < cnt; ++t) lists[pp_bot + off + t] = first + t;
+                leafsum += (uint32_t)total;
+            }
         }
         __syncwarp();
     }
@@ -283,12 +299,24 @@ __device__ __forceinline__ bool list_group(ListWarpShared* ws, const int lane, c
         if (fits) {
             const uint32_t* src_c = lists + sw->spc_off;
             const uint32_t* src_p = lists + sw->spp_off;
-#pragma unroll 4
-            for (uint32_t i = lane; i < nc; i += 32) lists[pc_top + i] = __ldcg(src_c + i);
+            for (uint32_t i0 = 0; i0 < nc; i0 += 256) {                 // eight loads in flight per lane
+                uint32_t v[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) v[u] = __ldcg(src_c + min(i0 + 32 * u + lane, nc - 1));
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    if (i0 + 32 * u + lane < nc) lists[pc_top + i0 + 32 * u + lane] = v[u];
+            }
             pc_top += nc;
             pp_bot -= np;
-#pragma unroll 4
-            for (uint32_t i = lane; i < np; i += 32) lists[pp_bot + i] = __ldcg(src_p + i);
+            for (uint32_t i0 = 0; i0 < np; i0 += 256) {
+                uint32_t v[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) v[u] = __ldcg(src_p + min(i0 + 32 * u + lane, np - 1));
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    if (i0 + 32 * u + lane < np) lists[pp_bot + i0 + 32 * u + lane] = v[u];
+            }
             npp = sw->leafsum;
             // the ambiguous cells, 32 at a time, each followed by the walk below the nodes it opened
             const uint32_t na = sw->n_amb;
@@ -400,12 +428,14 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
         if (lane == 0) claim = atomicAdd(&o.ctl->list_next[wave], 1u);
         claim = __shfl_sync(0xFFFFFFFFu, claim, 0);
         const uint32_t Gw = g1 - g0;
-        const uint32_t nA = (uint32_t)(0.70f * (float)Gw) / kSG, gA = nA * kSG;
-        const uint32_t szB = kSG >= 4 ? kSG / 2 : kSG;
+        // (few groups per warp, e.g. 16 K particles: a warp that walks for eight groups leaves seven warps idle: smaller tasks)
+        const uint32_t szA = min(max(Gw / (gridDim.x * kListWarps), 1u), (uint32_t)kSG);
+        const uint32_t nA = (uint32_t)(0.70f * (float)Gw) / szA, gA = nA * szA;
+        const uint32_t szB = szA >= 4 ? szA / 2 : szA;
         const uint32_t nB = ((uint32_t)(0.93f * (float)Gw) > gA ? (uint32_t)(0.93f * (float)Gw) - gA : 0u) / szB, gB = gA + nB * szB;
-        const uint32_t szC = kSG >= 4 ? kSG / 4 : kSG;
+        const uint32_t szC = szA >= 4 ? szA / 4 : szA;
         uint32_t off, sz;
-        if (claim < nA) { off = claim * kSG; sz = kSG; }
+        if (claim < nA) { off = claim * szA; sz = szA; }
         else if (claim < nA + nB) { off = gA + (claim - nA) * szB; sz = szB; }
         else { off = gB + (claim - nA - nB) * szC; sz = szC; }
         if (off >= Gw) break;

@@ -236,3 +236,40 @@ def test_block_call_order(BH):
     bh.set_particles(pm, vel)
     with pytest.raises(BhError):
         bh.block_step(0.5, 0.01)                            # new particles: the block state is gone
+
+
+def test_active_walk_is_bit_identical_with_shared_super_group_walks(BH):
+    """At this size the list walk shares the common part of the walks of neighbouring groups (walk_lists.cu); which groups
+    share must depend on the group index only, so a walk of an active subset reproduces the full walk's sums bit for bit,
+    and the counts stay those of the oracle."""
+    n = 400000
+    pm, vel, prm = bh_inputs.make("c2", n=n, seed=103)
+    bh = BH(n)
+    g = gpu_tree(bh, pm, vel, prm["theta"], prm["eps"])
+    assert g["stats"].sum_mac < 1100 * g["n_groups"]                 # the shared walk is in use: far fewer MAC tests than ~1300 per group
+    acc_full = g["acc_pot"].copy()
+    rng = np.random.default_rng(7)
+    active = (rng.random(n) < 0.03).astype(np.uint8)
+    bh.kick_drift(0.0, 0.0); bh.refresh_moments()
+    bh.compute_forces_active(prm["theta"], prm["eps"], torch.from_numpy(active).cuda())
+    g2 = export_numpy(bh)
+    gb = g2["group_begin"].astype(np.int64)
+    gact = np.add.reduceat(active.astype(np.int64), gb[:-1]) > 0
+    walked = np.repeat(gact, np.diff(gb))
+    assert 0.2 < gact.mean() < 0.9
+    assert np.array_equal(g2["acc_pot"][walked], acc_full[walked]) and np.array_equal(g2["acc_pot"][~walked], acc_full[~walked])
+    assert np.array_equal(g2["group_npc"][gact], g["group_npc"][gact]) and np.all(g2["group_npc"][~gact] == 0)
+    # counts against the oracle on a sample of the walked groups
+    st = oracle.tree_build(pm, vel)
+    sel = np.nonzero(gact)[0][::40].astype(np.int64)
+    oracle.compute_forces(st, prm["theta"], prm["eps"], sel=sel)
+    bad = compare_counts(g2, st, sel=sel)
+    assert not bad, "\n".join(bad)
+    check_forces(g2, st, sel=sel)
+    # and a context that walks every group on its own gives the same counts (the order of the entries, hence the last bits, differ)
+    priv = BH(n, walk_private=1)
+    g3 = gpu_tree(priv, pm, vel, prm["theta"], prm["eps"])
+    assert np.array_equal(g3["group_npc"], g["group_npc"]) and np.array_equal(g3["group_npp"], g["group_npp"])
+    assert g3["stats"].sum_mac > 1200 * g3["n_groups"]
+    err = np.abs(g3["acc_pot"][:, :3] - acc_full[:, :3]).max() / np.abs(acc_full[:, :3]).max()
+    assert err < 1e-5
