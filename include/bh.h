@@ -58,7 +58,10 @@ typedef struct bh_config {
                          * k > 1: at least k waves, run as a pipeline (list walk of wave w + 1 beside the evaluation of
                          * wave w on internal streams); 0..255 */
     int32_t front_mode; /* 0 (default): S0-S3 in one cooperative launch whenever every sort tile is resident at once
-                         * (n <= 4096 x 2 x SMs, 1.2 M on B200); 1: always one launch per step and sort pass (any n) */
+                         * (n <= 4096 x 2 x SMs, 1.2 M on B200), with the short sort (radix passes over the leading key bits only,
+                         * then every run of equal leading bits finished in place; the full sort is redone on the device if a
+                         * run is too long: bh_stats.sort_retries); 1: always one launch per step and sort pass (any n);
+                         * 2: the cooperative launch with all 8 radix passes.  The result is the same stable order in all three */
     int32_t walk_private; /* 0 (default): the eight groups of a block share the common part of their walks (cells every one of
                            * them accepts / opens, decided once against the union of their boxes; exact, see walk_lists.cu);
                            * 1: every group walks from the root on its own.  Counts are identical; the order of the list
@@ -81,7 +84,7 @@ typedef struct bh_stats {
     float   lo[3];         /* S0: domain corner */
     float   hi[3];         /* S0: per-axis maximum */
     int32_t domain_exp;    /* S0: cube side = 2^domain_exp */
-    int32_t reserved;
+    int32_t sort_retries;  /* S2: times since bh_create the short sort (leading key bits + fix-up) had to be redone in full */
 } bh_stats;
 
 /* Device pointers into the workspace, valid until the next bh_tree_build / bh_set_particles (particle arrays) or

@@ -45,7 +45,7 @@ static bool make_geometry(int64_t n_max, const bh_config* cfg, Geometry* g) {
     g->walk_private = cfg ? cfg->walk_private : 0;
     if (g->walk_private < 0 || g->walk_private > 1) return false;
     g->front_mode = cfg ? cfg->front_mode : 0;
-    if (g->front_mode < 0 || g->front_mode > 1) return false;
+    if (g->front_mode < 0 || g->front_mode > 2) return false;
     g->sort_tiles = div_up(n_max, kSortTile);
     g->tree_tiles = div_up(n_max + 1, kTreeTile);
     return true;
@@ -159,7 +159,8 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
     c->walk_waves = g.walk_waves;
     c->sort_tiles = g.sort_tiles;
     c->tree_tiles = g.tree_tiles;
-    c->front_enabled = g.front_mode == 0;
+    c->front_enabled = g.front_mode != 1;
+    c->front_full = g.front_mode == 2;
     c->walk_share = g.walk_private ? 0 : 1;
     carve(g, static_cast<unsigned char*>(d_workspace), &c->ws);
     int rc = BH_OK;
@@ -488,6 +489,7 @@ int bh_sync_status(bh_ctx* c, void* stream, bh_stats* out) {
         out->status = h.status;
         out->n = c->n;
         out->launches = c->launches;
+        out->sort_retries = (int32_t)h.sort_retries;
         if (c->have_tree) {
             out->n_levels = (int32_t)h.n_levels;
             out->n_cells = h.n_cells;

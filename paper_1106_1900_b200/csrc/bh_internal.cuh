@@ -54,6 +54,7 @@ struct DevScalars {
     uint32_t tick_next[2];   // next system time, per step parity (the idle slot is reset to ~0)
     uint32_t n_active;       // particles moved by the last block step
     unsigned long long deg_now, deg_base;   // interactions of the groups walked in the last block step / when each was first walked on this tree
+    uint32_t sort_retries;   // full re-sorts since bh_create: the short sort of k_front / stage_sort met a run of equal leading key bits it could not finish
 };
 
 // Walk control block (device): wave boundaries in groups, work counters, the groups deferred to the fused kernel.
@@ -107,8 +108,8 @@ struct Ws {
     float* front_part;    // [sortTiles][8] per-tile box of k_front
     uint32_t* front_matrix; // [frontTiles][kRadix] per-tile digit counts of the current pass
     uint32_t* front_gsum;   // [kSortPasses][kFrontGroupCap][kRadix] digit counts per pass and group of 16 tiles (zero between launches)
-    uint32_t* front_ctl;    // control words that are zero between launches: front_bar[2]
-    uint32_t* front_bar;    // [2] grid barrier of k_front: arrivals, generation
+    uint32_t* front_ctl;    // control words that are zero between launches: front_bar[5]
+    uint32_t* front_bar;    // [5] grid barriers of k_front and its retry flag (front.cu: FrontArgs::bar)
     uint8_t* c_dirty;     // [max_cells] partial refresh (block time-steps): the cell has an active particle below it
     uint4* c_topo;        // [max_cells] (first particle, end particle, first child, end child); children (0, 0) for a leaf
     uint32_t* c_parent;
@@ -167,6 +168,7 @@ struct bh_ctx {
     int64_t sort_tiles, tree_tiles;
     int64_t front_max_tiles;   // sort tiles that are resident at once in a cooperative launch of k_front (0: not available)
     bool front_enabled;        // bh_config.front_mode != 1
+    bool front_full;           // bh_config.front_mode == 2: k_front always sorts with all 8 passes
     // block time-steps
     bool block_on;             // bh_block_init done on this particle set
     int bcur;                  // which of accb / tick / rung / bactive is live

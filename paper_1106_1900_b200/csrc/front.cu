@@ -49,8 +49,13 @@ struct FrontArgs {
     float* part;         // [tiles][8]   per-tile box: min xyz, max xyz, bad flag
     uint32_t* matrix;    // [tiles][256] digit counts of every tile in the current pass
     uint32_t* gsum;      // [8][groups][256] digit counts per pass and group of 16 tiles; zero on entry, zeroed again on exit
-    uint32_t* bar;       // [2]          barrier: arrivals, generation
+    uint32_t* bar;       // [5]          control words, zero between launches: [0] arrivals at the barriers of the first sort, [1] arrivals at
+                         //              the closing barriers (only ever grows), [2] arrivals at the barriers of a full re-sort,
+                         //              [3] "the short sort met a run of equal leading bits it could not finish" (set in the fix-up)
+    int short_passes;    // passes of the first sort: 8 = all 60 bits; < 8: only the leading 8 x short_passes bits, then the fix-up
 };
+
+constexpr int kFixHalo = 64;   // the fix-up of the short sort finishes runs of keys with equal leading bits of at most this length
 
 __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
     uint32_t v;
@@ -74,15 +79,17 @@ __device__ __forceinline__ void grid_barrier(uint32_t* bar, uint32_t target, Dev
     }
     __syncthreads();
 }
-__device__ __forceinline__ void grid_barrier_last(uint32_t* bar, uint32_t b0, uint32_t nblocks, DevScalars* sc) {
+// `closing`: the counter of the closing barriers (bar[1]), passed at `arrivals` arrivals since this block started; `used`: the
+// counter of the barriers before it, which block 0 puts back to zero.
+__device__ __forceinline__ void grid_barrier_last(uint32_t* closing, uint32_t b0, uint32_t arrivals, uint32_t* used, DevScalars* sc) {
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
-        atomicAdd(bar + 1, 1u);
+        atomicAdd(closing, 1u);
         uint32_t spins = 0;
-        while (ld_acquire_u32(bar + 1) - b0 < nblocks)
+        while (ld_acquire_u32(closing) - b0 < arrivals)
             if (++spins > kBarSpinLimit) { atomicMin(&sc->status, (int)BH_ERR_CUDA); break; }
-        if (blockIdx.x == 0) atomicExch(bar, 0u);
+        if (blockIdx.x == 0) atomicExch(used, 0u);
         __threadfence();
     }
     __syncthreads();
@@ -243,149 +250,211 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
                 a.sc->dom_e = e;
                 a.sc->status = status;
                 a.sc->n_cells = 0; a.sc->n_groups = 0; a.sc->n_levels = 0;
+                a.bar[3] = 0u;                                  // (nobody looks at it before the fix-up, many barriers from here)
             }
         }
         __syncthreads();
     }
 
-    // ---------------------------------------------------------------- S1: keys, in registers
-    uint64_t k[kFrontItems];
-    uint32_t v[kFrontItems];
-    {
-        const float lox = s_lo[0], loy = s_lo[1], loz = s_lo[2];
-        const int sh = s_sh;
-        const float scale = (sh >= -126 && sh <= 127) ? __int_as_float((127 + sh) << 23) : 0.0f;
-#pragma unroll
-        for (int it = 0; it < kFrontItems; ++it) {
-            const int i = wbase + it * 32 + lane;
-            k[it] = 0ull;
-            v[it] = (uint32_t)i;
-            if (it * 32 < pw && i < n) {
-                const float4 p = a.pos_in[i];
-                k[it] = (dilate20f(grid_coordf(p.x, lox, sh, scale)) << 2) | (dilate20f(grid_coordf(p.y, loy, sh, scale)) << 1) | dilate20f(grid_coordf(p.z, loz, sh, scale));
-            }
-        }
-    }
-
-    TL();
-    // ---------------------------------------------------------------- S2: 8 passes of 8 bits
+    // Two attempts at most.  The first sorts by the leading 8 x short_passes bits of the key only (LSD over those bits,
+    // stable) and then finishes every run of keys with equal leading bits in place (the fix-up below); if a run is too long for
+    // that, every block learns so at the closing barrier and the second attempt is the full 8-pass sort from the keys made
+    // afresh.  Either way the result is THE stable order of the 60-bit keys, in buffer 1.
     const int cnt_tile = min(a.tile_n, n - (int)tile * a.tile_n);
+    uint32_t* barw = a.bar;                                   // counter of this attempt's barriers (continues the count of S0's)
+    bool gather = a.fuse_reorder != 0;                        // S3 as a gather by the finished permutation (after a full sort)
 #pragma unroll 1
-    for (int pass = 0; pass < kSortPasses; ++pass) {
-        const int shift = pass * kRadixBits;
-        const uint64_t* kin = (pass & 1) ? a.key0 : a.key1;      // pass p reads what pass p - 1 wrote: buffer (p - 1) & 1
-        const uint32_t* vin = (pass & 1) ? a.val0 : a.val1;
-        uint64_t* kout = (pass & 1) ? a.key1 : a.key0;
-        uint32_t* vout = (pass & 1) ? a.val1 : a.val0;
-        if (pass > 0) {
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        const bool full = attempt == 1 || a.short_passes >= kSortPasses;
+        const int npass = full ? kSortPasses : a.short_passes;
+        const int shift0 = full ? 0 : 60 - kRadixBits * npass;           // the short sort covers bits [shift0, 60)
+        const int flip = full ? 0 : (npass - 1) & 1;                      // pass p writes buffer (p + flip) & 1: the last write of an attempt lands in buffer 1
+        if (attempt == 1 && tile == 0 && tid == 0) a.sc->sort_retries += 1u;
+
+        // ------------------------------------------------------------ S1: keys, in registers
+        uint64_t k[kFrontItems];
+        uint32_t v[kFrontItems];
+        {
+            const float lox = s_lo[0], loy = s_lo[1], loz = s_lo[2];
+            const int sh = s_sh;
+            const float scale = (sh >= -126 && sh <= 127) ? __int_as_float((127 + sh) << 23) : 0.0f;
 #pragma unroll
             for (int it = 0; it < kFrontItems; ++it) {
                 const int i = wbase + it * 32 + lane;
-                const bool ok = it * 32 < pw && i < n;
-                k[it] = ok ? __ldcg(kin + i) : 0ull;
-                v[it] = ok ? __ldcg(vin + i) : 0u;
+                k[it] = 0ull;
+                v[it] = (uint32_t)i;
+                if (it * 32 < pw && i < n) {
+                    const float4 p = a.pos_in[i];
+                    k[it] = (dilate20f(grid_coordf(p.x, lox, sh, scale)) << 2) | (dilate20f(grid_coordf(p.y, loy, sh, scale)) << 1) | dilate20f(grid_coordf(p.z, loz, sh, scale));
+                }
             }
         }
-        for (int j = tid; j < kFrontWarps * kRadix / 2; j += kFrontThreads) reinterpret_cast<uint32_t*>(&wcnt[0][0])[j] = 0u;
-        __syncthreads();
+
         TL();
-        uint32_t rank[kFrontItems];
+        // ------------------------------------------------------------ S2: passes of 8 bits
+#pragma unroll 1
+        for (int pass = 0; pass < npass; ++pass) {
+            const int shift = shift0 + pass * kRadixBits;
+            const int ob = (pass + flip) & 1;                             // pass p reads what pass p - 1 wrote
+            const uint64_t* kin = ob ? a.key0 : a.key1;
+            const uint32_t* vin = ob ? a.val0 : a.val1;
+            uint64_t* kout = ob ? a.key1 : a.key0;
+            uint32_t* vout = ob ? a.val1 : a.val0;
+            if (pass > 0) {
 #pragma unroll
-        for (int it = 0; it < kFrontItems; ++it) {
-            if (it * 32 >= pw) { rank[it] = 0u; continue; }                // (warp-uniform)
-            const int i = wbase + it * 32 + lane;
-            const bool ok = i < n;
-            const uint32_t d = (uint32_t)(k[it] >> shift) & (kRadix - 1);
-            uint32_t peers = __ballot_sync(0xFFFFFFFFu, ok);
-            if (!ok) peers = ~peers;
-#pragma unroll
-            for (int b = 0; b < kRadixBits; ++b) {
-                const bool bit = (d >> b) & 1u;
-                const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
-                peers &= bit ? m : ~m;
+                for (int it = 0; it < kFrontItems; ++it) {
+                    const int i = wbase + it * 32 + lane;
+                    const bool ok = it * 32 < pw && i < n;
+                    k[it] = ok ? __ldcg(kin + i) : 0ull;
+                    v[it] = ok ? __ldcg(vin + i) : 0u;
+                }
             }
-            const uint32_t before = __popc(peers & lt);
-            uint32_t old = 0;
-            if (ok) old = wcnt[w][d];
-            __syncwarp();
-            if (ok && before == 0) wcnt[w][d] = (uint16_t)(old + __popc(peers));
-            __syncwarp();
-            rank[it] = old + before;
-        }
-        __syncthreads();
-        TL();
-        // digit = tid (first 256 threads): exclusive prefix over the warps, the tile's count; publish it
-        uint32_t tcount = 0;
-        if (tid < kRadix) {
+            for (int j = tid; j < kFrontWarps * kRadix / 2; j += kFrontThreads) reinterpret_cast<uint32_t*>(&wcnt[0][0])[j] = 0u;
+            __syncthreads();
+            TL();
+            uint32_t rank[kFrontItems];
 #pragma unroll
-            for (int ww = 0; ww < kFrontWarps; ++ww) {
-                const uint32_t t = wcnt[ww][tid];
-                wcnt[ww][tid] = (uint16_t)tcount;
-                tcount += t;
+            for (int it = 0; it < kFrontItems; ++it) {
+                if (it * 32 >= pw) { rank[it] = 0u; continue; }                // (warp-uniform)
+                const int i = wbase + it * 32 + lane;
+                const bool ok = i < n;
+                const uint32_t d = (uint32_t)(k[it] >> shift) & (kRadix - 1);
+                uint32_t peers = __ballot_sync(0xFFFFFFFFu, ok);
+                if (!ok) peers = ~peers;
+#pragma unroll
+                for (int b = 0; b < kRadixBits; ++b) {
+                    const bool bit = (d >> b) & 1u;
+                    const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
+                    peers &= bit ? m : ~m;
+                }
+                const uint32_t before = __popc(peers & lt);
+                uint32_t old = 0;
+                if (ok) old = wcnt[w][d];
+                __syncwarp();
+                if (ok && before == 0) wcnt[w][d] = (uint16_t)(old + __popc(peers));
+                __syncwarp();
+                rank[it] = old + before;
             }
-            a.matrix[(size_t)tile * kRadix + tid] = tcount;
-            if (tcount) atomicAdd(a.gsum + ((size_t)pass * kFrontGroupCap + (tile >> 4)) * kRadix + tid, tcount);
-        }
-        const uint32_t dstart = block_excl_scan512(tcount, wsum);             // first slot of digit d inside the tile, sorted by digit
-        TL();
-        grid_barrier(a.bar, ++nbar * T, a.sc);
-        TL();
-        // keys of this digit in the whole input (-> first output slot of the digit) and in the earlier tiles: the sums of the
-        // groups of 16 tiles + the rows of the earlier tiles of this tile's own group; split between the two halves of the block
-        {
-            const int d = tid & (kRadix - 1), h = tid >> 8;
-            const uint32_t* gs = a.gsum + (size_t)pass * kFrontGroupCap * kRadix + d;
-            const uint32_t myg = tile >> 4;
-            uint32_t tot = 0, ex = 0;
+            __syncthreads();
+            TL();
+            // digit = tid (first 256 threads): exclusive prefix over the warps, the tile's count; publish it
+            uint32_t tcount = 0;
+            if (tid < kRadix) {
+#pragma unroll
+                for (int ww = 0; ww < kFrontWarps; ++ww) {
+                    const uint32_t t = wcnt[ww][tid];
+                    wcnt[ww][tid] = (uint16_t)tcount;
+                    tcount += t;
+                }
+                a.matrix[(size_t)tile * kRadix + tid] = tcount;
+                if (tcount) atomicAdd(a.gsum + ((size_t)pass * kFrontGroupCap + (tile >> 4)) * kRadix + tid, tcount);
+            }
+            const uint32_t dstart = block_excl_scan512(tcount, wsum);             // first slot of digit d inside the tile, sorted by digit
+            TL();
+            grid_barrier(barw, ++nbar * T, a.sc);
+            TL();
+            // keys of this digit in the whole input (-> first output slot of the digit) and in the earlier tiles: the sums of the
+            // groups of 16 tiles + the rows of the earlier tiles of this tile's own group; split between the two halves of the block
+            {
+                const int d = tid & (kRadix - 1), h = tid >> 8;
+                const uint32_t* gs = a.gsum + (size_t)pass * kFrontGroupCap * kRadix + d;
+                const uint32_t myg = tile >> 4;
+                uint32_t tot = 0, ex = 0;
 #pragma unroll 8
-            for (uint32_t g = h; g < G; g += 2) {
-                const uint32_t x = __ldcg(gs + (size_t)g * kRadix);
-                tot += x;
-                if (g < myg) ex += x;
-            }
+                for (uint32_t g = h; g < G; g += 2) {
+                    const uint32_t x = __ldcg(gs + (size_t)g * kRadix);
+                    tot += x;
+                    if (g < myg) ex += x;
+                }
 #pragma unroll 8
-            for (uint32_t t = (myg << 4) + h; t < tile; t += 2) ex += __ldcg(a.matrix + (size_t)t * kRadix + d);
-            ex2[h][d] = ex;
-            tot2[h][d] = tot;
-        }
-        __syncthreads();
-        const uint32_t gh = tid < kRadix ? tot2[0][tid] + tot2[1][tid] : 0u;
-        const uint32_t dbase = block_excl_scan512(gh, wsum);                  // first output slot of digit d
-        if (tid < kRadix) {
-            gbase[tid] = dbase + ex2[0][tid] + ex2[1][tid] - dstart;          // output slot = gbase[digit] + slot inside the sorted tile
-            lbase[tid] = dstart;
-        }
-        __syncthreads();
-        TL();
-        // exchange through shared memory: the tile leaves sorted by digit, so every digit's run is written contiguously
-#pragma unroll
-        for (int it = 0; it < kFrontItems; ++it) {
-            const int i = wbase + it * 32 + lane;
-            if (it * 32 < pw && i < n) {
-                const uint32_t dg = (uint32_t)(k[it] >> shift) & (kRadix - 1);
-                const uint32_t lp = lbase[dg] + wcnt[w][dg] + rank[it];
-                skey[lp] = k[it];
-                sval[lp] = v[it];
+                for (uint32_t t = (myg << 4) + h; t < tile; t += 2) ex += __ldcg(a.matrix + (size_t)t * kRadix + d);
+                ex2[h][d] = ex;
+                tot2[h][d] = tot;
             }
-        }
-        __syncthreads();
-        TL();
+            __syncthreads();
+            const uint32_t gh = tid < kRadix ? tot2[0][tid] + tot2[1][tid] : 0u;
+            const uint32_t dbase = block_excl_scan512(gh, wsum);                  // first output slot of digit d
+            if (tid < kRadix) {
+                gbase[tid] = dbase + ex2[0][tid] + ex2[1][tid] - dstart;          // output slot = gbase[digit] + slot inside the sorted tile
+                lbase[tid] = dstart;
+            }
+            __syncthreads();
+            TL();
+            // exchange through shared memory: the tile leaves sorted by digit, so every digit's run is written contiguously
+#pragma unroll
+            for (int it = 0; it < kFrontItems; ++it) {
+                const int i = wbase + it * 32 + lane;
+                if (it * 32 < pw && i < n) {
+                    const uint32_t dg = (uint32_t)(k[it] >> shift) & (kRadix - 1);
+                    const uint32_t lp = lbase[dg] + wcnt[w][dg] + rank[it];
+                    skey[lp] = k[it];
+                    sval[lp] = v[it];
+                }
+            }
+            __syncthreads();
+            TL();
 #pragma unroll 4
-        for (int lp = tid; lp < cnt_tile; lp += kFrontThreads) {
-            const uint64_t kk = skey[lp];
-            const uint32_t dst = gbase[(uint32_t)(kk >> shift) & (kRadix - 1)] + (uint32_t)lp;
-            kout[dst] = kk;
-            vout[dst] = sval[lp];
+            for (int lp = tid; lp < cnt_tile; lp += kFrontThreads) {
+                const uint64_t kk = skey[lp];
+                const uint32_t dst = gbase[(uint32_t)(kk >> shift) & (kRadix - 1)] + (uint32_t)lp;
+                kout[dst] = kk;
+                vout[dst] = sval[lp];
+            }
+            TL();
+            if (full && pass + 1 == npass) grid_barrier_last(a.bar + 1, b0, (uint32_t)(attempt + 1) * T, barw, a.sc);
+            else grid_barrier(barw, ++nbar * T, a.sc);
+            TL();
+            if (tile < G && tid < kRadix) a.gsum[((size_t)pass * kFrontGroupCap + tile) * kRadix + tid] = 0u;   // everyone has read it: zero for the next launch
+        }
+        if (full) break;
+
+        // ------------------------------------------------------------ fix-up of the short sort (buffer 0 -> buffer 1)
+        // Buffer 0 is ordered by the leading bits, keys with equal leading bits in their original order.  The stable order of
+        // the full keys differs from it only inside each run of equal leading bits: a key goes to (start of its run) + (number
+        // of keys of the run that are smaller, or equal and earlier).  A tile reads its own positions plus kFixHalo on either
+        // side; a run that reaches the edge of that window, or is longer than 2 x kFixHalo, is left to the full sort.
+        {
+            const int w0 = (int)tile * a.tile_n;
+            const int wlo = max(w0 - kFixHalo, 0), whi = min(w0 + cnt_tile + kFixHalo, n);
+            const int wn = max(whi - wlo, 0);
+            for (int j = tid; j < wn; j += kFrontThreads) skey[j] = __ldcg(a.key0 + wlo + j);
+            __syncthreads();
+            bool giveup = false;
+            for (int lp = tid; lp < cnt_tile; lp += kFrontThreads) {
+                const int p = w0 - wlo + lp;
+                const uint64_t kp = skey[p], top = kp >> shift0;
+                int s0 = p;
+                while (s0 > 0 && (skey[s0 - 1] >> shift0) == top) --s0;
+                if ((s0 == 0 && wlo > 0) || p - s0 > 2 * kFixHalo) giveup = true;
+                int r = 0, q = s0;
+                for (; q < wn && q - s0 <= 2 * kFixHalo; ++q) {
+                    const uint64_t kq = skey[q];
+                    if ((kq >> shift0) != top) break;
+                    r += (kq < kp || (kq == kp && q < p)) ? 1 : 0;
+                }
+                if ((q == wn && whi < n) || q - s0 > 2 * kFixHalo) giveup = true;
+                const uint32_t src = __ldcg(a.val0 + w0 + lp);
+                const int dst = wlo + s0 + r;                            // (inside [wlo, whi) even when this run is given up)
+                a.key1[dst] = kp;
+                a.val1[dst] = src;
+                if (a.fuse_reorder) {                                     // S3 as a scatter: the destination is known here
+                    a.pos_out[dst] = a.pos_in[src];
+                    a.vel_out[dst] = a.vel_in[src];
+                    a.id_out[dst] = a.id_in[src];
+                }
+            }
+            if (giveup) atomicOr(a.bar + 3, 1u);
         }
         TL();
-        if (pass + 1 < kSortPasses) grid_barrier(a.bar, ++nbar * T, a.sc);
-        else grid_barrier_last(a.bar, b0, T, a.sc);
+        grid_barrier_last(a.bar + 1, b0, T, barw, a.sc);
         TL();
-        if (tile < G && tid < kRadix) a.gsum[((size_t)pass * kFrontGroupCap + tile) * kRadix + tid] = 0u;   // everyone has read it: zero for the next launch
+        if (__ldcg(a.bar + 3) == 0u) { gather = false; break; }          // (the same for every thread of the grid; reset by the next launch)
+        barw = a.bar + 2;
+        nbar = 0;
     }
 
     // ---------------------------------------------------------------- S3: gather by the permutation (sorted keys / perm are in buffer 1)
-    if (a.fuse_reorder) {
+    if (gather) {
 #pragma unroll 2
         for (int it = 0; it < kFrontItems; ++it) {
             const int j = wbase + it * 32 + lane;
@@ -421,6 +490,15 @@ static int front_tile(const bh_ctx* c) {
     return (int)std::min<int64_t>(std::max<int64_t>(t, 512), kSortTile);
 }
 
+// Passes of the short sort: the leading floor(log2 n) + 20 bits of the key, in whole digits.  With n particles spread over the
+// cube, runs of keys that agree on that many leading bits hold a handful of particles even in the core of a Plummer sphere
+// (1 M particles, 40 bits: longest run 5); what is more strongly clustered than that is caught by the fix-up and re-sorted in full.
+static int front_short_passes(int64_t n) {
+    int lg = 0;
+    while ((int64_t(2) << lg) <= n) ++lg;
+    return std::min(kSortPasses, (lg + 20 + kRadixBits - 1) / kRadixBits);
+}
+
 // S0-S2 (and S3 unless velocities / ids are still arriving on the side stream) in one cooperative launch.
 int stage_front(bh_ctx* c, bool fuse_reorder, cudaStream_t s) {
     const int n = (int)c->n;
@@ -440,11 +518,12 @@ int stage_front(bh_ctx* c, bool fuse_reorder, cudaStream_t s) {
     a.matrix = c->ws.front_matrix;
     a.gsum = c->ws.front_gsum;
     a.bar = c->ws.front_bar;
+    a.short_passes = c->front_full ? kSortPasses : front_short_passes(c->n);
     void* args[] = {(void*)&a};
     cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_front, dim3(tiles), dim3(kFrontThreads), args, (size_t)kSortTile * 12, s);
     c->launches += 1;
     if (e != cudaSuccess) { c->last_cuda = (int)e; return BH_ERR_CUDA; }
-    c->sorted = 1;                 // pass 7 wrote buffer 1
+    c->sorted = 1;                 // the last write of either attempt lands in buffer 1
     if (fuse_reorder) c->cur = b0;
     return BH_OK;
 }

@@ -35,10 +35,55 @@ def _full_parity(BH, pm, vel, theta, eps, mac=0, **cfg):
     return g, st, e
 
 
+@pytest.mark.parametrize("front_mode", [0, 1, 2])
 @pytest.mark.parametrize("cfg,n", [("c1", 16384), ("c1", 5000), ("c1", 4097), ("c1", 257), ("c3", 30000), ("c3", 12289)])
-def test_full_pipeline_parity(BH, cfg, n):
+def test_full_pipeline_parity(BH, cfg, n, front_mode):
+    """Through every front end: the one-launch front end with the short sort (leading key bits + fix-up), the one launch per
+    pass of large inputs, and the one-launch front end with all 8 passes."""
     pm, vel, prm = bh_inputs.make(cfg, n=n)
-    _full_parity(BH, pm, vel, prm["theta"], prm["eps"])
+    g, _, _ = _full_parity(BH, pm, vel, prm["theta"], prm["eps"], front_mode=front_mode)
+    assert g["stats"].sort_retries == 0
+
+
+def _with_clump(n, clump, radius, seed):
+    """A c1 sphere with `clump` of its particles moved into a ball of `radius` around one of them (radius 0: coincident)."""
+    pm, vel, prm = bh_inputs.make("c1", n=n, seed=seed)
+    rng = np.random.Generator(np.random.Philox(seed + 1))
+    idx = rng.choice(n, size=clump, replace=False)
+    centre = pm[idx[0], :3].astype(np.float64)
+    off = rng.standard_normal((clump, 3)) * radius
+    pm[idx, :3] = (centre + off).astype(np.float32)
+    return pm, vel, prm
+
+
+@pytest.mark.parametrize("front_mode", [0, 1])
+@pytest.mark.parametrize("n,clump,radius,retries", [(20000, 48, 3e-4, 0), (20000, 700, 3e-4, 1), (9000, 300, 0.0, 1), (4097, 4000, 1e-4, 1)])
+def test_short_sort_on_clustered_keys(BH, n, clump, radius, retries, front_mode):
+    """Runs of keys that agree on the leading bits the short sort looks at: a short run is finished by the fix-up (order of the
+    trailing bits, equal keys in their original order), a long one makes the device redo the sort in full.  The permutation is
+    bit-exact either way."""
+    pm, vel, prm = _with_clump(n, clump, radius, seed=300 + clump)
+    bh = BH(n, front_mode=front_mode)
+    g = gpu_tree(bh, pm, vel, prm["theta"], 0.05)
+    st = oracle_state(pm, vel, prm["theta"], 0.05)
+    # the input really has what the case is about: the longest run of equal leading 40 bits
+    top = st.keys >> np.uint64(20)
+    runs = np.diff(np.flatnonzero(np.concatenate([[True], top[1:] != top[:-1], [True]])))
+    assert (runs.max() > 128) == bool(retries) and runs.max() > 16
+    bad = compare_tree(g, st)
+    compare_counts(g, st, problems=bad)
+    assert not bad, "\n".join(bad)
+    if front_mode == 0:
+        assert g["stats"].sort_retries == retries
+    # a second build on the same context (the retry flag and the barrier words are back to their idle values)
+    bh.set_particles(pm, vel)
+    bh.tree_build()
+    bh.compute_forces(prm["theta"], 0.05)
+    g2 = export_numpy(bh)
+    assert np.array_equal(g2["perm"], g["perm"]) and np.array_equal(g2["key"], g["key"])
+    if front_mode == 0:
+        assert g2["stats"].sort_retries == 2 * retries
+    bh.close()
 
 
 @pytest.mark.parametrize("theta,eps", [(0.5, 0.01), (0.3, 0.0), (1.0, 0.05)])
