@@ -55,6 +55,7 @@ struct FrontArgs {
     int short_passes;    // passes of the first sort: 8 = all 60 bits; < 8: only the leading 8 x short_passes bits, then the fix-up
 };
 
+constexpr int kFewDigits = 8;   // distinct digits in a row of 32 keys up to which MATCH.ANY beats nine ballots
 constexpr int kFixHalo = 64;   // the fix-up of the short sort finishes runs of keys with equal leading bits of at most this length
 
 __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
@@ -313,21 +314,30 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
             __syncthreads();
             TL();
             uint32_t rank[kFrontItems];
+            bool few = pass > 0;                                               // (warp-uniform)
 #pragma unroll
             for (int it = 0; it < kFrontItems; ++it) {
                 if (it * 32 >= pw) { rank[it] = 0u; continue; }                // (warp-uniform)
                 const int i = wbase + it * 32 + lane;
                 const bool ok = i < n;
                 const uint32_t d = (uint32_t)(k[it] >> shift) & (kRadix - 1);
-                uint32_t peers = __ballot_sync(0xFFFFFFFFu, ok);
-                if (!ok) peers = ~peers;
+                // the lanes of this row with the same digit: MATCH costs one round per distinct value, the ballots a fixed nine
+                // votes; the row before says which is cheaper (leading digits of clustered inputs take few values per row)
+                uint32_t peers;
+                if (few) {
+                    peers = __match_any_sync(0xFFFFFFFFu, ok ? d : (uint32_t)kRadix);
+                } else {
+                    peers = __ballot_sync(0xFFFFFFFFu, ok);
+                    if (!ok) peers = ~peers;
 #pragma unroll
-                for (int b = 0; b < kRadixBits; ++b) {
-                    const bool bit = (d >> b) & 1u;
-                    const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
-                    peers &= bit ? m : ~m;
+                    for (int b = 0; b < kRadixBits; ++b) {
+                        const bool bit = (d >> b) & 1u;
+                        const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
+                        peers &= bit ? m : ~m;
+                    }
                 }
                 const uint32_t before = __popc(peers & lt);
+                few = __popc(__ballot_sync(0xFFFFFFFFu, before == 0u)) <= kFewDigits;
                 uint32_t old = 0;
                 if (ok) old = wcnt[w][d];
                 __syncwarp();
@@ -420,7 +430,18 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
             for (int j = tid; j < wn; j += kFrontThreads) skey[j] = __ldcg(a.key0 + wlo + j);
             __syncthreads();
             bool giveup = false;
-            for (int lp = tid; lp < cnt_tile; lp += kFrontThreads) {
+            uint32_t src[kFrontItems];
+            int dst[kFrontItems];
+#pragma unroll
+            for (int it = 0; it < kFrontItems; ++it) {                    // (the permutation entries are requested first: nothing below waits for them)
+                const int lp = tid + it * kFrontThreads;
+                src[it] = lp < cnt_tile ? __ldcg(a.val0 + w0 + lp) : 0u;
+            }
+#pragma unroll
+            for (int it = 0; it < kFrontItems; ++it) {
+                const int lp = tid + it * kFrontThreads;
+                dst[it] = -1;
+                if (lp >= cnt_tile) continue;
                 const int p = w0 - wlo + lp;
                 const uint64_t kp = skey[p], top = kp >> shift0;
                 int s0 = p;
@@ -433,15 +454,28 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
                     r += (kq < kp || (kq == kp && q < p)) ? 1 : 0;
                 }
                 if ((q == wn && whi < n) || q - s0 > 2 * kFixHalo) giveup = true;
-                const uint32_t src = __ldcg(a.val0 + w0 + lp);
-                const int dst = wlo + s0 + r;                            // (inside [wlo, whi) even when this run is given up)
-                a.key1[dst] = kp;
-                a.val1[dst] = src;
-                if (a.fuse_reorder) {                                     // S3 as a scatter: the destination is known here
-                    a.pos_out[dst] = a.pos_in[src];
-                    a.vel_out[dst] = a.vel_in[src];
-                    a.id_out[dst] = a.id_in[src];
+                dst[it] = wlo + s0 + r;                                   // (inside [wlo, whi) even when this run is given up)
+                a.key1[dst[it]] = kp;
+                a.val1[dst[it]] = src[it];
+            }
+            if (a.fuse_reorder) {                                         // S3 as a scatter: the destinations are known here
+#pragma unroll
+                for (int h = 0; h < kFrontItems; h += 4) {                // four gathers in flight per array
+                    float4 x[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) if (dst[h + u] >= 0) x[u] = a.pos_in[src[h + u]];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) if (dst[h + u] >= 0) a.pos_out[dst[h + u]] = x[u];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) if (dst[h + u] >= 0) x[u] = a.vel_in[src[h + u]];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) if (dst[h + u] >= 0) a.vel_out[dst[h + u]] = x[u];
                 }
+                uint32_t y[kFrontItems];
+#pragma unroll
+                for (int it = 0; it < kFrontItems; ++it) if (dst[it] >= 0) y[it] = a.id_in[src[it]];
+#pragma unroll
+                for (int it = 0; it < kFrontItems; ++it) if (dst[it] >= 0) a.id_out[dst[it]] = y[it];
             }
             if (giveup) atomicOr(a.bar + 3, 1u);
         }
