@@ -26,9 +26,15 @@ extern "C" int bh_debug_front(unsigned long long* host1024) { return (int)cudaMe
 
 namespace bh {
 
-constexpr int kFrontThreads = 512;
-constexpr int kFrontWarps = kFrontThreads / 32;                 // 16
-constexpr int kFrontItems = kSortTile / kFrontThreads;          // 8 keys per thread
+#ifndef BH_FRONT_THREADS
+#define BH_FRONT_THREADS 1024
+#endif
+constexpr int kFrontThreads = BH_FRONT_THREADS;                 // 1024: one block per SM (half as many arrivals at every grid barrier); 512: two
+constexpr int kFrontBlocksPerSM = 1024 / kFrontThreads;
+constexpr int kFrontWarps = kFrontThreads / 32;
+constexpr int kFrontItems = 8;                                  // keys per thread
+constexpr int kFrontTile = kFrontThreads * kFrontItems;         // most keys of a tile (block)
+constexpr int kFrontParts = kFrontThreads / kRadix;             // threads per digit in the prefix step
 constexpr uint32_t kBarSpinLimit = 1u << 24;
 
 struct FrontArgs {
@@ -115,9 +121,9 @@ __device__ __forceinline__ uint32_t grid_coordf(float x, float lo, int sh, float
     return min(__float2uint_rz(s), (1u << kKeyBits) - 1u);
 }
 
-// exclusive prefix of v over the first 256 threads of a 512-thread block (threads >= 256 pass 0); every thread gets
+// exclusive prefix of v over the first 256 threads of the block (threads >= 256 pass 0); every thread gets
 // the prefix of its own index
-__device__ __forceinline__ uint32_t block_excl_scan512(uint32_t v, uint32_t* wsum /*[16]*/) {
+__device__ __forceinline__ uint32_t block_excl_scan512(uint32_t v, uint32_t* wsum /*[kFrontWarps]*/) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint32_t inc = v;
 #pragma unroll
@@ -137,12 +143,12 @@ __device__ __forceinline__ uint32_t block_excl_scan512(uint32_t v, uint32_t* wsu
     return base + inc - v;
 }
 
-__global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
+__global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(const FrontArgs a) {
     extern __shared__ __align__(16) unsigned char xch[];
     uint64_t* skey = reinterpret_cast<uint64_t*>(xch);
-    uint32_t* sval = reinterpret_cast<uint32_t*>(xch + kSortTile * 8);
+    uint32_t* sval = reinterpret_cast<uint32_t*>(xch + kFrontTile * 8);
     __shared__ uint16_t wcnt[kFrontWarps][kRadix];
-    __shared__ uint32_t gbase[kRadix], lbase[kRadix], ex2[2][kRadix], tot2[2][kRadix];
+    __shared__ uint32_t gbase[kRadix], lbase[kRadix], ex2[kFrontParts][kRadix], tot2[kFrontParts][kRadix];
     __shared__ uint32_t wsum[kFrontWarps];
     __shared__ float redf[kFrontWarps][8];
     __shared__ float s_lo[3];
@@ -371,21 +377,25 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
                 const uint32_t myg = tile >> 4;
                 uint32_t tot = 0, ex = 0;
 #pragma unroll 8
-                for (uint32_t g = h; g < G; g += 2) {
+                for (uint32_t g = h; g < G; g += kFrontParts) {
                     const uint32_t x = __ldcg(gs + (size_t)g * kRadix);
                     tot += x;
                     if (g < myg) ex += x;
                 }
 #pragma unroll 8
-                for (uint32_t t = (myg << 4) + h; t < tile; t += 2) ex += __ldcg(a.matrix + (size_t)t * kRadix + d);
+                for (uint32_t t = (myg << 4) + h; t < tile; t += kFrontParts) ex += __ldcg(a.matrix + (size_t)t * kRadix + d);
                 ex2[h][d] = ex;
                 tot2[h][d] = tot;
             }
             __syncthreads();
-            const uint32_t gh = tid < kRadix ? tot2[0][tid] + tot2[1][tid] : 0u;
+            uint32_t gh = 0u, exs = 0u;
+            if (tid < kRadix) {
+#pragma unroll
+                for (int hh = 0; hh < kFrontParts; ++hh) { gh += tot2[hh][tid]; exs += ex2[hh][tid]; }
+            }
             const uint32_t dbase = block_excl_scan512(gh, wsum);                  // first output slot of digit d
             if (tid < kRadix) {
-                gbase[tid] = dbase + ex2[0][tid] + ex2[1][tid] - dstart;          // output slot = gbase[digit] + slot inside the sorted tile
+                gbase[tid] = dbase + exs - dstart;          // output slot = gbase[digit] + slot inside the sorted tile
                 lbase[tid] = dstart;
             }
             __syncthreads();
@@ -418,6 +428,8 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
         }
         if (full) break;
 
+        uint32_t src[kFrontItems];                                        // fix-up: where each of this thread's keys comes from / goes to
+        int dst[kFrontItems];
         // ------------------------------------------------------------ fix-up of the short sort (buffer 0 -> buffer 1)
         // Buffer 0 is ordered by the leading bits, keys with equal leading bits in their original order.  The stable order of
         // the full keys differs from it only inside each run of equal leading bits: a key goes to (start of its run) + (number
@@ -430,8 +442,6 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
             for (int j = tid; j < wn; j += kFrontThreads) skey[j] = __ldcg(a.key0 + wlo + j);
             __syncthreads();
             bool giveup = false;
-            uint32_t src[kFrontItems];
-            int dst[kFrontItems];
 #pragma unroll
             for (int it = 0; it < kFrontItems; ++it) {                    // (the permutation entries are requested first: nothing below waits for them)
                 const int lp = tid + it * kFrontThreads;
@@ -458,7 +468,15 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
                 a.key1[dst[it]] = kp;
                 a.val1[dst[it]] = src[it];
             }
-            if (a.fuse_reorder) {                                         // S3 as a scatter: the destinations are known here
+            if (giveup) atomicOr(a.bar + 3, 1u);
+        }
+        TL();
+        grid_barrier_last(a.bar + 1, b0, T, barw, a.sc);
+        TL();
+        if (__ldcg(a.bar + 3) == 0u) {                                    // (the same for every thread of the grid; reset by the next launch)
+            // S3 as a scatter: the destinations are still in registers; behind the closing barrier, so that the barrier does
+            // not wait for these stores
+            if (a.fuse_reorder) {
 #pragma unroll
                 for (int h = 0; h < kFrontItems; h += 4) {                // four gathers in flight per array
                     float4 x[4];
@@ -477,12 +495,9 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
 #pragma unroll
                 for (int it = 0; it < kFrontItems; ++it) if (dst[it] >= 0) a.id_out[dst[it]] = y[it];
             }
-            if (giveup) atomicOr(a.bar + 3, 1u);
+            gather = false;
+            break;
         }
-        TL();
-        grid_barrier_last(a.bar + 1, b0, T, barw, a.sc);
-        TL();
-        if (__ldcg(a.bar + 3) == 0u) { gather = false; break; }          // (the same for every thread of the grid; reset by the next launch)
         barw = a.bar + 2;
         nbar = 0;
     }
@@ -507,21 +522,21 @@ __global__ void __launch_bounds__(kFrontThreads, 2) k_front(const FrontArgs a) {
 }
 
 int front_init(bh_ctx* c) {
-    BH_CUDA(c, cudaFuncSetAttribute(k_front, cudaFuncAttributeMaxDynamicSharedMemorySize, kSortTile * 12));
+    BH_CUDA(c, cudaFuncSetAttribute(k_front, cudaFuncAttributeMaxDynamicSharedMemorySize, kFrontTile * 12));
     int per_sm = 0;
-    BH_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_front, kFrontThreads, kSortTile * 12));
+    BH_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_front, kFrontThreads, kFrontTile * 12));
     int coop = 0;
     BH_CUDA(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device));
     c->front_max_tiles = coop ? std::min<int64_t>((int64_t)per_sm * c->sm_count, kFrontTileCap) : 0;
     return BH_OK;
 }
 
-bool front_fits(const bh_ctx* c) { return c->front_enabled && div_up(c->n, kSortTile) <= c->front_max_tiles; }
+bool front_fits(const bh_ctx* c) { return c->front_enabled && div_up(c->n, kFrontTile) <= c->front_max_tiles; }
 
 // Keys per tile: the input spread evenly over every resident block slot (two per SM), in multiples of 512.
 static int front_tile(const bh_ctx* c) {
-    const int64_t t = div_up(div_up(c->n, c->front_max_tiles), 512) * 512;
-    return (int)std::min<int64_t>(std::max<int64_t>(t, 512), kSortTile);
+    const int64_t t = div_up(div_up(c->n, c->front_max_tiles), kFrontThreads) * kFrontThreads;
+    return (int)std::min<int64_t>(std::max<int64_t>(t, kFrontThreads), kFrontTile);
 }
 
 // Passes of the short sort: the leading floor(log2 n) + 20 bits of the key, in whole digits.  With n particles spread over the
@@ -554,7 +569,7 @@ int stage_front(bh_ctx* c, bool fuse_reorder, cudaStream_t s) {
     a.bar = c->ws.front_bar;
     a.short_passes = c->front_full ? kSortPasses : front_short_passes(c->n);
     void* args[] = {(void*)&a};
-    cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_front, dim3(tiles), dim3(kFrontThreads), args, (size_t)kSortTile * 12, s);
+    cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_front, dim3(tiles), dim3(kFrontThreads), args, (size_t)kFrontTile * 12, s);
     c->launches += 1;
     if (e != cudaSuccess) { c->last_cuda = (int)e; return BH_ERR_CUDA; }
     c->sorted = 1;                 // the last write of either attempt lands in buffer 1
