@@ -85,6 +85,8 @@ typedef struct bh_stats {
     float   hi[3];         /* S0: per-axis maximum */
     int32_t domain_exp;    /* S0: cube side = 2^domain_exp */
     int32_t sort_retries;  /* S2: times since bh_create the short sort (leading key bits + fix-up) had to be redone in full */
+    int32_t sort_passes;   /* S2: radix passes of the last build's first sort (8: the full sort; fewer: the short sort) */
+    int32_t reserved;
 } bh_stats;
 
 /* Device pointers into the workspace, valid until the next bh_tree_build / bh_set_particles (particle arrays) or

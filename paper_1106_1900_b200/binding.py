@@ -35,7 +35,7 @@ class BhStats(C.Structure):
     _fields_ = [("status", C.c_int32), ("n_levels", C.c_int32), ("n", C.c_int64), ("n_cells", C.c_int64),
                 ("n_groups", C.c_int64), ("sum_pc", C.c_int64), ("sum_pp", C.c_int64), ("sum_mac", C.c_int64),
                 ("launches", C.c_int64), ("lo", C.c_float * 3), ("hi", C.c_float * 3), ("domain_exp", C.c_int32),
-                ("sort_retries", C.c_int32)]
+                ("sort_retries", C.c_int32), ("sort_passes", C.c_int32), ("reserved", C.c_int32)]
 
 
 class BhBlockConfig(C.Structure):

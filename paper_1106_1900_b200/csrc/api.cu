@@ -74,9 +74,9 @@ static size_t carve(const Geometry& g, unsigned char* base, Ws* w) {
     o.g_cell = c.take<uint32_t>(n);
     o.g_npc = c.take<uint32_t>(n);
     o.g_npp = c.take<uint32_t>(n);
-    o.sort_ghist = c.take<uint32_t>((size_t)kSortPasses * kRadix + kSortPasses + (size_t)kSortPasses * kRadix * g.sort_tiles);
+    o.sort_ghist = c.take<uint32_t>(sort_words(g.sort_tiles));
     o.sort_ticket = o.sort_ghist ? o.sort_ghist + kSortPasses * kRadix : nullptr;
-    o.sort_status = o.sort_ghist ? o.sort_ticket + kSortPasses : nullptr;
+    o.sort_status = o.sort_ghist ? o.sort_ticket + 2 * kSortPasses : nullptr;
     o.tile_cnt = c.take<uint32_t>((size_t)kTreeRows * g.tree_tiles);
     o.row_total = c.take<uint32_t>(kTreeRows);
     o.mom_span = c.take<uint32_t>((size_t)kLevels * kMomBlockCap);
@@ -490,6 +490,7 @@ int bh_sync_status(bh_ctx* c, void* stream, bh_stats* out) {
         out->n = c->n;
         out->launches = c->launches;
         out->sort_retries = (int32_t)h.sort_retries;
+        out->sort_passes = (int32_t)(kSortPasses - h.sort_skip);
         if (c->have_tree) {
             out->n_levels = (int32_t)h.n_levels;
             out->n_cells = h.n_cells;

@@ -54,6 +54,8 @@ struct DevScalars {
     uint32_t tick_next[2];   // next system time, per step parity (the idle slot is reset to ~0)
     uint32_t n_active;       // particles moved by the last block step
     unsigned long long deg_now, deg_base;   // interactions of the groups walked in the last block step / when each was first walked on this tree
+    uint32_t sort_skip;      // stage_sort: trailing (low) digits this build's first sort leaves to the fix-up (0: all 8 passes); set by k_reset_build
+    uint32_t sort_redo;      // stage_sort: the fix-up met a run it could not finish: the full sort follows
     uint32_t sort_retries;   // full re-sorts since bh_create: the short sort of k_front / stage_sort met a run of equal leading key bits it could not finish
 };
 
@@ -100,8 +102,8 @@ struct Ws {
     uint32_t* g_npc;      // [n]
     uint32_t* g_npp;      // [n]
     uint32_t* sort_ghist;  // [kSortPasses][kRadix] keys per digit value, all passes (counted by k_keys)
-    uint32_t* sort_ticket; // [kSortPasses] tile tickets                       (contiguous with sort_ghist and
-    uint32_t* sort_status; // [kSortPasses][sortTiles][kRadix] look-back words  sort_status: one memset)
+    uint32_t* sort_ticket; // [2][kSortPasses] tile tickets                       (contiguous with sort_ghist and sort_status: one
+    uint32_t* sort_status; // [2][kSortPasses][sortTiles][kRadix] look-back words  memset); [1]: the full re-sort after a failed short sort
     uint32_t* tile_cnt;   // [kTreeRows][treeTiles] starts per tile; after k_bounds: exclusive scan of every row over the tiles
     uint32_t* row_total;  // [kTreeRows] cells per level, groups
     uint32_t* mom_span;   // [kLevels][momentBlocks] cell of each level that straddles the end of a block's particle range (kNone: none)
@@ -216,6 +218,8 @@ namespace bh {
     } while (0)
 
 static inline int64_t div_up(int64_t a, int64_t b) { return (a + b - 1) / b; }
+// words of sort bookkeeping (digit histograms, tickets, look-back status words for the first sort and for a re-sort)
+static inline size_t sort_words(int64_t tiles) { return (size_t)kSortPasses * kRadix + 2 * (size_t)kSortPasses + 2 * (size_t)kSortPasses * kRadix * (size_t)tiles; }
 
 // Stage-boundary event k on stream s.  While the step is being captured into a graph (bh_step_graph_build) the record
 // becomes an external event node, so the stage times of a replayed graph can be read like those of plain launches.

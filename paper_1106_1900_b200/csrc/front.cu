@@ -258,6 +258,7 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
                 a.sc->status = status;
                 a.sc->n_cells = 0; a.sc->n_groups = 0; a.sc->n_levels = 0;
                 a.bar[3] = 0u;                                  // (nobody looks at it before the fix-up, many barriers from here)
+                a.sc->sort_skip = (uint32_t)(kSortPasses - min(a.short_passes, kSortPasses));
             }
         }
         __syncthreads();

@@ -15,10 +15,28 @@ __device__ __forceinline__ float ord2f(uint32_t u) {
     return __uint_as_float((u & 0x80000000u) ? (u & 0x7FFFFFFFu) : ~u);
 }
 
-__global__ void k_reset_build(DevScalars* sc) {
+// Also decides how much of the key this build's first sort looks at (the short sort, see k_sort_fix): the tree of the
+// previous build on this context had n_levels levels, so keys that agree on 3 n_levels leading bits were at most nleaf then
+// (and are few now: particles move little between two builds); the first sort covers those bits in whole digits.  No
+// previous tree, an overflowed one, or short_ok = 0: all 8 passes.  A wrong guess costs time, never the result.
+__global__ void k_reset_build(DevScalars* sc, int short_ok) {
     const int t = threadIdx.x;
     if (t < 3) { sc->bb_min[t] = 0xFFFFFFFFu; sc->bb_max[t] = 0u; }
-    if (t == 0) { sc->status = BH_OK; sc->n_cells = 0; sc->n_groups = 0; sc->n_levels = 0; }
+    if (t == 0) {
+        const uint32_t L = sc->n_levels;
+        uint32_t np = kSortPasses;
+        if (short_ok && L > 0u) np = min((uint32_t)kSortPasses, (3u * L + kRadixBits - 1u) / kRadixBits);
+        sc->sort_skip = kSortPasses - np;
+        sc->sort_redo = 0u;
+        sc->status = BH_OK; sc->n_cells = 0; sc->n_groups = 0; sc->n_levels = 0;
+    }
+}
+
+// Which of the two key / permutation buffers the sort of this build starts in, so that its last write lands in buffer 0:
+// the first sort makes np = 8 - skip passes plus the fix-up (none when np = 8), the re-sort 8 passes.
+__device__ __forceinline__ uint32_t sort_start_buffer(uint32_t skip, int redo) {
+    if (redo || skip == 0u) return 0u;
+    return (kSortPasses - skip + 1u) & 1u;
 }
 
 // Per-axis min / max (exact) and input validation (A27: finite positions, finite mass > 0).
@@ -105,8 +123,15 @@ __device__ __forceinline__ uint32_t grid_coord(float x, float lo, int sh) {
 
 // Also counts, for every sort pass, how many keys carry each digit value (ghist[pass][digit]): the sort then needs no
 // histogram pass of its own.
-__global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pos, int n, const DevScalars* __restrict__ sc,
-                                              uint64_t* __restrict__ key, uint32_t* __restrict__ val, uint32_t* __restrict__ ghist) {
+// redo = 1: the keys again for the full re-sort, only if the fix-up asked for it (the histograms are still valid).
+__global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pos, int n, DevScalars* __restrict__ sc,
+                                              uint64_t* __restrict__ key0, uint64_t* __restrict__ key1, uint32_t* __restrict__ val0,
+                                              uint32_t* __restrict__ val1, uint32_t* __restrict__ ghist, int redo) {
+    if (redo && sc->sort_redo == 0u) return;
+    if (redo && blockIdx.x == 0 && threadIdx.x == 0) sc->sort_retries += 1u;
+    const uint32_t sb = sort_start_buffer(sc->sort_skip, redo);
+    uint64_t* __restrict__ key = sb ? key1 : key0;
+    uint32_t* __restrict__ val = sb ? val1 : val0;
     __shared__ uint32_t h[kSortPasses * kRadix];
     for (int j = threadIdx.x; j < kSortPasses * kRadix; j += blockDim.x) h[j] = 0;
     __syncthreads();
@@ -118,10 +143,12 @@ __global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pos, in
         const uint64_t k = (dilate20(ix) << 2) | (dilate20(iy) << 1) | dilate20(iz);   // x most significant in a triple (A4)
         key[i] = k;
         val[i] = (uint32_t)i;
+        if (redo) continue;
 #pragma unroll
         for (int q = 0; q < kSortPasses; ++q) atomicAdd(&h[q * kRadix + ((uint32_t)(k >> (q * kRadixBits)) & (kRadix - 1))], 1u);
     }
     __syncthreads();
+    if (redo) return;
     for (int j = threadIdx.x; j < kSortPasses * kRadix; j += blockDim.x)
         if (h[j]) atomicAdd(&ghist[j], h[j]);
 }
@@ -176,10 +203,20 @@ __device__ __forceinline__ void st_relaxed(uint32_t* p, uint32_t v) {
 }
 
 // Warp w of the block owns the contiguous sub-tile [w*512, (w+1)*512): order = (warp, iteration, lane).
-__global__ void __launch_bounds__(kSortThreads) k_radix_pass(const uint64_t* __restrict__ key_in, const uint32_t* __restrict__ val_in,
-                                                             int n, int shift, const uint32_t* __restrict__ ghist, uint32_t* ticket,
-                                                             uint32_t* status, uint64_t* __restrict__ key_out,
-                                                             uint32_t* __restrict__ val_out, DevScalars* sc) {
+// Pass `pass` (digit = key bits [8 pass, 8 pass + 8)) of the first sort (redo = 0: skipped when the short sort leaves this
+// digit to the fix-up) or of the full re-sort (redo = 1: skipped unless the fix-up asked for it).  The buffers alternate from
+// sort_start_buffer().
+__global__ void __launch_bounds__(kSortThreads) k_radix_pass(uint64_t* key0, uint64_t* key1, uint32_t* val0, uint32_t* val1,
+                                                             int n, int pass, int redo, const uint32_t* __restrict__ ghist, uint32_t* ticket,
+                                                             uint32_t* status, DevScalars* sc) {
+    const uint32_t skip = redo ? 0u : sc->sort_skip;
+    if (redo ? sc->sort_redo == 0u : (uint32_t)pass < skip) return;              // (the whole grid)
+    const uint32_t ib = (sort_start_buffer(skip, redo) + (uint32_t)pass - skip) & 1u;
+    const uint64_t* __restrict__ key_in = ib ? key1 : key0;
+    const uint32_t* __restrict__ val_in = ib ? val1 : val0;
+    uint64_t* __restrict__ key_out = ib ? key0 : key1;
+    uint32_t* __restrict__ val_out = ib ? val0 : val1;
+    const int shift = pass * kRadixBits;
     constexpr int kWarps = kSortThreads / 32;
     constexpr int kIters = kSortTile / kWarps / 32;   // 16
     __shared__ uint32_t wcnt[kWarps][kRadix];
@@ -291,6 +328,45 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_pass(const uint64_t* __r
     }
 }
 
+// The fix-up of the short sort.  After the passes over the digits above bit 8 skip, buffer 1 is ordered by those leading bits,
+// keys with equal leading bits in their original order; the stable order of the full keys differs from it only inside each
+// run of equal leading bits: a key goes to (start of its run) + (number of keys of the run that are smaller, or equal and
+// earlier).  A tile of 4096 positions reads kFixHaloBig more on either side; a run that reaches the edge of that window (or
+// is longer than twice the halo) cannot be finished here: sort_redo makes the kernels that follow sort again, in full.
+constexpr int kFixHaloBig = 256;
+__global__ void __launch_bounds__(kSortThreads) k_sort_fix(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin, int n,
+                                                           uint64_t* __restrict__ kout, uint32_t* __restrict__ vout, DevScalars* sc) {
+    const uint32_t skip = sc->sort_skip;
+    if (skip == 0u) return;
+    const int cut = (int)skip * kRadixBits;
+    __shared__ uint64_t skey[kSortTile + 2 * kFixHaloBig];
+    const int w0 = (int)blockIdx.x * kSortTile;
+    const int own = min(kSortTile, n - w0);
+    const int wlo = max(w0 - kFixHaloBig, 0), whi = min(w0 + own + kFixHaloBig, n);
+    const int wn = whi - wlo;
+    for (int j = threadIdx.x; j < wn; j += kSortThreads) skey[j] = kin[wlo + j];
+    __syncthreads();
+    bool giveup = false;
+    for (int lp = threadIdx.x; lp < own; lp += kSortThreads) {
+        const int p = w0 - wlo + lp;
+        const uint64_t kp = skey[p], top = kp >> cut;
+        int s0 = p;
+        while (s0 > 0 && p - s0 <= 2 * kFixHaloBig && (skey[s0 - 1] >> cut) == top) --s0;
+        if ((s0 == 0 && wlo > 0) || p - s0 > 2 * kFixHaloBig) giveup = true;
+        int r = 0, q = s0;
+        for (; q < wn && q - s0 <= 2 * kFixHaloBig; ++q) {
+            const uint64_t kq = skey[q];
+            if ((kq >> cut) != top) break;
+            r += (kq < kp || (kq == kp && q < p)) ? 1 : 0;
+        }
+        if ((q == wn && whi < n) || q - s0 > 2 * kFixHaloBig) giveup = true;
+        const int dst = wlo + s0 + r;                                    // (inside [wlo, whi) even when this run is given up)
+        kout[dst] = kp;
+        vout[dst] = vin[w0 + lp];
+    }
+    if (giveup) atomicOr(&sc->sort_redo, 1u);
+}
+
 int sort_init(bh_ctx* c) {
     BH_CUDA(c, cudaFuncSetAttribute(k_radix_pass, cudaFuncAttributeMaxDynamicSharedMemorySize, kSortTile * 12));
     return BH_OK;
@@ -317,30 +393,37 @@ int stage_iota(bh_ctx* c, uint32_t* dst, int64_t n, cudaStream_t s) {
 
 int stage_bbox_keys(bh_ctx* c, cudaStream_t s) {
     const int n = (int)c->n;
-    BH_LAUNCH(c, k_reset_build, 1, 32, 0, s, c->ws.sc);
+    BH_LAUNCH(c, k_reset_build, 1, 32, 0, s, c->ws.sc, c->front_full ? 0 : 1);
     // sort bookkeeping (digit histograms, tile tickets, look-back status words of every pass): one memset per build
     const int tiles = (int)div_up(n, kSortTile);
-    BH_CUDA(c, cudaMemsetAsync(c->ws.sort_ghist, 0, sizeof(uint32_t) * ((size_t)kSortPasses * kRadix + kSortPasses + (size_t)kSortPasses * kRadix * tiles), s));
+    BH_CUDA(c, cudaMemsetAsync(c->ws.sort_ghist, 0, sizeof(uint32_t) * sort_words(tiles), s));
     const int grid = (int)std::min<int64_t>(div_up(n, 256 * 4), (int64_t)c->sm_count * 8);
     BH_LAUNCH(c, k_bbox, grid, 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc);
     BH_LAUNCH(c, k_domain, 1, 32, 0, s, c->ws.sc);
     if (c->timing) stage_mark(c, 1, s);
     const int kgrid = (int)std::min<int64_t>(div_up(n, 256), (int64_t)c->sm_count * 8);
-    BH_LAUNCH(c, k_keys, kgrid, 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc, c->ws.key[0], c->ws.val[0], c->ws.sort_ghist);
+    BH_LAUNCH(c, k_keys, kgrid, 256, 0, s, c->ws.pos[c->cur], n, c->ws.sc, c->ws.key[0], c->ws.key[1], c->ws.val[0], c->ws.val[1], c->ws.sort_ghist, 0);
     return BH_OK;
 }
 
+// The first sort (as many passes as k_reset_build decided, then the fix-up), and the launches of the full re-sort, which
+// return at once unless the fix-up asked for it: the sequence of launches does not depend on the data (no host round
+// trip; capturable), and the result is in buffer 0 either way.
 int stage_sort(bh_ctx* c, cudaStream_t s) {
     const int n = (int)c->n;
     const int tiles = (int)div_up(n, kSortTile);
-    int src = 0;
-    for (int p = 0; p < kSortPasses; ++p) {
-        const int shift = p * kRadixBits;
-        BH_LAUNCH(c, k_radix_pass, tiles, kSortThreads, kSortTile * 12, s, c->ws.key[src], c->ws.val[src], n, shift, c->ws.sort_ghist + p * kRadix,
-                  c->ws.sort_ticket + p, c->ws.sort_status + (size_t)p * kRadix * tiles, c->ws.key[src ^ 1], c->ws.val[src ^ 1], c->ws.sc);
-        src ^= 1;
+    const Ws& w = c->ws;
+    for (int redo = 0; redo < 2; ++redo) {
+        if (redo) {
+            BH_LAUNCH(c, k_sort_fix, tiles, kSortThreads, 0, s, w.key[1], w.val[1], n, w.key[0], w.val[0], w.sc);
+            const int kgrid = (int)std::min<int64_t>(div_up(n, 256), (int64_t)c->sm_count * 8);
+            BH_LAUNCH(c, k_keys, kgrid, 256, 0, s, w.pos[c->cur], n, w.sc, w.key[0], w.key[1], w.val[0], w.val[1], w.sort_ghist, 1);
+        }
+        for (int p = 0; p < kSortPasses; ++p)
+            BH_LAUNCH(c, k_radix_pass, tiles, kSortThreads, kSortTile * 12, s, w.key[0], w.key[1], w.val[0], w.val[1], n, p, redo, w.sort_ghist + p * kRadix,
+                      w.sort_ticket + redo * kSortPasses + p, w.sort_status + ((size_t)redo * kSortPasses + p) * kRadix * tiles, w.sc);
     }
-    c->sorted = src;
+    c->sorted = 0;
     return BH_OK;
 }
 

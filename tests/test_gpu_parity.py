@@ -86,6 +86,35 @@ def test_short_sort_on_clustered_keys(BH, n, clump, radius, retries, front_mode)
     bh.close()
 
 
+@pytest.mark.parametrize("cfg,n", [("c1", 20000), ("c3", 12289)])
+def test_short_sort_of_large_inputs_follows_the_previous_tree(BH, cfg, n):
+    """The one-launch-per-pass front end (any n): the first build sorts in full; the next one sorts only the leading 3 x levels
+    bits of the previous tree (whole digits) and finishes the rest in the fix-up; a particle set that is far more clustered
+    than the previous tree suggests makes the device sort again in full.  Bit-exact against the oracle every time."""
+    pm, vel, prm = bh_inputs.make(cfg, n=n, seed=77)
+    bh = BH(n, front_mode=1)
+    g = gpu_tree(bh, pm, vel, prm["theta"], prm["eps"])
+    assert g["stats"].sort_passes == 8 and g["stats"].sort_retries == 0
+    levels = g["stats"].n_levels
+    st = oracle_state(pm, vel, prm["theta"], prm["eps"])
+    g2 = gpu_tree(bh, pm, vel, prm["theta"], prm["eps"])
+    assert g2["stats"].sort_passes == min(8, -(-3 * levels // 8)) < 8 and g2["stats"].sort_retries == 0
+    bad = compare_tree(g2, st)
+    compare_counts(g2, st, problems=bad)
+    assert not bad, "\n".join(bad)
+    pm3, vel3, _ = _with_clump(n, 900, 3e-4, seed=78) if cfg == "c1" else (None, None, None)
+    if pm3 is not None:
+        g3 = gpu_tree(bh, pm3, vel3, prm["theta"], 0.05)
+        assert g3["stats"].sort_passes < 8 and g3["stats"].sort_retries == 1
+        st3 = oracle_state(pm3, vel3, prm["theta"], 0.05)
+        bad = compare_tree(g3, st3)
+        compare_counts(g3, st3, problems=bad)
+        assert not bad, "\n".join(bad)
+        g4 = gpu_tree(bh, pm3, vel3, prm["theta"], 0.05)          # the deep tree of the clump now says how much to sort
+        assert g4["stats"].sort_retries == 1 and np.array_equal(g4["perm"], g3["perm"])
+    bh.close()
+
+
 @pytest.mark.parametrize("theta,eps", [(0.5, 0.01), (0.3, 0.0), (1.0, 0.05)])
 def test_parity_other_opening_angles_and_softening(BH, theta, eps):
     pm, vel, _ = bh_inputs.make("c1", n=8192, seed=7)
