@@ -17,8 +17,9 @@ __device__ __forceinline__ float ord2f(uint32_t u) {
 
 // Also decides how much of the key this build's first sort looks at (the short sort, see k_sort_fix): the tree of the
 // previous build on this context had n_levels levels, so keys that agree on 3 n_levels leading bits were at most nleaf then
-// (and are few now: particles move little between two builds); the first sort covers those bits in whole digits.  No
-// previous tree, an overflowed one, or short_ok = 0: all 8 passes.  A wrong guess costs time, never the result.
+// (and are few now: particles move little between two builds); the first sort covers those bits in whole digits.  (Fewer
+// bits were tried: 3 (n_levels - 2) saves a pass at 16 M but the fix-up's loops over runs of ~17 keys cost more than the pass.)
+// No previous tree, an overflowed one, or short_ok = 0: all 8 passes.  A wrong guess costs time, never the result.
 __global__ void k_reset_build(DevScalars* sc, int short_ok) {
     const int t = threadIdx.x;
     if (t < 3) { sc->bb_min[t] = 0xFFFFFFFFu; sc->bb_max[t] = 0u; }
@@ -160,8 +161,9 @@ __global__ void k_iota(uint32_t* dst, int n) {
 
 // ------------------------------------------------------------------------------------------ block scan
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* total) {
-    // 256 threads; returns the exclusive prefix of v over the block
-    __shared__ uint32_t wsum[8];
+    // returns the exclusive prefix of v over the block
+    constexpr int kW = kSortThreads / 32;
+    __shared__ uint32_t wsum[kW];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint32_t inc = v;
 #pragma unroll
@@ -173,7 +175,7 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* t
     __syncthreads();
     uint32_t base = 0, tot = 0;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
+    for (int k = 0; k < kW; ++k) {
         const uint32_t s = wsum[k];
         if (k < w) base += s;
         tot += s;
@@ -190,6 +192,9 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* t
 // (status word = flag | count: AGGREGATE = this tile only, PREFIX = this tile and all before it), so no key is read
 // twice and there is no separate histogram or scan launch.  Tiles are numbered by an atomic ticket, so a tile only ever
 // waits for tiles whose blocks are already running: the look-back cannot deadlock.
+#ifndef BH_FEW
+#define BH_FEW 8
+#endif
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kCountMask = (1u << 30) - 1u;
 constexpr uint32_t kSpinLimit = 1u << 22;   // ~1 s of polling
 
@@ -219,7 +224,7 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_pass(uint64_t* key0, uin
     const int shift = pass * kRadixBits;
     constexpr int kWarps = kSortThreads / 32;
     constexpr int kIters = kSortTile / kWarps / 32;   // 16
-    __shared__ uint32_t wcnt[kWarps][kRadix];
+    __shared__ uint16_t wcnt[kWarps][kRadix];      // (a warp holds kSortTile / kWarps <= 512 keys)
     __shared__ uint32_t gbase[kRadix], lbase[kRadix];
     __shared__ uint32_t s_tile;
     extern __shared__ __align__(16) unsigned char xch[];
@@ -227,7 +232,7 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_pass(uint64_t* key0, uin
     uint32_t* sval = reinterpret_cast<uint32_t*>(xch + kSortTile * 8);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
-    for (int j = threadIdx.x; j < kWarps * kRadix; j += kSortThreads) (&wcnt[0][0])[j] = 0;
+    for (int j = threadIdx.x; j < kWarps * kRadix / 2; j += kSortThreads) reinterpret_cast<uint32_t*>(&wcnt[0][0])[j] = 0u;
     __syncthreads();
     const uint32_t tile = s_tile;
 
@@ -243,68 +248,88 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_pass(uint64_t* key0, uin
         k[it] = ok ? key_in[i] : 0ull;
         v[it] = ok ? val_in[i] : 0u;
     }
+#ifdef BH_NO_MATCH
+    bool few = false;
+#else
+    bool few = pass >= kSortPasses / 2;              // (warp-uniform)
+#endif
 #pragma unroll
     for (int it = 0; it < kIters; ++it) {
         const int i = wbase + it * 32 + lane;
         const bool ok = i < n;
         const uint32_t d = (uint32_t)(k[it] >> shift) & (kRadix - 1);
-        // lanes with the same digit: one ballot per digit bit (the MATCH instruction is far slower than nine votes)
-        uint32_t peers = __ballot_sync(0xFFFFFFFFu, ok);
-        if (!ok) peers = ~peers;
+        // lanes with the same digit: MATCH costs one round per distinct value, the ballots a fixed nine votes; the row before
+        // says which is cheaper (the leading digits of clustered inputs take few values per row of 32 keys)
+        uint32_t peers;
+        if (few) {
+            peers = __match_any_sync(0xFFFFFFFFu, ok ? d : (uint32_t)kRadix);
+        } else {
+            peers = __ballot_sync(0xFFFFFFFFu, ok);
+            if (!ok) peers = ~peers;
 #pragma unroll
-        for (int b = 0; b < kRadixBits; ++b) {
-            const bool bit = (d >> b) & 1u;
-            const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
-            peers &= bit ? m : ~m;
+            for (int b = 0; b < kRadixBits; ++b) {
+                const bool bit = (d >> b) & 1u;
+                const uint32_t m = __ballot_sync(0xFFFFFFFFu, bit);
+                peers &= bit ? m : ~m;
+            }
         }
         const uint32_t before = __popc(peers & lt);
+#ifndef BH_NO_MATCH
+        few = __popc(__ballot_sync(0xFFFFFFFFu, before == 0u)) <= BH_FEW;
+#endif
         uint32_t old = 0;
         if (ok) old = wcnt[w][d];
         __syncwarp();
-        if (ok && before == 0) wcnt[w][d] = old + __popc(peers);
+        if (ok && before == 0) wcnt[w][d] = (uint16_t)(old + __popc(peers));
         __syncwarp();
         rank[it] = old + before;
     }
     __syncthreads();
-    // ---- digit = threadIdx.x: exclusive prefix over the warps, the tile's count, and the look-back over earlier tiles
+    // ---- digit = threadIdx.x (the first 256 threads): exclusive prefix over the warps, the tile's count, and the look-back
+    // over earlier tiles
     const uint32_t d = threadIdx.x;
+    const bool isd = d < (uint32_t)kRadix;
     uint32_t tcount = 0;
-#pragma unroll
-    for (int ww = 0; ww < kWarps; ++ww) {
-        const uint32_t t = wcnt[ww][d];
-        wcnt[ww][d] = tcount;
-        tcount += t;
-    }
     uint32_t excl = 0;
-    if (tile == 0) {
-        st_relaxed(status + d, kFlagPrefix | tcount);
-    } else {
-        st_relaxed(status + (size_t)tile * kRadix + d, kFlagAgg | tcount);
-        // look back eight tiles per round trip; the words are consumed in order, nearest tile first
-        int t = (int)tile - 1;
-        uint32_t spins = 0;
-        bool done = false;
-        while (!done) {
-            uint32_t wd[8];
+    if (isd) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) wd[j] = (t - j >= 0) ? ld_relaxed(status + (size_t)(t - j) * kRadix + d) : kFlagPrefix;
-            int used = 0;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                if (done || used != j) continue;
-                if (wd[j] & kFlagPrefix) { excl += wd[j] & kCountMask; done = true; }
-                else if (wd[j] & kFlagAgg) { excl += wd[j] & kCountMask; used = j + 1; }
-            }
-            t -= used;                                   // resume at the first tile that had nothing to report yet
-            if (!done && used == 0 && ++spins > kSpinLimit) { atomicMin(&sc->status, (int)BH_ERR_CUDA); break; }   // never hang the device
+        for (int ww = 0; ww < kWarps; ++ww) {
+            const uint32_t t = wcnt[ww][d];
+            wcnt[ww][d] = (uint16_t)tcount;
+            tcount += t;
         }
-        st_relaxed(status + (size_t)tile * kRadix + d, kFlagPrefix | (excl + tcount));
+        if (tile == 0) {
+            st_relaxed(status + d, kFlagPrefix | tcount);
+        } else {
+            st_relaxed(status + (size_t)tile * kRadix + d, kFlagAgg | tcount);
+            // look back eight tiles per round trip; the words are consumed in order, nearest tile first
+            int t = (int)tile - 1;
+            uint32_t spins = 0;
+            bool done = false;
+            while (!done) {
+                uint32_t wd[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) wd[j] = (t - j >= 0) ? ld_relaxed(status + (size_t)(t - j) * kRadix + d) : kFlagPrefix;
+                int used = 0;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    if (done || used != j) continue;
+                    if (wd[j] & kFlagPrefix) { excl += wd[j] & kCountMask; done = true; }
+                    else if (wd[j] & kFlagAgg) { excl += wd[j] & kCountMask; used = j + 1; }
+                }
+                t -= used;                                   // resume at the first tile that had nothing to report yet
+                if (!done && used == 0 && ++spins > kSpinLimit) { atomicMin(&sc->status, (int)BH_ERR_CUDA); break; }   // never hang the device
+            }
+            st_relaxed(status + (size_t)tile * kRadix + d, kFlagPrefix | (excl + tcount));
+        }
     }
     uint32_t dummy;
-    const uint32_t dbase = block_exclusive_scan(ghist[d], &dummy);   // first output slot of digit d
-    const uint32_t dstart = block_exclusive_scan(tcount, &dummy);    // first slot of digit d inside the tile, sorted by digit
-    gbase[d] = dbase + excl - dstart;                                // output slot = gbase[digit] + slot inside the sorted tile
-    lbase[d] = dstart;
+    const uint32_t dbase = block_exclusive_scan(isd ? ghist[d] : 0u, &dummy);   // first output slot of digit d
+    const uint32_t dstart = block_exclusive_scan(tcount, &dummy);               // first slot of digit d inside the tile, sorted by digit
+    if (isd) {
+        gbase[d] = dbase + excl - dstart;                                       // output slot = gbase[digit] + slot inside the sorted tile
+        lbase[d] = dstart;
+    }
     __syncthreads();
     // ---- exchange through shared memory: the tile leaves sorted by digit, so every digit's run is written contiguously
 #pragma unroll
