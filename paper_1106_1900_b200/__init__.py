@@ -5,4 +5,5 @@ Nothing here imports ``oracle/`` (test infrastructure); there is no CPU fallback
 """
 from .binding import (BarnesHut, BhError, BhStats, LIB_PATH, STAGES, SYMBOLS, direct_forces, load_library,  # noqa: F401
                       probe_fp32, workspace_bytes)
+from .pipeline import HostStepPipeline  # noqa: F401
 from .sharded import ShardedBarnesHut, balanced_bounds, keep_own_rows, share_bounds, share_mask  # noqa: F401

@@ -77,3 +77,41 @@ def test_graph_needs_forces_and_survives_new_particles_of_the_same_size(BH):
     bh.tree_build(); bh.compute_forces(0.75, 0.01)
     with pytest.raises(BhError):
         bh.step_graph_launch()                   # other n: the graphs were dropped
+
+
+def test_host_step_pipeline_matches_single_context_steps(BH):
+    """HostStepPipeline (two contexts on two streams, copies of one step beside the kernels of the other): every ticket returns
+    what the same calls give on one context, bit for bit, whatever the order of completion."""
+    import torch
+    from paper_1106_1900_b200 import HostStepPipeline
+    sets = []
+    for k in range(5):
+        pm, vel, prm = bh_inputs.make("c1", n=6000, seed=500 + k)
+        sets.append((torch.from_numpy(pm).pin_memory(), torch.from_numpy(vel).pin_memory(), torch.arange(6000, dtype=torch.int32).pin_memory()))
+    theta, eps, dt = prm["theta"], prm["eps"], prm["dt"]
+    ref = []
+    bh = BH(6000)
+    for hp, hv, hid in sets:
+        bh.set_particles(hp, hv, hid)
+        bh.tree_build()
+        bh.compute_forces(theta, eps)
+        bh.kick_drift(dt, dt)
+        out = (torch.empty((6000, 4)), torch.empty((6000, 4)), torch.empty((6000, 4)), torch.empty(6000, dtype=torch.int32))
+        bh.get_particles(*out)
+        torch.cuda.synchronize()
+        ref.append([o.clone() for o in out])
+    bh.close()
+    pipe = HostStepPipeline(6000, theta, eps, dt, depth=2)
+    tickets = []
+    for k, (hp, hv, hid) in enumerate(sets):
+        tickets.append(pipe.submit(hp, hv, hid))
+        if k >= 1:                                   # read the previous step while this one runs
+            got = pipe.result(tickets[k - 1])
+            for a, b in zip(got, ref[k - 1]):
+                assert torch.equal(a, b)
+    got = pipe.result(tickets[-1])
+    for a, b in zip(got, ref[-1]):
+        assert torch.equal(a, b)
+    with pytest.raises(ValueError):
+        pipe.result(tickets[0])                      # its buffers have been reused
+    pipe.close()
