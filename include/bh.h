@@ -58,7 +58,7 @@ typedef struct bh_config {
                          * k > 1: at least k waves, run as a pipeline (list walk of wave w + 1 beside the evaluation of
                          * wave w on internal streams); 0..255 */
     int32_t front_mode; /* 0 (default): S0-S3 in one cooperative launch whenever every sort tile is resident at once
-                         * (n <= 4096 x 2 x SMs, 1.2 M on B200), with the short sort (radix passes over the leading key bits only,
+                         * (n <= 8192 x SMs, 1.2 M on B200), with the short sort (radix passes over the leading key bits only,
                          * then every run of equal leading bits finished in place; the full sort is redone on the device if a
                          * run is too long: bh_stats.sort_retries); 1: always one launch per step and sort pass (any n);
                          * 2: the cooperative launch with all 8 radix passes.  The result is the same stable order in all three */
@@ -142,7 +142,13 @@ int bh_set_particles(bh_ctx* ctx, int64_t n, const float* pos_mass, const float*
  * accelerations would be in the previous order. */
 int bh_get_particles(bh_ctx* ctx, float* pos_mass, float* vel, float* acc_pot, uint32_t* id, void* stream);
 
-/* S0-S6: domain, keys, sort, reorder, octree, groups, fp64 moments and boxes (L55-65, L107-115).  theta-independent. */
+/* S0-S6: domain, keys, sort, reorder, octree, groups, fp64 moments and boxes (L55-65, L107-115).  theta-independent.
+ * S2 produces THE stable ascending order of the 60-bit keys (L362).  How: radix passes over the leading key bits only, every
+ * run of keys with equal leading bits finished in place, and the full 8-pass sort redone ON THE DEVICE when a run is too long
+ * for that (no host round trip; bh_stats.sort_passes / sort_retries say what happened; bh_config.front_mode = 2 sorts all 60
+ * bits in the first place).  The number of leading bits is a guess from n (one-launch front end) or from the depth of the
+ * previous tree on this context (any n): it changes the time, never the result.  A grid barrier or look-back that exceeds its
+ * spin limit (a device fault) sets the deferred status BH_ERR_CUDA and lets the kernel finish with an unspecified order. */
 int bh_tree_build(bh_ctx* ctx, void* stream);
 
 /* S7-S8 on the current tree: opening radii for `theta` (Eq.1), group walk, p-p and p-c forces + potentials

@@ -1,19 +1,26 @@
 // front.cu -- S0 domain box, S1 Morton keys, S2 stable LSD radix sort and S3 reorder in ONE cooperative launch, for
-// inputs whose sort tiles are all resident on the device at once (n <= 4096 x 2 x SMs: 1.2 M particles on B200).
+// inputs whose sort tiles are all resident on the device at once (n <= 8192 x SMs: 1.2 M particles on B200).
 // PAPER.md:374-392 (keys), PAPER.md:350-370 (split / radix sort), PAPER.md:174 ("moving").
 //
 // Why: at 1 M particles the whole front end moves ~0.3 GB that sits in the 126 MB L2; the round-1 sequence of 14
 // launches (box, domain, keys, 8 sort passes with a decoupled look-back each, reorder) spent its time in launch gaps and
-// in the look-back chain, not in bandwidth.  Here one block owns one tile of 4096 particles for the whole kernel:
+// in the look-back chain, not in bandwidth.  Here one block of 1024 threads per SM owns one tile of up to 8192 particles for
+// the whole kernel:
 //   * the box is reduced per tile and combined by every block after a grid barrier (no atomics, no reset launch);
 //   * the keys are made in registers and go straight into the first sort pass (the unsorted keys are never written);
-//   * a pass = rank the tile (one ballot per digit bit, as in keys_sort.cu), publish the tile's digit counts as a row
-//     of a [tiles][256] matrix (+ a reduction into the pass's global digit histogram), GRID BARRIER, sum the rows of
-//     the earlier tiles (all co-resident: no look-back chain), exchange through shared memory, scatter, GRID BARRIER;
-//   * the last phase gathers positions, velocities and ids by the permutation.
-// The barrier is a sense-reversing counter pair in the workspace (cooperative launch guarantees co-residency).
+//   * a pass = rank the tile (one ballot per digit bit, or MATCH.ANY where a row of 32 keys holds few distinct digits),
+//     publish the tile's digit counts as a row of a [tiles][256] matrix (+ a reduction into the sums of its group of 16
+//     tiles), GRID BARRIER, sum the group sums and the rows of the earlier tiles of the own group (all co-resident: no
+//     look-back chain), exchange through shared memory, scatter, GRID BARRIER;
+//   * THE SHORT SORT: the passes cover only the leading 8 x short_passes key bits; what is left to do is to order each run
+//     of keys with equal leading bits by the trailing bits (equal keys in their original order), which the fix-up does in
+//     a shared-memory window, and the particles are scattered to their final places from registers (S3).  A run too long
+//     for the window raises a flag that every block reads behind the closing barrier; the full 8-pass sort then follows
+//     in the same launch, from the keys made afresh.
+// The barriers are counters in the workspace (cooperative launch guarantees co-residency): barrier k of an attempt is
+// passed at k x blocks arrivals, the closing barrier counts on a word that only grows, so block 0 can zero the others.
 // Values other blocks wrote during this launch are read with ld.global.cg: L1 may hold lines from earlier passes.
-// Result: identical to keys_sort.cu (stable LSD order is unique), which still serves larger inputs.
+// Result: the stable order of the 60-bit keys, identical to keys_sort.cu's, which serves larger inputs.
 #include <algorithm>
 #include <cstdio>
 #include "bh_internal.cuh"
@@ -45,7 +52,7 @@ struct FrontArgs {
     float4* vel_out;
     uint32_t* id_out;
     int n;
-    int tile_n;          // keys per tile (block): a multiple of 512, <= kSortTile; the tiles are spread evenly over the SMs
+    int tile_n;          // keys per tile (block): a multiple of kFrontThreads, <= kFrontTile; the tiles are spread evenly over the SMs
     int fuse_reorder;
     uint64_t* key0;
     uint64_t* key1;
@@ -534,7 +541,7 @@ int front_init(bh_ctx* c) {
 
 bool front_fits(const bh_ctx* c) { return c->front_enabled && div_up(c->n, kFrontTile) <= c->front_max_tiles; }
 
-// Keys per tile: the input spread evenly over every resident block slot (two per SM), in multiples of 512.
+// Keys per tile: the input spread evenly over every resident block slot (one per SM), in multiples of the block size.
 static int front_tile(const bh_ctx* c) {
     const int64_t t = div_up(div_up(c->n, c->front_max_tiles), kFrontThreads) * kFrontThreads;
     return (int)std::min<int64_t>(std::max<int64_t>(t, kFrontThreads), kFrontTile);
