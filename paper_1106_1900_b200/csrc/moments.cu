@@ -438,85 +438,106 @@ k_moments_span(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo
     if (tid == 0) sh.cnt[nlev] = 0;
     __syncthreads();
     TLM();
-    for (int L = nlev - 1; L >= 0; --L) {
-        const int cur = L & 1, below = cur ^ 1;
-        const uint32_t cnt = sh.cnt[L], cntb = sh.cnt[L + 1];
-        const uint32_t* listb = sh.list[L + 1 < kLevels ? L + 1 : L];
-        // this CTA's nodes: q = rank + kSpanCtas * local, local = 0, 1, ...; lane group `grp` takes local = grp, grp + kSpanGroups, ...
-        // The stores to the cell arrays of a node are issued AFTER the cluster barrier has been signalled: the peers only
-        // need the shared-memory copy, and the barrier's release would otherwise wait for the global stores.
-        bool pend = false;
-        Mom pm;
-        uint4 pt = make_uint4(0u, 0u, 0u, 0u);
-        uint32_t pc = 0;
-        auto flush = [&]() {
-            if (!pend) return;
-            if (sub == 0) mom_store(pm, mom64, box, pc);
-            if (ro.enabled && sub == 1) rec_store(make_record(pm, ro.theta, ro.mac_kind, pt.x, pt.y, pt.z, pt.w), ro, pc);
-            pend = false;
-        };
-        for (uint32_t l0 = 0; rank + kSpanCtas * l0 < cnt; l0 += kSpanGroups) {
-            const uint32_t local = l0 + grp, q = rank + kSpanCtas * local;
-            if (rank + kSpanCtas * (local & ~3u) >= cnt) break;        // (warp-uniform) no node left for this warp's four groups
-            flush();
-            const bool have = q < cnt;
-            uint32_t c = 0;
-            uint4 t = make_uint4(0u, 0u, 0u, 0u);
-            if (have) { c = sh.list[L][q]; t = sh.topo[L][q]; }
-            int nch = have ? (int)(t.w - t.z) : 0;
-            bool clean = false;
-            if (partial) {                                              // all children clean: hand on what the cell arrays hold
-                uint32_t d = 0;
-                if (sub < nch) d = __ldcg(dirty + t.z + sub);
-                d |= __shfl_xor_sync(0xFFFFFFFFu, d, 1, 8); d |= __shfl_xor_sync(0xFFFFFFFFu, d, 2, 8); d |= __shfl_xor_sync(0xFFFFFFFFu, d, 4, 8);
-                if (have && sub == 0) dirty[c] = (uint8_t)(d ? 1 : 0);
-                clean = have && d == 0;
-                if (clean) nch = 0;
+    // A node's children are (a) cells that k_moments finished before this kernel started, or (b) straddling nodes of the
+    // level below.  (a) does not depend on anything computed here: while the cluster barrier of level L is pending (between
+    // its arrive and its wait), the lanes work out where the children of their node of level L - 1 are (binary search) and
+    // request the (a)-children, so that the chain over the levels holds only the shared-memory reads of the (b)-children,
+    // the sums and the barrier.  With at most kMomMaxBlocks straddling nodes per level a CTA has at most one node per lane
+    // group and level: node q = rank + kSpanCtas * grp.
+    struct Desc { bool have; uint32_t c; uint4 t; int nch; int src; };
+    auto describe = [&](int L) {
+        Desc d;
+        d.have = false; d.c = 0; d.t = make_uint4(0u, 0u, 0u, 0u); d.nch = 0; d.src = -1;
+        if (L < 0) return d;
+        const uint32_t q = rank + kSpanCtas * (uint32_t)grp;
+        if (q >= sh.cnt[L]) return d;
+        d.have = true;
+        d.c = sh.list[L][q];
+        d.t = sh.topo[L][q];
+        d.nch = (int)(d.t.w - d.t.z);
+        if (sub < d.nch) {
+            const uint32_t cc = d.t.z + sub;
+            const uint32_t* listb = sh.list[L + 1 < kLevels ? L + 1 : L];
+            const int cntb = (int)sh.cnt[L + 1];
+            int lo2 = 0, hi2 = cntb;
+            while (lo2 < hi2) {
+                const int mid = (lo2 + hi2) >> 1;
+                if (listb[mid] < cc) lo2 = mid + 1; else hi2 = mid;
             }
-            Child ch;
-            child_clear(ch);
-            if (clean && sub == 0) child_load_global(ch, mom64, box, c);   // (its own record, for the parent)
-            if (sub < nch) {
-                const uint32_t cc = t.z + sub;
-                int lo2 = 0, hi2 = (int)cntb;
-                while (lo2 < hi2) {
-                    const int mid = (lo2 + hi2) >> 1;
-                    if (listb[mid] < cc) lo2 = mid + 1; else hi2 = mid;
-                }
-                if (lo2 < (int)cntb && listb[lo2] == cc) {              // computed one level ago by CTA lo2 mod 8, kept in its slot lo2 / 8
-                    const SpanCell* remote = cluster.map_shared_rank(&sh.cell[below][lo2 / kSpanCtas], lo2 % kSpanCtas);
-                    child_load_shared(ch, *remote);
-                } else {
-                    child_load_global(ch, mom64, box, cc);
-                }
-            }
-            Mom m;
-            node_moments8(m, ch, nch, sub, sh.sx[grp]);
-            if (clean) {
-                if (sub == 0) {
-                    SpanCell& o = sh.cell[cur][local];
-                    o.m[0] = ch.M; o.m[1] = ch.c[0]; o.m[2] = ch.c[1]; o.m[3] = ch.c[2];
-#pragma unroll
-                    for (int k = 0; k < 6; ++k) o.m[4 + k] = ch.Q[k];
-#pragma unroll
-                    for (int k = 0; k < 3; ++k) { o.b[k] = ch.bn[k]; o.b[3 + k] = ch.bx[k]; }
-                }
-            } else if (have) {
-                if (sub == 0) {
-                    SpanCell& o = sh.cell[cur][local];
-                    o.m[0] = m.M; o.m[1] = m.com[0]; o.m[2] = m.com[1]; o.m[3] = m.com[2];
-#pragma unroll
-                    for (int k = 0; k < 6; ++k) o.m[4 + k] = m.Q[k];
-#pragma unroll
-                    for (int k = 0; k < 3; ++k) { o.b[k] = m.bmin[k]; o.b[3 + k] = m.bmax[k]; }
-                }
-                pend = true; pm = m; pt = t; pc = c;
-            }
+            if (lo2 < cntb && listb[lo2] == cc) d.src = lo2;             // computed one level earlier by CTA lo2 mod 8, kept in its slot lo2 / 8
         }
-        cluster.barrier_arrive();                                      // this CTA's part of the level is in its shared memory
-        flush();
-        cluster.barrier_wait();                                        // ... and so is everybody else's
+        return d;
+    };
+    auto request = [&](const Desc& d, Child& ch, Child& own, uint32_t& dflag) {
+        child_clear(ch);
+        child_clear(own);
+        dflag = 0;
+        if (d.have && sub < d.nch && d.src < 0) {
+            child_load_global(ch, mom64, box, d.t.z + sub);
+            if (partial) dflag = __ldcg(dirty + d.t.z + sub);
+        }
+        if (partial && d.have && sub == 0) child_load_global(own, mom64, box, d.c);   // (handed on unchanged when no child is dirty)
+    };
+    int Lc = nlev - 1;
+    while (Lc >= 0 && sh.cnt[Lc] == 0u) --Lc;                              // (levels without a straddling node: the same for every CTA)
+    Desc cur_d = describe(Lc);
+    Child cur_ch, cur_own;
+    uint32_t cur_df;
+    request(cur_d, cur_ch, cur_own, cur_df);
+    while (Lc >= 0) {
+        const int L = Lc;
+        const int cur = L & 1, below = cur ^ 1;
+        int Ln = L - 1;
+        while (Ln >= 0 && sh.cnt[Ln] == 0u) --Ln;
+        const bool have = cur_d.have;
+        const uint4 t = cur_d.t;
+        const uint32_t c = cur_d.c;
+        int nch = cur_d.nch;
+        Child ch = cur_ch;
+        uint32_t d = cur_df;
+        if (cur_d.src >= 0) {                                              // (b): from the shared memory of the CTA that owns it (DSMEM)
+            const SpanCell* remote = cluster.map_shared_rank(&sh.cell[below][cur_d.src / kSpanCtas], cur_d.src % kSpanCtas);
+            child_load_shared(ch, *remote);
+            d = __float_as_uint(remote->pad[0]);
+        }
+        bool clean = false;
+        if (partial) {                                                     // all children clean: hand on what the cell arrays hold
+            d |= __shfl_xor_sync(0xFFFFFFFFu, d, 1, 8); d |= __shfl_xor_sync(0xFFFFFFFFu, d, 2, 8); d |= __shfl_xor_sync(0xFFFFFFFFu, d, 4, 8);
+            if (have && sub == 0) dirty[c] = (uint8_t)(d ? 1 : 0);
+            clean = have && d == 0;
+            if (clean) { nch = 0; child_clear(ch); }
+        }
+        Mom m;
+        node_moments8(m, ch, nch, sub, sh.sx[grp]);
+        if (have && sub == 0) {
+            SpanCell& o = sh.cell[cur][grp];
+            if (clean) {
+                o.m[0] = cur_own.M; o.m[1] = cur_own.c[0]; o.m[2] = cur_own.c[1]; o.m[3] = cur_own.c[2];
+#pragma unroll
+                for (int k = 0; k < 6; ++k) o.m[4 + k] = cur_own.Q[k];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) { o.b[k] = cur_own.bn[k]; o.b[3 + k] = cur_own.bx[k]; }
+            } else {
+                o.m[0] = m.M; o.m[1] = m.com[0]; o.m[2] = m.com[1]; o.m[3] = m.com[2];
+#pragma unroll
+                for (int k = 0; k < 6; ++k) o.m[4 + k] = m.Q[k];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) { o.b[k] = m.bmin[k]; o.b[3 + k] = m.bmax[k]; }
+            }
+            o.pad[0] = __uint_as_float(partial ? (d ? 1u : 0u) : 1u);
+        }
+        cluster.barrier_arrive();                                          // this CTA's part of the level is in its shared memory
+        // while the barrier is pending: the stores to the cell arrays (the peers only need the shared-memory copy) and
+        // everything about the next level that does not depend on this one
+        if (have && !clean) {
+            if (sub == 0) mom_store(m, mom64, box, c);
+            if (ro.enabled && sub == 1) rec_store(make_record(m, ro.theta, ro.mac_kind, t.x, t.y, t.z, t.w), ro, c);
+        }
+        cur_d = describe(Ln);
+        request(cur_d, cur_ch, cur_own, cur_df);
+        cluster.barrier_wait();                                            // ... and so is everybody else's
         TLM();
+        Lc = Ln;
     }
 #ifdef BH_TIMELINE
     if (tid == 0 && rank == 0) { for (int q = 0; q < ntl; ++q) g_bh_dbg[384 + q] = tl[q]; g_bh_dbg[384 + 127] = ntl; }
