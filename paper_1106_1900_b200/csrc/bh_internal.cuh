@@ -87,6 +87,46 @@ __device__ __forceinline__ unsigned long long global_ns() {
     return t;
 }
 
+// ---- grid barriers of the cooperative kernels (front.cu, keys_sort.cu): counters in the workspace, bounded spins
+constexpr uint32_t kBarSpinLimit = 1u << 24;
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// All blocks of the (cooperative) grid meet here.  bar[0] counts the arrivals of every barrier but the last (barrier k is
+// passed at k x blocks arrivals); the last barrier of the launch counts on bar[1], which only ever grows (`b0` = its value
+// when this block started, read before any block can arrive there), so that block 0 can put bar[0] back to zero for the
+// next launch once everybody is known to have left it.
+__device__ __forceinline__ void grid_barrier(uint32_t* bar, uint32_t target, DevScalars* sc) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();                                   // release what this block wrote
+        atomicAdd(bar, 1u);
+        uint32_t spins = 0;
+        while (ld_acquire_u32(bar) < target)
+            if (++spins > kBarSpinLimit) { atomicMin(&sc->status, (int)BH_ERR_CUDA); break; }   // never hang the device
+        __threadfence();
+    }
+    __syncthreads();
+}
+// `closing`: the counter of the closing barriers (bar[1]), passed at `arrivals` arrivals since this block started; `used`: the
+// counter of the barriers before it, which block 0 puts back to zero.
+__device__ __forceinline__ void grid_barrier_last(uint32_t* closing, uint32_t b0, uint32_t arrivals, uint32_t* used, DevScalars* sc) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(closing, 1u);
+        uint32_t spins = 0;
+        while (ld_acquire_u32(closing) - b0 < arrivals)
+            if (++spins > kBarSpinLimit) { atomicMin(&sc->status, (int)BH_ERR_CUDA); break; }
+        if (blockIdx.x == 0) atomicExch(used, 0u);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
 // Pointers into the caller's workspace.
 struct Ws {
     DevScalars* sc;
@@ -113,7 +153,7 @@ struct Ws {
     float* front_part;    // [sortTiles][8] per-tile box of k_front
     uint32_t* front_matrix; // [frontTiles][kRadix] per-tile digit counts of the current pass
     uint32_t* front_gsum;   // [kSortPasses][kFrontGroupCap][kRadix] digit counts per pass and group of 16 tiles (zero between launches)
-    uint32_t* front_ctl;    // control words that are zero between launches: front_bar[5]
+    uint32_t* front_ctl;    // control words that are zero between launches: front_bar[5], then [5..6] the grid barrier of k_sort_passes
     uint32_t* front_bar;    // [5] grid barriers of k_front and its retry flag (front.cu: FrontArgs::bar)
     uint8_t* c_dirty;     // [max_cells] partial refresh (block time-steps): the cell has an active particle below it
     uint4* c_topo;        // [max_cells] (first particle, end particle, first child, end child); children (0, 0) for a leaf
@@ -171,6 +211,7 @@ struct bh_ctx {
     int mac_kind;          // 0: Eq.1, 1: minimum distance (bh_set_mac)
     bh::Ws ws;
     int64_t sort_tiles, tree_tiles;
+    int sort_grid;             // resident blocks of k_sort_passes (cooperative launch)
     int64_t front_max_tiles;   // sort tiles that are resident at once in a cooperative launch of k_front (0: not available)
     bool front_enabled;        // bh_config.front_mode != 1
     bool front_full;           // bh_config.front_mode == 2: k_front always sorts with all 8 passes

@@ -42,7 +42,6 @@ constexpr int kFrontWarps = kFrontThreads / 32;
 constexpr int kFrontItems = 8;                                  // keys per thread
 constexpr int kFrontTile = kFrontThreads * kFrontItems;         // most keys of a tile (block)
 constexpr int kFrontParts = kFrontThreads / kRadix;             // threads per digit in the prefix step
-constexpr uint32_t kBarSpinLimit = 1u << 24;
 
 struct FrontArgs {
     const float4* pos_in;
@@ -70,44 +69,6 @@ struct FrontArgs {
 
 constexpr int kFewDigits = 8;   // distinct digits in a row of 32 keys up to which MATCH.ANY beats nine ballots
 constexpr int kFixHalo = 64;   // the fix-up of the short sort finishes runs of keys with equal leading bits of at most this length
-
-__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
-    uint32_t v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-
-// All blocks of the (cooperative) grid meet here.  bar[0] counts the arrivals of every barrier but the last (barrier k is
-// passed at k x blocks arrivals); the last barrier of the launch counts on bar[1], which only ever grows (`b0` = its value
-// when this block started, read before any block can arrive there), so that block 0 can put bar[0] back to zero for the
-// next launch once everybody is known to have left it.
-__device__ __forceinline__ void grid_barrier(uint32_t* bar, uint32_t target, DevScalars* sc) {
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();                                   // release what this block wrote
-        atomicAdd(bar, 1u);
-        uint32_t spins = 0;
-        while (ld_acquire_u32(bar) < target)
-            if (++spins > kBarSpinLimit) { atomicMin(&sc->status, (int)BH_ERR_CUDA); break; }   // never hang the device
-        __threadfence();
-    }
-    __syncthreads();
-}
-// `closing`: the counter of the closing barriers (bar[1]), passed at `arrivals` arrivals since this block started; `used`: the
-// counter of the barriers before it, which block 0 puts back to zero.
-__device__ __forceinline__ void grid_barrier_last(uint32_t* closing, uint32_t b0, uint32_t arrivals, uint32_t* used, DevScalars* sc) {
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        atomicAdd(closing, 1u);
-        uint32_t spins = 0;
-        while (ld_acquire_u32(closing) - b0 < arrivals)
-            if (++spins > kBarSpinLimit) { atomicMin(&sc->status, (int)BH_ERR_CUDA); break; }
-        if (blockIdx.x == 0) atomicExch(used, 0u);
-        __threadfence();
-    }
-    __syncthreads();
-}
 
 __device__ __forceinline__ uint64_t dilate20f(uint32_t v) {
     uint64_t x = v & 0xFFFFFu;

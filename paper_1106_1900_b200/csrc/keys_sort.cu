@@ -114,23 +114,25 @@ __device__ __forceinline__ uint64_t dilate20(uint32_t v) {
     return x;
 }
 
-__device__ __forceinline__ uint32_t grid_coord(float x, float lo, int sh) {
-    const float d = __fsub_rn(x, lo);              // the only rounding
-    const float s = ldexpf(d, sh);                 // exact power-of-two scaling
-    const float t = truncf(s);
-    uint32_t v = (t > 0.0f) ? (uint32_t)t : 0u;
-    return min(v, (1u << kKeyBits) - 1u);
+// (x - lo) * 2^sh truncated and clamped to 20 bits.  The subtraction is the only rounding (O2): `scale` = 2^sh exactly
+// when sh is in the normal range (the product of a float and a power of two is exact unless it underflows, and then it is
+// < 1 either way); otherwise ldexpf.  cvt.rzi.u32.f32 truncates, sends negatives and NaN to 0 and saturates.
+__device__ __forceinline__ uint32_t grid_coord(float x, float lo, int sh, float scale) {
+    const float d = __fsub_rn(x, lo);
+    const float s = scale != 0.0f ? __fmul_rn(d, scale) : ldexpf(d, sh);
+    return min(__float2uint_rz(s), (1u << kKeyBits) - 1u);
 }
 
 // Also counts, for every sort pass, how many keys carry each digit value (ghist[pass][digit]): the sort then needs no
 // histogram pass of its own.
-// redo = 1: the keys again for the full re-sort, only if the fix-up asked for it (the histograms are still valid).
+// redo = 1: the keys again for the full re-sort, only if the fix-up asked for it.
 __global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pos, int n, DevScalars* __restrict__ sc,
                                               uint64_t* __restrict__ key0, uint64_t* __restrict__ key1, uint32_t* __restrict__ val0,
                                               uint32_t* __restrict__ val1, uint32_t* __restrict__ ghist, int redo) {
     if (redo && sc->sort_redo == 0u) return;
     if (redo && blockIdx.x == 0 && threadIdx.x == 0) sc->sort_retries += 1u;
-    const uint32_t sb = sort_start_buffer(sc->sort_skip, redo);
+    const uint32_t skip = sc->sort_skip;
+    const uint32_t sb = sort_start_buffer(skip, redo);
     uint64_t* __restrict__ key = sb ? key1 : key0;
     uint32_t* __restrict__ val = sb ? val1 : val0;
     __shared__ uint32_t h[kSortPasses * kRadix];
@@ -138,18 +140,19 @@ __global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pos, in
     __syncthreads();
     const float lox = sc->lo[0], loy = sc->lo[1], loz = sc->lo[2];
     const int sh = kKeyBits - sc->dom_e;
+    const float scale = (sh >= -126 && sh <= 127) ? __int_as_float((127 + sh) << 23) : 0.0f;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const float4 p = pos[i];
-        const uint32_t ix = grid_coord(p.x, lox, sh), iy = grid_coord(p.y, loy, sh), iz = grid_coord(p.z, loz, sh);
+        const uint32_t ix = grid_coord(p.x, lox, sh, scale), iy = grid_coord(p.y, loy, sh, scale), iz = grid_coord(p.z, loz, sh, scale);
         const uint64_t k = (dilate20(ix) << 2) | (dilate20(iy) << 1) | dilate20(iz);   // x most significant in a triple (A4)
         key[i] = k;
         val[i] = (uint32_t)i;
-        if (redo) continue;
+        // digit histograms: of the passes the first sort makes (digits skip..7); the re-sort adds those of the digits below
 #pragma unroll
-        for (int q = 0; q < kSortPasses; ++q) atomicAdd(&h[q * kRadix + ((uint32_t)(k >> (q * kRadixBits)) & (kRadix - 1))], 1u);
+        for (int q = 0; q < kSortPasses; ++q)
+            if (redo ? q < (int)skip : q >= (int)skip) atomicAdd(&h[q * kRadix + ((uint32_t)(k >> (q * kRadixBits)) & (kRadix - 1))], 1u);
     }
     __syncthreads();
-    if (redo) return;
     for (int j = threadIdx.x; j < kSortPasses * kRadix; j += blockDim.x)
         if (h[j]) atomicAdd(&ghist[j], h[j]);
 }
@@ -207,20 +210,11 @@ __device__ __forceinline__ void st_relaxed(uint32_t* p, uint32_t v) {
     asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// Warp w of the block owns the contiguous sub-tile [w*512, (w+1)*512): order = (warp, iteration, lane).
-// Pass `pass` (digit = key bits [8 pass, 8 pass + 8)) of the first sort (redo = 0: skipped when the short sort leaves this
-// digit to the fix-up) or of the full re-sort (redo = 1: skipped unless the fix-up asked for it).  The buffers alternate from
-// sort_start_buffer().
-__global__ void __launch_bounds__(kSortThreads) k_radix_pass(uint64_t* key0, uint64_t* key1, uint32_t* val0, uint32_t* val1,
-                                                             int n, int pass, int redo, const uint32_t* __restrict__ ghist, uint32_t* ticket,
-                                                             uint32_t* status, DevScalars* sc) {
-    const uint32_t skip = redo ? 0u : sc->sort_skip;
-    if (redo ? sc->sort_redo == 0u : (uint32_t)pass < skip) return;              // (the whole grid)
-    const uint32_t ib = (sort_start_buffer(skip, redo) + (uint32_t)pass - skip) & 1u;
-    const uint64_t* __restrict__ key_in = ib ? key1 : key0;
-    const uint32_t* __restrict__ val_in = ib ? val1 : val0;
-    uint64_t* __restrict__ key_out = ib ? key0 : key1;
-    uint32_t* __restrict__ val_out = ib ? val0 : val1;
+// One tile of one pass.  Warp w of the block owns the contiguous sub-tile [w*256, (w+1)*256): order = (warp, iteration, lane).
+// Returns false when the pass has no tile left (every thread of the block gets the same answer).
+__device__ __forceinline__ bool radix_tile(const uint64_t* __restrict__ key_in, const uint32_t* __restrict__ val_in, int n, int tiles, int pass,
+                                           const uint32_t* __restrict__ ghist, uint32_t* ticket, uint32_t* status,
+                                           uint64_t* __restrict__ key_out, uint32_t* __restrict__ val_out, DevScalars* sc) {
     const int shift = pass * kRadixBits;
     constexpr int kWarps = kSortThreads / 32;
     constexpr int kIters = kSortTile / kWarps / 32;   // 16
@@ -231,10 +225,12 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_pass(uint64_t* key0, uin
     uint64_t* skey = reinterpret_cast<uint64_t*>(xch);
     uint32_t* sval = reinterpret_cast<uint32_t*>(xch + kSortTile * 8);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    __syncthreads();                                   // (the previous tile of this block is done with the shared arrays)
     if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
     for (int j = threadIdx.x; j < kWarps * kRadix / 2; j += kSortThreads) reinterpret_cast<uint32_t*>(&wcnt[0][0])[j] = 0u;
     __syncthreads();
     const uint32_t tile = s_tile;
+    if (tile >= (uint32_t)tiles) return false;
 
     const int wbase = (int)tile * kSortTile + w * (kIters * 32);
     const uint32_t lt = (1u << lane) - 1u;
@@ -351,6 +347,34 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_pass(uint64_t* key0, uin
         key_out[dst] = kk;
         val_out[dst] = sval[lp];
     }
+    return true;
+}
+
+// All passes of a sort in ONE cooperative launch: the first sort (redo = 0: the passes from digit sort_skip up) or the full
+// re-sort (redo = 1: returns at once unless the fix-up asked for it).  The resident blocks draw tiles from the pass's ticket
+// counter until it runs out (a tile only ever waits for tiles with smaller tickets, whose blocks are running: the look-back
+// cannot deadlock), then meet at a grid barrier: the next pass reads what this one scattered.  Buffers alternate from
+// sort_start_buffer().  (One launch per pass cost ~4 us per launch, and the number of passes is only known on the device:
+// eight launches for the first sort and nine for the re-sort, most of them returning at once.)
+__global__ void __launch_bounds__(kSortThreads, 2) k_sort_passes(uint64_t* key0, uint64_t* key1, uint32_t* val0, uint32_t* val1, int n, int tiles, int redo,
+                                                              const uint32_t* __restrict__ ghist, uint32_t* ticket, uint32_t* status,
+                                                              DevScalars* sc, uint32_t* bar /* [2]: arrivals, closing arrivals */) {
+    const uint32_t skip = redo ? 0u : sc->sort_skip;
+    if (redo && sc->sort_redo == 0u) return;                                   // (the whole grid, before any barrier)
+    uint32_t b0 = 0, nbar = 0;
+    if (threadIdx.x == 0) b0 = ld_acquire_u32(bar + 1);
+    const uint32_t sb = sort_start_buffer(skip, redo);
+#pragma unroll 1
+    for (int pass = (int)skip; pass < kSortPasses; ++pass) {
+        const uint32_t ib = (sb + (uint32_t)pass - skip) & 1u;
+        const uint64_t* key_in = ib ? key1 : key0;
+        const uint32_t* val_in = ib ? val1 : val0;
+        uint64_t* key_out = ib ? key0 : key1;
+        uint32_t* val_out = ib ? val0 : val1;
+        while (radix_tile(key_in, val_in, n, tiles, pass, ghist + pass * kRadix, ticket + pass, status + (size_t)pass * kRadix * tiles, key_out, val_out, sc)) {}
+        if (pass + 1 < kSortPasses) grid_barrier(bar, ++nbar * gridDim.x, sc);
+        else grid_barrier_last(bar + 1, b0, gridDim.x, bar, sc);              // (puts bar[0] back to zero for the next launch)
+    }
 }
 
 // The fix-up of the short sort.  After the passes over the digits above bit 8 skip, buffer 1 is ordered by those leading bits,
@@ -393,7 +417,13 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_fix(const uint64_t* __res
 }
 
 int sort_init(bh_ctx* c) {
-    BH_CUDA(c, cudaFuncSetAttribute(k_radix_pass, cudaFuncAttributeMaxDynamicSharedMemorySize, kSortTile * 12));
+    BH_CUDA(c, cudaFuncSetAttribute(k_sort_passes, cudaFuncAttributeMaxDynamicSharedMemorySize, kSortTile * 12));
+    int per_sm = 0;
+    BH_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sort_passes, kSortThreads, kSortTile * 12));
+    int coop = 0;
+    BH_CUDA(c, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, c->device));
+    if (!coop || per_sm < 1) return BH_ERR_CUDA;
+    c->sort_grid = per_sm * c->sm_count;
     return BH_OK;
 }
 
@@ -431,23 +461,37 @@ int stage_bbox_keys(bh_ctx* c, cudaStream_t s) {
     return BH_OK;
 }
 
-// The first sort (as many passes as k_reset_build decided, then the fix-up), and the launches of the full re-sort, which
-// return at once unless the fix-up asked for it: the sequence of launches does not depend on the data (no host round
-// trip; capturable), and the result is in buffer 0 either way.
+// The first sort (as many passes as k_reset_build decided, in one cooperative launch, then the fix-up), and the launches of
+// the full re-sort, which return at once unless the fix-up asked for it: the sequence of launches does not depend on the data
+// (no host round trip; capturable), and the result is in buffer 0 either way.
+static int launch_sort_passes(bh_ctx* c, int redo, cudaStream_t s) {
+    const Ws& w = c->ws;
+    int n = (int)c->n, tiles = (int)div_up(c->n, kSortTile);
+    uint64_t *k0 = w.key[0], *k1 = w.key[1];
+    uint32_t *v0 = w.val[0], *v1 = w.val[1];
+    const uint32_t* gh = w.sort_ghist;
+    uint32_t* ticket = w.sort_ticket + redo * kSortPasses;
+    uint32_t* status = w.sort_status + (size_t)redo * kSortPasses * kRadix * tiles;
+    DevScalars* sc = w.sc;
+    uint32_t* bar = w.front_ctl + 5;
+    void* args[] = {&k0, &k1, &v0, &v1, &n, &tiles, &redo, &gh, &ticket, &status, &sc, &bar};
+    const int grid = std::min(c->sort_grid, tiles);
+    cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_sort_passes, dim3(grid), dim3(kSortThreads), args, (size_t)kSortTile * 12, s);
+    c->launches += 1;
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return BH_ERR_CUDA; }
+    return BH_OK;
+}
+
 int stage_sort(bh_ctx* c, cudaStream_t s) {
     const int n = (int)c->n;
     const int tiles = (int)div_up(n, kSortTile);
     const Ws& w = c->ws;
-    for (int redo = 0; redo < 2; ++redo) {
-        if (redo) {
-            BH_LAUNCH(c, k_sort_fix, tiles, kSortThreads, 0, s, w.key[1], w.val[1], n, w.key[0], w.val[0], w.sc);
-            const int kgrid = (int)std::min<int64_t>(div_up(n, 256), (int64_t)c->sm_count * 8);
-            BH_LAUNCH(c, k_keys, kgrid, 256, 0, s, w.pos[c->cur], n, w.sc, w.key[0], w.key[1], w.val[0], w.val[1], w.sort_ghist, 1);
-        }
-        for (int p = 0; p < kSortPasses; ++p)
-            BH_LAUNCH(c, k_radix_pass, tiles, kSortThreads, kSortTile * 12, s, w.key[0], w.key[1], w.val[0], w.val[1], n, p, redo, w.sort_ghist + p * kRadix,
-                      w.sort_ticket + redo * kSortPasses + p, w.sort_status + ((size_t)redo * kSortPasses + p) * kRadix * tiles, w.sc);
-    }
+    int rc = launch_sort_passes(c, 0, s);
+    if (rc != BH_OK) return rc;
+    BH_LAUNCH(c, k_sort_fix, tiles, kSortThreads, 0, s, w.key[1], w.val[1], n, w.key[0], w.val[0], w.sc);
+    const int kgrid = (int)std::min<int64_t>(div_up(n, 256), (int64_t)c->sm_count * 8);
+    BH_LAUNCH(c, k_keys, kgrid, 256, 0, s, w.pos[c->cur], n, w.sc, w.key[0], w.key[1], w.val[0], w.val[1], w.sort_ghist, 1);
+    if ((rc = launch_sort_passes(c, 1, s)) != BH_OK) return rc;
     c->sorted = 0;
     return BH_OK;
 }
