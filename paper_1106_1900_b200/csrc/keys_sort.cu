@@ -44,12 +44,19 @@ __device__ __forceinline__ uint32_t sort_start_buffer(uint32_t skip, int redo) {
 __global__ void __launch_bounds__(256) k_bbox(const float4* __restrict__ pos, int n, DevScalars* sc) {
     float mn[3] = {INFINITY, INFINITY, INFINITY}, mx[3] = {-INFINITY, -INFINITY, -INFINITY};
     int bad = 0;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const float4 p = pos[i];
+    const int stride = gridDim.x * blockDim.x;
+    for (int i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < n; i0 += 4 * stride) {
+        float4 q[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) q[u] = pos[min(i0 + u * stride, n - 1)];   // four loads in flight (a repeated last particle changes nothing)
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+        const float4 p = q[u];
         bad |= !(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(p.w) && p.w > 0.0f);
         mn[0] = fminf(mn[0], p.x); mx[0] = fmaxf(mx[0], p.x);
         mn[1] = fminf(mn[1], p.y); mx[1] = fmaxf(mx[1], p.y);
         mn[2] = fminf(mn[2], p.z); mx[2] = fmaxf(mx[2], p.z);
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -141,8 +148,12 @@ __global__ void __launch_bounds__(256) k_keys(const float4* __restrict__ pos, in
     const float lox = sc->lo[0], loy = sc->lo[1], loz = sc->lo[2];
     const int sh = kKeyBits - sc->dom_e;
     const float scale = (sh >= -126 && sh <= 127) ? __int_as_float((127 + sh) << 23) : 0.0f;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const float4 p = pos[i];
+    const int stride = gridDim.x * blockDim.x;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float4 pn = i < n ? pos[i] : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    for (; i < n; i += stride) {
+        const float4 p = pn;
+        if (i + stride < n) pn = pos[i + stride];          // (the next particle is on its way while this one is encoded)
         const uint32_t ix = grid_coord(p.x, lox, sh, scale), iy = grid_coord(p.y, loy, sh, scale), iz = grid_coord(p.z, loz, sh, scale);
         const uint64_t k = (dilate20(ix) << 2) | (dilate20(iy) << 1) | dilate20(iz);   // x most significant in a triple (A4)
         key[i] = k;
