@@ -1,5 +1,7 @@
-// keys_sort.cu -- S0 domain box, S1 Morton keys, S2 stable LSD radix sort, S3 reorder: one kernel per step, for inputs of
-// any size (inputs whose sort tiles are all resident at once take the single cooperative launch of front.cu instead).
+// keys_sort.cu -- S0 domain box, S1 Morton keys, S2 stable LSD radix sort, S3 reorder, for inputs of any size (inputs whose sort
+// tiles are all resident at once take the single cooperative launch of front.cu instead).  S2 is the SHORT sort of DESIGN.md
+// section 8: k_sort_passes (all radix passes over the leading key bits in one cooperative launch), k_sort_fix (every run of equal
+// leading bits finished in place), and the launches of a full re-sort that return at once unless the fix-up asked for it.
 // PAPER.md:374-392 (Appendix B: keys), PAPER.md:350-370 (Appendix A: scan, split, radix sort), PAPER.md:174 ("moving").
 #include <algorithm>
 #include "bh_internal.cuh"
@@ -200,8 +202,8 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* t
 }
 
 // ------------------------------------------------------------------------------------------ S2
-// Stable LSD radix sort, 8 bits per pass (the paper's 1-bit split generalised: PAPER.md:352, 362), ONE kernel
-// per pass.  The digit histograms of all passes were counted while the keys were made (k_keys).  A pass ranks a tile of
+// Stable LSD radix sort, 8 bits per pass (the paper's 1-bit split generalised: PAPER.md:352, 362).  The digit
+// histograms of the passes were counted while the keys were made (k_keys).  A pass ranks a tile of
 // 4096 keys, publishes the tile's digit counts and obtains the counts of all earlier tiles by a decoupled look-back
 // (status word = flag | count: AGGREGATE = this tile only, PREFIX = this tile and all before it), so no key is read
 // twice and there is no separate histogram or scan launch.  Tiles are numbered by an atomic ticket, so a tile only ever
