@@ -168,6 +168,30 @@ def oracle_sample(pm, vel, theta, eps, dt, budget_groups=None, seed=1):
                 interactions_per_s=inter / t_walk, cores=os.cpu_count())
 
 
+def _oracle_one_thread(args, theta, groups=2048):
+    """oracle_sample on `groups` seeded random groups of the same workload with OMP_NUM_THREADS=1 (a few seconds)."""
+    code = ("import json, sys; sys.path.insert(0, %r); import bench; cfg, n = %r, %d; "
+            "pm, vel, prm = bench._make_inputs(cfg, n, 0); "
+            "r = bench.oracle_sample(pm, vel, %r, prm['eps'], prm['dt'], budget_groups=%d); "
+            "print('ONE_THREAD ' + json.dumps(dict(value=r['value'], particles=r['particles'], groups=r['groups'], t_build=r['t_build'], "
+            "t_walk=r['t_walk'], interactions_per_s=r['interactions_per_s'])))") % (ROOT, _workload(args)[0], _workload(args)[1], float(theta), groups)
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    for k in ("RANK", "WORLD_SIZE", "LOCAL_RANK"):
+        env.pop(k, None)
+    try:
+        out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
+        for ln in out.stdout.splitlines():
+            if ln.startswith("ONE_THREAD "):
+                d = json.loads(ln[len("ONE_THREAD "):])
+                d.update(unit="particles/s", cores=1,
+                         sample=f"full oracle tree build (1 thread, {d['t_build']:.2f} s) + walk/forces of {d['groups']} seeded random groups = "
+                                f"{d['particles']} particles (1 thread, {d['t_walk']:.2f} s)")
+                return d
+    except Exception:
+        pass
+    return None
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -493,6 +517,10 @@ def run_ours(args):
                           f"random groups = {r['particles']} particles (OpenMP, {r['t_walk']:.2f} s); particles/s = sampled "
                           f"particles / (walk time + the sample's share of build+integration)"),
                "interactions_per_s": r["interactions_per_s"]}
+        # the same oracle with ONE thread, in a process of its own (OMP_NUM_THREADS is read when libgomp starts)
+        one = _oracle_one_thread(args, theta)
+        if one:
+            cpu["one_thread"] = one
 
     line = {
         "metric": "particles/sec per full step (build+walk+integrate)", "value": value, "unit": "particles/s",
