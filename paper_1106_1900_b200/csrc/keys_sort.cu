@@ -211,6 +211,10 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* t
 #ifndef BH_FEW
 #define BH_FEW 8
 #endif
+#ifndef BH_LOOK
+#define BH_LOOK 8
+#endif
+constexpr int kLook = BH_LOOK;   // earlier tiles a digit thread reads per round trip of the look-back
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kCountMask = (1u << 30) - 1u;
 constexpr uint32_t kSpinLimit = 1u << 22;   // ~1 s of polling
 
@@ -311,17 +315,17 @@ __device__ __forceinline__ bool radix_tile(const uint64_t* __restrict__ key_in, 
             st_relaxed(status + d, kFlagPrefix | tcount);
         } else {
             st_relaxed(status + (size_t)tile * kRadix + d, kFlagAgg | tcount);
-            // look back eight tiles per round trip; the words are consumed in order, nearest tile first
+            // look back kLook tiles per round trip; the words are consumed in order, nearest tile first
             int t = (int)tile - 1;
             uint32_t spins = 0;
             bool done = false;
             while (!done) {
-                uint32_t wd[8];
+                uint32_t wd[kLook];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) wd[j] = (t - j >= 0) ? ld_relaxed(status + (size_t)(t - j) * kRadix + d) : kFlagPrefix;
+                for (int j = 0; j < kLook; ++j) wd[j] = (t - j >= 0) ? ld_relaxed(status + (size_t)(t - j) * kRadix + d) : kFlagPrefix;
                 int used = 0;
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < kLook; ++j) {
                     if (done || used != j) continue;
                     if (wd[j] & kFlagPrefix) { excl += wd[j] & kCountMask; done = true; }
                     else if (wd[j] & kFlagAgg) { excl += wd[j] & kCountMask; used = j + 1; }
