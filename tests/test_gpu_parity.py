@@ -57,7 +57,7 @@ def _with_clump(n, clump, radius, seed):
 
 
 @pytest.mark.parametrize("front_mode", [0, 1])
-@pytest.mark.parametrize("n,clump,radius,retries", [(20000, 48, 3e-4, 0), (20000, 700, 3e-4, 1), (9000, 300, 0.0, 1), (4097, 4000, 1e-4, 1)])
+@pytest.mark.parametrize("n,clump,radius,retries", [(20000, 48, 3e-4, 0), (20000, 30, 0.0, 0), (20000, 700, 3e-4, 1), (9000, 300, 0.0, 1), (4097, 4000, 1e-4, 1)])
 def test_short_sort_on_clustered_keys(BH, n, clump, radius, retries, front_mode):
     """Runs of keys that agree on the leading bits the short sort looks at: a short run is finished by the fix-up (order of the
     trailing bits, equal keys in their original order), a long one makes the device redo the sort in full.  The permutation is
@@ -102,6 +102,17 @@ def test_short_sort_of_large_inputs_follows_the_previous_tree(BH, cfg, n):
     bad = compare_tree(g2, st)
     compare_counts(g2, st, problems=bad)
     assert not bad, "\n".join(bad)
+    if cfg == "c1":
+        # equal keys inside a run the fix-up finishes (40 coincident particles, the shallow tree's hint): their original order stays
+        pm5, vel5, _ = _with_clump(n, 40, 0.0, seed=79)
+        g5 = gpu_tree(bh, pm5, vel5, prm["theta"], 0.05)
+        assert g5["stats"].sort_passes < 8 and g5["stats"].sort_retries == 0
+        st5 = oracle_state(pm5, vel5, prm["theta"], 0.05)
+        assert np.unique(st5.keys).size < n
+        bad = compare_tree(g5, st5)
+        assert not bad, "\n".join(bad)
+        g = gpu_tree(bh, pm, vel, prm["theta"], prm["eps"])         # back to the plain set (and a shallow tree for the next hint)
+        g = gpu_tree(bh, pm, vel, prm["theta"], prm["eps"])
     pm3, vel3, _ = _with_clump(n, 900, 3e-4, seed=78) if cfg == "c1" else (None, None, None)
     if pm3 is not None:
         g3 = gpu_tree(bh, pm3, vel3, prm["theta"], 0.05)
