@@ -86,6 +86,48 @@ def test_short_sort_on_clustered_keys(BH, n, clump, radius, retries, front_mode)
     bh.close()
 
 
+def _many_clumps(n, clumps, size, radius, seed):
+    pm, vel, prm = bh_inputs.make("c1", n=n, seed=seed)
+    rng = np.random.Generator(np.random.Philox(seed + 1))
+    idx = rng.choice(n, size=clumps * size, replace=False).reshape(clumps, size)
+    for row in idx:
+        centre = pm[row[0], :3].astype(np.float64)
+        pm[row, :3] = (centre + rng.standard_normal((size, 3)) * radius).astype(np.float32)
+    return pm, vel, prm
+
+
+@pytest.mark.parametrize("seed,size", [(611, 100), (612, 100), (621, 60), (622, 60), (623, 60)])
+def test_short_sort_runs_across_tile_boundaries(BH, seed, size):
+    """Runs of ~100 / ~60 keys with equal leading bits, many of them, so that some lie across the boundary between two sort tiles:
+    inside the halo of 64 the fix-up finishes them from either side; a run that reaches further into the neighbouring tile
+    must be given up (full re-sort).  What the device has to decide is predicted here from the oracle's keys and the tiling."""
+    import torch
+    n = 30000
+    pm, vel, prm = _many_clumps(n, 6000 // size, size, 2e-4, seed)
+    st = oracle_state(pm, vel, prm["theta"], 0.05)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    tile = min(max(-(-(-(-n // sms)) // 1024) * 1024, 1024), 8192)
+    top = st.keys >> np.uint64(20)
+    edges = np.flatnonzero(np.concatenate([[True], top[1:] != top[:-1], [True]]))
+    halo, giveup, crossing = 64, False, 0
+    for a, b in zip(edges[:-1], edges[1:]):
+        if b - a > 2 * halo:
+            giveup = True
+        for w0 in range(tile, n, tile):
+            if a < w0 < b:
+                crossing += 1
+                if w0 - a >= halo or b - w0 >= halo:      # the window of one of the two tiles ends inside the run
+                    giveup = True
+    assert crossing > 0 and giveup == (size > 64)
+    bh = BH(n)
+    g = gpu_tree(bh, pm, vel, prm["theta"], 0.05)
+    bad = compare_tree(g, st)
+    compare_counts(g, st, problems=bad)
+    assert not bad, "\n".join(bad)
+    assert g["stats"].sort_retries == (1 if giveup else 0), (giveup, crossing)
+    bh.close()
+
+
 @pytest.mark.parametrize("cfg,n", [("c1", 20000), ("c3", 12289)])
 def test_short_sort_of_large_inputs_follows_the_previous_tree(BH, cfg, n):
     """The one-launch-per-pass front end (any n): the first build sorts in full; the next one sorts only the leading 3 x levels
