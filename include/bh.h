@@ -42,7 +42,8 @@ typedef enum bh_status {
                               * bounded device-side wait (grid barrier of the front end, look-back of a sort pass) ran out:
                               * the kernels then finish without writing out of bounds, but the build is not valid */
     BH_ERR_NONFINITE = -5,   /* deferred: NaN/Inf position or mass <= 0 seen by S0 (A27) */
-    BH_ERR_CAPACITY = -6     /* deferred: more cells than max_cells */
+    BH_ERR_CAPACITY = -6,    /* deferred: more cells than max_cells */
+    BH_ERR_TOO_LARGE = -7    /* bh_domain_box_static only: n is above BH_DOMAIN_STATIC_MAX_N, the built-in scratch cannot hold it */
 } bh_status;
 
 /* Tunables.  Zero-initialise and override; 0 means "default". */
@@ -264,6 +265,45 @@ int bh_get_walk_timeline(bh_ctx* ctx, void* stream, int64_t* ns, int capacity_wa
  * a_i = sum_{j != i} m_j (x_j - x_i) / rho_ij^3, rho^2 = |x_j - x_i|^2 + eps^2.  Needs no ctx; only enqueues work on
  * `stream`; both pointers are borrowed.  Not on the per-step path.  Returns BH_OK, BH_ERR_INVALID_ARG or BH_ERR_CUDA. */
 int bh_direct_forces(const float* d_pos_mass, int64_t n, float eps, int64_t t0, int64_t t1, double* d_acc_pot, void* stream);
+
+/* S0 on its own, WITHOUT a workspace and without any allocation: the domain box of n particles (per-axis minimum and
+ * maximum, exact), the cube side 2^domain_exp that bh_tree_build would use for them (the smallest power of two strictly above
+ * the largest extent, Appendix B "the domain"; O1) and the input check of S0 (finite positions, finite
+ * mass > 0; A27).  The result is bit for bit what bh_tree_build + bh_sync_status report in bh_stats.lo / hi /
+ * domain_exp for the same particles.
+ *
+ * For callers that cannot allocate device memory and so cannot create a bh_ctx (which needs a workspace): code living inside
+ * an application whose allocator already owns the whole GPU, processes held to a fixed device-memory budget where a cudaMalloc
+ * mid-run can fail, and time-step loops that must not call cudaMalloc / cudaFree because those stall every stream of the
+ * device.  This call makes no cudaMalloc, cudaFree or other allocating call.  Its intermediates (one partial box per 4096
+ * particles and a counter) sit in a 256 KiB array that is part of the library image, resident on every GPU that runs this
+ * library's kernels until the process ends; its fixed size is the reason for the limit:
+ *     n <= BH_DOMAIN_STATIC_MAX_N (2^25 = 33 554 432 particles; also returned by bh_domain_box_static_max_n).
+ * A larger n is refused with BH_ERR_TOO_LARGE before anything is enqueued -- split the input and merge the boxes, or use a ctx.
+ *
+ * d_pos_mass: float[n][4] DEVICE pointer (x, y, z, m), borrowed.  d_out: DEVICE pointer to one bh_domain_box (32 bytes) on the
+ * same device, written by the kernel: the caller copies it to the host (or reads it from a kernel of its own) after the work
+ * on `stream` has completed.  out->status is BH_OK or BH_ERR_NONFINITE (then lo / hi are the box of the finite coordinates
+ * and domain_exp is still a usable exponent).  Only enqueues work on `stream` (one 256-byte memset + one kernel); no host
+ * synchronisation.  The device is taken from the pointers; the caller's current device is restored on return.
+ *
+ * First call on each device: looks up the device address of the built-in array (cudaGetSymbolAddress, which may make the
+ * driver load the library's kernels on that device).  Make this first call during set-up, outside any stream capture.
+ *
+ * Sharing: every call on a device uses the same array, which still holds the previous call's contents; the call clears the
+ * one word that must start at zero itself.  Calls whose GPU work may OVERLAP on one device (two streams, two host threads)
+ * race on that array and return garbage: issue them on one stream, or order them with events.  Calls on different devices
+ * are independent.  Thread-safe on the host side.
+ * Returns BH_OK, BH_ERR_INVALID_ARG (null / host pointers, pointers on different devices, n < 1), BH_ERR_TOO_LARGE, BH_ERR_CUDA. */
+#define BH_DOMAIN_STATIC_MAX_N 33554432
+typedef struct bh_domain_box {
+    float   lo[3];        /* per-axis minimum = corner of the key grid */
+    float   hi[3];        /* per-axis maximum */
+    int32_t domain_exp;   /* cube side = 2^domain_exp */
+    int32_t status;       /* BH_OK or BH_ERR_NONFINITE */
+} bh_domain_box;
+int bh_domain_box_static(const float* d_pos_mass, int64_t n, bh_domain_box* d_out, void* stream);
+int64_t bh_domain_box_static_max_n(void);
 
 /* FP32 issue-rate probes ("a register-resident FFMA-chain probe"); a measurement aid, not on the
  * per-step path.  Runs one kernel on every SM of the current device (512 threads per block: four warps per scheduler,

@@ -16,14 +16,15 @@ LIB_PATH = os.path.join(HERE, "libbh_b200.so")
 
 BH_OK = 0
 STATUS = {0: "BH_OK", -1: "BH_ERR_INVALID_ARG", -2: "BH_ERR_WORKSPACE", -3: "BH_ERR_STATE", -4: "BH_ERR_CUDA",
-          -5: "BH_ERR_NONFINITE", -6: "BH_ERR_CAPACITY"}
+          -5: "BH_ERR_NONFINITE", -6: "BH_ERR_CAPACITY", -7: "BH_ERR_TOO_LARGE"}
 
 # every symbol include/bh.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", "bh_get_particles", "bh_tree_build",
            "bh_compute_forces", "bh_refresh_moments", "bh_compute_forces_active", "bh_refresh_moments_active", "bh_block_init", "bh_block_step",
            "bh_block_state", "bh_set_mac", "bh_leapfrog_step", "bh_step_graph_build",
            "bh_step_graph_launch", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
-           "bh_get_stage_ms", "bh_get_walk_timeline", "bh_direct_forces", "bh_probe_fp32", "bh_last_cuda_error", "bh_status_string"]
+           "bh_get_stage_ms", "bh_get_walk_timeline", "bh_direct_forces", "bh_domain_box_static", "bh_domain_box_static_max_n", "bh_probe_fp32", "bh_last_cuda_error",
+           "bh_status_string"]
 
 
 class BhConfig(C.Structure):
@@ -36,6 +37,10 @@ class BhStats(C.Structure):
                 ("n_groups", C.c_int64), ("sum_pc", C.c_int64), ("sum_pp", C.c_int64), ("sum_mac", C.c_int64),
                 ("launches", C.c_int64), ("lo", C.c_float * 3), ("hi", C.c_float * 3), ("domain_exp", C.c_int32),
                 ("sort_retries", C.c_int32), ("sort_passes", C.c_int32), ("reserved", C.c_int32)]
+
+
+class BhDomainBox(C.Structure):
+    _fields_ = [("lo", C.c_float * 3), ("hi", C.c_float * 3), ("domain_exp", C.c_int32), ("status", C.c_int32)]
 
 
 class BhBlockConfig(C.Structure):
@@ -109,6 +114,10 @@ def load_library():
     lib.bh_get_walk_timeline.restype = C.c_int
     lib.bh_direct_forces.argtypes = [C.c_void_p, C.c_int64, C.c_float, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
     lib.bh_direct_forces.restype = C.c_int
+    lib.bh_domain_box_static.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+    lib.bh_domain_box_static.restype = C.c_int
+    lib.bh_domain_box_static_max_n.argtypes = []
+    lib.bh_domain_box_static_max_n.restype = C.c_int64
     lib.bh_probe_fp32.argtypes = [C.c_int, C.c_void_p, C.c_size_t, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.bh_probe_fp32.restype = C.c_int
     lib.bh_last_cuda_error.argtypes = [C.c_void_p]
@@ -143,6 +152,41 @@ def direct_forces(pos_mass: torch.Tensor, eps: float, t0: int = 0, t1: int | Non
     if rc != BH_OK:
         raise BhError(rc, "bh_direct_forces")
     return out
+
+
+def domain_box_static_max_n() -> int:
+    """Most particles bh_domain_box_static accepts (the size of its built-in scratch array fixes it)."""
+    return int(load_library().bh_domain_box_static_max_n())
+
+
+def domain_box_static(pos_mass: torch.Tensor, out: torch.Tensor) -> torch.Tensor:
+    """bh_domain_box_static: the S0 domain box of ``pos_mass`` (CUDA float32[n,4]) without a context, a workspace or any
+    allocation by the library -- for callers that have no device memory to hand over and may not call cudaMalloc (all of the
+    card owned by another allocator, a fixed memory budget, a loop that cannot take cudaMalloc's device-wide stall).
+
+    ``out``: a CUDA int32[8] tensor on the same device that the CALLER provides (this wrapper allocates nothing either); the
+    kernel fills it with the 32 bytes of ``bh_domain_box``: lo xyz and hi xyz as float32 bit patterns, domain_exp, status.
+    Only enqueues work on the current stream of that device and returns ``out``; decode it with ``decode_domain_box`` after
+    synchronising.  n above ``domain_box_static_max_n()`` raises BhError(BH_ERR_TOO_LARGE).  All calls on one GPU share one
+    scratch array inside the library: keep them on one stream (or otherwise ordered); overlapping calls race.  The first call
+    on a device also looks up that array's address, so make it during set-up."""
+    if not (pos_mass.is_cuda and pos_mass.dtype == torch.float32 and pos_mass.is_contiguous() and pos_mass.dim() == 2 and pos_mass.shape[1] == 4):
+        raise BhError(-1, "pos_mass must be a contiguous CUDA float32[n,4] tensor")
+    if not (out.is_cuda and out.dtype == torch.int32 and out.is_contiguous() and out.numel() == 8 and out.device == pos_mass.device):
+        raise BhError(-1, "out must be a contiguous CUDA int32[8] tensor on the device of pos_mass")
+    n = int(pos_mass.shape[0])
+    rc = load_library().bh_domain_box_static(pos_mass.data_ptr(), n, out.data_ptr(),
+                                             C.c_void_p(torch.cuda.current_stream(pos_mass.device).cuda_stream))
+    if rc != BH_OK:
+        what = f"bh_domain_box_static: n = {n} exceeds the limit of {domain_box_static_max_n()} particles" if rc == -7 else "bh_domain_box_static"
+        raise BhError(rc, what)
+    return out
+
+
+def decode_domain_box(out: torch.Tensor) -> BhDomainBox:
+    """The int32[8] result of ``domain_box_static`` as a BhDomainBox (copies 32 bytes to the host: synchronises)."""
+    raw = out.detach().cpu().numpy().astype(np.int32, copy=False).tobytes()
+    return BhDomainBox.from_buffer_copy(raw)
 
 
 PROBE_KINDS = {"ffma": 0, "ffma2": 1, "ffma2_shared_operand": 2, "ffma2_broadcast_scalar": 3, "pc_body": 4, "pp_body": 5}

@@ -604,6 +604,7 @@ const char* bh_status_string(int status) {
         case BH_ERR_CUDA: return "CUDA runtime error";
         case BH_ERR_NONFINITE: return "non-finite position or mass <= 0 in the input";
         case BH_ERR_CAPACITY: return "tree needs more cells than max_cells";
+        case BH_ERR_TOO_LARGE: return "n is above BH_DOMAIN_STATIC_MAX_N: the built-in scratch of bh_domain_box_static cannot hold it";
         default: return "unknown status";
     }
 }
