@@ -73,7 +73,8 @@ typedef struct bh_ctx bh_ctx;
 
 /* What a step produced.  Filled by bh_sync_status (which synchronises the stream). */
 typedef struct bh_stats {
-    int32_t status;        /* deferred device status: BH_OK, BH_ERR_NONFINITE or BH_ERR_CAPACITY */
+    int32_t status;        /* deferred device status: BH_OK, BH_ERR_NONFINITE, BH_ERR_CAPACITY, BH_ERR_CUDA (a bounded device-side
+                            * wait ran out) or BH_ERR_STATE (block time-steps: the 32-bit tick counter is about to end) */
     int32_t n_levels;      /* deepest occupied level + 1 */
     int64_t n;             /* particles */
     int64_t n_cells;       /* tree cells (S4) */
@@ -139,8 +140,10 @@ int bh_destroy(bh_ctx* ctx);
 int bh_set_particles(bh_ctx* ctx, int64_t n, const float* pos_mass, const float* vel, const uint32_t* id, void* stream);
 
 /* Copy the current (key-sorted) state out; any pointer may be NULL; host or device destinations.  BH_ERR_STATE when
- * acc_pot is asked for between a bh_tree_build (which re-sorts the particles) and the next force evaluation: the stored
- * accelerations would be in the previous order. */
+ * acc_pot is asked for between a bh_tree_build (which re-sorts the particles) and the next evaluation that puts every row
+ * in the new order (bh_compute_forces, bh_leapfrog_step, bh_step_graph_launch, bh_block_step with a rebuild): the stored
+ * accelerations would be in the previous order.  bh_compute_forces_active alone does not lift this: it writes the rows of
+ * the walked groups only. */
 int bh_get_particles(bh_ctx* ctx, float* pos_mass, float* vel, float* acc_pot, uint32_t* id, void* stream);
 
 /* S0-S6: domain, keys, sort, reorder, octree, groups, fp64 moments and boxes (L55-65, L107-115).  theta-independent.
@@ -189,7 +192,13 @@ int bh_refresh_moments_active(bh_ctx* ctx, const uint8_t* d_active, void* stream
  *   tick, rung, the active flags of the last step, the held accelerations (float[n][4]).  interactions_now /
  *   interactions_first = the list lengths of the groups walked in the last step, now and when each group was first walked
  *   on the current cells: their ratio is the decline L266 speaks of ("the tree-cell size increases, which causes more
- *   cells to be opened"); the caller rebuilds when it has grown too far. */
+ *   cells to be opened"); the caller rebuilds when it has grown too far.
+ * Time is counted in 32-bit ticks of dt_max / 2^max_rung: a run can cover 2^(32 - max_rung) dt_max (4096 dt_max at max_rung = 20).
+ *   When the system time comes within two dt_max of that end, the deferred status (bh_sync_status) of the step becomes
+ *   BH_ERR_STATE; that step and the next are still exact.  Start over with bh_block_init (ticks restart at 0).
+ * acc_pot (bh_get_particles) after a block step: the new acceleration for the active particles; for the others either the one
+ *   held by the scheme (after a step with rebuild != 0) or a newer by-product of a walk of their group.  The scheme's own
+ *   accelerations are acc_held of bh_block_state. */
 typedef struct bh_block_config {
     float len_scale;    /* length in the criterion (e.g. the softening eps), > 0 */
     float eta;          /* accuracy parameter, > 0 */

@@ -304,7 +304,9 @@ static int compute_forces_impl(bh_ctx* c, float theta, float eps, const uint8_t*
     if (rc != BH_OK) return rc;
     c->theta_last = theta;
     c->have_forces = true;
-    c->acc_in_order = true;    // (after an active-subset walk the rows of the other groups keep what they held)
+    // A full walk writes every row of acc_pot in the current order.  An active-subset walk writes the rows of the walked
+    // groups only: the others keep what they held, which is in order only if nothing re-sorted the particles since.
+    if (!d_active) c->acc_in_order = true;
     return BH_OK;
 }
 
@@ -360,6 +362,10 @@ int bh_block_step(bh_ctx* c, float theta, float eps, int rebuild, void* stream) 
         // S0-S6 on the current positions (the active ones predicted); the block state then follows the sort
         if ((rc = bh_tree_build(c, stream)) != BH_OK) return rc;
         if ((rc = stage_block_permute(c, s)) != BH_OK) return rc;
+        // acc_pot did not follow the sort.  Put the held accelerations (which did) there, so that the rows the walk below does
+        // not write belong to the right particles: for those, acc_pot = the acceleration of the particle's last own update.
+        BH_CUDA(c, cudaMemcpyAsync(c->ws.acc, c->ws.accb[c->bcur], sizeof(float4) * (size_t)c->n, cudaMemcpyDeviceToDevice, s));
+        c->acc_in_order = true;
         c->blk_since_rebuild = 0;
         act = c->ws.bactive[c->bcur];
     } else {
@@ -429,6 +435,11 @@ int bh_step_graph_build(bh_ctx* c, float theta, float eps, float dt, void* strea
     // parity; capturing only records the launches, nothing runs, and after the second capture the host-side state is back
     // where it started.
     const int64_t launches0 = c->launches;
+    // ... except for what describes the DEVICE: capturing bh_leapfrog_step walks through its bookkeeping (records written for
+    // theta, accelerations in order, split walk timed) although no kernel ran.  Keep the truth and put it back afterwards.
+    const bool rec_valid0 = c->rec_valid, acc_in_order0 = c->acc_in_order, split0 = c->walk_split_timed;
+    const float rec_theta0 = c->rec_theta, theta_last0 = c->theta_last;
+    const int rec_mac0 = c->rec_mac;
     int rc = BH_OK;
     for (int k = 0; k < 2 && rc == BH_OK; ++k) {
         const int parity = c->cur;
@@ -447,6 +458,9 @@ int bh_step_graph_build(bh_ctx* c, float theta, float eps, float dt, void* strea
     }
     c->graph_launches = (c->launches - launches0) / 2;
     c->launches = launches0;
+    c->graph_split_timed = c->walk_split_timed;               // what a replay leaves behind (bh_step_graph_launch)
+    c->rec_valid = rec_valid0; c->rec_theta = rec_theta0; c->rec_mac = rec_mac0;
+    c->acc_in_order = acc_in_order0; c->walk_split_timed = split0; c->theta_last = theta_last0;
     if (rc != BH_OK) { (void)cudaGetLastError(); drop_step_graph(c); return rc; }
     c->graph_theta = theta; c->graph_eps = eps; c->graph_dt = dt;
     c->step_graph_valid = true;
@@ -463,6 +477,12 @@ int bh_step_graph_launch(bh_ctx* c, void* stream) {
     c->cur ^= 1;
     c->theta_last = c->graph_theta;
     c->launches += c->graph_launches;
+    c->rec_valid = true;                                      // S6 of the captured step wrote the fp32 records for its theta
+    c->rec_theta = c->graph_theta;                            // (bh_set_mac drops the graphs, so mac_kind is the captured one)
+    c->rec_mac = c->mac_kind;
+    c->acc_in_order = true;                                   // a full walk
+    c->walk_split_timed = c->graph_split_timed;
+    c->have_topology = c->have_tree = c->have_forces = true;
     return BH_OK;
 }
 

@@ -231,6 +231,7 @@ struct bh_ctx {
     bool step_graph_valid;
     float graph_theta, graph_eps, graph_dt;
     int64_t graph_launches;          // kernels in one captured step
+    bool graph_split_timed;          // walk_split_timed as the captured step leaves it
     cudaEvent_t ev[13];     // [0..10] stage boundaries; [11], [12]: after the list walk / the evaluation of a one-wave walk
     bool copies_pending;    // bh_set_particles left copies on s_lists; ev_join marks their end (api.cu: join_copies)
     bool walk_split_timed;  // the last walk was one wave: ev[11], ev[12] are valid

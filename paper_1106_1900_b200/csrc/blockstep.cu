@@ -99,9 +99,14 @@ __global__ void __launch_bounds__(256) k_block_permute(const uint32_t* __restric
 __global__ void __launch_bounds__(256) k_block_correct(float4* __restrict__ vel, float4* __restrict__ accb, const float4* __restrict__ acc,
                                                        uint32_t* __restrict__ tick, uint8_t* __restrict__ rung, const uint8_t* __restrict__ active,
                                                        int n, int R, float dt_max, float len, float eta, const uint32_t* __restrict__ tick_next,
-                                                       uint32_t* tick_next_idle) {
+                                                       uint32_t* tick_next_idle, DevScalars* sc) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i == 0) *tick_next_idle = 0xFFFFFFFFu;              // the other parity's slot, for the next step
+    if (i == 0) {
+        *tick_next_idle = 0xFFFFFFFFu;                      // the other parity's slot, for the next step
+        // ticks are 32-bit: tick + 2^(R - rung) must not wrap.  Within two longest steps of 2^32 the deferred status says so
+        // (this step and the next are still exact); the caller starts over with bh_block_init.
+        if (*tick_next >= 0xFFFFFFFFu - (2u << R)) atomicMin(&sc->status, (int)BH_ERR_STATE);
+    }
     if (i >= n || !active[i]) return;
     const uint32_t now = *tick_next;
     const int r = rung[i];
@@ -148,7 +153,8 @@ int stage_block_predict(bh_ctx* c, cudaStream_t s) {
     const int n = (int)c->n, b = c->bcur;
     uint32_t* tn = &c->ws.sc->tick_next[c->blk_steps & 1];
     const int grid = (int)std::min<int64_t>(div_up(n, 256), (int64_t)c->sm_count * 8);
-    BH_CUDA(c, cudaMemsetAsync(&c->ws.sc->n_active, 0, sizeof(DevScalars) - offsetof(DevScalars, n_active), s));   // n_active, deg_now, deg_base (the last members)
+    // n_active, deg_now, deg_base and nothing else (the sort's words behind them keep their values: sort_retries counts since bh_create)
+    BH_CUDA(c, cudaMemsetAsync(&c->ws.sc->n_active, 0, offsetof(DevScalars, sort_skip) - offsetof(DevScalars, n_active), s));
     BH_LAUNCH(c, k_block_next, grid, 256, 0, s, c->ws.tick[b], c->ws.rung[b], n, c->blk_R, tn);
     BH_LAUNCH(c, k_block_predict, (unsigned)div_up(n, 256), 256, 0, s, c->ws.pos[c->cur], c->ws.vel[c->cur], c->ws.accb[b], c->ws.tick[b], c->ws.rung[b],
               n, c->blk_R, c->blk_dt_max, tn, c->ws.bactive[b], c->ws.sc);
@@ -168,7 +174,7 @@ int stage_block_correct(bh_ctx* c, cudaStream_t s) {
     uint32_t* tn = &c->ws.sc->tick_next[c->blk_steps & 1];
     uint32_t* idle = &c->ws.sc->tick_next[(c->blk_steps + 1) & 1];
     BH_LAUNCH(c, k_block_correct, (unsigned)div_up(n, 256), 256, 0, s, c->ws.vel[c->cur], c->ws.accb[b], c->ws.acc, c->ws.tick[b], c->ws.rung[b],
-              c->ws.bactive[b], n, c->blk_R, c->blk_dt_max, c->blk_len, c->blk_eta, tn, idle);
+              c->ws.bactive[b], n, c->blk_R, c->blk_dt_max, c->blk_len, c->blk_eta, tn, idle, c->ws.sc);
     const int grid = (int)std::min<int64_t>(div_up(n, 256), (int64_t)c->sm_count * 4);
     BH_LAUNCH(c, k_block_degrade, grid, 256, 0, s, c->ws.sc, c->ws.gflag, c->ws.g_npc, c->ws.g_npp, c->ws.g_base);
     return BH_OK;

@@ -584,11 +584,15 @@ int stage_moments(bh_ctx* c, float theta, const uint8_t* d_active, cudaStream_t 
     const int nb = (int)div_up(n + 1, P);
     const int tiles = (int)div_up(n + 1, kTreeTile);
     const bool rec = theta > 0.0f;
+    // A partial refresh rewrites the fp32 records of the dirty cells only; the others keep what they hold, which is good only
+    // if that was written for this same criterion.  Otherwise the records are not valid as a whole and stage_walk redoes them.
+    const bool partial = d_active != nullptr;
+    const bool kept = c->rec_valid && c->rec_theta == theta && c->rec_mac == c->mac_kind;
     BH_LAUNCH(c, k_moments, nb, kMomThreads, sizeof(NodeScratch) * kMomGroups, s, c->ws.sc, c->ws.pos[c->cur], (int)n, (int)P, tiles, c->ws.tile_cnt, c->ws.c_topo,
               c->ws.mom64, c->ws.box, c->ws.mom_span, rec_out(c, theta, rec), d_active, c->ws.c_dirty);
     BH_LAUNCH(c, k_moments_span, kSpanCtas, kSpanThreads, sizeof(SpanShared), s, c->ws.sc, c->ws.c_topo, c->ws.mom64, c->ws.box,
               c->ws.mom_span, (uint32_t)nb, rec_out(c, theta, rec), c->ws.c_dirty, d_active ? 1 : 0);
-    c->rec_valid = rec;
+    c->rec_valid = rec && (!partial || kept);
     c->rec_theta = theta;
     c->rec_mac = c->mac_kind;
     return BH_OK;
