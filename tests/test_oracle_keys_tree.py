@@ -233,3 +233,37 @@ def test_groups_overflow_leaf_is_chunked():
     t = oracle.make_groups(oracle.build_tree(ks))
     assert list(t.gcount) == [64, 64, 22] and list(t.gbegin) == [0, 64, 128]
     assert np.all(t.gcell == 20)
+
+
+# ---------------------------------------------------------------- A13: group boxes (the walk's targets, S7)
+@pytest.mark.parametrize("cfg,n", [("c1", 16384), ("c3", 30000), ("c1", 50), ("c1", 1)])
+def test_group_boxes_are_the_min_and_max_of_the_groups_particles(cfg, n):
+    """orc_group_boxes against numpy's own min / max over each group's slice, the cell a group comes from (a group is all
+    of one cell's particles unless it is a chunk of an overflow leaf: then the cell's box contains it) and the domain."""
+    pm, vel, _ = bh_inputs.make(cfg, n=n)
+    st = oracle.tree_build(pm, vel)
+    t = st.tree
+    assert t.gbox.shape == (t.ngroups, 6) and t.gbox.dtype == np.float32
+    for g in range(t.ngroups):
+        p = st.pos[t.gbegin[g]: t.gbegin[g] + t.gcount[g], :3]
+        assert np.array_equal(t.gbox[g, :3], p.min(axis=0)) and np.array_equal(t.gbox[g, 3:], p.max(axis=0))
+    whole = t.pcount[t.gcell] == t.gcount
+    assert np.array_equal(t.gbox[whole], t.box[t.gcell[whole]])
+    assert np.all(t.gbox[:, :3] >= t.box[t.gcell][:, :3]) and np.all(t.gbox[:, 3:] <= t.box[t.gcell][:, 3:])
+    assert np.array_equal(t.gbox[:, :3].min(axis=0), st.pos[:, :3].min(axis=0)) and np.array_equal(t.gbox[:, 3:].max(axis=0), st.pos[:, :3].max(axis=0))
+
+
+def test_group_boxes_of_overflow_chunks():
+    """150 particles on one key: groups of 64, 64, 22 consecutive particles, each with its own box inside the leaf's."""
+    rng = np.random.default_rng(3)
+    pm = np.zeros((150, 4), np.float32)
+    pm[:, :3] = (0.25 + rng.random((150, 3)) * 1e-9).astype(np.float32)      # one level-20 cell of the unit cube
+    pm[:, 3] = 1.0 / 150
+    far = np.array([[0.0, 0.0, 0.0, 1e-3], [1.0, 1.0, 1.0, 1e-3]], np.float32)  # fixes the domain to [0, 2)^3
+    st = oracle.tree_build(np.concatenate([far[:1], pm, far[1:]]), None)
+    t = st.tree
+    big = np.nonzero(t.gcount == 64)[0]
+    assert big.size == 2 and sorted(t.gcount.tolist()) == [1, 1, 22, 64, 64]
+    for g in range(t.ngroups):
+        p = st.pos[t.gbegin[g]: t.gbegin[g] + t.gcount[g], :3]
+        assert np.array_equal(t.gbox[g, :3], p.min(axis=0)) and np.array_equal(t.gbox[g, 3:], p.max(axis=0))
