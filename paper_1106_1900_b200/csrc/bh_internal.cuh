@@ -19,10 +19,7 @@ constexpr uint32_t kSkip = 0xFFFFFFFEu;   // g_pcoff of a group that is not acti
 constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kSortPasses = 8;                 // 8 x 8 bits covers the 60-bit key
-#ifndef BH_SORT_THREADS
-#define BH_SORT_THREADS 512
-#endif
-constexpr int kSortThreads = BH_SORT_THREADS;    // 512 x 8 keys: 64 registers per thread, 48 warps per SM (256 x 16: 128 registers, 16 warps)
+constexpr int kSortThreads = 512;    // 512 x 8 keys: 64 registers per thread, 48 warps per SM (256 x 16: 128 registers, 16 warps)
 constexpr int kSortItemsPerThread = 4096 / kSortThreads;
 constexpr int kSortTile = kSortThreads * kSortItemsPerThread;   // 4096 keys per block
 

@@ -25,18 +25,10 @@
 #include <cstdio>
 #include "bh_internal.cuh"
 
-#ifdef BH_TIMELINE
-// working aid (-DBH_TIMELINE builds only): %globaltimer stamps of this file's kernel, read back by bh_debug_front
-__device__ unsigned long long g_bh_dbg[1024];
-extern "C" int bh_debug_front(unsigned long long* host1024) { return (int)cudaMemcpyFromSymbol(host1024, g_bh_dbg, sizeof(unsigned long long) * 1024); }
-#endif
 
 namespace bh {
 
-#ifndef BH_FRONT_THREADS
-#define BH_FRONT_THREADS 1024
-#endif
-constexpr int kFrontThreads = BH_FRONT_THREADS;                 // 1024: one block per SM (half as many arrivals at every grid barrier); 512: two
+constexpr int kFrontThreads = 1024;                             // 1024: one block per SM (half as many arrivals at every grid barrier); 512: two
 constexpr int kFrontBlocksPerSM = 1024 / kFrontThreads;
 constexpr int kFrontWarps = kFrontThreads / 32;
 constexpr int kFrontItems = 8;                                  // keys per thread
@@ -130,13 +122,6 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
     const uint32_t lt = (1u << lane) - 1u;
     uint32_t b0 = 0, nbar = 0;                             // barrier bookkeeping (thread 0)
     if (tid == 0) b0 = ld_acquire_u32(a.bar + 1);
-#ifdef BH_TIMELINE
-    int ntl = 0;
-#define TL() do { if (tid == 0 && (tile == 0 || tile == T - 1) && ntl < 120) g_bh_dbg[(tile == 0 ? 0 : 128) + ntl++] = global_ns(); } while (0)
-#else
-#define TL() do {} while (0)
-#endif
-    TL();
 
     // ---------------------------------------------------------------- S0: box of this tile
     {
@@ -174,9 +159,7 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
             a.part[(size_t)tile * 8 + tid] = v;
         }
     }
-    TL();
     grid_barrier(a.bar, ++nbar * T, a.sc);
-    TL();
 
     // ---------------------------------------------------------------- domain (every block, redundantly): DESIGN.md O1
     {
@@ -266,7 +249,6 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
             }
         }
 
-        TL();
         // ------------------------------------------------------------ S2: passes of 8 bits
 #pragma unroll 1
         for (int pass = 0; pass < npass; ++pass) {
@@ -287,7 +269,6 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
             }
             for (int j = tid; j < kFrontWarps * kRadix / 2; j += kFrontThreads) reinterpret_cast<uint32_t*>(&wcnt[0][0])[j] = 0u;
             __syncthreads();
-            TL();
             uint32_t rank[kFrontItems];
             bool few = pass > 0;                                               // (warp-uniform)
 #pragma unroll
@@ -321,7 +302,6 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
                 rank[it] = old + before;
             }
             __syncthreads();
-            TL();
             // digit = tid (first 256 threads): exclusive prefix over the warps, the tile's count; publish it
             uint32_t tcount = 0;
             if (tid < kRadix) {
@@ -335,9 +315,7 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
                 if (tcount) atomicAdd(a.gsum + ((size_t)pass * kFrontGroupCap + (tile >> 4)) * kRadix + tid, tcount);
             }
             const uint32_t dstart = block_excl_scan512(tcount, wsum);             // first slot of digit d inside the tile, sorted by digit
-            TL();
             grid_barrier(barw, ++nbar * T, a.sc);
-            TL();
             // keys of this digit in the whole input (-> first output slot of the digit) and in the earlier tiles: the sums of the
             // groups of 16 tiles + the rows of the earlier tiles of this tile's own group; split between the two halves of the block
             {
@@ -368,7 +346,6 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
                 lbase[tid] = dstart;
             }
             __syncthreads();
-            TL();
             // exchange through shared memory: the tile leaves sorted by digit, so every digit's run is written contiguously
 #pragma unroll
             for (int it = 0; it < kFrontItems; ++it) {
@@ -381,7 +358,6 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
                 }
             }
             __syncthreads();
-            TL();
 #pragma unroll 4
             for (int lp = tid; lp < cnt_tile; lp += kFrontThreads) {
                 const uint64_t kk = skey[lp];
@@ -389,10 +365,8 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
                 kout[dst] = kk;
                 vout[dst] = sval[lp];
             }
-            TL();
             if (full && pass + 1 == npass) grid_barrier_last(a.bar + 1, b0, (uint32_t)(attempt + 1) * T, barw, a.sc);
             else grid_barrier(barw, ++nbar * T, a.sc);
-            TL();
             if (tile < G && tid < kRadix) a.gsum[((size_t)pass * kFrontGroupCap + tile) * kRadix + tid] = 0u;   // everyone has read it: zero for the next launch
         }
         if (full) break;
@@ -439,9 +413,7 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
             }
             if (giveup) atomicOr(a.bar + 3, 1u);
         }
-        TL();
         grid_barrier_last(a.bar + 1, b0, T, barw, a.sc);
-        TL();
         if (__ldcg(a.bar + 3) == 0u) {                                    // (the same for every thread of the grid; reset by the next launch)
             // S3 as a scatter: the destinations are still in registers; behind the closing barrier, so that the barrier does
             // not wait for these stores
@@ -484,10 +456,6 @@ __global__ void __launch_bounds__(kFrontThreads, kFrontBlocksPerSM) k_front(cons
             }
         }
     }
-    TL();
-#ifdef BH_TIMELINE
-    if (tid == 0 && (tile == 0 || tile == T - 1)) g_bh_dbg[(tile == 0 ? 0 : 128) + 127] = (unsigned long long)ntl;
-#endif
 }
 
 int front_init(bh_ctx* c) {

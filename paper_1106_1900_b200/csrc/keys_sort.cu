@@ -208,13 +208,8 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* t
 // (status word = flag | count: AGGREGATE = this tile only, PREFIX = this tile and all before it), so no key is read
 // twice and there is no separate histogram or scan launch.  Tiles are numbered by an atomic ticket, so a tile only ever
 // waits for tiles whose blocks are already running: the look-back cannot deadlock.
-#ifndef BH_FEW
-#define BH_FEW 8
-#endif
-#ifndef BH_LOOK
-#define BH_LOOK 8
-#endif
-constexpr int kLook = BH_LOOK;   // earlier tiles a digit thread reads per round trip of the look-back
+constexpr int kFew = 8;          // a warp whose keys carry at most this many distinct digit values ranks them leader by leader
+constexpr int kLook = 8;         // earlier tiles a digit thread reads per round trip of the look-back
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagPrefix = 2u << 30, kCountMask = (1u << 30) - 1u;
 constexpr uint32_t kSpinLimit = 1u << 22;   // ~1 s of polling
 
@@ -261,11 +256,7 @@ __device__ __forceinline__ bool radix_tile(const uint64_t* __restrict__ key_in, 
         k[it] = ok ? key_in[i] : 0ull;
         v[it] = ok ? val_in[i] : 0u;
     }
-#ifdef BH_NO_MATCH
-    bool few = false;
-#else
     bool few = pass >= kSortPasses / 2;              // (warp-uniform)
-#endif
 #pragma unroll
     for (int it = 0; it < kIters; ++it) {
         const int i = wbase + it * 32 + lane;
@@ -287,9 +278,7 @@ __device__ __forceinline__ bool radix_tile(const uint64_t* __restrict__ key_in, 
             }
         }
         const uint32_t before = __popc(peers & lt);
-#ifndef BH_NO_MATCH
-        few = __popc(__ballot_sync(0xFFFFFFFFu, before == 0u)) <= BH_FEW;
-#endif
+        few = __popc(__ballot_sync(0xFFFFFFFFu, before == 0u)) <= kFew;
         uint32_t old = 0;
         if (ok) old = wcnt[w][d];
         __syncwarp();

@@ -10,11 +10,11 @@
 //     deepest one, separated by __syncthreads only: a node's children lie inside the same range.  A node is computed by
 //     EIGHT LANES, one child each: the lanes load their child at once, and the sums run over the children in ascending
 //     order through shuffles -- the same sequence of roundings as a sequential loop (bit-identical);
-//   * the cells that straddle a range boundary (at most one per level and block) are left to the block that finishes
-//     last, which computes them level by level in the same way: their children are either owned cells (all published
-//     by then: read from L2) or straddling cells of the level below, which that block keeps in shared memory -- the
-//     dependent chain over the levels of the tree never leaves the SM.
-// No thread ever waits for another block.  Cells of the same level are numbered in ascending first particle, so the
+//   * the cells that straddle a range boundary (at most one per level and block) are left to k_moments_span, a second
+//     launch of ONE cluster of eight blocks, which computes them level by level in the same way: their children are
+//     either owned cells (all published by the first launch: read from L2) or straddling cells of the level below, which
+//     the cluster keeps in (distributed) shared memory -- the dependent chain over the levels of the tree never leaves it.
+// No thread ever waits for another block of k_moments.  Cells of the same level are numbered in ascending first particle, so the
 // owned cells of a block are one index range per level, read off the per-tile scans of tree.cu.
 // The fp32 records (what the walk tests and what the force loop consumes) are written in the same pass when the caller
 // knows theta (bh_leapfrog_step, or the theta of the last bh_compute_forces as a hint); k_cell_record writes them alone
@@ -26,11 +26,6 @@
 
 namespace cg = cooperative_groups;
 
-#ifdef BH_TIMELINE
-// working aid (-DBH_TIMELINE builds only): %globaltimer stamps of this file's kernel, read back by bh_debug_moments
-__device__ unsigned long long g_bh_dbg[1024];
-extern "C" int bh_debug_moments(unsigned long long* host1024) { return (int)cudaMemcpyFromSymbol(host1024, g_bh_dbg, sizeof(unsigned long long) * 1024); }
-#endif
 
 namespace bh {
 
@@ -145,11 +140,6 @@ __device__ __forceinline__ void leaf_moments(Mom& m, Loader ld, uint32_t b, uint
     }
 }
 
-#ifdef BH_TIMELINE
-#define TLM() do { if (tid == 0 && ntl < 48) tl[ntl++] = global_ns(); } while (0)
-#else
-#define TLM() do {} while (0)
-#endif
 
 // What a parent reads of a child.
 struct Child {
@@ -300,10 +290,6 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
     const int tid = threadIdx.x;
     const uint32_t b = blockIdx.x, nb = gridDim.x;
     const int nlev = (int)sc->n_levels;                       // 0: capacity overflow, the tree is empty
-#ifdef BH_TIMELINE
-    unsigned long long tl[48]; int ntl = 0;
-#endif
-    TLM();
     // ---- the cells that start inside this block's particle range [b P, (b + 1) P): one index range per level
     if (tid < kLevels) {
         const int L = tid;
@@ -329,17 +315,12 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
         s_pre[kLevels] = run;
     }
     __syncthreads();
-    TLM();
     // ---- the block's particles, once, coalesced, into shared memory (the node scratch is not in use yet) when they fit
     float4* spos = reinterpret_cast<float4*>(mom_smem);
     const uint32_t p0 = b * (uint32_t)P;
     const uint32_t staged = P <= kMomStage ? min((uint32_t)P, (uint32_t)n - min((uint32_t)n, p0)) : 0u;
-#ifdef BH_NO_TMA
-    for (uint32_t i = tid; i < staged; i += kMomThreads) spos[i] = __ldg(pos + p0 + i);
-    __syncthreads();
-#else
     // one contiguous run of up to 128 KB: a 1-D bulk copy (TMA, cp.async.bulk) issued by one thread and completed on an
-    // mbarrier, instead of seven 16-byte loads and stores per thread (A/B: -DBH_NO_TMA)
+    // mbarrier, instead of seven 16-byte loads and stores per thread (measured against plain loads: profiles/r2_tma_ab.md)
     __shared__ __align__(8) unsigned long long s_bar;
     const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&s_bar);
     if (tid == 0) {
@@ -362,7 +343,6 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
         while (!done)
             asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(bar) : "memory");
     }
-#endif
     auto ld = [&](uint32_t i) -> float4 { return (i - p0 < staged) ? spos[i - p0] : __ldg(pos + i); };
     // ---- leaves: one thread each
     const uint32_t total = s_pre[kLevels];
@@ -385,17 +365,12 @@ __global__ void __launch_bounds__(kMomThreads, 1) k_moments(const DevScalars* __
         if (ro.enabled) rec_store(make_record(m, ro.theta, ro.mac_kind, t.x, t.y, t.z, t.w), ro, c);
     }
     __syncthreads();
-    TLM();
     // ---- owned nodes, deepest level first
     for (int L = nlev - 2; L >= 0; --L) {
         if (s_hin[L] == s_lo[L]) continue;                    // (uniform over the block)
         node_pass(s_lo[L], s_hin[L], topo, mom64, box, ro, sx, dirty, partial);
         __syncthreads();
     }
-    TLM();
-#ifdef BH_TIMELINE
-    if (tid == 0 && b == nb / 2) { for (int q = 0; q < ntl; ++q) g_bh_dbg[256 + q] = tl[q]; g_bh_dbg[256 + 127] = ntl; }
-#endif
 }
 
 // The straddling nodes, level by level from the deepest one, by ONE THREAD-BLOCK CLUSTER of eight CTAs that keeps them in
@@ -413,10 +388,6 @@ k_moments_span(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo
     const uint32_t rank = cluster.block_rank();
     const int tid = threadIdx.x, lane = tid & 31;
     const int nlev = (int)sc->n_levels;
-#ifdef BH_TIMELINE
-    unsigned long long tl[48]; int ntl = 0;
-#endif
-    TLM();
     const int grp = tid >> 3, sub = tid & 7;
     // the straddling nodes of every level, in ascending order (= block order), and their topology (every CTA builds the
     // same lists): warp w takes levels w, w + 8, ...
@@ -437,7 +408,6 @@ k_moments_span(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo
     }
     if (tid == 0) sh.cnt[nlev] = 0;
     __syncthreads();
-    TLM();
     // A node's children are (a) cells that k_moments finished before this kernel started, or (b) straddling nodes of the
     // level below.  (a) does not depend on anything computed here: while the cluster barrier of level L is pending (between
     // its arrive and its wait), the lanes work out where the children of their node of level L - 1 are (binary search) and
@@ -536,12 +506,8 @@ k_moments_span(const DevScalars* __restrict__ sc, const uint4* __restrict__ topo
         cur_d = describe(Ln);
         request(cur_d, cur_ch, cur_own, cur_df);
         cluster.barrier_wait();                                            // ... and so is everybody else's
-        TLM();
         Lc = Ln;
     }
-#ifdef BH_TIMELINE
-    if (tid == 0 && rank == 0) { for (int q = 0; q < ntl; ++q) g_bh_dbg[384 + q] = tl[q]; g_bh_dbg[384 + 127] = ntl; }
-#endif
 }
 
 // fp32 records alone (theta or the MAC changed on an existing tree).

@@ -28,24 +28,14 @@ namespace bh {
 
 constexpr int kEvalWarps = 4;
 constexpr int kEvalThreads = kEvalWarps * 32;
-#ifndef BH_EVAL_BLOCKS
-#define BH_EVAL_BLOCKS 4
-#endif
-constexpr int kEvalBlocksPerSM = BH_EVAL_BLOCKS;          // 4: 16 warps / SM at <= 128 registers
-#ifndef BH_EVAL_BATCH
-#define BH_EVAL_BATCH 128
-#endif
-constexpr int kBatch = BH_EVAL_BATCH;        // list entries per batch
+constexpr int kEvalBlocksPerSM = 4;          // 16 warps / SM at <= 128 registers
+constexpr int kBatch = 128;                  // list entries per batch
 constexpr int kPerLane = kBatch / 32;        // entries a lane gathers per batch
 
 struct __align__(16) EvalShared {
     float4 buf[2][kBatch * 3];               // cp.async landing zones: 3 x float4 per cell, 1 x float4 per particle
     uint32_t idx[2][kBatch];                 // list indices of the next batches (cp.async as well)
     float tx[64], ty[64], tz[64];            // negated target coordinates: a lane reads its pairs with one 64-bit load each
-#ifdef BH_EVAL_SELF_TMA
-    unsigned long long bar;                  // mbarrier of the bulk copy of the group's own particles (A/B: profiles/r2_tma_ab.md)
-    unsigned long long pad;
-#endif
 };
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
@@ -64,7 +54,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 template <int R2>
 __device__ __forceinline__ void eval_group(EvalShared* ws, const int lane, const uint32_t gb, const int ng, const float4* __restrict__ pos,
                                            const float4* __restrict__ erec, const uint32_t* __restrict__ lpc, const int npc,
-                                           const uint32_t* __restrict__ lpp, const int npp, const Consts& k, float4* __restrict__ acc_out, uint32_t& tma_phase) {
+                                           const uint32_t* __restrict__ lpp, const int npp, const Consts& k, float4* __restrict__ acc_out) {
     constexpr int R = 2 * R2;
     constexpr int U = R2 == 1 ? 2 : 1;           // entries per iteration: two independent chains per lane in every case but R2 = 3 (three)
     const int L = (ng + R - 1) / R, S = 32 / L;
@@ -130,24 +120,11 @@ __device__ __forceinline__ void eval_group(EvalShared* ws, const int lane, const
                 if (le < len) cp_async16(dst + le, pos + sidx[le]);
             }
         } else {
-#ifdef BH_EVAL_SELF_TMA
-            // the group's own particles are one contiguous run of ng x 16 bytes: a 1-D bulk copy (TMA) issued by one lane
-            if (lane == 0) {
-                const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&ws->bar);
-                const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst);
-                const uint32_t bytes = (uint32_t)len * 16u;
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // (the buffer was last read through the generic proxy)
-                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                             ::"r"(d), "l"(pos + gb), "r"(bytes), "r"(bar) : "memory");
-            }
-#else
 #pragma unroll
             for (int j = 0; j < kPerLane; ++j) {
                 const int le = j * 32 + lane;
                 if (le < len) cp_async16(dst + le, pos + gb + le);
             }
-#endif
         }
     };
 
@@ -160,15 +137,6 @@ __device__ __forceinline__ void eval_group(EvalShared* ws, const int lane, const
     cp_async_commit();
     for (int b = 0; b < nb; ++b) {
         cp_async_wait_all();
-#ifdef BH_EVAL_SELF_TMA
-        if (b + 1 == nb) {             // the self batch came by the bulk copy: wait for its mbarrier phase
-            const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&ws->bar);
-            uint32_t done = 0;
-            while (!done)
-                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(done) : "r"(bar), "r"(tma_phase & 1u) : "memory");
-            tma_phase ^= 1u;
-        }
-#endif
         __syncwarp();                  // batch b (and the indices of b + 1) have landed; everyone is done sweeping batch b - 1
         if (b + 1 < nb) { issue(b + 1); fetch_idx(b + 2); cp_async_commit(); }
         const float4* buf = ws->buf[b & 1];
@@ -258,15 +226,6 @@ __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(co
     const int lane = threadIdx.x & 31;
     const uint32_t g0 = ctl->wave_g[wave], g1 = ctl->wave_g[wave + 1];
     const Consts k = make_consts(eps2);
-    uint32_t tma_phase = 0;
-#ifdef BH_EVAL_SELF_TMA
-    if (lane == 0) {
-        const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&ws->bar);
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncwarp();
-#endif
     if (threadIdx.x == 0) atomicMin(&ctl->t_start[1][wave], global_ns());
     // three sweeps over the wave's groups with one counter: first the groups with more than 3 times the average work
     // (targets x list entries), then those above 1.5 times, then the rest -- the long groups start early and the kernel
@@ -294,9 +253,9 @@ __global__ void __launch_bounds__(kEvalThreads, kEvalBlocksPerSM) k_walk_eval(co
         const uint32_t* lpc = lists + pcoff;
         const uint32_t* lpp = lists + __ldg(g_ppoff + g);
         switch (choose_r2(ng)) {
-            case 1: eval_group<1>(ws, lane, gb, ng, pos, erec, lpc, npc, lpp, npp, k, acc_out, tma_phase); break;
-            case 2: eval_group<2>(ws, lane, gb, ng, pos, erec, lpc, npc, lpp, npp, k, acc_out, tma_phase); break;
-            default: eval_group<3>(ws, lane, gb, ng, pos, erec, lpc, npc, lpp, npp, k, acc_out, tma_phase); break;
+            case 1: eval_group<1>(ws, lane, gb, ng, pos, erec, lpc, npc, lpp, npp, k, acc_out); break;
+            case 2: eval_group<2>(ws, lane, gb, ng, pos, erec, lpc, npc, lpp, npp, k, acc_out); break;
+            default: eval_group<3>(ws, lane, gb, ng, pos, erec, lpc, npc, lpp, npp, k, acc_out); break;
         }
         __syncwarp();
     }

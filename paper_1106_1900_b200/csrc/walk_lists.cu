@@ -6,8 +6,8 @@
 // FP32 loop that wants 128 registers per thread.  The lists travel through device memory as 4-byte indices -- 4 B against
 // ~20 x 64 flops per entry, i.e. nothing next to the arithmetic they feed.
 //
-// One warp walks one group; the eight warps of a block draw from a chunk of 32 CONSECUTIVE groups (Morton neighbours test
-// nearly the same cells, so the block's loads hit L1).  Per group:
+// One warp walks one group at a time.  A warp claims a TASK of up to eight CONSECUTIVE groups (a super-group, see below:
+// Morton neighbours test nearly the same cells), walks what they have in common once and then each of them.  Per group:
 //   * frontier: a LIFO of OPENED NODES (first child, child count) in shared memory.  The paper walks breadth-first with two
 //     stacks of cells (L83-87); the interaction lists are SETS, so any traversal order produces the same lists and counts.
 //     A step pops up to four nodes and gives each of their (up to 8, consecutive) children to one lane: a node of the
@@ -33,14 +33,7 @@ constexpr int kListThreads = kListWarps * 32;
 constexpr int kLStackCap = 512;       // opened nodes
 constexpr int kLStackReserve = 160;   // >= 7 * 20 + 7: room for a pure depth-first descent
 constexpr int kLeafQueue = 64;
-#ifndef BH_GROUP_CHUNK
-#define BH_GROUP_CHUNK 32
-#endif
-#ifndef BH_KSUB
-#define BH_KSUB 2
-#endif
-constexpr int kGroupChunk = BH_GROUP_CHUNK;   // consecutive groups a block claims at a time
-constexpr int kSub = BH_KSUB;               // sub-batches of 4 nodes (32 children) popped per step: 4 records in flight per lane
+constexpr int kSub = 2;               // sub-batches of 4 nodes (32 children) popped per step: 4 records in flight per lane
 
 struct ListArena { uint32_t pc_top, pp_bot; };
 struct WalkSums { unsigned long long pc, pp, mac; };
@@ -82,10 +75,7 @@ __device__ __forceinline__ bool flush_leaves(const uint2* q, int k, int lane, ui
 // Every member then copies the shared lists into its own lists (4 bytes per entry against ~120 instructions per MAC
 // test and append) and continues the walk from the frontier with its own box.  The lists are sets, so the counts are
 // exactly those of O9; which groups form a super-group depends on the group index only, never on the active subset.
-#ifndef BH_SG
-#define BH_SG 8
-#endif
-constexpr int kSG = BH_SG;              // groups per super-group
+constexpr int kSG = 8;                  // groups per super-group
 constexpr int kAmbCap = 384;
 struct SharedWalk {                     // the result of a shared walk: the two shared lists sit in the list region like a group's
     uint32_t amb[kAmbCap];
@@ -371,9 +361,7 @@ __device__ __forceinline__ bool alloc_chunk(WalkCtl* ctl, int wave, int lane, ui
     return true;
 }
 
-constexpr int kChunkSG = kListWarps;                                   // super-groups per chunk: one shared walk per warp
-constexpr int kShareChunk = kSG * kChunkSG;                             // 64 consecutive groups a block claims at a time
-constexpr size_t kListSmem = sizeof(ListWarpShared) * kListWarps + sizeof(SharedWalk) * kChunkSG;
+constexpr size_t kListSmem = (sizeof(ListWarpShared) + sizeof(SharedWalk)) * kListWarps;   // per warp: its walk state + one shared walk
 
 // The box of group g (A13).  A group that is a whole cell has that cell's box (exact min / max of the same particles); a
 // chunk of an over-full leaf takes it from its particles (all lanes take part).
@@ -402,7 +390,6 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
     extern __shared__ __align__(16) unsigned char list_smem[];
     ListWarpShared* s_ws = reinterpret_cast<ListWarpShared*>(list_smem);
     SharedWalk* s_sw = reinterpret_cast<SharedWalk*>(list_smem + sizeof(ListWarpShared) * kListWarps);
-    __shared__ uint32_t s_chunk;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t g0 = o.ctl->wave_g[wave], g1 = o.ctl->wave_g[wave + 1];
     if (threadIdx.x == 0) atomicMin(&o.ctl->t_start[0][wave], global_ns());
@@ -411,15 +398,6 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
     WalkSums sums = {0ull, 0ull, 0ull};
     const bool sharing = share && kMac == kMacEq1;
     for (;;) {
-#ifdef BH_LIST_BLOCK_CHUNKS
-        __syncthreads();               // everyone is done with the previous chunk
-        if (threadIdx.x == 0) s_chunk = atomicAdd(&o.ctl->list_next[wave], (uint32_t)kShareChunk);
-        __syncthreads();
-        const uint32_t base = g0 + s_chunk;
-        if (base >= g1) break;
-        const uint32_t nchunk = min((uint32_t)kShareChunk, g1 - base);
-        const uint32_t s0 = (uint32_t)warp * kSG;
-#else
         // every warp claims its own super-group: no warp ever waits for another.  Task t covers a FIXED range of groups (the
         // partition depends on the number of groups only, so the lists, and with them the order of the fp32 sums, do not
         // depend on timing or on the active subset): eight groups per task over the first 70 % of the groups, four up to
@@ -442,7 +420,6 @@ __global__ void __launch_bounds__(kListThreads, 4) k_walk_lists(WalkListOut o, i
         const uint32_t base = g0 + off;
         const uint32_t nchunk = min(sz, g1 - base);
         const uint32_t s0 = 0u;
-#endif
         // ---- warp w takes the super-group w of the chunk (groups base + kSG w ...): one shared walk, then its members one by
         //      one from where the shared walk stopped.  No warp waits for another inside a chunk.
         SharedWalk* sw = s_sw + warp;
