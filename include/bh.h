@@ -13,7 +13,8 @@
  *   - Particle layout: pos_mass = float[n][4] (x, y, z, m); vel = float[n][4] (vx, vy, vz, unused);
  *     acc_pot = float[n][4] (ax, ay, az, phi); id = uint32[n] (caller identity).
  *   - The library keeps the particle state inside the caller-provided WORKSPACE, in key-sorted order
- *     (bh_tree_build re-sorts it; `id` follows the particles).  bh_set_particles / bh_get_particles copy in / out.
+ *     (bh_tree_build re-sorts it; `id` follows the particles).  bh_set_particles / bh_get_particles copy in / out;
+ *     bh_bind_particles borrows the caller's device arrays as that state instead (no copy).
  *   - Memory: the library never allocates device memory.  `d_workspace` is device memory owned by the caller
  *     (e.g. a torch tensor) and must stay alive until bh_destroy.  Host objects are owned by the ctx.
  *   - Streams: `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  bh_tree_build,
@@ -138,6 +139,24 @@ int bh_destroy(bh_ctx* ctx);
  * capture every copy stays on `stream`.  All source buffers must stay valid until the work enqueued on `stream` by the
  * next bh_tree_build / bh_get_particles (or a synchronisation after it) has completed. */
 int bh_set_particles(bh_ctx* ctx, int64_t n, const float* pos_mass, const float* vel, const uint32_t* id, void* stream);
+
+/* Borrow the caller's DEVICE arrays as the simulation state instead of copying it in (section 1 and PAPER.md:264
+ * section 5: the particles live on the GPU and no step moves them to the host or back).
+ * d_pos_mass, d_vel, d_acc_pot: float[n][4], 16-byte aligned; d_id: uint32[n]; all on the context's device, n <= n_max.
+ * Nothing is copied, zeroed or enqueued: the four arrays take the place of the workspace's first set of particle arrays
+ * and of its acc_pot array, and every later call reads and writes them directly on the stream it is given (the caller orders
+ * its own accesses against those streams).  Invalidates tree and forces, like bh_set_particles; acc_pot is not read before
+ * the first force evaluation has written it.  The arrays are borrowed until bh_set_particles (which goes back to the
+ * workspace's own arrays), another bh_bind_particles or bh_destroy.
+ * Where the state is afterwards.  acc_pot: always the caller's array, rows in the current key-sorted order.  Positions,
+ * velocities and ids: S3 gathers them from one set of arrays into the other (caller's -> workspace's, workspace's -> caller's),
+ * so after an EVEN number of builds since the binding (bh_tree_build, and the one inside every bh_leapfrog_step,
+ * bh_step_graph_launch and bh_block_step with rebuild) the caller's arrays hold the current sorted state, and after an odd
+ * number the workspace does (bh_export_tree gives the pointers either way).  bh_land_particles makes the caller's arrays
+ * current in that case with one device-to-device copy of 36 bytes per particle (nothing is enqueued when they already are);
+ * tree, forces and block state stay valid.  A run that steps in pairs never copies a particle. */
+int bh_bind_particles(bh_ctx* ctx, int64_t n, float* d_pos_mass, float* d_vel, float* d_acc_pot, uint32_t* d_id);
+int bh_land_particles(bh_ctx* ctx, void* stream);
 
 /* Copy the current (key-sorted) state out; any pointer may be NULL; host or device destinations.  BH_ERR_STATE when
  * acc_pot is asked for between a bh_tree_build (which re-sorts the particles) and the next evaluation that puts every row

@@ -19,7 +19,7 @@ STATUS = {0: "BH_OK", -1: "BH_ERR_INVALID_ARG", -2: "BH_ERR_WORKSPACE", -3: "BH_
           -5: "BH_ERR_NONFINITE", -6: "BH_ERR_CAPACITY", -7: "BH_ERR_TOO_LARGE"}
 
 # every symbol include/bh.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", "bh_get_particles", "bh_tree_build",
+SYMBOLS = ["bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_particles", "bh_bind_particles", "bh_land_particles", "bh_get_particles", "bh_tree_build",
            "bh_compute_forces", "bh_refresh_moments", "bh_compute_forces_active", "bh_refresh_moments_active", "bh_block_init", "bh_block_step",
            "bh_block_state", "bh_set_mac", "bh_leapfrog_step", "bh_step_graph_build",
            "bh_step_graph_launch", "bh_kick_drift", "bh_sync_status", "bh_export_tree", "bh_set_stage_timing",
@@ -83,6 +83,10 @@ def load_library():
     lib.bh_create.argtypes = [C.POINTER(C.c_void_p), C.c_int64, C.POINTER(BhConfig), C.c_void_p, C.c_size_t]
     lib.bh_destroy.argtypes = [C.c_void_p]
     lib.bh_set_particles.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.bh_bind_particles.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.bh_bind_particles.restype = C.c_int
+    lib.bh_land_particles.argtypes = [C.c_void_p, C.c_void_p]
+    lib.bh_land_particles.restype = C.c_int
     lib.bh_get_particles.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.bh_tree_build.argtypes = [C.c_void_p, C.c_void_p]
     lib.bh_compute_forces.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p]
@@ -278,7 +282,26 @@ class BarnesHut:
         n = int(pos_mass.shape[0])
         self._keep = (pos_mass, vel, ids)   # keep host buffers alive until the async copies are done
         self._check(self.lib.bh_set_particles(self.h, n, _ptr(pos_mass), _ptr(vel), _ptr(ids), self._stream()), "bh_set_particles")
+        if getattr(self, "_bound", None) is not None:
+            self._bound = None             # back to the workspace's own arrays
+            self._acc_ptr = None
         self.n = n
+
+    def bind_particles(self, pos_mass: torch.Tensor, vel: torch.Tensor, acc_pot: torch.Tensor, ids: torch.Tensor):
+        """bh_bind_particles: the caller's CUDA tensors (float32[n,4] x 3, int32[n] ids) become the simulation state; no copy.
+        The tensors are kept alive by this object until set_particles / another bind_particles / close."""
+        n = int(pos_mass.shape[0])
+        for t, shape, dt in ((pos_mass, (n, 4), torch.float32), (vel, (n, 4), torch.float32), (acc_pot, (n, 4), torch.float32), (ids, (n,), torch.int32)):
+            if not (t.is_cuda and t.device == self.device and t.dtype == dt and t.is_contiguous() and tuple(t.shape) == shape):
+                raise BhError(-1, "bind_particles wants contiguous CUDA tensors on this device: float32[n,4] x 3 and int32[n]")
+        self._check(self.lib.bh_bind_particles(self.h, n, pos_mass.data_ptr(), vel.data_ptr(), acc_pot.data_ptr(), ids.data_ptr()), "bh_bind_particles")
+        self._bound = (pos_mass, vel, acc_pot, ids)
+        self._acc_ptr = None
+        self.n = n
+
+    def land_particles(self):
+        """bh_land_particles: make the bound tensors hold the current sorted state (one device copy, or nothing)."""
+        self._check(self.lib.bh_land_particles(self.h, self._stream()), "bh_land_particles")
 
     def get_particles(self, pos_mass=None, vel=None, acc_pot=None, ids=None):
         self._check(self.lib.bh_get_particles(self.h, _ptr(pos_mass), _ptr(vel), _ptr(acc_pot), _ptr(ids), self._stream()),
@@ -377,6 +400,9 @@ class BarnesHut:
     def _view(self, ptr: int, count: int, dtype: torch.dtype, shape=None):
         if ptr is None or count == 0:
             return torch.empty(0, dtype=dtype, device=self.device)
+        for t in (getattr(self, "_bound", None) or ()):          # bh_bind_particles: the pointer may be one of the caller's tensors
+            if t.data_ptr() == ptr:
+                return t.view(dtype).view(shape) if shape is not None else t.view(dtype).reshape(-1)
         off = ptr - self.workspace.data_ptr()
         nb = count * torch.empty(0, dtype=dtype).element_size()
         t = self.workspace[off: off + nb].view(dtype)

@@ -163,6 +163,7 @@ int bh_create(bh_ctx** out, int64_t n_max, const bh_config* cfg, void* d_workspa
     c->front_full = g.front_mode == 2;
     c->walk_share = g.walk_private ? 0 : 1;
     carve(g, static_cast<unsigned char*>(d_workspace), &c->ws);
+    c->home_pos0 = c->ws.pos[0]; c->home_vel0 = c->ws.vel[0]; c->home_id0 = c->ws.idb[0]; c->home_acc = c->ws.acc;
     int rc = BH_OK;
     do {
         if (cudaSetDevice(c->device) != cudaSuccess) { rc = BH_ERR_CUDA; break; }
@@ -197,6 +198,11 @@ int bh_set_particles(bh_ctx* c, int64_t n, const float* pos_mass, const float* v
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     BH_CUDA(c, cudaSetDevice(c->device));
     if (c->step_graph_valid && n != c->n) drop_step_graph(c);   // captured for the old particle count
+    if (c->bound) {                                             // back to the workspace's own arrays: the caller's are released
+        c->ws.pos[0] = c->home_pos0; c->ws.vel[0] = c->home_vel0; c->ws.idb[0] = c->home_id0; c->ws.acc = c->home_acc;
+        c->bound = false;
+        drop_step_graph(c);                                     // (the captured kernels hold the caller's pointers)
+    }
     c->n = n;
     c->cur = 0;
     c->have_particles = c->have_topology = c->have_tree = c->have_forces = false;
@@ -224,6 +230,47 @@ int bh_set_particles(bh_ctx* c, int64_t n, const float* pos_mass, const float* v
         c->copies_pending = true;
     }
     c->have_particles = true;
+    return BH_OK;
+}
+
+int bh_bind_particles(bh_ctx* c, int64_t n, float* d_pos_mass, float* d_vel, float* d_acc_pot, uint32_t* d_id) {
+    if (!c || !d_pos_mass || !d_vel || !d_acc_pot || !d_id || n < 1 || n > c->n_max) return BH_ERR_INVALID_ARG;
+    const void* ptrs[4] = {d_pos_mass, d_vel, d_acc_pot, d_id};
+    for (int k = 0; k < 4; ++k) {
+        cudaPointerAttributes a;
+        if (cudaPointerGetAttributes(&a, ptrs[k]) != cudaSuccess || a.type != cudaMemoryTypeDevice || a.device != c->device) {
+            (void)cudaGetLastError();
+            return BH_ERR_INVALID_ARG;
+        }
+        if (reinterpret_cast<uintptr_t>(ptrs[k]) % (k < 3 ? 16u : 4u)) return BH_ERR_INVALID_ARG;   // float4 rows are moved as 16-byte words
+    }
+    drop_step_graph(c);                                         // captured kernels hold the previous pointers
+    c->ws.pos[0] = reinterpret_cast<float4*>(d_pos_mass);
+    c->ws.vel[0] = reinterpret_cast<float4*>(d_vel);
+    c->ws.acc = reinterpret_cast<float4*>(d_acc_pot);
+    c->ws.idb[0] = d_id;
+    c->bound = true;
+    c->n = n;
+    c->cur = 0;
+    c->have_particles = true;
+    c->have_topology = c->have_tree = c->have_forces = false;
+    c->block_on = false;
+    c->acc_in_order = true;                                     // the caller's acc_pot belongs to the caller's particles, row by row
+    return BH_OK;
+}
+
+int bh_land_particles(bh_ctx* c, void* stream) {
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->have_particles) return BH_ERR_STATE;
+    if (c->cur == 0) return BH_OK;                              // already there
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    BH_CUDA(c, cudaSetDevice(c->device));
+    { int rcj = join_copies(c, s); if (rcj != BH_OK) return rcj; }
+    const size_t n = (size_t)c->n;
+    BH_CUDA(c, cudaMemcpyAsync(c->ws.pos[0], c->ws.pos[1], sizeof(float4) * n, cudaMemcpyDeviceToDevice, s));
+    BH_CUDA(c, cudaMemcpyAsync(c->ws.vel[0], c->ws.vel[1], sizeof(float4) * n, cudaMemcpyDeviceToDevice, s));
+    BH_CUDA(c, cudaMemcpyAsync(c->ws.idb[0], c->ws.idb[1], sizeof(uint32_t) * n, cudaMemcpyDeviceToDevice, s));
+    c->cur = 0;                                                 // tree, forces and block state stay valid: same particles, same order
     return BH_OK;
 }
 

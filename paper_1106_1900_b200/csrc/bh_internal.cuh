@@ -124,6 +124,8 @@ __device__ __forceinline__ void grid_barrier_last(uint32_t* closing, uint32_t b0
     __syncthreads();
 }
 
+typedef float4* float4_ptr;
+
 // Pointers into the caller's workspace.
 struct Ws {
     DevScalars* sc;
@@ -196,6 +198,9 @@ struct bh_ctx {
     int cur;               // which of pos[2]/vel[2]/idb[2] holds the live state
     int sorted;            // which of key[2]/val[2] holds the sorted keys / perm
     bool have_particles, have_topology, have_tree, have_forces;   // topology: cells + groups; tree: topology + current moments
+    bool bound;            // bh_bind_particles: ws.pos[0] / vel[0] / idb[0] / acc are the CALLER's arrays (home_*: the workspace's own)
+    bh::float4_ptr home_pos0, home_vel0, home_acc;
+    uint32_t* home_id0;
     bool acc_in_order;     // ws.acc is in the order of the current particle arrays (false between a re-sort and the next full forces)
     const uint8_t* active;   // per-particle flags of bh_compute_forces_active during that call (nullptr: every group)
     int64_t launches;
