@@ -24,7 +24,8 @@
 // Eq.1's l, delta, r_open: hand-built cells with closed-form values and a target one ulp on either side of the
 // threshold, plus a numpy-float32 restatement over every cell and a root-to-leaf walk with it; block time-steps: rung
 // closed forms and thresholds, commensurate times, the one-rung case against the shared-step leapfrog, second order on a
-// two-body orbit with unequal steps, energy over a macro-step.
+// two-body orbit with unequal steps, energy over a macro-step; group boxes (orc_group_boxes): numpy min / max over every
+// group's slice, equality with the cell's box for whole-cell groups, overflow-leaf chunks.
 // Parity unpinned against the paper: magnitudes of the interaction counts (Fig.6 inset is an image).
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
